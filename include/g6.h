@@ -1,0 +1,187 @@
+/*
+ * g6.h -- C ABI of libg6b200: a GRAPE-6-style direct-summation force engine for NVIDIA B200
+ * (sm_100a), after Sapporo (arxiv 0902.4463; cited below as PAPER.md:LINE).
+ *
+ * The paper reproduces "the calling sequence of the GRAPE-6 library" but
+ * prints no prototypes, and the GRAPE-6 header is not available to this build.  The g6_* names
+ * and argument ORDER below follow the historical convention as recalled (Taylor coefficients
+ * are passed pre-divided: acc/2, jerk/6, snap/18); binary drop-in compatibility with the
+ * original header is NOT claimed.  g6x_* are extensions of this library.
+ *
+ * What one force call computes (PAPER.md:31, :41 fn.3, :80-118, :126):
+ * for every i-particle of the block, over all stored j-particles with address in [0, nj) and
+ * index_j != index_i, predicted to the time set by g6_set_ti (Eq. 1-2),
+ *     dx = x_j - x_i (double-single, Eq. 3), dv = v_j - v_i, s^2 = dx.dx + eps2
+ *     acc  = sum m_j dx / s^3
+ *     jerk = sum m_j [ dv / s^3 - 3 (dx.dv) dx / s^5 ]          (d acc / dt, physical, not /6)
+ *     pot  = - sum m_j / s                                       (negative; no self term)
+ *     nearest neighbour = argmin over j of the UNSOFTENED dx.dx, ties -> smallest address.
+ * Units G = 1.  Arithmetic: FP32 with double-single separations, partial
+ * sums folded into fp64.  All j-particles live on the device; only
+ * i-particles and results cross the host-device link per call.
+ *
+ * General rules
+ *  - Every function returns G6_OK (0) or a negative G6_ERR_* code; g6x_last_error() gives text.
+ *    No C++ exception crosses this boundary and the library never aborts.
+ *  - Pointers are HOST pointers unless the parameter name starts with d_ (DEVICE pointers,
+ *    valid on the library's device, 8-byte aligned).  The caller owns every array; the library
+ *    copies what it needs before returning and keeps no caller pointer, except that the d_
+ *    outputs of g6x_calc_dev are written asynchronously on the library's stream.
+ *  - [][3] arrays are C row-major (x,y,z per particle), fp64.
+ *  - One host thread per clusterid (not thread-safe, like the original).  clusterid in [0, 4).
+ *  - The library never falls back to a CPU path: without a usable CUDA device g6_open fails.
+ */
+#ifndef G6_B200_H
+#define G6_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define G6_OK                0
+#define G6_ERR_NOT_OPEN     -1   /* cluster not opened                                  */
+#define G6_ERR_CLUSTER      -2   /* clusterid out of range                              */
+#define G6_ERR_ADDRESS      -3   /* j address < 0 or >= capacity                        */
+#define G6_ERR_NI           -4   /* ni < 1 or ni > g6_npipes()                          */
+#define G6_ERR_NJ           -5   /* nj < 1 or nj > highest stored address + 1           */
+#define G6_ERR_SEQUENCE     -6   /* lasthalf without firsthalf, firsthalf twice, ...    */
+#define G6_ERR_CUDA         -7   /* a CUDA call failed (text in g6x_last_error)         */
+#define G6_ERR_ARG          -8   /* NULL pointer / bad value / mismatch with firsthalf  */
+#define G6_ERR_ALREADY_OPEN -9
+#define G6_ERR_NOMEM        -10
+
+/* ---- GRAPE-6 calling sequence ------------------------------------- */
+
+/* Acquire device `G6_DEVICE` (env, default 0), a stream, pinned staging and the j-particle
+ * store.  Capacity = env G6_NJMAX (default 2^21 addresses), fixed until g6_close. */
+int g6_open(int clusterid);
+
+/* Wait for outstanding work and free everything the cluster owns. */
+int g6_close(int clusterid);
+
+/* Largest ni accepted by one firsthalf/lasthalf pair.  The paper's value is 256
+ * (PAPER.md:132 fn.7); that is the default.  env G6_NPIPES or g6x_set_npipes raise it (up to
+ * 2^21) so that a whole sweep fits one call; larger blocks are tiled inside the library
+ * (the paper's "segments"). */
+int g6_npipes(void);
+
+/* Store / overwrite j-memory slot `address` (x, v, a, j and time per particle).
+ *   index      caller's particle id: what neighbour queries return and what self-exclusion
+ *              compares against the i-particle's index
+ *   tj         time at which x, v, acc, jerk are valid
+ *   dtj        the particle's step; accepted, not used by the formulas (reading 3)
+ *   snap_by18  accepted and ignored (4th-order scheme); may be NULL
+ *   jerk_by6, acc_by2   jerk/6 and acc/2 at tj (GRAPE convention, reading 13)
+ *   v, x       velocity and position at tj; x is kept in full fp64, the rest in FP32
+ *
+ * The data is copied before return; the device copy is refreshed at the next firsthalf. */
+int g6_set_j_particle(int clusterid, int address, int index, double tj, double dtj, double mass,
+                      const double snap_by18[3], const double jerk_by6[3], const double acc_by2[3],
+                      const double v[3], const double x[3]);
+
+/* Time to which the j-particles are predicted by the next force call (Eq. 1-2, dt = ti - tj). */
+int g6_set_ti(int clusterid, double ti);
+
+/* Start a force calculation on ni i-particles against j addresses [0, nj).
+ *   index[ni]          ids of the i-particles (for self-exclusion)
+ *   xi, vi [ni][3]     positions / velocities ALREADY PREDICTED to ti by the host
+ *
+ *   acc_old, jerk6_old, phi_old   GRAPE fixed-point scaling hints: ignored, may be NULL
+ *   eps2               softening length squared for this block, >= 0
+ *   h2[ni]             neighbour-sphere radius squared (reserved for neighbour lists,
+ *                      PAPER.md:206): ignored, may be NULL
+ * Copies the block to pinned staging, uploads j-particles changed since the last call, and
+ * enqueues predictor -> force -> combine -> download.  Returns without waiting. */
+int g6calc_firsthalf(int clusterid, int nj, int ni, const int index[],
+                     const double xi[][3], const double vi[][3],
+                     const double acc_old[][3], const double jerk6_old[][3], const double phi_old[],
+                     double eps2, const double h2[]);
+
+/* Wait for the matching firsthalf (same clusterid, nj, ni) and return its results:
+ * acc[ni][3], jerk[ni][3] (physical d acc/dt), pot[ni].  index/xi/vi/eps2/h2 are accepted for
+ * signature compatibility and not read. */
+int g6calc_lasthalf(int clusterid, int nj, int ni, const int index[],
+                    const double xi[][3], const double vi[][3], double eps2, const double h2[],
+                    double acc[][3], double jerk[][3], double pot[]);
+
+/* As g6calc_lasthalf, and also the nearest neighbour's index per i (-1 if none). */
+int g6calc_lasthalf2(int clusterid, int nj, int ni, const int index[],
+                     const double xi[][3], const double vi[][3], double eps2, const double h2[],
+                     double acc[][3], double jerk[][3], double pot[], int nnb_index[]);
+
+/* Make the neighbour results of the last completed force call readable.  Returns 0
+ * (a positive value would mean list overflow once neighbour lists exist). */
+int g6_read_neighbour_list(int clusterid);
+
+/* Neighbour "list" of pipe `ipipe` (the ipipe-th i-particle of the last call).  In this
+ * version the list is the single nearest neighbour: *n = 1 and list[0] = its index, or
+ * *n = 0.  maxlen must be >= 1. */
+int g6_get_neighbour_list(int clusterid, int ipipe, int maxlen, int *n, int list[]);
+
+/* ---- extensions ------------------------------------------------------------------------ */
+
+/* Text of the last error of this cluster (never NULL; valid until the next call). */
+const char *g6x_last_error(int clusterid);
+
+/* Raise/lower g6_npipes() (1 .. 2^21).  Global, like g6_npipes itself. */
+int g6x_set_npipes(int npipes);
+
+/* Bulk loader, HOST arrays: addresses addr0 .. addr0+n-1.  acc and jerk are PHYSICAL here
+ * (not pre-divided).  Same effect as n calls of g6_set_j_particle. */
+int g6x_set_j_particles(int clusterid, int addr0, int n, const int index[], const double tj[],
+                        const double mass[], const double jerk[][3], const double acc[][3],
+                        const double v[][3], const double x[][3]);
+
+/* Bulk loader, DEVICE arrays (fp64, same shapes).  Asynchronous on the library's stream. */
+int g6x_set_j_particles_dev(int clusterid, int addr0, int n, const int *d_index, const double *d_tj,
+                            const double *d_mass, const double *d_jerk, const double *d_acc,
+                            const double *d_v, const double *d_x);
+
+/* Whole force call with DEVICE inputs and outputs (fp64 [ni][3] / [ni]; d_nn_index int32,
+ * d_nn_r2 fp64, either may be NULL).  ni <= g6_npipes().  Asynchronous on the library's
+ * stream; outputs are complete after g6x_synchronize (or any sync of that stream). */
+int g6x_calc_dev(int clusterid, int nj, int ni, const int *d_index, const double *d_xi,
+                 const double *d_vi, double eps2, double *d_acc, double *d_jerk, double *d_pot,
+                 int *d_nn_index, double *d_nn_r2);
+
+/* Nearest neighbour of each i of the last completed host force call: index (-1 if none) and
+ * UNSOFTENED squared distance (+inf if none). */
+int g6x_get_nearest(int clusterid, int ni, int nn_index[], double nn_r2[]);
+
+/* Use the caller's CUDA stream (a cudaStream_t / CUstream handle cast to void*, NULL for the
+ * library's own) for all further work of this cluster.  The cluster must be idle. */
+int g6x_set_stream(int clusterid, void *cuda_stream);
+
+/* Block until all work of this cluster has finished. */
+int g6x_synchronize(int clusterid);
+
+/* Device times (microseconds, CUDA events) of the phases of the last completed force call:
+ * us[0] j upload + scatter, [1] predictor, [2] force kernel, [3] combine, [4] download,
+ * [5] whole call enqueue->done; [6] number of force-kernel CTAs, [7] j-splits S. */
+int g6x_get_timers(int clusterid, double us[8]);
+
+/* Variant switches (for experiments and tests).  Keys:
+ *   "ds"      1 (default) double-single positions; 0 = pure FP32 positions (lo words zeroed)
+ *   "newton"  1 = one Newton step after rsqrt.approx, 0 = none
+ *   "jsplit"  0 = automatic; S > 0 forces S j-splits
+ *   "kernel"  0 = automatic; 1 = checked reference kernel everywhere; 2 = fast kernel
+ *   "timers"  1 (default) record CUDA events per phase
+ * Returns G6_ERR_ARG for an unknown key or value. */
+int g6x_set_option(int clusterid, const char *key, int value);
+int g6x_get_option(int clusterid, const char *key, int *value);
+
+/* Predicted j-particles (Eq. 1-2 at the current ti) for addresses addr0..addr0+n-1, read back
+ * from the device as fp64: xp = hi + lo, vp.  Runs the predictor if needed.  For parity tests. */
+int g6x_get_predicted(int clusterid, int addr0, int n, double xp[][3], double vp[][3]);
+
+/* Debug: the kernel's own Eq.-3 separation dx[k][3] (binary32) for pairs (i-slot ipipe[k] of
+ * the last host force call, j address jaddr[k]).  For the bit-exactness pin of DESIGN.md. */
+int g6x_debug_dx(int clusterid, int n, const int ipipe[], const int jaddr[], float dx[][3]);
+
+/* Library build information: a static string (arch, variant flags). */
+const char *g6x_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* G6_B200_H */

@@ -1,0 +1,53 @@
+/*
+ * g6_hermite.h -- host-side 4th-order Hermite predictor-corrector with block time steps (fp64)
+ * that drives libg6b200 through the g6_* calling sequence of g6.h, exactly as a GRAPE-6 host
+ * code does (section 2; task split of Fig. 1: the host predicts
+ * the i-particles and corrects, the device predicts the j-particles and computes the forces).
+ *
+ * The paper cites the scheme (Makino & Aarseth 1992) and the step criterion
+ * (Aarseth 1985) without printing them; the textbook formulas used are
+ * listed in DESIGN.md reading 16:
+ *   corrector  a2 = [-6 (a0 - a1) - h (4 adot0 + 2 adot1)] / h^2,  a3 = [12 (a0 - a1) + 6 h (adot0 + adot1)] / h^3
+ *              x1 = x_p + h^4 a2 / 24 + h^5 a3 / 120,  v1 = v_p + h^3 a2 / 6 + h^4 a3 / 24
+ *   step       dt_want = sqrt(eta (|a1||a2'| + |adot1|^2) / (|adot1||a3| + |a2'|^2)),  a2' = a2 + h a3;
+ *              power-of-two steps, halved while dt > dt_want, doubled only when dt_want >= 2 dt and the
+ *              time is a multiple of 2 dt, dt <= dt_max; first step eta_start |a| / |adot| rounded down.
+ *
+ * All pointers are HOST pointers, [][3] arrays row-major fp64; the caller owns them.
+ * Functions return 0 or a negative G6_ERR_* code (g6h_create: NULL on failure; the text is in
+ * g6x_last_error(clusterid)).  The cluster must have been opened with g6_open and must not be
+ * used by anything else while the system exists.  Particle p lives at j address p with index p.
+ */
+#ifndef G6_B200_HERMITE_H
+#define G6_B200_HERMITE_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct g6h_system g6h_system;
+
+/* Load n particles (t = 0), compute initial acc/jerk on the device and the initial steps. */
+g6h_system *g6h_create(int clusterid, int n, const double x[][3], const double v[][3], const double m[],
+                       double eps2, double eta, double eta_start, double dt_max);
+
+void g6h_destroy(g6h_system *s);
+
+/* Advance block step by block step until t_end (a multiple of dt_max: all particles are then
+ * synchronised) or for at most max_block_steps (> 0) block steps. */
+int g6h_evolve(g6h_system *s, double t_end, long long max_block_steps);
+
+/* Positions and velocities at the current system time: corrected values for particles that
+ * are at that time, Eq. 1-2 predictions (host, fp64) for the others. */
+int g6h_get_state(g6h_system *s, double x[][3], double v[][3]);
+
+/* stats[0] block steps, [1] particle steps, [2] system time, [3] smallest step used,
+ * [4] pairwise interactions (n_i * N per block step), [5] wall seconds spent in g6h_evolve,
+ * [6] wall seconds of that inside the g6 force calls.  ni_hist_log2[b] = block steps with
+ * 2^b <= n_i < 2^(b+1) (64 entries). */
+int g6h_get_stats(g6h_system *s, double stats[8], long long ni_hist_log2[64]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,747 @@
+// g6_api.cu -- the C ABI of libg6b200 (include/g6.h): host state, staging, launch scheduling.
+// Every step of the path runs in the CUDA kernels; there is no CPU fallback: without a CUDA
+// device g6_open fails with G6_ERR_CUDA.
+#include "../../include/g6.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <vector>
+
+#include "g6_device.cuh"
+#include "g6_force_ref.cuh"
+#include "g6_force_fast.cuh"
+
+using namespace g6;
+
+namespace {
+
+constexpr int MAX_CLUSTERS = 4;
+constexpr int MAX_NPIPES = 1 << 21;
+constexpr int N_EVENTS = 6;
+
+int g_npipes = 0;   // 0 = not initialised yet (env G6_NPIPES or 256)
+
+struct Cluster {
+    bool open = false;
+    int device = 0;
+    int n_sm = 148;
+    cudaStream_t stream = nullptr;
+    cudaStream_t own_stream = nullptr;
+    char err[512] = "no error";
+
+    // j store
+    int capacity = 0;        // addresses
+    int n_stored = 0;        // highest address set + 1
+    JStore js{};
+    float *pred = nullptr;   // predicted tiles
+    int *tile_imin = nullptr, *tile_imax = nullptr;
+    bool pred_valid = false;
+    double pred_ti = 0.0;
+    int pred_ds = 1;
+    int pred_n = 0;
+
+    // host -> device staging of changed j particles
+    JRecord *h_rec = nullptr;   // pinned
+    JRecord *d_rec = nullptr;
+    int rec_cap = 0, n_rec = 0;
+    std::vector<int> slot_of_addr;   // address -> slot in h_rec (or -1)
+
+    // i block + results
+    int i_cap = 0;
+    int *h_idx = nullptr, *d_idx = nullptr;
+    double *h_xi = nullptr, *h_vi = nullptr, *d_xi = nullptr, *d_vi = nullptr;
+    double *d_acc = nullptr, *d_jerk = nullptr, *d_pot = nullptr, *d_nnr2 = nullptr;
+    int *d_nnidx = nullptr;
+    double *h_acc = nullptr, *h_jerk = nullptr, *h_pot = nullptr, *h_nnr2 = nullptr;
+    int *h_nnidx = nullptr;
+
+    // partial results
+    Partials part{};
+    void *part_block = nullptr;
+    size_t part_elems = 0;
+
+    // bulk-load staging (host fp64 arrays -> device)
+    void *h_bulk = nullptr, *d_bulk = nullptr;
+    size_t bulk_bytes = 0;
+
+    // call state
+    double ti = 0.0;
+    bool pending = false;      // firsthalf issued, lasthalf not yet
+    bool have_result = false;  // a host force call completed (neighbour / debug queries)
+    int pend_nj = 0, pend_ni = 0;
+    int last_ni = 0;
+    cudaEvent_t ev[N_EVENTS] = {};
+    cudaEvent_t ev_bulk = nullptr;
+    bool ev_valid = false;
+    int last_ctas = 0, last_S = 0;
+
+    // options
+    int opt_ds = 1, opt_newton = 1, opt_jsplit = 0, opt_kernel = 0, opt_timers = 1, opt_variant = 0;
+};
+
+Cluster g_cl[MAX_CLUSTERS];
+
+int fail(Cluster &c, int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(c.err, sizeof(c.err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CK(call)                                                                                  \
+    do {                                                                                          \
+        cudaError_t e_ = (call);                                                                  \
+        if (e_ != cudaSuccess)                                                                    \
+            return fail(c, G6_ERR_CUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_),  \
+                        __FILE__, __LINE__);                                                      \
+    } while (0)
+
+#define GET_CLUSTER(id)                                                     \
+    if ((id) < 0 || (id) >= MAX_CLUSTERS) return G6_ERR_CLUSTER;            \
+    Cluster &c = g_cl[(id)];                                                \
+    if (!c.open) return fail(c, G6_ERR_NOT_OPEN, "cluster %d is not open", (id))
+
+int env_int(const char *name, int dflt)
+{
+    const char *v = getenv(name);
+    if (!v || !*v) return dflt;
+    char *end = nullptr;
+    long x = strtol(v, &end, 0);
+    return (end && *end == 0) ? (int)x : dflt;
+}
+
+void init_npipes()
+{
+    if (g_npipes == 0) g_npipes = std::min(std::max(env_int("G6_NPIPES", 256), 1), MAX_NPIPES);
+}
+
+template <class T>
+cudaError_t dalloc(T *&p, size_t n) { return cudaMalloc((void **)&p, n * sizeof(T)); }
+template <class T>
+cudaError_t halloc(T *&p, size_t n) { return cudaMallocHost((void **)&p, n * sizeof(T)); }
+template <class T>
+void dfree(T *&p) { if (p) cudaFree(p); p = nullptr; }
+template <class T>
+void hfree(T *&p) { if (p) cudaFreeHost(p); p = nullptr; }
+
+void free_i(Cluster &c)
+{
+    hfree(c.h_idx); hfree(c.h_xi); hfree(c.h_vi);
+    dfree(c.d_idx); dfree(c.d_xi); dfree(c.d_vi);
+    dfree(c.d_acc); dfree(c.d_jerk); dfree(c.d_pot); dfree(c.d_nnr2); dfree(c.d_nnidx);
+    hfree(c.h_acc); hfree(c.h_jerk); hfree(c.h_pot); hfree(c.h_nnr2); hfree(c.h_nnidx);
+    c.i_cap = 0;
+}
+
+int ensure_i(Cluster &c, int ni)
+{
+    if (ni <= c.i_cap) return G6_OK;
+    CK(cudaStreamSynchronize(c.stream));
+    free_i(c);
+    size_t n = std::max(ni, 256);
+    CK(halloc(c.h_idx, n)); CK(halloc(c.h_xi, 3 * n)); CK(halloc(c.h_vi, 3 * n));
+    CK(dalloc(c.d_idx, n)); CK(dalloc(c.d_xi, 3 * n)); CK(dalloc(c.d_vi, 3 * n));
+    CK(dalloc(c.d_acc, 3 * n)); CK(dalloc(c.d_jerk, 3 * n)); CK(dalloc(c.d_pot, n));
+    CK(dalloc(c.d_nnr2, n)); CK(dalloc(c.d_nnidx, n));
+    CK(halloc(c.h_acc, 3 * n)); CK(halloc(c.h_jerk, 3 * n)); CK(halloc(c.h_pot, n));
+    CK(halloc(c.h_nnr2, n)); CK(halloc(c.h_nnidx, n));
+    c.i_cap = (int)n;
+    return G6_OK;
+}
+
+int ensure_partials(Cluster &c, size_t elems)
+{
+    if (elems <= c.part_elems) return G6_OK;
+    CK(cudaStreamSynchronize(c.stream));
+    if (c.part_block) cudaFree(c.part_block);
+    c.part_block = nullptr;
+    c.part_elems = 0;
+    elems = (elems + 63) & ~(size_t)63;
+    CK(cudaMalloc(&c.part_block, elems * (7 * sizeof(double) + sizeof(float) + sizeof(int))));
+    double *d = (double *)c.part_block;
+    for (int k = 0; k < 3; ++k) c.part.acc[k] = d + (size_t)k * elems;
+    for (int k = 0; k < 3; ++k) c.part.jrk[k] = d + (size_t)(3 + k) * elems;
+    c.part.pot = d + 6 * elems;
+    c.part.nn_r2 = (float *)(d + 7 * elems);
+    c.part.nn_addr = (int *)(c.part.nn_r2 + elems);
+    c.part_elems = elems;
+    return G6_OK;
+}
+
+int ensure_bulk(Cluster &c, size_t bytes)
+{
+    if (bytes <= c.bulk_bytes) return G6_OK;
+    CK(cudaStreamSynchronize(c.stream));
+    if (c.h_bulk) cudaFreeHost(c.h_bulk);
+    if (c.d_bulk) cudaFree(c.d_bulk);
+    c.h_bulk = c.d_bulk = nullptr;
+    c.bulk_bytes = 0;
+    CK(cudaMallocHost(&c.h_bulk, bytes));
+    CK(cudaMalloc(&c.d_bulk, bytes));
+    c.bulk_bytes = bytes;
+    return G6_OK;
+}
+
+int ensure_rec(Cluster &c, int n)
+{
+    if (n <= c.rec_cap) return G6_OK;
+    int cap = std::max(std::max(n, 2 * c.rec_cap), 4096);
+    JRecord *h = nullptr, *d = nullptr;
+    CK(halloc(h, cap));
+    CK(dalloc(d, cap));
+    if (c.n_rec) memcpy(h, c.h_rec, sizeof(JRecord) * c.n_rec);
+    CK(cudaStreamSynchronize(c.stream));   // the old device buffer may still be read by a scatter
+    hfree(c.h_rec);
+    dfree(c.d_rec);
+    c.h_rec = h;
+    c.d_rec = d;
+    c.rec_cap = cap;
+    return G6_OK;
+}
+
+void release(Cluster &c)
+{
+    if (c.stream) cudaStreamSynchronize(c.stream);
+    for (int k = 0; k < 3; ++k) { dfree(c.js.x[k]); dfree(c.js.v[k]); dfree(c.js.a2[k]); dfree(c.js.j6[k]); }
+    dfree(c.js.t); dfree(c.js.m); dfree(c.js.idx);
+    dfree(c.pred); dfree(c.tile_imin); dfree(c.tile_imax);
+    hfree(c.h_rec); dfree(c.d_rec);
+    free_i(c);
+    if (c.part_block) cudaFree(c.part_block);
+    if (c.h_bulk) cudaFreeHost(c.h_bulk);
+    if (c.d_bulk) cudaFree(c.d_bulk);
+    for (auto &e : c.ev) if (e) { cudaEventDestroy(e); e = nullptr; }
+    if (c.ev_bulk) cudaEventDestroy(c.ev_bulk);
+    if (c.own_stream) cudaStreamDestroy(c.own_stream);
+    char keep[sizeof(c.err)];
+    memcpy(keep, c.err, sizeof(keep));
+    c = Cluster{};
+    memcpy(c.err, keep, sizeof(keep));
+}
+
+// upload + scatter of the j particles changed since the last force call (step a-1)
+int flush_j(Cluster &c)
+{
+    if (c.n_rec == 0) return G6_OK;
+    CK(cudaMemcpyAsync(c.d_rec, c.h_rec, sizeof(JRecord) * c.n_rec, cudaMemcpyHostToDevice, c.stream));
+    k_scatter_records<<<(c.n_rec + 255) / 256, 256, 0, c.stream>>>(c.js, c.d_rec, c.n_rec);
+    CK(cudaGetLastError());
+    // the pinned buffer is rewritten by the next g6_set_j_particle: wait for the copy engine
+    CK(cudaEventRecord(c.ev_bulk, c.stream));
+    for (int k = 0; k < c.n_rec; ++k) c.slot_of_addr[c.h_rec[k].addr] = -1;
+    CK(cudaEventSynchronize(c.ev_bulk));
+    c.n_rec = 0;
+    c.pred_valid = false;
+    return G6_OK;
+}
+
+// predictor over all stored particles (step a-2); skipped when nothing changed
+int run_predict(Cluster &c)
+{
+    if (c.pred_valid && c.pred_ti == c.ti && c.pred_ds == c.opt_ds && c.pred_n == c.n_stored) return G6_OK;
+    int ntiles = (c.n_stored + JT - 1) / JT;
+    if (ntiles > 0) {
+        k_predict<<<ntiles, JT, 0, c.stream>>>(c.js, c.n_stored, c.ti, c.opt_ds, c.pred, c.tile_imin, c.tile_imax);
+        CK(cudaGetLastError());
+    }
+    c.pred_valid = true;
+    c.pred_ti = c.ti;
+    c.pred_ds = c.opt_ds;
+    c.pred_n = c.n_stored;
+    return G6_OK;
+}
+
+// force + combine (steps a-4, a-5) on device-resident i-blocks; all asynchronous
+int run_force(Cluster &c, int nj, int ni, const int *d_index, const double *d_xi, const double *d_vi,
+              double eps2, double *d_acc, double *d_jerk, double *d_pot, int *d_nn_index, double *d_nn_r2,
+              cudaEvent_t ev_force_done)
+{
+    ForceArgs A{};
+    A.pred = c.pred;
+    A.jidx = c.js.idx;
+    A.tile_imin = c.tile_imin;
+    A.tile_imax = c.tile_imax;
+    A.nj = nj;
+    A.ntiles = (nj + JT - 1) / JT;
+    A.i_index = d_index;
+    A.xi = d_xi;
+    A.vi = d_vi;
+    A.ni = ni;
+    A.eps2 = (float)eps2;
+    A.ds = c.opt_ds;
+
+    // kernel choice: the fast kernel needs a normal FP32 eps2 > 0 (its unchecked tiles rely on s2 > 0)
+    const bool fast_ok = A.eps2 >= std::numeric_limits<float>::min() && std::isfinite(A.eps2);
+    const bool use_fast = (c.opt_kernel == 2 || c.opt_kernel == 0) && fast_ok && fast_available();
+
+    const FastVariant fv = fast_pick(ni, c.n_sm, c.opt_variant);
+    const int itile = use_fast ? fv.threads * fv.it : REF_THREADS;
+    const int n_itiles = (ni + itile - 1) / itile;
+    int S;
+    if (c.opt_jsplit > 0) {
+        S = c.opt_jsplit;
+    } else {
+        // i/j-split scheduler (PAPER.md:82, :104 generalised): enough CTAs to fill the SMs at any n_i
+        const int slots = c.n_sm * (use_fast ? fast_ctas_per_sm(fv) : 8);
+        S = n_itiles >= slots ? 1 : (slots + n_itiles - 1) / n_itiles;
+        // keep at least 2 tiles per split so the staging pipeline has something to overlap
+        S = std::min(S, std::max(1, A.ntiles / 2));
+    }
+    S = std::max(1, std::min(S, A.ntiles));
+    A.S = S;
+    int rc = ensure_partials(c, (size_t)S * ni);
+    if (rc) return rc;
+    A.P = c.part;
+    A.P.stride = ni;
+
+    if (use_fast) {
+        rc = launch_force_fast(A, c.opt_newton != 0, fv, n_itiles, S, c.stream);
+        if (rc) return fail(c, G6_ERR_CUDA, "fast force kernel launch failed: %s", cudaGetErrorString((cudaError_t)rc));
+    } else {
+        dim3 grid(n_itiles, S);
+        if (c.opt_newton) k_force_ref<true><<<grid, REF_THREADS, 0, c.stream>>>(A);
+        else k_force_ref<false><<<grid, REF_THREADS, 0, c.stream>>>(A);
+        CK(cudaGetLastError());
+    }
+    if (ev_force_done) CK(cudaEventRecord(ev_force_done, c.stream));
+    k_combine<<<(ni + 255) / 256, 256, 0, c.stream>>>(A.P, S, ni, c.js.idx, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2);
+    CK(cudaGetLastError());
+    c.last_ctas = n_itiles * S;
+    c.last_S = S;
+    return G6_OK;
+}
+
+int check_force_args(Cluster &c, int nj, int ni)
+{
+    init_npipes();
+    if (ni < 1 || ni > g_npipes) return fail(c, G6_ERR_NI, "ni = %d outside [1, g6_npipes() = %d]", ni, g_npipes);
+    if (nj < 1 || nj > c.n_stored) return fail(c, G6_ERR_NJ, "nj = %d outside [1, stored = %d]", nj, c.n_stored);
+    return G6_OK;
+}
+
+}  // namespace
+
+// ================================================================================ C ABI =====
+extern "C" {
+
+int g6_npipes(void)
+{
+    init_npipes();
+    return g_npipes;
+}
+
+int g6x_set_npipes(int npipes)
+{
+    if (npipes < 1 || npipes > MAX_NPIPES) return G6_ERR_ARG;
+    g_npipes = npipes;
+    return G6_OK;
+}
+
+const char *g6x_version(void)
+{
+    return "libg6b200 0.1 (sm_100a; FP32 + double-single separations; kernels: ref, fast[FFMA2+TMA])";
+}
+
+const char *g6x_last_error(int clusterid)
+{
+    if (clusterid < 0 || clusterid >= MAX_CLUSTERS) return "clusterid out of range";
+    return g_cl[clusterid].err;
+}
+
+int g6_open(int clusterid)
+{
+    if (clusterid < 0 || clusterid >= MAX_CLUSTERS) return G6_ERR_CLUSTER;
+    Cluster &c = g_cl[clusterid];
+    if (c.open) return fail(c, G6_ERR_ALREADY_OPEN, "cluster %d is already open", clusterid);
+    init_npipes();
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev < 1)
+        return fail(c, G6_ERR_CUDA, "no CUDA device (%s); this library has no CPU path",
+                    e == cudaSuccess ? "device count 0" : cudaGetErrorString(e));
+    c.device = env_int("G6_DEVICE", 0);
+    if (c.device < 0 || c.device >= ndev) return fail(c, G6_ERR_CUDA, "G6_DEVICE = %d but %d devices", c.device, ndev);
+    CK(cudaSetDevice(c.device));
+    cudaDeviceProp prop;
+    CK(cudaGetDeviceProperties(&prop, c.device));
+    if (prop.major < 10)
+        return fail(c, G6_ERR_CUDA, "device %s is sm_%d%d; this library is built for sm_100a only", prop.name,
+                    prop.major, prop.minor);
+    c.n_sm = prop.multiProcessorCount;
+    c.capacity = std::max(JT, env_int("G6_NJMAX", 1 << 21));
+    c.capacity = ((c.capacity + JT - 1) / JT) * JT;
+    const size_t n = c.capacity;
+    int rc = [&]() -> int {
+        CK(cudaStreamCreateWithFlags(&c.own_stream, cudaStreamNonBlocking));
+        c.stream = c.own_stream;
+        for (int k = 0; k < 3; ++k) {
+            CK(dalloc(c.js.x[k], n)); CK(dalloc(c.js.v[k], n)); CK(dalloc(c.js.a2[k], n)); CK(dalloc(c.js.j6[k], n));
+        }
+        CK(dalloc(c.js.t, n)); CK(dalloc(c.js.m, n)); CK(dalloc(c.js.idx, n));
+        CK(dalloc(c.pred, n * NF));
+        CK(dalloc(c.tile_imin, n / JT)); CK(dalloc(c.tile_imax, n / JT));
+        for (auto &ev : c.ev) CK(cudaEventCreate(&ev));
+        CK(cudaEventCreateWithFlags(&c.ev_bulk, cudaEventDisableTiming));
+        int r = fast_kernel_init();
+        if (r) return fail(c, G6_ERR_CUDA, "fast kernel attribute setup failed: %s", cudaGetErrorString((cudaError_t)r));
+        return G6_OK;
+    }();
+    if (rc != G6_OK) { release(c); return rc; }
+    try {
+        c.slot_of_addr.assign(n, -1);
+    } catch (const std::bad_alloc &) {
+        release(c);
+        return fail(c, G6_ERR_NOMEM, "host allocation failed");
+    }
+    c.open = true;
+    c.opt_newton = env_int("G6_NEWTON", 1) ? 1 : 0;
+    c.opt_kernel = env_int("G6_KERNEL", 0);
+    snprintf(c.err, sizeof(c.err), "no error");
+    return G6_OK;
+}
+
+int g6_close(int clusterid)
+{
+    GET_CLUSTER(clusterid);
+    release(c);
+    return G6_OK;
+}
+
+int g6_set_j_particle(int clusterid, int address, int index, double tj, double dtj, double mass,
+                      const double snap_by18[3], const double jerk_by6[3], const double acc_by2[3],
+                      const double v[3], const double x[3])
+{
+    GET_CLUSTER(clusterid);
+    (void)dtj; (void)snap_by18;
+    if (address < 0 || address >= c.capacity)
+        return fail(c, G6_ERR_ADDRESS, "address %d outside [0, capacity = %d)", address, c.capacity);
+    if (!jerk_by6 || !acc_by2 || !v || !x) return fail(c, G6_ERR_ARG, "NULL array in g6_set_j_particle");
+    int slot = c.slot_of_addr[address];
+    if (slot < 0) {
+        int rc = ensure_rec(c, c.n_rec + 1);
+        if (rc) return rc;
+        slot = c.n_rec++;
+        c.slot_of_addr[address] = slot;
+    }
+    JRecord &r = c.h_rec[slot];
+    for (int k = 0; k < 3; ++k) {
+        r.x[k] = x[k];
+        r.v[k] = (float)v[k];
+        r.a2[k] = (float)acc_by2[k];
+        r.j6[k] = (float)jerk_by6[k];
+    }
+    r.t = tj;
+    r.m = (float)mass;
+    r.idx = index;
+    r.addr = address;
+    c.n_stored = std::max(c.n_stored, address + 1);
+    return G6_OK;
+}
+
+int g6x_set_j_particles_dev(int clusterid, int addr0, int n, const int *d_index, const double *d_tj,
+                            const double *d_mass, const double *d_jerk, const double *d_acc,
+                            const double *d_v, const double *d_x)
+{
+    GET_CLUSTER(clusterid);
+    if (n < 1) return fail(c, G6_ERR_ARG, "n = %d", n);
+    if (addr0 < 0 || (long long)addr0 + n > c.capacity)
+        return fail(c, G6_ERR_ADDRESS, "addresses [%d, %lld) outside capacity %d", addr0, (long long)addr0 + n, c.capacity);
+    if (!d_index || !d_tj || !d_mass || !d_jerk || !d_acc || !d_v || !d_x) return fail(c, G6_ERR_ARG, "NULL device array");
+    int rc = flush_j(c);   // keep program order with earlier g6_set_j_particle calls
+    if (rc) return rc;
+    k_store_from_f64<<<(n + 255) / 256, 256, 0, c.stream>>>(c.js, addr0, n, d_index, d_tj, d_mass, d_jerk, d_acc, d_v, d_x);
+    CK(cudaGetLastError());
+    c.n_stored = std::max(c.n_stored, addr0 + n);
+    c.pred_valid = false;
+    return G6_OK;
+}
+
+int g6x_set_j_particles(int clusterid, int addr0, int n, const int index[], const double tj[],
+                        const double mass[], const double jerk[][3], const double acc[][3],
+                        const double v[][3], const double x[][3])
+{
+    GET_CLUSTER(clusterid);
+    if (n < 1) return fail(c, G6_ERR_ARG, "n = %d", n);
+    if (addr0 < 0 || (long long)addr0 + n > c.capacity)
+        return fail(c, G6_ERR_ADDRESS, "addresses [%d, %lld) outside capacity %d", addr0, (long long)addr0 + n, c.capacity);
+    if (!index || !tj || !mass || !jerk || !acc || !v || !x) return fail(c, G6_ERR_ARG, "NULL array");
+    // staging layout: x v acc jerk [n][3] f64, tj mass [n] f64, index [n] i32
+    const size_t n3 = 3 * (size_t)n * sizeof(double), n1 = (size_t)n * sizeof(double);
+    const size_t bytes = 4 * n3 + 2 * n1 + (size_t)n * sizeof(int);
+    int rc = ensure_bulk(c, bytes);
+    if (rc) return rc;
+    CK(cudaStreamSynchronize(c.stream));   // previous bulk upload must have left the pinned buffer
+    char *h = (char *)c.h_bulk, *d = (char *)c.d_bulk;
+    memcpy(h, x, n3); memcpy(h + n3, v, n3); memcpy(h + 2 * n3, acc, n3); memcpy(h + 3 * n3, jerk, n3);
+    memcpy(h + 4 * n3, tj, n1); memcpy(h + 4 * n3 + n1, mass, n1); memcpy(h + 4 * n3 + 2 * n1, index, (size_t)n * sizeof(int));
+    CK(cudaMemcpyAsync(d, h, bytes, cudaMemcpyHostToDevice, c.stream));
+    return g6x_set_j_particles_dev(clusterid, addr0, n, (const int *)(d + 4 * n3 + 2 * n1), (const double *)(d + 4 * n3),
+                                   (const double *)(d + 4 * n3 + n1), (const double *)(d + 3 * n3),
+                                   (const double *)(d + 2 * n3), (const double *)(d + n3), (const double *)d);
+}
+
+int g6_set_ti(int clusterid, double ti)
+{
+    GET_CLUSTER(clusterid);
+    c.ti = ti;
+    return G6_OK;
+}
+
+int g6x_calc_dev(int clusterid, int nj, int ni, const int *d_index, const double *d_xi, const double *d_vi,
+                 double eps2, double *d_acc, double *d_jerk, double *d_pot, int *d_nn_index, double *d_nn_r2)
+{
+    GET_CLUSTER(clusterid);
+    if (c.pending) return fail(c, G6_ERR_SEQUENCE, "g6x_calc_dev between firsthalf and lasthalf");
+    int rc = flush_j(c);
+    if (rc) return rc;
+    rc = check_force_args(c, nj, ni);
+    if (rc) return rc;
+    if (!d_index || !d_xi || !d_vi || !d_acc || !d_jerk || !d_pot) return fail(c, G6_ERR_ARG, "NULL device array");
+    if (!(eps2 >= 0.0)) return fail(c, G6_ERR_ARG, "eps2 = %g", eps2);
+    const bool tm = c.opt_timers != 0;
+    if (tm) { CK(cudaEventRecord(c.ev[0], c.stream)); CK(cudaEventRecord(c.ev[1], c.stream)); }
+    rc = run_predict(c);
+    if (rc) return rc;
+    if (tm) CK(cudaEventRecord(c.ev[2], c.stream));
+    rc = run_force(c, nj, ni, d_index, d_xi, d_vi, eps2, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2, tm ? c.ev[3] : nullptr);
+    if (rc) return rc;
+    if (tm) { CK(cudaEventRecord(c.ev[4], c.stream)); CK(cudaEventRecord(c.ev[5], c.stream)); }
+    c.ev_valid = tm;
+    return G6_OK;
+}
+
+int g6calc_firsthalf(int clusterid, int nj, int ni, const int index[], const double xi[][3], const double vi[][3],
+                     const double acc_old[][3], const double jerk6_old[][3], const double phi_old[],
+                     double eps2, const double h2[])
+{
+    GET_CLUSTER(clusterid);
+    (void)acc_old; (void)jerk6_old; (void)phi_old; (void)h2;
+    if (c.pending) return fail(c, G6_ERR_SEQUENCE, "g6calc_firsthalf called twice without g6calc_lasthalf");
+    int rc = check_force_args(c, nj, ni);
+    if (rc) return rc;
+    if (!index || !xi || !vi) return fail(c, G6_ERR_ARG, "NULL i-particle array");
+    if (!(eps2 >= 0.0)) return fail(c, G6_ERR_ARG, "eps2 = %g", eps2);
+    rc = ensure_i(c, ni);
+    if (rc) return rc;
+    const bool tm = c.opt_timers != 0;
+    if (tm) CK(cudaEventRecord(c.ev[0], c.stream));
+    // a-3: i-block to pinned staging, then to the device (the only per-step H2D payload)
+    memcpy(c.h_idx, index, sizeof(int) * ni);
+    memcpy(c.h_xi, xi, sizeof(double) * 3 * ni);
+    memcpy(c.h_vi, vi, sizeof(double) * 3 * ni);
+    CK(cudaMemcpyAsync(c.d_idx, c.h_idx, sizeof(int) * ni, cudaMemcpyHostToDevice, c.stream));
+    CK(cudaMemcpyAsync(c.d_xi, c.h_xi, sizeof(double) * 3 * ni, cudaMemcpyHostToDevice, c.stream));
+    CK(cudaMemcpyAsync(c.d_vi, c.h_vi, sizeof(double) * 3 * ni, cudaMemcpyHostToDevice, c.stream));
+    // a-1
+    rc = flush_j(c);
+    if (rc) return rc;
+    if (tm) CK(cudaEventRecord(c.ev[1], c.stream));
+    // a-2
+    rc = run_predict(c);
+    if (rc) return rc;
+    if (tm) CK(cudaEventRecord(c.ev[2], c.stream));
+    // a-4, a-5
+    rc = run_force(c, nj, ni, c.d_idx, c.d_xi, c.d_vi, eps2, c.d_acc, c.d_jerk, c.d_pot, c.d_nnidx, c.d_nnr2,
+                   tm ? c.ev[3] : nullptr);
+    if (rc) return rc;
+    if (tm) CK(cudaEventRecord(c.ev[4], c.stream));
+    // a-6
+    CK(cudaMemcpyAsync(c.h_acc, c.d_acc, sizeof(double) * 3 * ni, cudaMemcpyDeviceToHost, c.stream));
+    CK(cudaMemcpyAsync(c.h_jerk, c.d_jerk, sizeof(double) * 3 * ni, cudaMemcpyDeviceToHost, c.stream));
+    CK(cudaMemcpyAsync(c.h_pot, c.d_pot, sizeof(double) * ni, cudaMemcpyDeviceToHost, c.stream));
+    CK(cudaMemcpyAsync(c.h_nnidx, c.d_nnidx, sizeof(int) * ni, cudaMemcpyDeviceToHost, c.stream));
+    CK(cudaMemcpyAsync(c.h_nnr2, c.d_nnr2, sizeof(double) * ni, cudaMemcpyDeviceToHost, c.stream));
+    CK(cudaEventRecord(c.ev[5], c.stream));
+    c.ev_valid = tm;
+    c.pending = true;
+    c.pend_nj = nj;
+    c.pend_ni = ni;
+    return G6_OK;
+}
+
+int g6calc_lasthalf2(int clusterid, int nj, int ni, const int index[], const double xi[][3], const double vi[][3],
+                     double eps2, const double h2[], double acc[][3], double jerk[][3], double pot[], int nnb_index[])
+{
+    GET_CLUSTER(clusterid);
+    (void)index; (void)xi; (void)vi; (void)eps2; (void)h2;
+    if (!c.pending) return fail(c, G6_ERR_SEQUENCE, "g6calc_lasthalf without g6calc_firsthalf");
+    if (nj != c.pend_nj || ni != c.pend_ni)
+        return fail(c, G6_ERR_ARG, "lasthalf (nj=%d, ni=%d) does not match firsthalf (nj=%d, ni=%d)", nj, ni, c.pend_nj, c.pend_ni);
+    if (!acc || !jerk || !pot) return fail(c, G6_ERR_ARG, "NULL result array");
+    c.pending = false;
+    CK(cudaEventSynchronize(c.ev[5]));
+    memcpy(acc, c.h_acc, sizeof(double) * 3 * ni);
+    memcpy(jerk, c.h_jerk, sizeof(double) * 3 * ni);
+    memcpy(pot, c.h_pot, sizeof(double) * ni);
+    if (nnb_index) memcpy(nnb_index, c.h_nnidx, sizeof(int) * ni);
+    c.have_result = true;
+    c.last_ni = ni;
+    return G6_OK;
+}
+
+int g6calc_lasthalf(int clusterid, int nj, int ni, const int index[], const double xi[][3], const double vi[][3],
+                    double eps2, const double h2[], double acc[][3], double jerk[][3], double pot[])
+{
+    return g6calc_lasthalf2(clusterid, nj, ni, index, xi, vi, eps2, h2, acc, jerk, pot, nullptr);
+}
+
+int g6_read_neighbour_list(int clusterid)
+{
+    GET_CLUSTER(clusterid);
+    if (c.pending || !c.have_result) return fail(c, G6_ERR_SEQUENCE, "no completed force call to read neighbours of");
+    return 0;
+}
+
+int g6_get_neighbour_list(int clusterid, int ipipe, int maxlen, int *n, int list[])
+{
+    GET_CLUSTER(clusterid);
+    if (c.pending || !c.have_result) return fail(c, G6_ERR_SEQUENCE, "no completed force call");
+    if (ipipe < 0 || ipipe >= c.last_ni) return fail(c, G6_ERR_ARG, "ipipe = %d outside [0, %d)", ipipe, c.last_ni);
+    if (!n || !list || maxlen < 1) return fail(c, G6_ERR_ARG, "bad neighbour list buffer");
+    if (c.h_nnidx[ipipe] >= 0) { *n = 1; list[0] = c.h_nnidx[ipipe]; }
+    else *n = 0;
+    return G6_OK;
+}
+
+int g6x_get_nearest(int clusterid, int ni, int nn_index[], double nn_r2[])
+{
+    GET_CLUSTER(clusterid);
+    if (c.pending || !c.have_result) return fail(c, G6_ERR_SEQUENCE, "no completed force call");
+    if (ni != c.last_ni) return fail(c, G6_ERR_ARG, "ni = %d but the last call had %d", ni, c.last_ni);
+    if (nn_index) memcpy(nn_index, c.h_nnidx, sizeof(int) * ni);
+    if (nn_r2) memcpy(nn_r2, c.h_nnr2, sizeof(double) * ni);
+    return G6_OK;
+}
+
+int g6x_set_stream(int clusterid, void *cuda_stream)
+{
+    GET_CLUSTER(clusterid);
+    if (c.pending) return fail(c, G6_ERR_SEQUENCE, "stream change between firsthalf and lasthalf");
+    CK(cudaStreamSynchronize(c.stream));
+    c.stream = cuda_stream ? (cudaStream_t)cuda_stream : c.own_stream;
+    return G6_OK;
+}
+
+int g6x_synchronize(int clusterid)
+{
+    GET_CLUSTER(clusterid);
+    CK(cudaStreamSynchronize(c.stream));
+    return G6_OK;
+}
+
+int g6x_get_timers(int clusterid, double us[8])
+{
+    GET_CLUSTER(clusterid);
+    if (!us) return fail(c, G6_ERR_ARG, "NULL");
+    if (c.pending) return fail(c, G6_ERR_SEQUENCE, "force call still pending");
+    if (!c.ev_valid) return fail(c, G6_ERR_SEQUENCE, "no timed force call (option timers = 0?)");
+    CK(cudaEventSynchronize(c.ev[5]));
+    for (int k = 0; k < 5; ++k) {
+        float ms = 0;
+        CK(cudaEventElapsedTime(&ms, c.ev[k], c.ev[k + 1]));
+        us[k] = 1e3 * ms;
+    }
+    float ms = 0;
+    CK(cudaEventElapsedTime(&ms, c.ev[0], c.ev[5]));
+    us[5] = 1e3 * ms;
+    us[6] = c.last_ctas;
+    us[7] = c.last_S;
+    return G6_OK;
+}
+
+static int *option_slot(Cluster &c, const char *key)
+{
+    if (!key) return nullptr;
+    if (!strcmp(key, "ds")) return &c.opt_ds;
+    if (!strcmp(key, "newton")) return &c.opt_newton;
+    if (!strcmp(key, "jsplit")) return &c.opt_jsplit;
+    if (!strcmp(key, "kernel")) return &c.opt_kernel;
+    if (!strcmp(key, "timers")) return &c.opt_timers;
+    if (!strcmp(key, "variant")) return &c.opt_variant;
+    return nullptr;
+}
+
+int g6x_set_option(int clusterid, const char *key, int value)
+{
+    GET_CLUSTER(clusterid);
+    int *slot = option_slot(c, key);
+    if (!slot) return fail(c, G6_ERR_ARG, "unknown option '%s'", key ? key : "(null)");
+    const bool is_flag = slot == &c.opt_ds || slot == &c.opt_newton || slot == &c.opt_timers;
+    if (value < 0 || (is_flag && value > 1) || (slot == &c.opt_kernel && value > 2) || (slot == &c.opt_jsplit && value > 65535) ||
+        (slot == &c.opt_variant && value != 0 && fast_ctas_per_sm(FastVariant{value / 8, value % 8}) < 1))
+        return fail(c, G6_ERR_ARG, "bad value %d for option '%s'", value, key);
+    *slot = value;
+    return G6_OK;
+}
+
+int g6x_get_option(int clusterid, const char *key, int *value)
+{
+    GET_CLUSTER(clusterid);
+    int *slot = option_slot(c, key);
+    if (!slot || !value) return fail(c, G6_ERR_ARG, "unknown option '%s'", key ? key : "(null)");
+    *value = *slot;
+    return G6_OK;
+}
+
+int g6x_get_predicted(int clusterid, int addr0, int n, double xp[][3], double vp[][3])
+{
+    GET_CLUSTER(clusterid);
+    if (c.pending) return fail(c, G6_ERR_SEQUENCE, "force call pending");
+    int rc = flush_j(c);
+    if (rc) return rc;
+    if (n < 1 || addr0 < 0 || (long long)addr0 + n > c.n_stored)
+        return fail(c, G6_ERR_ADDRESS, "addresses [%d, %lld) outside stored [0, %d)", addr0, (long long)addr0 + n, c.n_stored);
+    if (!xp || !vp) return fail(c, G6_ERR_ARG, "NULL");
+    rc = run_predict(c);
+    if (rc) return rc;
+    const int t0 = addr0 / JT, t1 = (addr0 + n - 1) / JT + 1;
+    std::vector<float> h;
+    try { h.resize((size_t)(t1 - t0) * TILE_FLOATS); } catch (const std::bad_alloc &) { return fail(c, G6_ERR_NOMEM, "host allocation failed"); }
+    CK(cudaMemcpyAsync(h.data(), c.pred + (size_t)t0 * TILE_FLOATS, h.size() * sizeof(float), cudaMemcpyDeviceToHost, c.stream));
+    CK(cudaStreamSynchronize(c.stream));
+    for (int p = 0; p < n; ++p) {
+        const int a = addr0 + p;
+        const float *t = h.data() + (size_t)(a / JT - t0) * TILE_FLOATS + (a % JT);
+        for (int k = 0; k < 3; ++k) {
+            xp[p][k] = (double)t[(F_XH + k) * JT] + (double)t[(F_XL + k) * JT];
+            vp[p][k] = (double)t[(F_V + k) * JT];
+        }
+    }
+    return G6_OK;
+}
+
+int g6x_debug_dx(int clusterid, int n, const int ipipe[], const int jaddr[], float dx[][3])
+{
+    GET_CLUSTER(clusterid);
+    if (c.pending || !c.have_result) return fail(c, G6_ERR_SEQUENCE, "no completed host force call");
+    if (n < 1 || !ipipe || !jaddr || !dx) return fail(c, G6_ERR_ARG, "bad arguments");
+    for (int k = 0; k < n; ++k)
+        if (ipipe[k] < 0 || ipipe[k] >= c.last_ni || jaddr[k] < 0 || jaddr[k] >= c.pred_n)
+            return fail(c, G6_ERR_ARG, "pair %d out of range", k);
+    int *d_ip = nullptr, *d_ja = nullptr;
+    float *d_out = nullptr;
+    int rc = [&]() -> int {
+        CK(dalloc(d_ip, n)); CK(dalloc(d_ja, n)); CK(dalloc(d_out, 3 * (size_t)n));
+        CK(cudaMemcpyAsync(d_ip, ipipe, sizeof(int) * n, cudaMemcpyHostToDevice, c.stream));
+        CK(cudaMemcpyAsync(d_ja, jaddr, sizeof(int) * n, cudaMemcpyHostToDevice, c.stream));
+        k_debug_dx<<<(n + 127) / 128, 128, 0, c.stream>>>(n, d_ip, d_ja, c.d_xi, c.opt_ds, c.pred, d_out);
+        CK(cudaGetLastError());
+        CK(cudaMemcpyAsync(dx, d_out, sizeof(float) * 3 * n, cudaMemcpyDeviceToHost, c.stream));
+        CK(cudaStreamSynchronize(c.stream));
+        return G6_OK;
+    }();
+    dfree(d_ip); dfree(d_ja); dfree(d_out);
+    return rc;
+}
+
+}  // extern "C"

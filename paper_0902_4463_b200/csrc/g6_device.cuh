@@ -1,0 +1,225 @@
+// g6_device.cuh -- device data layout and the small kernels of libg6b200 (sm_100a).
+//
+// Steps of the path:
+//   a-1  k_store_from_f64 / k_scatter_records : keep the j-particle store on the device
+//   a-2  k_predict                            : Eq. 1-2, DS positions
+//   a-4  force kernels (g6_force_ref.cuh, g6_force_fast.cuh)
+//   a-5  k_combine                            : sum the per-split partial forces on the GPU
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace g6 {
+
+// ---- j-particle store (raw Hermite state at t_j), structure of arrays --------------------
+// "Only the position is stored in DP, whereas the rest of the terms are stored in SP".
+// 8*3 + 8 + 4*(3+3+3+1) + 4 = 76 bytes per particle.
+struct JStore {
+    double *x[3];   // position at t_j, fp64
+    double *t;      // t_j
+    float *v[3];    // velocity
+    float *a2[3];   // acc / 2      (GRAPE convention, kept as handed in)
+    float *j6[3];   // jerk / 6
+    float *m;       // mass
+    int *idx;       // caller's particle id
+};
+
+// one j-particle on its way host -> device (g6_set_j_particle staging); 80 bytes
+struct JRecord {
+    double x[3];
+    double t;
+    float v[3], a2[3], j6[3];
+    float m;
+    int idx;
+    int addr;
+};
+
+// ---- predicted j-particles: tiles of JT particles, field-major inside a tile --------------
+// tile k = floats [k*JT*NF, (k+1)*JT*NF): x_hi[JT] y_hi z_hi x_lo y_lo z_lo vx vy vz m.
+// One contiguous 10 KiB block per tile = one TMA bulk copy into shared memory; consecutive
+// lanes reading consecutive j are coalesced; LDS.128 yields four consecutive j of one field.
+constexpr int JT = 256;
+constexpr int NF = 10;
+constexpr int F_XH = 0, F_XL = 3, F_V = 6, F_M = 9;
+constexpr int TILE_FLOATS = JT * NF;
+constexpr int TILE_BYTES = TILE_FLOATS * 4;
+
+// ---- partial results of one j-split, structure of arrays, element [s * stride + i] --------
+struct Partials {
+    double *acc[3];
+    double *jrk[3];
+    double *pot;
+    float *nn_r2;    // unsoftened, +inf when none
+    int *nn_addr;    // j address, -1 when none
+    int stride;
+};
+
+// double -> double-single (reading 12): hi = RN32(x), lo = RN32(x - hi)
+__device__ __forceinline__ void ds_split(double x, float &hi, float &lo)
+{
+    hi = __double2float_rn(x);
+    lo = __double2float_rn(x - (double)hi);
+}
+
+// Eq. 3: dx = (xj_hi - xi_hi) + (xj_lo - xi_lo), three binary32 adds
+__device__ __forceinline__ float ds_dx(float xj_hi, float xj_lo, float xi_hi, float xi_lo)
+{
+    return __fadd_rn(__fsub_rn(xj_hi, xi_hi), __fsub_rn(xj_lo, xi_lo));
+}
+
+__device__ __forceinline__ float rsqrt_approx(float x)
+{
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// ---- a-1: bulk load from fp64 device arrays (physical acc, jerk) --------------------------
+__global__ void __launch_bounds__(256)
+k_store_from_f64(JStore S, int addr0, int n, const int *__restrict__ index, const double *__restrict__ tj,
+                 const double *__restrict__ mass, const double *__restrict__ jerk, const double *__restrict__ acc,
+                 const double *__restrict__ v, const double *__restrict__ x)
+{
+    int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    int a = addr0 + p;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        S.x[k][a] = x[3 * (size_t)p + k];
+        S.v[k][a] = (float)v[3 * (size_t)p + k];
+        S.a2[k][a] = (float)(acc[3 * (size_t)p + k] * 0.5);
+        S.j6[k][a] = (float)(jerk[3 * (size_t)p + k] / 6.0);
+    }
+    S.t[a] = tj[p];
+    S.m[a] = (float)mass[p];
+    S.idx[a] = index[p];
+}
+
+// ---- a-1: scatter of the particles changed since the last force call -----------------------
+__global__ void __launch_bounds__(256)
+k_scatter_records(JStore S, const JRecord *__restrict__ rec, int n)
+{
+    int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    JRecord r = rec[p];
+    int a = r.addr;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        S.x[k][a] = r.x[k];
+        S.v[k][a] = r.v[k];
+        S.a2[k][a] = r.a2[k];
+        S.j6[k][a] = r.j6[k];
+    }
+    S.t[a] = r.t;
+    S.m[a] = r.m;
+    S.idx[a] = r.idx;
+}
+
+// ---- a-2: predictor, one thread per j, one CTA per tile ------------------------------------
+// Eq. 1-2 with dt = t_i - t_j (reading 3).  "the multiplications and
+// divisions can be carried out in SP, but the summation should be carried out in DP"
+// (PAPER.md:66): the Taylor increment is formed in FP32 (Horner), added to the fp64 x0 and the
+// sum is re-split into a double-single pair (reading 11).  The kernel is HBM-bound
+// (76 B read + 40 B written per particle); it also records the index range of every tile,
+// which lets the force kernel skip per-pair self checks on tiles that cannot hold the i-particle.
+__global__ void __launch_bounds__(JT)
+k_predict(JStore S, int n_stored, double ti, int ds, float *__restrict__ pred,
+          int *__restrict__ tile_imin, int *__restrict__ tile_imax)
+{
+    const int tile = blockIdx.x;
+    const int l = threadIdx.x;
+    const int j = tile * JT + l;
+    float f[NF];
+    int id_lo = INT32_MAX, id_hi = INT32_MIN;
+    if (j < n_stored) {
+        const float dt = (float)(ti - S.t[j]);
+        const float dt3 = 3.0f * dt;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const float v0 = S.v[k][j], a2 = S.a2[k][j], j6 = S.j6[k][j];
+            // dx = dt (v0 + dt (a0/2 + dt j0/6))
+            const float d = __fmul_rn(dt, __fmaf_rn(dt, __fmaf_rn(dt, j6, a2), v0));
+            const double xp = S.x[k][j] + (double)d;
+            float hi, lo;
+            ds_split(xp, hi, lo);
+            f[F_XH + k] = hi;
+            f[F_XL + k] = ds ? lo : 0.0f;
+            // v_p = v0 + dt (a0 + dt j0/2) = v0 + dt (2 (a0/2) + 3 dt (j0/6))
+            f[F_V + k] = __fmaf_rn(dt, __fmaf_rn(dt3, j6, __fadd_rn(a2, a2)), v0);
+        }
+        f[F_M] = S.m[j];
+        id_lo = id_hi = S.idx[j];
+    } else {
+#pragma unroll
+        for (int k = 0; k < NF; ++k) f[k] = 0.0f;      // padding of the last tile: finite, massless
+    }
+    float *out = pred + (size_t)tile * TILE_FLOATS + l;
+#pragma unroll
+    for (int k = 0; k < NF; ++k) out[k * JT] = f[k];
+
+    // index range of the tile
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        id_lo = min(id_lo, __shfl_xor_sync(0xffffffffu, id_lo, o));
+        id_hi = max(id_hi, __shfl_xor_sync(0xffffffffu, id_hi, o));
+    }
+    __shared__ int s_lo[JT / 32], s_hi[JT / 32];
+    if ((l & 31) == 0) { s_lo[l >> 5] = id_lo; s_hi[l >> 5] = id_hi; }
+    __syncthreads();
+    if (l == 0) {
+#pragma unroll
+        for (int w = 1; w < JT / 32; ++w) { id_lo = min(id_lo, s_lo[w]); id_hi = max(id_hi, s_hi[w]); }
+        tile_imin[tile] = id_lo;
+        tile_imax[tile] = id_hi;
+    }
+}
+
+// ---- a-5: combine the S partial results of every i (fixed order => bit-reproducible) --------
+// "reduce the partial forces directly in the GPU memory and only copy back the final result"
+// (PAPER.md:106).  Sums in fp64 in split order; nearest neighbour: smallest r2, ties -> lowest
+// split = lowest j address (reading 7); address -> caller's index.
+__global__ void __launch_bounds__(256)
+k_combine(Partials P, int S, int ni, const int *__restrict__ jidx,
+          double *__restrict__ acc, double *__restrict__ jerk, double *__restrict__ pot,
+          int *__restrict__ nn_index, double *__restrict__ nn_r2)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= ni) return;
+    double a[3] = {0, 0, 0}, jk[3] = {0, 0, 0}, ph = 0;
+    float best = __int_as_float(0x7f800000);
+    int baddr = -1;
+    for (int s = 0; s < S; ++s) {
+        size_t o = (size_t)s * P.stride + i;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { a[k] += P.acc[k][o]; jk[k] += P.jrk[k][o]; }
+        ph += P.pot[o];
+        float r2 = P.nn_r2[o];
+        int ad = P.nn_addr[o];
+        if (ad >= 0 && r2 < best) { best = r2; baddr = ad; }
+    }
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { acc[3 * (size_t)i + k] = a[k]; jerk[3 * (size_t)i + k] = jk[k]; }
+    pot[i] = ph;
+    if (nn_index) nn_index[i] = baddr >= 0 ? jidx[baddr] : -1;
+    if (nn_r2) nn_r2[i] = baddr >= 0 ? (double)best : (double)__int_as_float(0x7f800000);
+}
+
+// ---- debug: the kernel's Eq.-3 separation for chosen (i, j) pairs (DESIGN.md pin P11) -------
+__global__ void k_debug_dx(int n, const int *__restrict__ ipipe, const int *__restrict__ jaddr,
+                           const double *__restrict__ xi, int ds, const float *__restrict__ pred,
+                           float *__restrict__ out)
+{
+    int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    int i = ipipe[p], j = jaddr[p];
+    const float *t = pred + (size_t)(j / JT) * TILE_FLOATS + (j % JT);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        float hi, lo;
+        ds_split(xi[3 * (size_t)i + k], hi, lo);
+        if (!ds) lo = 0.0f;
+        out[3 * (size_t)p + k] = ds_dx(t[(F_XH + k) * JT], t[(F_XL + k) * JT], hi, lo);
+    }
+}
+
+}  // namespace g6

@@ -1,0 +1,446 @@
+// g6_force_fast.cuh -- the production force kernel for sm_100a (step a-4 of the path).
+//
+// What it computes is what k_force_ref computes (section 2.3, Eq. 3); how differs from the
+// paper's G80 kernel because the B200 bound is the FP32 issue slot, not shared
+// memory latency:
+//
+//  * i-particles live in registers, IT per thread ("one i-particle per thread",
+//    generalised).  Every FP32 operation of a pair is issued as a PACKED two-wide instruction
+//    (FADD2 / FMUL2 / FFMA2, new in sm_100) over TWO CONSECUTIVE j-particles: the i operand is
+//    duplicated once outside the loop, the j operands arrive already paired from shared memory
+//    (LDS.128 = four consecutive j of one field).  One issue slot then carries two pairs' worth
+//    of FMA-pipe work, which leaves slots for the MUFU.RSQ, the nearest-neighbour FMNMX3 and the
+//    shared-memory loads.  IEEE round-to-nearest per lane, so Eq. 3 stays bit-exact.
+//  * j-tiles (JT particles, 10 KiB, field-major) are staged global -> shared by ONE 1-D TMA bulk
+//    copy each (cp.async.bulk ... mbarrier::complete_tx::bytes) into a ring of NSTAGE buffers
+//    guarded by full/empty mbarriers; consumer warps drift by up to NSTAGE-2 tiles, no
+//    __syncthreads in the loop.  (PAPER.md:102 loads one j per thread and synchronises.)
+//  * self-exclusion is hoisted to tile level: the predictor recorded [min,max] of the j indices of
+//    every tile, and a warp takes the checked path (per-pair index compare, address < nj) only on
+//    tiles whose index range contains one of its i-particles, or on the ragged last tile.
+//    All other tiles run without any per-pair test (needs eps2 > 0 so that s2 > 0).
+//  * nearest neighbour: the loop keeps only min r2 (one FMNMX3 per two pairs) and the tile in
+//    which it last improved; the j address is recovered afterwards by re-scanning that one tile
+//    with the same arithmetic (first j that reproduces the minimum: ties -> smallest address).
+//  * FP32 partial sums run over one tile (two chains of JT/2 terms per component, even and odd j)
+//    and are folded into fp64 accumulators per tile (reading 9).
+//  * the grid is (i-tiles) x (S j-splits); S is chosen by the host scheduler so that the SMs are
+//    full at any n_i (PAPER.md:82, :104 generalised); partials go to k_combine.
+#pragma once
+#include "g6_force_ref.cuh"
+
+namespace g6 {
+
+// ---------------------------------------------------------------- PTX helpers (mbarrier + TMA)
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+// bounded wait: a protocol error traps (the launch fails) instead of hanging the device
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    uint32_t spins = 0;
+    while (!mbar_try_wait(bar, parity)) {
+        if (++spins > (1u << 24)) __trap();
+    }
+}
+// 1-D TMA bulk copy global -> shared, completion signalled on an mbarrier (bytes % 16 == 0)
+__device__ __forceinline__ void tma_load_1d(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// ---------------------------------------------------------------- packed FP32 helpers
+__device__ __forceinline__ float2 dup(float a) { return make_float2(a, a); }
+__device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 mul2(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+
+// per-i-particle register state
+struct IPart {
+    float2 nxh[3], nxl[3], nv[3];   // NEGATED hi/lo position words and velocity, duplicated
+    float2 a[3], j[3], p;           // FP32 tile accumulators: .x even j, .y odd j
+    float rmin;                     // min unsoftened r2 so far (over this CTA's j-range)
+};
+
+// One i-particle against two consecutive j-particles (packed lanes).  34 FMA-pipe packed
+// instructions (+4 with the Newton step), 2 MUFU, 1 FMNMX3.  MASKED: m and r2 already masked.
+template <bool NEWTON>
+__device__ __forceinline__ void pair2(IPart &I, const float2 xh, const float2 yh, const float2 zh, const float2 xl,
+                                      const float2 yl, const float2 zl, const float2 vx, const float2 vy, const float2 vz,
+                                      const float2 m, const float2 eps2, float2 &r2_out)
+{
+    // Eq. 3: dx = (xj_hi - xi_hi) + (xj_lo - xi_lo)
+    const float2 dx = add2(add2(xh, I.nxh[0]), add2(xl, I.nxl[0]));
+    const float2 dy = add2(add2(yh, I.nxh[1]), add2(yl, I.nxl[1]));
+    const float2 dz = add2(add2(zh, I.nxh[2]), add2(zl, I.nxl[2]));
+    const float2 dvx = add2(vx, I.nv[0]);
+    const float2 dvy = add2(vy, I.nv[1]);
+    const float2 dvz = add2(vz, I.nv[2]);
+    const float2 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+    const float2 s2 = add2(r2, eps2);
+    float2 rinv = make_float2(rsqrt_approx(s2.x), rsqrt_approx(s2.y));
+    if (NEWTON) {
+        // y <- y - (y/2)(s2 y^2 - 1)
+        const float2 e = fma2(s2, mul2(rinv, rinv), dup(-1.0f));
+        rinv = fma2(mul2(dup(-0.5f), rinv), e, rinv);
+    }
+    const float2 rinv2 = mul2(rinv, rinv);
+    const float2 mrinv = mul2(m, rinv);
+    const float2 mrinv3 = mul2(mrinv, rinv2);
+    const float2 rv = fma2(dz, dvz, fma2(dy, dvy, mul2(dx, dvx)));
+    const float2 alpha = mul2(dup(-3.0f), mul2(rv, rinv2));
+    I.p = add2(I.p, mrinv);                       // +m/s; the sign is applied at the flush
+    I.a[0] = fma2(mrinv3, dx, I.a[0]);
+    I.a[1] = fma2(mrinv3, dy, I.a[1]);
+    I.a[2] = fma2(mrinv3, dz, I.a[2]);
+    I.j[0] = fma2(mrinv3, fma2(alpha, dx, dvx), I.j[0]);
+    I.j[1] = fma2(mrinv3, fma2(alpha, dy, dvy), I.j[1]);
+    I.j[2] = fma2(mrinv3, fma2(alpha, dz, dvz), I.j[2]);
+    r2_out = r2;
+}
+
+constexpr int FAST_NSTAGE = 4;
+
+template <int THREADS, int IT>
+struct FastSmem {
+    alignas(128) float tile[FAST_NSTAGE][TILE_FLOATS];
+    alignas(8) uint64_t full[FAST_NSTAGE];
+    alignas(8) uint64_t empty[FAST_NSTAGE];
+};
+
+template <int THREADS, int IT, bool NEWTON>
+__global__ void __launch_bounds__(THREADS)
+k_force_fast(ForceArgs A)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    FastSmem<THREADS, IT> &sm = *reinterpret_cast<FastSmem<THREADS, IT> *>(smem_raw);
+    constexpr int NWARP = THREADS / 32;
+    constexpr float INF = __builtin_huge_valf();
+
+    const int tid = threadIdx.x;
+    const int s = blockIdx.y;
+    const int t0 = (int)(((long long)A.ntiles * s) / A.S);
+    const int t1 = (int)(((long long)A.ntiles * (s + 1)) / A.S);
+    const int nt = t1 - t0;
+
+    if (tid == 0) {
+#pragma unroll
+        for (int k = 0; k < FAST_NSTAGE; ++k) { mbar_init(&sm.full[k], 1); mbar_init(&sm.empty[k], NWARP); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    // prologue: prefetch distance PD = NSTAGE-2 tiles (one tile of slack between warps, see below)
+    constexpr int PD = FAST_NSTAGE - 2;
+    if (tid == 0) {
+#pragma unroll
+        for (int k = 0; k < PD; ++k)
+            if (k < nt) {
+                mbar_expect_tx(&sm.full[k], TILE_BYTES);
+                tma_load_1d(sm.tile[k], A.pred + (size_t)(t0 + k) * TILE_FLOATS, TILE_BYTES, &sm.full[k]);
+            }
+    }
+
+    // ---- my IT i-particles -> registers (fp64 -> double-single / FP32, negated and duplicated)
+    IPart I[IT];
+    int my[IT];
+    double acc[IT][3], jrk[IT][3], pot[IT];
+    int btile[IT];
+#pragma unroll
+    for (int q = 0; q < IT; ++q) {
+        const int i = (blockIdx.x * IT + q) * THREADS + tid;
+        my[q] = i < A.ni ? A.i_index[i] : -1;
+        btile[q] = -1;
+        pot[q] = 0;
+        I[q].rmin = INF;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            float hi = 0.0f, lo = 0.0f, vv = 0.0f;
+            if (i < A.ni) {
+                ds_split(A.xi[3 * (size_t)i + k], hi, lo);
+                if (!A.ds) lo = 0.0f;
+                vv = (float)A.vi[3 * (size_t)i + k];
+            }
+            I[q].nxh[k] = dup(-hi);
+            I[q].nxl[k] = dup(-lo);
+            I[q].nv[k] = dup(-vv);
+            acc[q][k] = 0;
+            jrk[q][k] = 0;
+        }
+    }
+    const float2 eps2 = dup(A.eps2);
+
+    for (int it = 0; it < nt; ++it) {
+        const int t = t0 + it;
+        const int st = it % FAST_NSTAGE;
+        const uint32_t ph = (uint32_t)(it / FAST_NSTAGE) & 1u;
+
+        // producer: tile it+PD goes into the stage tile it-2 occupied; every warp must have released
+        // that one, so this thread never waits on a warp that is less than a tile behind it
+        if (tid == 0) {
+            const int nx = it + PD;
+            if (nx < nt) {
+                const int sx = nx % FAST_NSTAGE;
+                if (it >= 2) mbar_wait(&sm.empty[sx], (uint32_t)((it - 2) / FAST_NSTAGE) & 1u);
+                mbar_expect_tx(&sm.full[sx], TILE_BYTES);
+                tma_load_1d(sm.tile[sx], A.pred + (size_t)(t0 + nx) * TILE_FLOATS, TILE_BYTES, &sm.full[sx]);
+            }
+        }
+        // does this warp need the checked path on this tile?
+        const int imin = __ldg(A.tile_imin + t), imax = __ldg(A.tile_imax + t);
+        bool hit = false;
+#pragma unroll
+        for (int q = 0; q < IT; ++q) hit |= (my[q] >= imin) & (my[q] <= imax);
+        const bool checked = __any_sync(0xffffffffu, hit) || (t * JT + JT > A.nj);
+
+        mbar_wait(&sm.full[st], ph);
+        const float4 *T = reinterpret_cast<const float4 *>(sm.tile[st]);
+
+#pragma unroll
+        for (int q = 0; q < IT; ++q) {
+#pragma unroll
+            for (int k = 0; k < 3; ++k) { I[q].a[k] = dup(0.0f); I[q].j[k] = dup(0.0f); }
+            I[q].p = dup(0.0f);
+        }
+        float rmin0[IT];
+#pragma unroll
+        for (int q = 0; q < IT; ++q) rmin0[q] = I[q].rmin;
+
+        if (!checked) {
+#pragma unroll 2
+            for (int l4 = 0; l4 < JT / 4; ++l4) {
+                float4 f[NF];
+#pragma unroll
+                for (int k = 0; k < NF; ++k) f[k] = T[k * (JT / 4) + l4];
+#pragma unroll
+                for (int q = 0; q < IT; ++q) {
+                    float2 ra, rb;
+                    pair2<NEWTON>(I[q], make_float2(f[0].x, f[0].y), make_float2(f[1].x, f[1].y), make_float2(f[2].x, f[2].y),
+                                  make_float2(f[3].x, f[3].y), make_float2(f[4].x, f[4].y), make_float2(f[5].x, f[5].y),
+                                  make_float2(f[6].x, f[6].y), make_float2(f[7].x, f[7].y), make_float2(f[8].x, f[8].y),
+                                  make_float2(f[9].x, f[9].y), eps2, ra);
+                    pair2<NEWTON>(I[q], make_float2(f[0].z, f[0].w), make_float2(f[1].z, f[1].w), make_float2(f[2].z, f[2].w),
+                                  make_float2(f[3].z, f[3].w), make_float2(f[4].z, f[4].w), make_float2(f[5].z, f[5].w),
+                                  make_float2(f[6].z, f[6].w), make_float2(f[7].z, f[7].w), make_float2(f[8].z, f[8].w),
+                                  make_float2(f[9].z, f[9].w), eps2, rb);
+                    I[q].rmin = fminf(fminf(ra.x, ra.y), I[q].rmin);
+                    I[q].rmin = fminf(fminf(rb.x, rb.y), I[q].rmin);
+                }
+            }
+        } else {
+            // checked tile: mask out j >= nj and index_j == index_i (mass -> 0, r2 -> +inf)
+            const int4 *JX = reinterpret_cast<const int4 *>(A.jidx + (size_t)t * JT);
+            for (int l4 = 0; l4 < JT / 4; ++l4) {
+                float4 f[NF];
+#pragma unroll
+                for (int k = 0; k < NF; ++k) f[k] = T[k * (JT / 4) + l4];
+                const int j0 = t * JT + 4 * l4;
+                int4 jx = make_int4(0, 0, 0, 0);
+                if (j0 + 3 < A.nj) jx = __ldg(JX + l4);
+                else {
+                    if (j0 + 0 < A.nj) jx.x = __ldg(A.jidx + j0 + 0);
+                    if (j0 + 1 < A.nj) jx.y = __ldg(A.jidx + j0 + 1);
+                    if (j0 + 2 < A.nj) jx.z = __ldg(A.jidx + j0 + 2);
+                }
+#pragma unroll
+                for (int q = 0; q < IT; ++q) {
+                    const bool o0 = (j0 + 0 < A.nj) && (jx.x != my[q]);
+                    const bool o1 = (j0 + 1 < A.nj) && (jx.y != my[q]);
+                    const bool o2 = (j0 + 2 < A.nj) && (jx.z != my[q]);
+                    const bool o3 = (j0 + 3 < A.nj) && (jx.w != my[q]);
+                    float2 ra, rb;
+                    pair2<NEWTON>(I[q], make_float2(f[0].x, f[0].y), make_float2(f[1].x, f[1].y), make_float2(f[2].x, f[2].y),
+                                  make_float2(f[3].x, f[3].y), make_float2(f[4].x, f[4].y), make_float2(f[5].x, f[5].y),
+                                  make_float2(f[6].x, f[6].y), make_float2(f[7].x, f[7].y), make_float2(f[8].x, f[8].y),
+                                  make_float2(o0 ? f[9].x : 0.0f, o1 ? f[9].y : 0.0f), eps2, ra);
+                    pair2<NEWTON>(I[q], make_float2(f[0].z, f[0].w), make_float2(f[1].z, f[1].w), make_float2(f[2].z, f[2].w),
+                                  make_float2(f[3].z, f[3].w), make_float2(f[4].z, f[4].w), make_float2(f[5].z, f[5].w),
+                                  make_float2(f[6].z, f[6].w), make_float2(f[7].z, f[7].w), make_float2(f[8].z, f[8].w),
+                                  make_float2(o2 ? f[9].z : 0.0f, o3 ? f[9].w : 0.0f), eps2, rb);
+                    I[q].rmin = fminf(fminf(o0 ? ra.x : INF, o1 ? ra.y : INF), I[q].rmin);
+                    I[q].rmin = fminf(fminf(o2 ? rb.x : INF, o3 ? rb.y : INF), I[q].rmin);
+                }
+            }
+        }
+        // release the stage (one arrival per warp)
+        __syncwarp();
+        if ((tid & 31) == 0) mbar_arrive(&sm.empty[st]);
+
+        // fold the tile's FP32 sums into fp64; remember the tile if the minimum improved
+#pragma unroll
+        for (int q = 0; q < IT; ++q) {
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                acc[q][k] += (double)I[q].a[k].x + (double)I[q].a[k].y;
+                jrk[q][k] += (double)I[q].j[k].x + (double)I[q].j[k].y;
+            }
+            pot[q] -= (double)I[q].p.x + (double)I[q].p.y;
+            if (I[q].rmin < rmin0[q]) btile[q] = t;
+        }
+    }
+
+    // ---- recover the nearest neighbour's address: re-scan the one tile that set the minimum
+#pragma unroll
+    for (int q = 0; q < IT; ++q) {
+        const int i = (blockIdx.x * IT + q) * THREADS + tid;
+        if (i >= A.ni) continue;
+        int baddr = -1;
+        if (btile[q] >= 0) {
+            const int t = btile[q];
+            const float *g = A.pred + (size_t)t * TILE_FLOATS;
+            const float nxh0 = I[q].nxh[0].x, nxh1 = I[q].nxh[1].x, nxh2 = I[q].nxh[2].x;
+            const float nxl0 = I[q].nxl[0].x, nxl1 = I[q].nxl[1].x, nxl2 = I[q].nxl[2].x;
+            for (int l = 0; l < JT && baddr < 0; ++l) {
+                const int ja = t * JT + l;
+                if (ja >= A.nj) break;
+                const float dx = __fadd_rn(__fadd_rn(g[(F_XH + 0) * JT + l], nxh0), __fadd_rn(g[(F_XL + 0) * JT + l], nxl0));
+                const float dy = __fadd_rn(__fadd_rn(g[(F_XH + 1) * JT + l], nxh1), __fadd_rn(g[(F_XL + 1) * JT + l], nxl1));
+                const float dz = __fadd_rn(__fadd_rn(g[(F_XH + 2) * JT + l], nxh2), __fadd_rn(g[(F_XL + 2) * JT + l], nxl2));
+                const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+                if (r2 == I[q].rmin && A.jidx[ja] != my[q]) baddr = ja;
+            }
+        }
+        const size_t o = (size_t)s * A.P.stride + i;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { A.P.acc[k][o] = acc[q][k]; A.P.jrk[k][o] = jrk[q][k]; }
+        A.P.pot[o] = pot[q];
+        A.P.nn_r2[o] = baddr >= 0 ? I[q].rmin : INF;
+        A.P.nn_addr[o] = baddr;
+    }
+}
+
+// ---------------------------------------------------------------- host side: variants + launch
+struct FastVariant { int threads, it; };
+
+inline bool fast_available() { return true; }
+
+template <int THREADS, int IT>
+inline int fast_attr()
+{
+    const int bytes = (int)sizeof(FastSmem<THREADS, IT>);
+    cudaError_t e = cudaFuncSetAttribute(k_force_fast<THREADS, IT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e != cudaSuccess) return (int)e;
+    e = cudaFuncSetAttribute(k_force_fast<THREADS, IT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    return (int)e;
+}
+
+inline int fast_kernel_init()
+{
+    int r;
+    if ((r = fast_attr<128, 2>())) return r;
+    if ((r = fast_attr<128, 1>())) return r;
+    if ((r = fast_attr<64, 1>())) return r;
+    if ((r = fast_attr<32, 1>())) return r;
+    if ((r = fast_attr<256, 1>())) return r;
+    if ((r = fast_attr<256, 2>())) return r;
+    if ((r = fast_attr<128, 4>())) return r;
+    if ((r = fast_attr<64, 2>())) return r;
+    if ((r = fast_attr<64, 4>())) return r;
+    return 0;
+}
+
+// pick the (threads, i-per-thread) shape for a block of ni particles.  `force` (option
+// "variant" = threads * 8 + it) overrides for experiments.
+inline FastVariant fast_pick(int ni, int n_sm, int force)
+{
+    if (force > 0) return FastVariant{force / 8, force % 8};
+    if (ni <= 32) return FastVariant{32, 1};
+    if (ni <= 64) return FastVariant{64, 1};
+    if (ni <= 128 * n_sm) return FastVariant{128, 1};
+    return FastVariant{128, 2};
+}
+
+template <int THREADS, int IT>
+inline int fast_launch_t(const ForceArgs &A, bool newton, int n_itiles, int S, cudaStream_t st)
+{
+    dim3 grid(n_itiles, S);
+    const size_t bytes = sizeof(FastSmem<THREADS, IT>);
+    if (newton) k_force_fast<THREADS, IT, true><<<grid, THREADS, bytes, st>>>(A);
+    else k_force_fast<THREADS, IT, false><<<grid, THREADS, bytes, st>>>(A);
+    return (int)cudaGetLastError();
+}
+
+inline int launch_force_fast(const ForceArgs &A, bool newton, FastVariant v, int n_itiles, int S, cudaStream_t st)
+{
+    const int key = v.threads * 8 + v.it;
+    switch (key) {
+        case 128 * 8 + 2: return fast_launch_t<128, 2>(A, newton, n_itiles, S, st);
+        case 128 * 8 + 1: return fast_launch_t<128, 1>(A, newton, n_itiles, S, st);
+        case 64 * 8 + 1: return fast_launch_t<64, 1>(A, newton, n_itiles, S, st);
+        case 32 * 8 + 1: return fast_launch_t<32, 1>(A, newton, n_itiles, S, st);
+        case 256 * 8 + 1: return fast_launch_t<256, 1>(A, newton, n_itiles, S, st);
+        case 256 * 8 + 2: return fast_launch_t<256, 2>(A, newton, n_itiles, S, st);
+        case 128 * 8 + 4: return fast_launch_t<128, 4>(A, newton, n_itiles, S, st);
+        case 64 * 8 + 2: return fast_launch_t<64, 2>(A, newton, n_itiles, S, st);
+        case 64 * 8 + 4: return fast_launch_t<64, 4>(A, newton, n_itiles, S, st);
+        default: return (int)cudaErrorInvalidValue;
+    }
+}
+
+// resident CTAs per SM of a variant (for the j-split scheduler)
+template <int THREADS, int IT>
+inline int fast_occ_t()
+{
+    int n = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_force_fast<THREADS, IT, true>, THREADS, sizeof(FastSmem<THREADS, IT>)) != cudaSuccess) return 1;
+    return n > 0 ? n : 1;
+}
+inline int fast_ctas_per_sm(FastVariant v)
+{
+    static int cache[9] = {0};
+    const int key = v.threads * 8 + v.it;
+    int slot;
+    switch (key) {
+        case 128 * 8 + 2: slot = 0; break;
+        case 128 * 8 + 1: slot = 1; break;
+        case 64 * 8 + 1: slot = 2; break;
+        case 32 * 8 + 1: slot = 3; break;
+        case 256 * 8 + 1: slot = 4; break;
+        case 256 * 8 + 2: slot = 5; break;
+        case 128 * 8 + 4: slot = 6; break;
+        case 64 * 8 + 2: slot = 7; break;
+        case 64 * 8 + 4: slot = 8; break;
+        default: return 1;
+    }
+    if (!cache[slot]) {
+        switch (slot) {
+            case 0: cache[slot] = fast_occ_t<128, 2>(); break;
+            case 1: cache[slot] = fast_occ_t<128, 1>(); break;
+            case 2: cache[slot] = fast_occ_t<64, 1>(); break;
+            case 3: cache[slot] = fast_occ_t<32, 1>(); break;
+            case 4: cache[slot] = fast_occ_t<256, 1>(); break;
+            case 5: cache[slot] = fast_occ_t<256, 2>(); break;
+            case 6: cache[slot] = fast_occ_t<128, 4>(); break;
+            case 7: cache[slot] = fast_occ_t<64, 2>(); break;
+            case 8: cache[slot] = fast_occ_t<64, 4>(); break;
+        }
+    }
+    return cache[slot];
+}
+
+}  // namespace g6

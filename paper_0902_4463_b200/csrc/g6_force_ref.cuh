@@ -1,0 +1,124 @@
+// g6_force_ref.cuh -- the checked force kernel: every pair is tested (address < nj,
+// index_j != index_i, s2 > 0) and the nearest neighbour is tracked pair by pair.
+// It is the semantic baseline of the CUDA path (option "kernel" = 1), the path for eps2 == 0,
+// and the model the fast kernel's checked tiles follow.  Layout like the paper's kernel
+// (Fig. 2-3): one i-particle per thread, a tile of j-particles staged in
+// shared memory by the whole block and then processed sequentially; the j-range is split over
+// the grid's y dimension and the partial sums go to the combine kernel (:106).
+#pragma once
+#include "g6_device.cuh"
+
+namespace g6 {
+
+struct ForceArgs {
+    const float *pred;        // predicted j tiles
+    const int *jidx;          // caller's index of every j address (JStore.idx)
+    const int *tile_imin;     // per-tile index range (from the predictor)
+    const int *tile_imax;
+    int nj;                   // j addresses [0, nj)
+    int ntiles;               // ceil(nj / JT)
+    const int *i_index;       // i-block: ids, fp64 positions and velocities [ni][3]
+    const double *xi;
+    const double *vi;
+    int ni;
+    float eps2;
+    int ds;                   // 0: pure-FP32 positions (lo words dropped)
+    int S;                    // number of j-splits (gridDim.y)
+    Partials P;
+};
+
+constexpr int REF_THREADS = 128;
+
+template <bool NEWTON>
+__global__ void __launch_bounds__(REF_THREADS)
+k_force_ref(ForceArgs A)
+{
+    __shared__ float sj[TILE_FLOATS];
+    __shared__ int sidx[JT];
+
+    const int tid = threadIdx.x;
+    const int i = blockIdx.x * REF_THREADS + tid;
+    const int s = blockIdx.y;
+    const int t0 = (int)(((long long)A.ntiles * s) / A.S);
+    const int t1 = (int)(((long long)A.ntiles * (s + 1)) / A.S);
+    const bool active = i < A.ni;
+
+    float xh[3], xl[3], vi[3];
+    int my = -1;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { xh[k] = xl[k] = vi[k] = 0.0f; }
+    if (active) {
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            ds_split(A.xi[3 * (size_t)i + k], xh[k], xl[k]);
+            if (!A.ds) xl[k] = 0.0f;
+            vi[k] = (float)A.vi[3 * (size_t)i + k];
+        }
+        my = A.i_index[i];
+    }
+
+    double acc[3] = {0, 0, 0}, jrk[3] = {0, 0, 0}, pot = 0;
+    float best = __int_as_float(0x7f800000);
+    int baddr = -1;
+
+    for (int t = t0; t < t1; ++t) {
+        __syncthreads();
+        const float *g = A.pred + (size_t)t * TILE_FLOATS;
+        for (int k = tid; k < TILE_FLOATS; k += REF_THREADS) sj[k] = g[k];
+        for (int k = tid; k < JT; k += REF_THREADS) {
+            int ja = t * JT + k;
+            sidx[k] = ja < A.nj ? A.jidx[ja] : 0;
+        }
+        __syncthreads();
+
+        float a32[3] = {0, 0, 0}, j32[3] = {0, 0, 0}, p32 = 0;
+        const int jn = min(JT, A.nj - t * JT);
+        for (int l = 0; l < jn; ++l) {
+            const float dx = ds_dx(sj[(F_XH + 0) * JT + l], sj[(F_XL + 0) * JT + l], xh[0], xl[0]);
+            const float dy = ds_dx(sj[(F_XH + 1) * JT + l], sj[(F_XL + 1) * JT + l], xh[1], xl[1]);
+            const float dz = ds_dx(sj[(F_XH + 2) * JT + l], sj[(F_XL + 2) * JT + l], xh[2], xl[2]);
+            const float dvx = __fsub_rn(sj[(F_V + 0) * JT + l], vi[0]);
+            const float dvy = __fsub_rn(sj[(F_V + 1) * JT + l], vi[1]);
+            const float dvz = __fsub_rn(sj[(F_V + 2) * JT + l], vi[2]);
+            const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+            const float s2 = __fadd_rn(r2, A.eps2);
+            const bool ok = (sidx[l] != my) && (s2 > 0.0f);
+            const float s2c = ok ? s2 : 1.0f;
+            float rinv = rsqrt_approx(s2c);
+            if (NEWTON) {
+                // one Newton-Raphson step: y <- y + (y/2) (1 - s2 y^2)
+                const float e = __fmaf_rn(-s2c, __fmul_rn(rinv, rinv), 1.0f);
+                rinv = __fmaf_rn(__fmul_rn(0.5f, rinv), e, rinv);
+            }
+            const float m = ok ? sj[F_M * JT + l] : 0.0f;
+            const float rinv2 = __fmul_rn(rinv, rinv);
+            const float mrinv = __fmul_rn(m, rinv);
+            const float mrinv3 = __fmul_rn(mrinv, rinv2);
+            const float rv = __fmaf_rn(dz, dvz, __fmaf_rn(dy, dvy, __fmul_rn(dx, dvx)));
+            const float alpha = __fmul_rn(-3.0f, __fmul_rn(rv, rinv2));
+            p32 = __fsub_rn(p32, mrinv);
+            a32[0] = __fmaf_rn(mrinv3, dx, a32[0]);
+            a32[1] = __fmaf_rn(mrinv3, dy, a32[1]);
+            a32[2] = __fmaf_rn(mrinv3, dz, a32[2]);
+            j32[0] = __fmaf_rn(mrinv3, __fmaf_rn(alpha, dx, dvx), j32[0]);
+            j32[1] = __fmaf_rn(mrinv3, __fmaf_rn(alpha, dy, dvy), j32[1]);
+            j32[2] = __fmaf_rn(mrinv3, __fmaf_rn(alpha, dz, dvz), j32[2]);
+            if (ok && r2 < best) { best = r2; baddr = t * JT + l; }
+        }
+        // FP32 chains are at most JT pairs long; fold into fp64 (reading 9)
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { acc[k] += (double)a32[k]; jrk[k] += (double)j32[k]; }
+        pot += (double)p32;
+    }
+
+    if (active) {
+        const size_t o = (size_t)s * A.P.stride + i;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { A.P.acc[k][o] = acc[k]; A.P.jrk[k][o] = jrk[k]; }
+        A.P.pot[o] = pot;
+        A.P.nn_r2[o] = best;
+        A.P.nn_addr[o] = baddr;
+    }
+}
+
+}  // namespace g6
