@@ -1,0 +1,338 @@
+#!/usr/bin/env python
+"""bench.py -- BASELINE.json's headline metric on its headline workload.
+
+  metric    interactions/s of the full force sweep (every particle against every particle:
+            acceleration + jerk + potential + nearest neighbour, double-single separations)
+  workload  C4 of BASELINE.json: N = 1 048 576 equal-mass Plummer sphere, eps = 1e-4, synthetic
+            (seeded generator, paper_0902_4463_b200/inputs.py)
+
+One "step" = one pass of the whole hot path over the particle set:
+  a-1 j-store update (all N particles re-sent: in a sweep every particle was "corrected"),
+  a-2 predictor, a-3 i-block, a-4 force kernel, a-5 combine, a-6 results.
+`value`  : inputs (fp64) already resident in HBM, results left in HBM  (g6x_*_dev entry points)
+`e2e`    : the same step through the host entry points (g6x_set_j_particles, g6calc_firsthalf,
+           g6calc_lasthalf2) with HOST buffers; H2D and D2H copies inside the timed region.
+
+Multi-GPU (torchrun, one rank per GPU): the sweep is sharded over the i-particles -- every rank
+holds and predicts all N j-particles and computes the forces on its N/G i-particles; no
+data-path collective (SURVEY.md 8(e) option 2).  Total work is fixed => "scaling": "strong".
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same
+workload on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+WORKLOAD = "C4"
+METRIC = "interactions/s (N=1048576 Plummer full force sweep: acc+jerk+pot+nearest neighbour, DS separations)"
+# algorithmic work of one pairwise interaction
+FP32_INSTR_PER_INTERACTION = 33      # FP32-pipe lane-instructions
+FLOP47 = 47                          # same work counted as flops with FMA = 2
+FLOP_PAPER = 60                      # the paper's convention (PAPER.md:164 fn.9); 66 with DS
+SM_COUNT = 148
+FP32_LANES_PER_SM = 128
+SM_MAX_MHZ_FALLBACK = 1965.0
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)), "measured"
+        except Exception:
+            pass
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": SM_MAX_MHZ_FALLBACK}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled while the timed region runs."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index=0):
+        self.gpu = gpu_index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.gpu}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            f = [s.strip() for s in line.split(",")]
+            if len(f) >= 9:
+                self.rows.append(f)
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, power = [], [], set(), []
+        for f in self.rows:
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2])); power.append(float(f[3]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        busy = [c for c, p in zip(sm, power) if p > 0.5 * max(power)] or sm
+        return {"sm_mhz": float(np.median(busy)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
+                "power_w_max": float(max(power)), "samples": len(sm)}
+
+
+def cpu_oracle_rate(x, v, m, eps2, idx, target_s, seed=7):
+    """interactions/s of the oracle (as it stands) on a bounded sample of rows of the sweep."""
+    from oracle import oracle as orc
+    n = len(m)
+    rng = np.random.default_rng(seed)
+    probe = np.sort(rng.choice(n, 64, replace=False))
+    t0 = time.perf_counter()
+    orc.force(idx[probe], x[probe], v[probe], idx, x, v, m, eps2)
+    dt = time.perf_counter() - t0
+    rows = int(min(n, max(64, 64 * target_s / max(dt, 1e-3))))
+    rows = max(orc.threads(), rows)
+    sel = np.sort(rng.choice(n, rows, replace=False))
+    t0 = time.perf_counter()
+    orc.force(idx[sel], x[sel], v[sel], idx, x, v, m, eps2)
+    dt = time.perf_counter() - t0
+    return rows * float(n) / dt, rows, dt, orc.threads()
+
+
+def run_reference(args):
+    """--impl reference: the oracle, timed on the host cores on a bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import oracle as orc
+    from paper_0902_4463_b200 import inputs
+    orc.build(False)
+    x, v, m, eps2 = inputs.config(WORKLOAD, n=args.n)
+    n = len(m)
+    idx = np.arange(n, dtype=np.int32)
+    rng = np.random.default_rng(11)
+    # size one step to ~args.ref_seconds of CPU work
+    probe = np.sort(rng.choice(n, 64, replace=False))
+    t0 = time.perf_counter(); orc.force(idx[probe], x[probe], v[probe], idx, x, v, m, eps2); dt = time.perf_counter() - t0
+    rows = int(min(n, max(orc.threads(), 64 * args.ref_seconds / max(dt, 1e-3))))
+    times = []
+    for step in range(args.warmup + args.steps):
+        sel = np.sort(rng.choice(n, rows, replace=False))
+        t0 = time.perf_counter()
+        orc.force(idx[sel], x[sel], v[sel], idx, x, v, m, eps2)
+        if step >= args.warmup:
+            times.append(time.perf_counter() - t0)
+    total = sum(times)
+    value = args.steps * rows * float(n) / total
+    sample = f"{rows} randomly chosen i-rows x all {n} j per step (a bounded sample of the sweep), {args.steps} steps"
+    out = {"impl": "reference", "metric": METRIC, "value": value, "unit": "interactions/s", "n_gpus": args.gpus, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True, "scaling": "strong",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": f"{WORKLOAD}: N={n} equal-mass Plummer, eps=1e-4, full sweep (sampled rows)", "n": n},
+           "cpu_baseline": {"value": value, "unit": "interactions/s", "cores": orc.threads(), "kind": "oracle", "sample": sample},
+           "e2e": {"value": value, "unit": "interactions/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gflops_60": value * FLOP_PAPER / 1e9}
+    print(json.dumps(out), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--n", type=int, default=None, help="override N (same seed) for quick checks; the headline is the default")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="CPU work of the cpu_baseline leg")
+    ap.add_argument("--ref-seconds", type=float, default=8.0, help="CPU work per step of --impl reference")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--newton", type=int, default=None, help="override the library default (1 = rsqrt + one Newton step)")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = max(args.warmup, 0)
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_0902_4463_b200 import build, g6, inputs
+    from paper_0902_4463_b200.sharding import i_range
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    os.environ["G6_DEVICE"] = str(local)
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+
+    x, v, m, eps2 = inputs.config(WORKLOAD, n=args.n)
+    n = len(m)
+    idx = np.arange(n, dtype=np.int32)
+    i0, i1 = i_range(rank, world, n)
+    ni = i1 - i0
+
+    g6.g6_open(0)
+    g6.g6x_set_npipes(1 << 21)
+    if args.newton is not None:
+        g6.g6x_set_option(0, "newton", args.newton)
+    newton = g6.g6x_get_option(0, "newton")
+    stream = torch.cuda.Stream(device=dev)             # a real (non-default) stream: handle != 0
+    torch.cuda.set_stream(stream)
+    g6.g6x_set_stream(0, stream.cuda_stream)          # so that torch events bracket the library's kernels
+
+    f64 = torch.float64
+    to = lambda a, dt=f64: torch.from_numpy(np.ascontiguousarray(a)).to(dev, dt)
+    d_x, d_v, d_m, d_idx = to(x), to(v), to(m), to(idx, torch.int32)
+    d_t = torch.zeros(n, dtype=f64, device=dev); d_z3 = torch.zeros(n, 3, dtype=f64, device=dev)
+    d_xi, d_vi, d_ii = d_x[i0:i1].contiguous(), d_v[i0:i1].contiguous(), d_idx[i0:i1].contiguous()
+    d_acc = torch.empty(ni, 3, dtype=f64, device=dev); d_jerk = torch.empty_like(d_acc)
+    d_pot = torch.empty(ni, dtype=f64, device=dev); d_nn = torch.empty(ni, dtype=torch.int32, device=dev); d_r2 = torch.empty_like(d_pot)
+    flush = torch.empty(512 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)      # 512 MiB > 126 MB L2
+
+    def step_dev():
+        g6.g6x_set_j_particles_dev(0, 0, n, d_idx, d_t, d_m, d_z3, d_z3, d_v, d_x)       # a-1
+        g6.g6_set_ti(0, 0.0)
+        g6.g6x_calc_dev(0, n, ni, d_ii, d_xi, d_vi, eps2, d_acc, d_jerk, d_pot, d_nn, d_r2)   # a-2 .. a-5
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        flush.zero_()
+        step_dev()
+    barrier()
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    force_us, pred_us, comb_us = [], [], []
+    barrier()
+    wall0 = time.perf_counter()
+    for k in range(args.steps):
+        flush.zero_()                                     # L2 flush between timed iterations (outside the events)
+        ev[k][0].record(stream)
+        step_dev()
+        ev[k][1].record(stream)
+        torch.cuda.synchronize()
+        tm = g6.g6x_get_timers(0)                         # the library's own CUDA events, same stream
+        force_us.append(tm["force_us"]); pred_us.append(tm["predict_us"]); comb_us.append(tm["combine_us"])
+    barrier()
+    wall = time.perf_counter() - wall0
+    clocks = sampler.stop()
+    ms = sum(a.elapsed_time(b) for a, b in ev)
+    t_ms = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
+    ms_total = float(t_ms.item())
+    value = args.steps * float(n) * float(n) / (ms_total * 1e-3)
+
+    # ---- end to end through the host entry points (rank-local shard, host buffers) ------------------
+    e2e = None
+    if not args.no_e2e:
+        z3 = np.zeros((n, 3)); tz = np.zeros(n)
+        xi_h, vi_h, ii_h = np.ascontiguousarray(x[i0:i1]), np.ascontiguousarray(v[i0:i1]), np.ascontiguousarray(idx[i0:i1])
+
+        def step_host():
+            g6.g6x_set_j_particles(0, 0, idx, tz, m, z3, z3, v, x)
+            g6.g6_set_ti(0, 0.0)
+            g6.g6calc_firsthalf(0, n, ni, ii_h, xi_h, vi_h, eps2=eps2)
+            return g6.g6calc_lasthalf2(0, n, ni, eps2=eps2)
+        step_host()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            flush.zero_()
+            torch.cuda.synchronize()
+            r = step_host()
+        barrier()
+        e2e_s = time.perf_counter() - t0
+        t_e = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t_e, op=dist.ReduceOp.MAX)
+        h2d = (x.nbytes + v.nbytes + 2 * z3.nbytes + tz.nbytes + m.nbytes + idx.nbytes) + (xi_h.nbytes + vi_h.nbytes + ii_h.nbytes)
+        d2h = ni * (3 * 8 + 3 * 8 + 8 + 4 + 8)
+        e2e = {"value": args.steps * float(n) * float(n) / float(t_e.item()), "unit": "interactions/s",
+               "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+               "note": "host arrays in, host arrays out (library stages through its own pinned buffers); includes the L2 flush"}
+
+    if rank == 0:
+        peaks, peaks_src = measured_peaks()
+        sm_max = float(peaks.get("sm_max_mhz", SM_MAX_MHZ_FALLBACK))
+        peak_inst = SM_COUNT * FP32_LANES_PER_SM * sm_max * 1e6                 # FP32 lane-instructions / s
+        f_us = float(np.mean(force_us))
+        inter_per_launch = float(ni) * float(n)
+        ach_inst = FP32_INSTR_PER_INTERACTION * inter_per_launch / (f_us * 1e-6)
+        roofline = {"bound": "alu", "kernel": "k_force_fast",
+                    "achieved": 2 * ach_inst / 1e12, "peak": 2 * peak_inst / 1e12,
+                    "unit": "TFLOP/s", "frac": ach_inst / peak_inst, "traffic": None,
+                    "how": ("FP32-pipe issue-slot equivalent: 33 algorithmic FP32 lane-instructions per interaction (SURVEY 8(d)) x "
+                            "interactions per launch / mean force-kernel time (CUDA events on the launching stream, live in this run); "
+                            f"peak = 148 SM x 128 lanes x {sm_max:.0f} MHz ({peaks_src} max SM clock) x 2"),
+                    "kernel_ms": f_us / 1e3,
+                    "kernel_interactions_per_s": inter_per_launch / (f_us * 1e-6),
+                    "flops47_tflops": FLOP47 * inter_per_launch / (f_us * 1e-6) / 1e12,
+                    "frac_at_measured_clock": (ach_inst / (SM_COUNT * FP32_LANES_PER_SM * clocks["sm_mhz"] * 1e6)) if clocks.get("sm_mhz") else None,
+                    "kernel_share_of_step": f_us * args.steps / (ms_total * 1e3) if world == 1 else None,
+                    "predictor_gbs": (n * (76 + 40)) / (float(np.mean(pred_us)) * 1e-6) / 1e9,
+                    "hbm_peak_gbs": peaks.get("hbm_gbs")}
+        out = {"metric": METRIC, "value": value, "unit": "interactions/s", "n_gpus": world, "steps": args.steps,
+               "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+               "scaling": "strong", "vs_baseline": None, "dtype": "f32 (double-single separations, fp64 accumulation across tiles)",
+               "data": "synthetic",
+               "config": {"workload": f"{WORKLOAD}: N={n} equal-mass Plummer sphere, eps=1e-4, full force sweep n_i=N_j=N",
+                          "n": n, "eps2": eps2, "seed": inputs.CONFIGS[WORKLOAD]["seed"], "newton_step": int(newton),
+                          "parallelism": f"i-split x{world}" if world > 1 else "1 GPU", "l2": "flushed between timed steps (512 MiB write)"},
+               "gflops_60": value * FLOP_PAPER / 1e9, "gflops_66": value * 66 / 1e9,
+               "clocks": clocks, "roofline": roofline, "gpu_launches": 4 * args.steps,
+               "wall_s_timed_region": wall}
+        if e2e:
+            out["e2e"] = e2e
+        if not args.no_cpu_baseline and world == 1:
+            rate, rows, dt, cores = cpu_oracle_rate(x, v, m, eps2, idx, args.cpu_seconds)
+            out["cpu_baseline"] = {"value": rate, "unit": "interactions/s", "cores": cores, "kind": "oracle",
+                                   "sample": f"{rows} randomly chosen i-rows x all {n} j of the same workload, {dt:.1f} s"}
+        print(json.dumps(out), flush=True)
+
+    g6.g6_close(0)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
