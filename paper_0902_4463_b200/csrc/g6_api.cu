@@ -18,6 +18,7 @@
 #include "g6_device.cuh"
 #include "g6_force_ref.cuh"
 #include "g6_force_fast.cuh"
+#include "g6_force_small.cuh"
 
 using namespace g6;
 
@@ -48,20 +49,24 @@ struct Cluster {
     int pred_ds = 1;
     int pred_n = 0;
 
-    // host -> device staging of changed j particles
-    JRecord *h_rec = nullptr;   // pinned
-    JRecord *d_rec = nullptr;
+    // host -> device staging of changed j particles: two pinned+mapped buffers used alternately,
+    // so the host can fill one while the device may still read the other
+    JRecord *h_rec[2] = {nullptr, nullptr};   // pinned, mapped
+    JRecord *hd_rec[2] = {nullptr, nullptr};  // device view of the same memory (zero-copy path)
+    JRecord *d_rec = nullptr;                 // device copy (DMA path)
+    cudaEvent_t ev_rec[2] = {nullptr, nullptr};
+    bool rec_used[2] = {false, false};
+    int rec_cur = 0;
     int rec_cap = 0, n_rec = 0;
-    std::vector<int> slot_of_addr;   // address -> slot in h_rec (or -1)
+    std::vector<int> slot_of_addr;   // address -> slot in h_rec[rec_cur] (or -1)
 
-    // i block + results
+    // i block and results: one pinned+mapped block each, compact layout by ni
+    //   i block : xi[3 ni] f64 | vi[3 ni] f64 | index[ni] i32
+    //   results : acc[3 ni] f64 | jerk[3 ni] f64 | pot[ni] f64 | nn_r2[ni] f64 | nn_index[ni] i32
     int i_cap = 0;
-    int *h_idx = nullptr, *d_idx = nullptr;
-    double *h_xi = nullptr, *h_vi = nullptr, *d_xi = nullptr, *d_vi = nullptr;
-    double *d_acc = nullptr, *d_jerk = nullptr, *d_pot = nullptr, *d_nnr2 = nullptr;
-    int *d_nnidx = nullptr;
-    double *h_acc = nullptr, *h_jerk = nullptr, *h_pot = nullptr, *h_nnr2 = nullptr;
-    int *h_nnidx = nullptr;
+    char *h_iblk = nullptr, *hd_iblk = nullptr, *d_iblk = nullptr;
+    char *h_res = nullptr, *hd_res = nullptr, *d_res = nullptr;
+    bool res_on_host = false;   // last call's results were written straight into h_res
 
     // partial results
     Partials part{};
@@ -79,12 +84,11 @@ struct Cluster {
     int pend_nj = 0, pend_ni = 0;
     int last_ni = 0;
     cudaEvent_t ev[N_EVENTS] = {};
-    cudaEvent_t ev_bulk = nullptr;
     bool ev_valid = false;
     int last_ctas = 0, last_S = 0;
 
     // options
-    int opt_ds = 1, opt_newton = 1, opt_jsplit = 0, opt_kernel = 0, opt_timers = 1, opt_variant = 0;
+    int opt_ds = 1, opt_newton = 1, opt_jsplit = 0, opt_kernel = 0, opt_timers = 1, opt_variant = 0, opt_small = 16;
 };
 
 Cluster g_cl[MAX_CLUSTERS];
@@ -134,12 +138,36 @@ void dfree(T *&p) { if (p) cudaFree(p); p = nullptr; }
 template <class T>
 void hfree(T *&p) { if (p) cudaFreeHost(p); p = nullptr; }
 
+inline size_t iblk_bytes(size_t ni) { return ni * (6 * sizeof(double) + sizeof(int)); }
+inline size_t res_bytes(size_t ni) { return ni * (8 * sizeof(double) + sizeof(int)); }
+
+// views into an i block / result block laid out for `ni` particles
+struct IView { const double *xi, *vi; const int *idx; };
+struct RView { double *acc, *jerk, *pot, *nnr2; int *nnidx; };
+inline IView iview(char *base, size_t ni)
+{
+    const double *d = (const double *)base;
+    return IView{d, d + 3 * ni, (const int *)(d + 6 * ni)};
+}
+inline RView rview(char *base, size_t ni)
+{
+    double *d = (double *)base;
+    return RView{d, d + 3 * ni, d + 6 * ni, d + 7 * ni, (int *)(d + 8 * ni)};
+}
+
+template <class T>
+cudaError_t mapped_alloc(T *&h, T *&hd, size_t bytes)
+{
+    cudaError_t e = cudaHostAlloc((void **)&h, bytes, cudaHostAllocMapped);
+    if (e != cudaSuccess) return e;
+    return cudaHostGetDevicePointer((void **)&hd, (void *)h, 0);
+}
+
 void free_i(Cluster &c)
 {
-    hfree(c.h_idx); hfree(c.h_xi); hfree(c.h_vi);
-    dfree(c.d_idx); dfree(c.d_xi); dfree(c.d_vi);
-    dfree(c.d_acc); dfree(c.d_jerk); dfree(c.d_pot); dfree(c.d_nnr2); dfree(c.d_nnidx);
-    hfree(c.h_acc); hfree(c.h_jerk); hfree(c.h_pot); hfree(c.h_nnr2); hfree(c.h_nnidx);
+    hfree(c.h_iblk); hfree(c.h_res);
+    dfree(c.d_iblk); dfree(c.d_res);
+    c.hd_iblk = c.hd_res = nullptr;
     c.i_cap = 0;
 }
 
@@ -148,14 +176,13 @@ int ensure_i(Cluster &c, int ni)
     if (ni <= c.i_cap) return G6_OK;
     CK(cudaStreamSynchronize(c.stream));
     free_i(c);
-    size_t n = std::max(ni, 256);
-    CK(halloc(c.h_idx, n)); CK(halloc(c.h_xi, 3 * n)); CK(halloc(c.h_vi, 3 * n));
-    CK(dalloc(c.d_idx, n)); CK(dalloc(c.d_xi, 3 * n)); CK(dalloc(c.d_vi, 3 * n));
-    CK(dalloc(c.d_acc, 3 * n)); CK(dalloc(c.d_jerk, 3 * n)); CK(dalloc(c.d_pot, n));
-    CK(dalloc(c.d_nnr2, n)); CK(dalloc(c.d_nnidx, n));
-    CK(halloc(c.h_acc, 3 * n)); CK(halloc(c.h_jerk, 3 * n)); CK(halloc(c.h_pot, n));
-    CK(halloc(c.h_nnr2, n)); CK(halloc(c.h_nnidx, n));
+    size_t n = std::max(ni, 4096);
+    CK(mapped_alloc(c.h_iblk, c.hd_iblk, iblk_bytes(n)));
+    CK(mapped_alloc(c.h_res, c.hd_res, res_bytes(n)));
+    CK(cudaMalloc((void **)&c.d_iblk, iblk_bytes(n)));
+    CK(cudaMalloc((void **)&c.d_res, res_bytes(n)));
     c.i_cap = (int)n;
+    c.have_result = false;
     return G6_OK;
 }
 
@@ -195,15 +222,14 @@ int ensure_bulk(Cluster &c, size_t bytes)
 int ensure_rec(Cluster &c, int n)
 {
     if (n <= c.rec_cap) return G6_OK;
-    int cap = std::max(std::max(n, 2 * c.rec_cap), 4096);
-    JRecord *h = nullptr, *d = nullptr;
-    CK(halloc(h, cap));
+    const int cap = std::max(std::max(n, 2 * c.rec_cap), 4096);
+    CK(cudaStreamSynchronize(c.stream));   // nothing may still read the old buffers
+    JRecord *h[2] = {nullptr, nullptr}, *hd[2] = {nullptr, nullptr}, *d = nullptr;
+    for (int b = 0; b < 2; ++b) CK(mapped_alloc(h[b], hd[b], sizeof(JRecord) * cap));
     CK(dalloc(d, cap));
-    if (c.n_rec) memcpy(h, c.h_rec, sizeof(JRecord) * c.n_rec);
-    CK(cudaStreamSynchronize(c.stream));   // the old device buffer may still be read by a scatter
-    hfree(c.h_rec);
+    if (c.n_rec) memcpy(h[c.rec_cur], c.h_rec[c.rec_cur], sizeof(JRecord) * c.n_rec);
+    for (int b = 0; b < 2; ++b) { hfree(c.h_rec[b]); c.h_rec[b] = h[b]; c.hd_rec[b] = hd[b]; c.rec_used[b] = false; }
     dfree(c.d_rec);
-    c.h_rec = h;
     c.d_rec = d;
     c.rec_cap = cap;
     return G6_OK;
@@ -215,13 +241,13 @@ void release(Cluster &c)
     for (int k = 0; k < 3; ++k) { dfree(c.js.x[k]); dfree(c.js.v[k]); dfree(c.js.a2[k]); dfree(c.js.j6[k]); }
     dfree(c.js.t); dfree(c.js.m); dfree(c.js.idx);
     dfree(c.pred); dfree(c.tile_imin); dfree(c.tile_imax);
-    hfree(c.h_rec); dfree(c.d_rec);
+    for (int b = 0; b < 2; ++b) { hfree(c.h_rec[b]); if (c.ev_rec[b]) cudaEventDestroy(c.ev_rec[b]); }
+    dfree(c.d_rec);
     free_i(c);
     if (c.part_block) cudaFree(c.part_block);
     if (c.h_bulk) cudaFreeHost(c.h_bulk);
     if (c.d_bulk) cudaFree(c.d_bulk);
     for (auto &e : c.ev) if (e) { cudaEventDestroy(e); e = nullptr; }
-    if (c.ev_bulk) cudaEventDestroy(c.ev_bulk);
     if (c.own_stream) cudaStreamDestroy(c.own_stream);
     char keep[sizeof(c.err)];
     memcpy(keep, c.err, sizeof(keep));
@@ -229,26 +255,57 @@ void release(Cluster &c)
     memcpy(c.err, keep, sizeof(keep));
 }
 
-// upload + scatter of the j particles changed since the last force call (step a-1)
-int flush_j(Cluster &c)
+// zero-copy thresholds: below these the kernels read the staging buffers / write the results
+// through mapped pinned memory (no DMA set-up latency); above, one packed copy each way
+constexpr int ZC_MAX_I = 2048;
+constexpr int ZC_MAX_REC = 2048;
+
+// Step a-1 (+ a-3): scatter of the j particles changed since the last force call and, when
+// `with_i`, the i block host staging -> device.  Small batches are read by the kernel straight
+// from mapped pinned memory; large ones are DMA-copied first.
+int stage_inputs(Cluster &c, bool with_i, int ni)
 {
-    if (c.n_rec == 0) return G6_OK;
-    CK(cudaMemcpyAsync(c.d_rec, c.h_rec, sizeof(JRecord) * c.n_rec, cudaMemcpyHostToDevice, c.stream));
-    k_scatter_records<<<(c.n_rec + 255) / 256, 256, 0, c.stream>>>(c.js, c.d_rec, c.n_rec);
-    CK(cudaGetLastError());
-    // the pinned buffer is rewritten by the next g6_set_j_particle: wait for the copy engine
-    CK(cudaEventRecord(c.ev_bulk, c.stream));
-    for (int k = 0; k < c.n_rec; ++k) c.slot_of_addr[c.h_rec[k].addr] = -1;
-    CK(cudaEventSynchronize(c.ev_bulk));
-    c.n_rec = 0;
-    c.pred_valid = false;
+    const int nrec = c.n_rec;
+    const int b = c.rec_cur;
+    const bool zc_rec = nrec <= ZC_MAX_REC;
+    const bool zc_i = with_i && ni <= ZC_MAX_I;
+    if (nrec == 0 && !with_i) return G6_OK;
+    if (nrec > 0 && !zc_rec)
+        CK(cudaMemcpyAsync(c.d_rec, c.h_rec[b], sizeof(JRecord) * nrec, cudaMemcpyHostToDevice, c.stream));
+    if (with_i && !zc_i)
+        CK(cudaMemcpyAsync(c.d_iblk, c.h_iblk, iblk_bytes(ni), cudaMemcpyHostToDevice, c.stream));
+    const int n_i_copy = zc_i ? ni : 0;
+    const int nthreads = std::max(nrec, n_i_copy);
+    if (nthreads > 0) {
+        const IView src = iview(c.hd_iblk, ni), dst = iview(c.d_iblk, ni);
+        k_stage<<<(nthreads + 127) / 128, 128, 0, c.stream>>>(c.js, zc_rec ? c.hd_rec[b] : c.d_rec, nrec, n_i_copy,
+                                                              src.xi, src.vi, src.idx, (double *)dst.xi, (double *)dst.vi, (int *)dst.idx);
+        CK(cudaGetLastError());
+    }
+    if (nrec > 0) {
+        CK(cudaEventRecord(c.ev_rec[b], c.stream));
+        c.rec_used[b] = true;
+        for (int k = 0; k < nrec; ++k) c.slot_of_addr[c.h_rec[b][k].addr] = -1;
+        c.n_rec = 0;
+        c.pred_valid = false;
+        // switch to the other staging buffer; its previous upload (two flushes ago) must be done
+        c.rec_cur = b ^ 1;
+        if (c.rec_used[c.rec_cur]) { CK(cudaEventSynchronize(c.ev_rec[c.rec_cur])); c.rec_used[c.rec_cur] = false; }
+    }
     return G6_OK;
+}
+
+int flush_j(Cluster &c) { return stage_inputs(c, false, 0); }
+
+bool pred_is_current(const Cluster &c)
+{
+    return c.pred_valid && c.pred_ti == c.ti && c.pred_ds == c.opt_ds && c.pred_n == c.n_stored;
 }
 
 // predictor over all stored particles (step a-2); skipped when nothing changed
 int run_predict(Cluster &c)
 {
-    if (c.pred_valid && c.pred_ti == c.ti && c.pred_ds == c.opt_ds && c.pred_n == c.n_stored) return G6_OK;
+    if (pred_is_current(c)) return G6_OK;
     int ntiles = (c.n_stored + JT - 1) / JT;
     if (ntiles > 0) {
         k_predict<<<ntiles, JT, 0, c.stream>>>(c.js, c.n_stored, c.ti, c.opt_ds, c.pred, c.tile_imin, c.tile_imax);
@@ -261,10 +318,32 @@ int run_predict(Cluster &c)
     return G6_OK;
 }
 
+// i/j-split scheduler (PAPER.md:82 "j-particles distributed evenly among the P MPs", :104 generalised):
+// pick the number of j-splits S that minimises  waves(S) x (tiles per CTA + per-CTA overhead),
+// waves(S) = ceil(i-tiles x S / resident CTA slots).  Small blocks get S ~ slots (every SM busy at
+// n_i = 1); big sweeps get the S that makes the last wave full.  Partials are capped at 1 GiB.
+int choose_jsplit(int n_itiles, int ntiles, int slots, int ni)
+{
+    const double OVH = 0.4;        // CTA prologue + epilogue, in tile times
+    const double COMBINE = 0.004;  // per extra split: partial traffic + combine work, in tile times
+    long long smax = std::min<long long>(ntiles, (1LL << 30) / (72LL * std::max(ni, 1)));
+    smax = std::max<long long>(1, std::min<long long>(smax, 2LL * slots / std::max(n_itiles, 1) + 2));
+    int best = 1;
+    double best_cost = 1e300;
+    for (int S = 1; S <= smax; ++S) {
+        const long long ctas = (long long)n_itiles * S;
+        const long long waves = (ctas + slots - 1) / slots;
+        const int per = (ntiles + S - 1) / S;
+        const double cost = waves * (per + OVH) + COMBINE * S;
+        if (cost < best_cost - 1e-9) { best_cost = cost; best = S; }
+    }
+    return best;
+}
+
 // force + combine (steps a-4, a-5) on device-resident i-blocks; all asynchronous
 int run_force(Cluster &c, int nj, int ni, const int *d_index, const double *d_xi, const double *d_vi,
               double eps2, double *d_acc, double *d_jerk, double *d_pot, int *d_nn_index, double *d_nn_r2,
-              cudaEvent_t ev_force_done)
+              cudaEvent_t ev_pred_done, cudaEvent_t ev_force_done)
 {
     ForceArgs A{};
     A.pred = c.pred;
@@ -280,6 +359,42 @@ int run_force(Cluster &c, int nj, int ni, const int *d_index, const double *d_xi
     A.eps2 = (float)eps2;
     A.ds = c.opt_ds;
 
+    // small active blocks: lanes over j, predictor fused in (g6_force_small.cuh)
+    if (ni <= c.opt_small && c.opt_kernel != 1 && c.opt_kernel != 2 && c.opt_jsplit == 0) {
+        SmallArgs B{};
+        B.js = c.js;
+        B.ti = c.ti;
+        B.pred = c.pred;
+        B.fused = pred_is_current(c) ? 0 : 1;
+        B.nj = nj;
+        B.ntiles = A.ntiles;
+        B.i_index = d_index; B.xi = d_xi; B.vi = d_vi;
+        B.ni = ni;
+        B.eps2 = A.eps2;
+        B.ds = c.opt_ds;
+        const int S = A.ntiles;
+        int rc = ensure_partials(c, (size_t)S * ni);
+        if (rc) return rc;
+        B.P = c.part;
+        B.P.stride_s = 1;
+        B.P.stride_i = S;
+        const int blocks = (A.ntiles + 3) / 4;
+        if (ev_pred_done) CK(cudaEventRecord(ev_pred_done, c.stream));     // predictor fused: no separate phase
+        if (c.opt_newton) k_force_small<true><<<blocks, 128, 0, c.stream>>>(B);
+        else k_force_small<false><<<blocks, 128, 0, c.stream>>>(B);
+        CK(cudaGetLastError());
+        if (ev_force_done) CK(cudaEventRecord(ev_force_done, c.stream));
+        if (S > 256) k_combine_block<<<ni, 128, 0, c.stream>>>(B.P, S, ni, c.js.idx, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2);
+        else k_combine_wide<<<(ni + 3) / 4, 128, 0, c.stream>>>(B.P, S, ni, c.js.idx, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2);
+        CK(cudaGetLastError());
+        c.last_ctas = blocks;
+        c.last_S = S;
+        return G6_OK;
+    }
+    int rcp = run_predict(c);
+    if (rcp) return rcp;
+    if (ev_pred_done) CK(cudaEventRecord(ev_pred_done, c.stream));
+
     // kernel choice: the fast kernel needs a normal FP32 eps2 > 0 (its unchecked tiles rely on s2 > 0)
     const bool fast_ok = A.eps2 >= std::numeric_limits<float>::min() && std::isfinite(A.eps2);
     const bool use_fast = (c.opt_kernel == 2 || c.opt_kernel == 0) && fast_ok && fast_available();
@@ -287,22 +402,16 @@ int run_force(Cluster &c, int nj, int ni, const int *d_index, const double *d_xi
     const FastVariant fv = fast_pick(ni, c.n_sm, c.opt_variant);
     const int itile = use_fast ? fv.threads * fv.it : REF_THREADS;
     const int n_itiles = (ni + itile - 1) / itile;
-    int S;
-    if (c.opt_jsplit > 0) {
-        S = c.opt_jsplit;
-    } else {
-        // i/j-split scheduler (PAPER.md:82, :104 generalised): enough CTAs to fill the SMs at any n_i
-        const int slots = c.n_sm * (use_fast ? fast_ctas_per_sm(fv) : 8);
-        S = n_itiles >= slots ? 1 : (slots + n_itiles - 1) / n_itiles;
-        // keep at least 2 tiles per split so the staging pipeline has something to overlap
-        S = std::min(S, std::max(1, A.ntiles / 2));
-    }
+    const int slots = c.n_sm * (use_fast ? fast_ctas_per_sm(fv) : 8);
+    int S = c.opt_jsplit > 0 ? c.opt_jsplit : choose_jsplit(n_itiles, A.ntiles, slots, ni);
     S = std::max(1, std::min(S, A.ntiles));
     A.S = S;
     int rc = ensure_partials(c, (size_t)S * ni);
     if (rc) return rc;
     A.P = c.part;
-    A.P.stride = ni;
+    const bool wide = S > 8;                 // many splits: [i][s] layout, one warp per i combines
+    A.P.stride_s = wide ? 1 : ni;
+    A.P.stride_i = wide ? S : 1;
 
     if (use_fast) {
         rc = launch_force_fast(A, c.opt_newton != 0, fv, n_itiles, S, c.stream);
@@ -314,7 +423,8 @@ int run_force(Cluster &c, int nj, int ni, const int *d_index, const double *d_xi
         CK(cudaGetLastError());
     }
     if (ev_force_done) CK(cudaEventRecord(ev_force_done, c.stream));
-    k_combine<<<(ni + 255) / 256, 256, 0, c.stream>>>(A.P, S, ni, c.js.idx, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2);
+    if (wide) k_combine_wide<<<(ni + 3) / 4, 128, 0, c.stream>>>(A.P, S, ni, c.js.idx, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2);
+    else k_combine<<<(ni + 255) / 256, 256, 0, c.stream>>>(A.P, S, ni, c.js.idx, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2);
     CK(cudaGetLastError());
     c.last_ctas = n_itiles * S;
     c.last_S = S;
@@ -391,7 +501,7 @@ int g6_open(int clusterid)
         CK(dalloc(c.pred, n * NF));
         CK(dalloc(c.tile_imin, n / JT)); CK(dalloc(c.tile_imax, n / JT));
         for (auto &ev : c.ev) CK(cudaEventCreate(&ev));
-        CK(cudaEventCreateWithFlags(&c.ev_bulk, cudaEventDisableTiming));
+        for (auto &ev : c.ev_rec) CK(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
         int r = fast_kernel_init();
         if (r) return fail(c, G6_ERR_CUDA, "fast kernel attribute setup failed: %s", cudaGetErrorString((cudaError_t)r));
         return G6_OK;
@@ -433,7 +543,7 @@ int g6_set_j_particle(int clusterid, int address, int index, double tj, double d
         slot = c.n_rec++;
         c.slot_of_addr[address] = slot;
     }
-    JRecord &r = c.h_rec[slot];
+    JRecord &r = c.h_rec[c.rec_cur][slot];
     for (int k = 0; k < 3; ++k) {
         r.x[k] = x[k];
         r.v[k] = (float)v[k];
@@ -510,10 +620,8 @@ int g6x_calc_dev(int clusterid, int nj, int ni, const int *d_index, const double
     if (!(eps2 >= 0.0)) return fail(c, G6_ERR_ARG, "eps2 = %g", eps2);
     const bool tm = c.opt_timers != 0;
     if (tm) { CK(cudaEventRecord(c.ev[0], c.stream)); CK(cudaEventRecord(c.ev[1], c.stream)); }
-    rc = run_predict(c);
-    if (rc) return rc;
-    if (tm) CK(cudaEventRecord(c.ev[2], c.stream));
-    rc = run_force(c, nj, ni, d_index, d_xi, d_vi, eps2, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2, tm ? c.ev[3] : nullptr);
+    rc = run_force(c, nj, ni, d_index, d_xi, d_vi, eps2, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2, tm ? c.ev[2] : nullptr,
+                   tm ? c.ev[3] : nullptr);
     if (rc) return rc;
     if (tm) { CK(cudaEventRecord(c.ev[4], c.stream)); CK(cudaEventRecord(c.ev[5], c.stream)); }
     c.ev_valid = tm;
@@ -535,33 +643,30 @@ int g6calc_firsthalf(int clusterid, int nj, int ni, const int index[], const dou
     if (rc) return rc;
     const bool tm = c.opt_timers != 0;
     if (tm) CK(cudaEventRecord(c.ev[0], c.stream));
-    // a-3: i-block to pinned staging, then to the device (the only per-step H2D payload)
-    memcpy(c.h_idx, index, sizeof(int) * ni);
-    memcpy(c.h_xi, xi, sizeof(double) * 3 * ni);
-    memcpy(c.h_vi, vi, sizeof(double) * 3 * ni);
-    CK(cudaMemcpyAsync(c.d_idx, c.h_idx, sizeof(int) * ni, cudaMemcpyHostToDevice, c.stream));
-    CK(cudaMemcpyAsync(c.d_xi, c.h_xi, sizeof(double) * 3 * ni, cudaMemcpyHostToDevice, c.stream));
-    CK(cudaMemcpyAsync(c.d_vi, c.h_vi, sizeof(double) * 3 * ni, cudaMemcpyHostToDevice, c.stream));
-    // a-1
-    rc = flush_j(c);
+    // a-3: i block to pinned staging (the only per-step H2D payload) ...
+    {
+        const IView hv = iview(c.h_iblk, ni);
+        memcpy((void *)hv.xi, xi, sizeof(double) * 3 * ni);
+        memcpy((void *)hv.vi, vi, sizeof(double) * 3 * ni);
+        memcpy((void *)hv.idx, index, sizeof(int) * ni);
+    }
+    // ... and, together with a-1 (changed j particles), on to the device
+    rc = stage_inputs(c, true, ni);
     if (rc) return rc;
     if (tm) CK(cudaEventRecord(c.ev[1], c.stream));
-    // a-2
-    rc = run_predict(c);
-    if (rc) return rc;
-    if (tm) CK(cudaEventRecord(c.ev[2], c.stream));
-    // a-4, a-5
-    rc = run_force(c, nj, ni, c.d_idx, c.d_xi, c.d_vi, eps2, c.d_acc, c.d_jerk, c.d_pot, c.d_nnidx, c.d_nnr2,
+    // a-2 (inside run_force: separate predictor kernel, or fused into the small-block force kernel), a-4, a-5;
+    // small blocks: the combine kernel writes the results straight into mapped host memory (a-6)
+    const bool zc_out = ni <= ZC_MAX_I;
+    const IView dv = iview(c.d_iblk, ni);
+    const RView out = rview(zc_out ? c.hd_res : c.d_res, ni);
+    rc = run_force(c, nj, ni, dv.idx, dv.xi, dv.vi, eps2, out.acc, out.jerk, out.pot, out.nnidx, out.nnr2, tm ? c.ev[2] : nullptr,
                    tm ? c.ev[3] : nullptr);
     if (rc) return rc;
     if (tm) CK(cudaEventRecord(c.ev[4], c.stream));
     // a-6
-    CK(cudaMemcpyAsync(c.h_acc, c.d_acc, sizeof(double) * 3 * ni, cudaMemcpyDeviceToHost, c.stream));
-    CK(cudaMemcpyAsync(c.h_jerk, c.d_jerk, sizeof(double) * 3 * ni, cudaMemcpyDeviceToHost, c.stream));
-    CK(cudaMemcpyAsync(c.h_pot, c.d_pot, sizeof(double) * ni, cudaMemcpyDeviceToHost, c.stream));
-    CK(cudaMemcpyAsync(c.h_nnidx, c.d_nnidx, sizeof(int) * ni, cudaMemcpyDeviceToHost, c.stream));
-    CK(cudaMemcpyAsync(c.h_nnr2, c.d_nnr2, sizeof(double) * ni, cudaMemcpyDeviceToHost, c.stream));
+    if (!zc_out) CK(cudaMemcpyAsync(c.h_res, c.d_res, res_bytes(ni), cudaMemcpyDeviceToHost, c.stream));
     CK(cudaEventRecord(c.ev[5], c.stream));
+    c.res_on_host = zc_out;
     c.ev_valid = tm;
     c.pending = true;
     c.pend_nj = nj;
@@ -580,10 +685,11 @@ int g6calc_lasthalf2(int clusterid, int nj, int ni, const int index[], const dou
     if (!acc || !jerk || !pot) return fail(c, G6_ERR_ARG, "NULL result array");
     c.pending = false;
     CK(cudaEventSynchronize(c.ev[5]));
-    memcpy(acc, c.h_acc, sizeof(double) * 3 * ni);
-    memcpy(jerk, c.h_jerk, sizeof(double) * 3 * ni);
-    memcpy(pot, c.h_pot, sizeof(double) * ni);
-    if (nnb_index) memcpy(nnb_index, c.h_nnidx, sizeof(int) * ni);
+    const RView r = rview(c.h_res, ni);
+    memcpy(acc, r.acc, sizeof(double) * 3 * ni);
+    memcpy(jerk, r.jerk, sizeof(double) * 3 * ni);
+    memcpy(pot, r.pot, sizeof(double) * ni);
+    if (nnb_index) memcpy(nnb_index, r.nnidx, sizeof(int) * ni);
     c.have_result = true;
     c.last_ni = ni;
     return G6_OK;
@@ -608,7 +714,8 @@ int g6_get_neighbour_list(int clusterid, int ipipe, int maxlen, int *n, int list
     if (c.pending || !c.have_result) return fail(c, G6_ERR_SEQUENCE, "no completed force call");
     if (ipipe < 0 || ipipe >= c.last_ni) return fail(c, G6_ERR_ARG, "ipipe = %d outside [0, %d)", ipipe, c.last_ni);
     if (!n || !list || maxlen < 1) return fail(c, G6_ERR_ARG, "bad neighbour list buffer");
-    if (c.h_nnidx[ipipe] >= 0) { *n = 1; list[0] = c.h_nnidx[ipipe]; }
+    const int nb = rview(c.h_res, c.last_ni).nnidx[ipipe];
+    if (nb >= 0) { *n = 1; list[0] = nb; }
     else *n = 0;
     return G6_OK;
 }
@@ -618,8 +725,9 @@ int g6x_get_nearest(int clusterid, int ni, int nn_index[], double nn_r2[])
     GET_CLUSTER(clusterid);
     if (c.pending || !c.have_result) return fail(c, G6_ERR_SEQUENCE, "no completed force call");
     if (ni != c.last_ni) return fail(c, G6_ERR_ARG, "ni = %d but the last call had %d", ni, c.last_ni);
-    if (nn_index) memcpy(nn_index, c.h_nnidx, sizeof(int) * ni);
-    if (nn_r2) memcpy(nn_r2, c.h_nnr2, sizeof(double) * ni);
+    const RView r = rview(c.h_res, ni);
+    if (nn_index) memcpy(nn_index, r.nnidx, sizeof(int) * ni);
+    if (nn_r2) memcpy(nn_r2, r.nnr2, sizeof(double) * ni);
     return G6_OK;
 }
 
@@ -668,6 +776,7 @@ static int *option_slot(Cluster &c, const char *key)
     if (!strcmp(key, "kernel")) return &c.opt_kernel;
     if (!strcmp(key, "timers")) return &c.opt_timers;
     if (!strcmp(key, "variant")) return &c.opt_variant;
+    if (!strcmp(key, "small")) return &c.opt_small;
     return nullptr;
 }
 
@@ -677,7 +786,7 @@ int g6x_set_option(int clusterid, const char *key, int value)
     int *slot = option_slot(c, key);
     if (!slot) return fail(c, G6_ERR_ARG, "unknown option '%s'", key ? key : "(null)");
     const bool is_flag = slot == &c.opt_ds || slot == &c.opt_newton || slot == &c.opt_timers;
-    if (value < 0 || (is_flag && value > 1) || (slot == &c.opt_kernel && value > 2) || (slot == &c.opt_jsplit && value > 65535) ||
+    if (value < 0 || (is_flag && value > 1) || (slot == &c.opt_kernel && value > 2) || (slot == &c.opt_jsplit && value > 65535) || (slot == &c.opt_small && value > SMALL_MAX_I) ||
         (slot == &c.opt_variant && value != 0 && fast_ctas_per_sm(FastVariant{value / 8, value % 8}) < 1))
         return fail(c, G6_ERR_ARG, "bad value %d for option '%s'", value, key);
     *slot = value;
@@ -730,11 +839,13 @@ int g6x_debug_dx(int clusterid, int n, const int ipipe[], const int jaddr[], flo
             return fail(c, G6_ERR_ARG, "pair %d out of range", k);
     int *d_ip = nullptr, *d_ja = nullptr;
     float *d_out = nullptr;
-    int rc = [&]() -> int {
+    int rc = run_predict(c);     // the small-block kernel predicts on the fly and leaves c.pred stale
+    if (rc) return rc;
+    rc = [&]() -> int {
         CK(dalloc(d_ip, n)); CK(dalloc(d_ja, n)); CK(dalloc(d_out, 3 * (size_t)n));
         CK(cudaMemcpyAsync(d_ip, ipipe, sizeof(int) * n, cudaMemcpyHostToDevice, c.stream));
         CK(cudaMemcpyAsync(d_ja, jaddr, sizeof(int) * n, cudaMemcpyHostToDevice, c.stream));
-        k_debug_dx<<<(n + 127) / 128, 128, 0, c.stream>>>(n, d_ip, d_ja, c.d_xi, c.opt_ds, c.pred, d_out);
+        k_debug_dx<<<(n + 127) / 128, 128, 0, c.stream>>>(n, d_ip, d_ja, iview(c.d_iblk, c.last_ni).xi, c.opt_ds, c.pred, d_out);
         CK(cudaGetLastError());
         CK(cudaMemcpyAsync(dx, d_out, sizeof(float) * 3 * n, cudaMemcpyDeviceToHost, c.stream));
         CK(cudaStreamSynchronize(c.stream));

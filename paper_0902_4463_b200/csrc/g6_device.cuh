@@ -1,7 +1,7 @@
 // g6_device.cuh -- device data layout and the small kernels of libg6b200 (sm_100a).
 //
 // Steps of the path:
-//   a-1  k_store_from_f64 / k_scatter_records : keep the j-particle store on the device
+//   a-1  k_store_from_f64 / k_stage           : keep the j-particle store on the device
 //   a-2  k_predict                            : Eq. 1-2, DS positions
 //   a-4  force kernels (g6_force_ref.cuh, g6_force_fast.cuh)
 //   a-5  k_combine                            : sum the per-split partial forces on the GPU
@@ -44,14 +44,16 @@ constexpr int F_XH = 0, F_XL = 3, F_V = 6, F_M = 9;
 constexpr int TILE_FLOATS = JT * NF;
 constexpr int TILE_BYTES = TILE_FLOATS * 4;
 
-// ---- partial results of one j-split, structure of arrays, element [s * stride + i] --------
+// ---- partial results of one j-split, structure of arrays, element [s * stride_s + i * stride_i]
+// few splits: (stride_s, stride_i) = (ni, 1), one thread per i combines; many splits (small
+// blocks): (1, S), one warp per i combines with coalesced reads.
 struct Partials {
     double *acc[3];
     double *jrk[3];
     double *pot;
     float *nn_r2;    // unsoftened, +inf when none
     int *nn_addr;    // j address, -1 when none
-    int stride;
+    int stride_s, stride_i;
 };
 
 // double -> double-single (reading 12): hi = RN32(x), lo = RN32(x - hi)
@@ -95,24 +97,37 @@ k_store_from_f64(JStore S, int addr0, int n, const int *__restrict__ index, cons
     S.idx[a] = index[p];
 }
 
-// ---- a-1: scatter of the particles changed since the last force call -----------------------
-__global__ void __launch_bounds__(256)
-k_scatter_records(JStore S, const JRecord *__restrict__ rec, int n)
+// ---- a-1 + a-3: scatter of the particles changed since the last force call, and the i block -----
+// `rec`, `xi_src`, ... may point into mapped pinned HOST memory (small batches: no DMA set-up
+// latency) or into device memory (large batches, after one packed copy).
+__global__ void __launch_bounds__(128)
+k_stage(JStore S, const JRecord *__restrict__ rec, int n_rec, int n_i, const double *__restrict__ xi_src,
+        const double *__restrict__ vi_src, const int *__restrict__ idx_src, double *__restrict__ xi_dst,
+        double *__restrict__ vi_dst, int *__restrict__ idx_dst)
 {
-    int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= n) return;
-    JRecord r = rec[p];
-    int a = r.addr;
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p < n_rec) {
+        const JRecord r = rec[p];
+        const int a = r.addr;
 #pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        S.x[k][a] = r.x[k];
-        S.v[k][a] = r.v[k];
-        S.a2[k][a] = r.a2[k];
-        S.j6[k][a] = r.j6[k];
+        for (int k = 0; k < 3; ++k) {
+            S.x[k][a] = r.x[k];
+            S.v[k][a] = r.v[k];
+            S.a2[k][a] = r.a2[k];
+            S.j6[k][a] = r.j6[k];
+        }
+        S.t[a] = r.t;
+        S.m[a] = r.m;
+        S.idx[a] = r.idx;
     }
-    S.t[a] = r.t;
-    S.m[a] = r.m;
-    S.idx[a] = r.idx;
+    if (p < n_i) {
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            xi_dst[3 * p + k] = xi_src[3 * p + k];
+            vi_dst[3 * p + k] = vi_src[3 * p + k];
+        }
+        idx_dst[p] = idx_src[p];
+    }
 }
 
 // ---- a-2: predictor, one thread per j, one CTA per tile ------------------------------------
@@ -189,7 +204,7 @@ k_combine(Partials P, int S, int ni, const int *__restrict__ jidx,
     float best = __int_as_float(0x7f800000);
     int baddr = -1;
     for (int s = 0; s < S; ++s) {
-        size_t o = (size_t)s * P.stride + i;
+        size_t o = (size_t)s * P.stride_s + (size_t)i * P.stride_i;
 #pragma unroll
         for (int k = 0; k < 3; ++k) { a[k] += P.acc[k][o]; jk[k] += P.jrk[k][o]; }
         ph += P.pot[o];
@@ -202,6 +217,104 @@ k_combine(Partials P, int S, int ni, const int *__restrict__ jidx,
     pot[i] = ph;
     if (nn_index) nn_index[i] = baddr >= 0 ? jidx[baddr] : -1;
     if (nn_r2) nn_r2[i] = baddr >= 0 ? (double)best : (double)__int_as_float(0x7f800000);
+}
+
+// many splits, few i (the small active blocks of block time steps): one warp per i.  Lane l sums
+// the splits s = l, l+32, ... in order, then a fixed xor-tree adds the 32 lane sums: the order is
+// fixed by (S) alone, so results are bit-reproducible.  Nearest neighbour: (r2, address)
+// lexicographic minimum = smallest r2, ties -> smallest address.
+__global__ void __launch_bounds__(128)
+k_combine_wide(Partials P, int S, int ni, const int *__restrict__ jidx,
+               double *__restrict__ acc, double *__restrict__ jerk, double *__restrict__ pot,
+               int *__restrict__ nn_index, double *__restrict__ nn_r2)
+{
+    const int i = blockIdx.x * 4 + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (i >= ni) return;
+    double v[7] = {0, 0, 0, 0, 0, 0, 0};
+    float best = __int_as_float(0x7f800000);
+    int baddr = 0x7fffffff;
+    for (int s = lane; s < S; s += 32) {
+        const size_t o = (size_t)s * P.stride_s + (size_t)i * P.stride_i;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { v[k] += P.acc[k][o]; v[3 + k] += P.jrk[k][o]; }
+        v[6] += P.pot[o];
+        const float r2 = P.nn_r2[o];
+        const int ad = P.nn_addr[o];
+        if (ad >= 0 && (r2 < best || (r2 == best && ad < baddr))) { best = r2; baddr = ad; }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int k = 0; k < 7; ++k) v[k] += __shfl_xor_sync(0xffffffffu, v[k], o);
+        const float r2 = __shfl_xor_sync(0xffffffffu, best, o);
+        const int ad = __shfl_xor_sync(0xffffffffu, baddr, o);
+        if (r2 < best || (r2 == best && ad < baddr)) { best = r2; baddr = ad; }
+    }
+    if (lane == 0) {
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { acc[3 * (size_t)i + k] = v[k]; jerk[3 * (size_t)i + k] = v[3 + k]; }
+        pot[i] = v[6];
+        const bool has = baddr != 0x7fffffff;
+        if (nn_index) nn_index[i] = has ? jidx[baddr] : -1;
+        if (nn_r2) nn_r2[i] = has ? (double)best : (double)__int_as_float(0x7f800000);
+    }
+}
+
+// very many splits (one per j-tile, small-block kernel at large N_j): one CTA of 128 threads per i.
+// Thread t sums s = t, t+128, ... in order; fixed xor tree inside each warp; the four warp sums are
+// added in warp order by thread 0.
+__global__ void __launch_bounds__(128)
+k_combine_block(Partials P, int S, int ni, const int *__restrict__ jidx,
+                double *__restrict__ acc, double *__restrict__ jerk, double *__restrict__ pot,
+                int *__restrict__ nn_index, double *__restrict__ nn_r2)
+{
+    const int i = blockIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    __shared__ double sv[4][7];
+    __shared__ float sr[4];
+    __shared__ int sa[4];
+    double v[7] = {0, 0, 0, 0, 0, 0, 0};
+    float best = __int_as_float(0x7f800000);
+    int baddr = 0x7fffffff;
+    for (int s = tid; s < S; s += 128) {
+        const size_t o = (size_t)s * P.stride_s + (size_t)i * P.stride_i;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { v[k] += P.acc[k][o]; v[3 + k] += P.jrk[k][o]; }
+        v[6] += P.pot[o];
+        const float r2 = P.nn_r2[o];
+        const int ad = P.nn_addr[o];
+        if (ad >= 0 && (r2 < best || (r2 == best && ad < baddr))) { best = r2; baddr = ad; }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int k = 0; k < 7; ++k) v[k] += __shfl_xor_sync(0xffffffffu, v[k], o);
+        const float r2 = __shfl_xor_sync(0xffffffffu, best, o);
+        const int ad = __shfl_xor_sync(0xffffffffu, baddr, o);
+        if (r2 < best || (r2 == best && ad < baddr)) { best = r2; baddr = ad; }
+    }
+    if (lane == 0) {
+#pragma unroll
+        for (int k = 0; k < 7; ++k) sv[w][k] = v[k];
+        sr[w] = best;
+        sa[w] = baddr;
+    }
+    __syncthreads();
+    if (tid == 0) {
+#pragma unroll
+        for (int q = 1; q < 4; ++q) {
+#pragma unroll
+            for (int k = 0; k < 7; ++k) v[k] += sv[q][k];
+            if (sr[q] < best || (sr[q] == best && sa[q] < baddr)) { best = sr[q]; baddr = sa[q]; }
+        }
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { acc[3 * (size_t)i + k] = v[k]; jerk[3 * (size_t)i + k] = v[3 + k]; }
+        pot[i] = v[6];
+        const bool has = baddr != 0x7fffffff;
+        if (nn_index) nn_index[i] = has ? jidx[baddr] : -1;
+        if (nn_r2) nn_r2[i] = has ? (double)best : (double)__int_as_float(0x7f800000);
+    }
 }
 
 // ---- debug: the kernel's Eq.-3 separation for chosen (i, j) pairs (DESIGN.md pin P11) -------

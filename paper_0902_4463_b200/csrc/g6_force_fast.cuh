@@ -19,8 +19,8 @@
 //    every tile, and a warp takes the checked path (per-pair index compare, address < nj) only on
 //    tiles whose index range contains one of its i-particles, or on the ragged last tile.
 //    All other tiles run without any per-pair test (needs eps2 > 0 so that s2 > 0).
-//  * nearest neighbour: the loop keeps only min r2 (one FMNMX3 per two pairs) and the tile in
-//    which it last improved; the j address is recovered afterwards by re-scanning that one tile
+//  * nearest neighbour: the loop keeps only min r2 (one FMNMX3 per two pairs) and the 8-j step in
+//    which it last improved; the j address is recovered afterwards by re-evaluating those 8 j
 //    with the same arithmetic (first j that reproduces the minimum: ties -> smallest address).
 //  * FP32 partial sums run over one tile (two chains of JT/2 terms per component, even and odd j)
 //    and are folded into fp64 accumulators per tile (reading 9).
@@ -170,12 +170,12 @@ k_force_fast(ForceArgs A)
     IPart I[IT];
     int my[IT];
     double acc[IT][3], jrk[IT][3], pot[IT];
-    int btile[IT];
+    int bstep[IT];          // the 8-j step (global numbering: address / 8) in which rmin last improved
 #pragma unroll
     for (int q = 0; q < IT; ++q) {
         const int i = (blockIdx.x * IT + q) * THREADS + tid;
         my[q] = i < A.ni ? A.i_index[i] : -1;
-        btile[q] = -1;
+        bstep[q] = -1;
         pot[q] = 0;
         I[q].rmin = INF;
 #pragma unroll
@@ -227,34 +227,42 @@ k_force_fast(ForceArgs A)
             for (int k = 0; k < 3; ++k) { I[q].a[k] = dup(0.0f); I[q].j[k] = dup(0.0f); }
             I[q].p = dup(0.0f);
         }
-        float rmin0[IT];
-#pragma unroll
-        for (int q = 0; q < IT; ++q) rmin0[q] = I[q].rmin;
 
         if (!checked) {
-#pragma unroll 2
-            for (int l4 = 0; l4 < JT / 4; ++l4) {
-                float4 f[NF];
+            // a step = 8 consecutive j: two LDS.128 per field, four packed pair-evaluations per i
+#pragma unroll 1
+            for (int s8 = 0; s8 < JT / 8; ++s8) {
+                float before[IT];
 #pragma unroll
-                for (int k = 0; k < NF; ++k) f[k] = T[k * (JT / 4) + l4];
+                for (int q = 0; q < IT; ++q) before[q] = I[q].rmin;
 #pragma unroll
-                for (int q = 0; q < IT; ++q) {
-                    float2 ra, rb;
-                    pair2<NEWTON>(I[q], make_float2(f[0].x, f[0].y), make_float2(f[1].x, f[1].y), make_float2(f[2].x, f[2].y),
-                                  make_float2(f[3].x, f[3].y), make_float2(f[4].x, f[4].y), make_float2(f[5].x, f[5].y),
-                                  make_float2(f[6].x, f[6].y), make_float2(f[7].x, f[7].y), make_float2(f[8].x, f[8].y),
-                                  make_float2(f[9].x, f[9].y), eps2, ra);
-                    pair2<NEWTON>(I[q], make_float2(f[0].z, f[0].w), make_float2(f[1].z, f[1].w), make_float2(f[2].z, f[2].w),
-                                  make_float2(f[3].z, f[3].w), make_float2(f[4].z, f[4].w), make_float2(f[5].z, f[5].w),
-                                  make_float2(f[6].z, f[6].w), make_float2(f[7].z, f[7].w), make_float2(f[8].z, f[8].w),
-                                  make_float2(f[9].z, f[9].w), eps2, rb);
-                    I[q].rmin = fminf(fminf(ra.x, ra.y), I[q].rmin);
-                    I[q].rmin = fminf(fminf(rb.x, rb.y), I[q].rmin);
+                for (int h = 0; h < 2; ++h) {
+                    float4 f[NF];
+#pragma unroll
+                    for (int k = 0; k < NF; ++k) f[k] = T[k * (JT / 4) + 2 * s8 + h];
+#pragma unroll
+                    for (int q = 0; q < IT; ++q) {
+                        float2 ra, rb;
+                        pair2<NEWTON>(I[q], make_float2(f[0].x, f[0].y), make_float2(f[1].x, f[1].y), make_float2(f[2].x, f[2].y),
+                                      make_float2(f[3].x, f[3].y), make_float2(f[4].x, f[4].y), make_float2(f[5].x, f[5].y),
+                                      make_float2(f[6].x, f[6].y), make_float2(f[7].x, f[7].y), make_float2(f[8].x, f[8].y),
+                                      make_float2(f[9].x, f[9].y), eps2, ra);
+                        pair2<NEWTON>(I[q], make_float2(f[0].z, f[0].w), make_float2(f[1].z, f[1].w), make_float2(f[2].z, f[2].w),
+                                      make_float2(f[3].z, f[3].w), make_float2(f[4].z, f[4].w), make_float2(f[5].z, f[5].w),
+                                      make_float2(f[6].z, f[6].w), make_float2(f[7].z, f[7].w), make_float2(f[8].z, f[8].w),
+                                      make_float2(f[9].z, f[9].w), eps2, rb);
+                        I[q].rmin = fminf(fminf(ra.x, ra.y), I[q].rmin);
+                        I[q].rmin = fminf(fminf(rb.x, rb.y), I[q].rmin);
+                    }
                 }
+#pragma unroll
+                for (int q = 0; q < IT; ++q)
+                    if (I[q].rmin < before[q]) bstep[q] = t * (JT / 8) + s8;
             }
         } else {
             // checked tile: mask out j >= nj and index_j == index_i (mass -> 0, r2 -> +inf)
             const int4 *JX = reinterpret_cast<const int4 *>(A.jidx + (size_t)t * JT);
+#pragma unroll 1
             for (int l4 = 0; l4 < JT / 4; ++l4) {
                 float4 f[NF];
 #pragma unroll
@@ -273,6 +281,7 @@ k_force_fast(ForceArgs A)
                     const bool o1 = (j0 + 1 < A.nj) && (jx.y != my[q]);
                     const bool o2 = (j0 + 2 < A.nj) && (jx.z != my[q]);
                     const bool o3 = (j0 + 3 < A.nj) && (jx.w != my[q]);
+                    const float before = I[q].rmin;
                     float2 ra, rb;
                     pair2<NEWTON>(I[q], make_float2(f[0].x, f[0].y), make_float2(f[1].x, f[1].y), make_float2(f[2].x, f[2].y),
                                   make_float2(f[3].x, f[3].y), make_float2(f[4].x, f[4].y), make_float2(f[5].x, f[5].y),
@@ -284,6 +293,7 @@ k_force_fast(ForceArgs A)
                                   make_float2(o2 ? f[9].z : 0.0f, o3 ? f[9].w : 0.0f), eps2, rb);
                     I[q].rmin = fminf(fminf(o0 ? ra.x : INF, o1 ? ra.y : INF), I[q].rmin);
                     I[q].rmin = fminf(fminf(o2 ? rb.x : INF, o3 ? rb.y : INF), I[q].rmin);
+                    if (I[q].rmin < before) bstep[q] = j0 >> 3;
                 }
             }
         }
@@ -291,7 +301,7 @@ k_force_fast(ForceArgs A)
         __syncwarp();
         if ((tid & 31) == 0) mbar_arrive(&sm.empty[st]);
 
-        // fold the tile's FP32 sums into fp64; remember the tile if the minimum improved
+        // fold the tile's FP32 sums into fp64 (chains of JT/2 terms, reading 9)
 #pragma unroll
         for (int q = 0; q < IT; ++q) {
 #pragma unroll
@@ -300,32 +310,44 @@ k_force_fast(ForceArgs A)
                 jrk[q][k] += (double)I[q].j[k].x + (double)I[q].j[k].y;
             }
             pot[q] -= (double)I[q].p.x + (double)I[q].p.y;
-            if (I[q].rmin < rmin0[q]) btile[q] = t;
         }
     }
 
-    // ---- recover the nearest neighbour's address: re-scan the one tile that set the minimum
+    // ---- recover the nearest neighbour's address: re-evaluate the 8 j of the step that set the
+    // minimum with the same arithmetic (packed and scalar IEEE ops round identically); the first j
+    // that reproduces rmin wins, so ties go to the smallest address (reading 7)
 #pragma unroll
     for (int q = 0; q < IT; ++q) {
         const int i = (blockIdx.x * IT + q) * THREADS + tid;
         if (i >= A.ni) continue;
         int baddr = -1;
-        if (btile[q] >= 0) {
-            const int t = btile[q];
-            const float *g = A.pred + (size_t)t * TILE_FLOATS;
-            const float nxh0 = I[q].nxh[0].x, nxh1 = I[q].nxh[1].x, nxh2 = I[q].nxh[2].x;
-            const float nxl0 = I[q].nxl[0].x, nxl1 = I[q].nxl[1].x, nxl2 = I[q].nxl[2].x;
-            for (int l = 0; l < JT && baddr < 0; ++l) {
-                const int ja = t * JT + l;
-                if (ja >= A.nj) break;
-                const float dx = __fadd_rn(__fadd_rn(g[(F_XH + 0) * JT + l], nxh0), __fadd_rn(g[(F_XL + 0) * JT + l], nxl0));
-                const float dy = __fadd_rn(__fadd_rn(g[(F_XH + 1) * JT + l], nxh1), __fadd_rn(g[(F_XL + 1) * JT + l], nxl1));
-                const float dz = __fadd_rn(__fadd_rn(g[(F_XH + 2) * JT + l], nxh2), __fadd_rn(g[(F_XL + 2) * JT + l], nxl2));
-                const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-                if (r2 == I[q].rmin && A.jidx[ja] != my[q]) baddr = ja;
+        if (bstep[q] >= 0) {
+            const int j0 = bstep[q] * 8;
+            const float *g = A.pred + (size_t)(j0 / JT) * TILE_FLOATS + (j0 % JT);
+            float r2[8];
+            int jx[8];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                float4 c[6];
+#pragma unroll
+                for (int k = 0; k < 6; ++k) c[k] = __ldg(reinterpret_cast<const float4 *>(g + k * JT) + h);
+                const float xs[6][4] = {{c[0].x, c[0].y, c[0].z, c[0].w}, {c[1].x, c[1].y, c[1].z, c[1].w}, {c[2].x, c[2].y, c[2].z, c[2].w},
+                                        {c[3].x, c[3].y, c[3].z, c[3].w}, {c[4].x, c[4].y, c[4].z, c[4].w}, {c[5].x, c[5].y, c[5].z, c[5].w}};
+#pragma unroll
+                for (int l = 0; l < 4; ++l) {
+                    const float dx = __fadd_rn(__fadd_rn(xs[0][l], I[q].nxh[0].x), __fadd_rn(xs[3][l], I[q].nxl[0].x));
+                    const float dy = __fadd_rn(__fadd_rn(xs[1][l], I[q].nxh[1].x), __fadd_rn(xs[4][l], I[q].nxl[1].x));
+                    const float dz = __fadd_rn(__fadd_rn(xs[2][l], I[q].nxh[2].x), __fadd_rn(xs[5][l], I[q].nxl[2].x));
+                    r2[4 * h + l] = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+                    const int ja = j0 + 4 * h + l;
+                    jx[4 * h + l] = ja < A.nj ? __ldg(A.jidx + ja) : my[q];
+                }
             }
+#pragma unroll
+            for (int l = 7; l >= 0; --l)
+                if (r2[l] == I[q].rmin && jx[l] != my[q]) baddr = j0 + l;
         }
-        const size_t o = (size_t)s * A.P.stride + i;
+        const size_t o = (size_t)s * A.P.stride_s + (size_t)i * A.P.stride_i;
 #pragma unroll
         for (int k = 0; k < 3; ++k) { A.P.acc[k][o] = acc[q][k]; A.P.jrk[k][o] = jrk[q][k]; }
         A.P.pot[o] = pot[q];

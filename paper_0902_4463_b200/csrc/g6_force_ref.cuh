@@ -112,7 +112,7 @@ k_force_ref(ForceArgs A)
     }
 
     if (active) {
-        const size_t o = (size_t)s * A.P.stride + i;
+        const size_t o = (size_t)s * A.P.stride_s + (size_t)i * A.P.stride_i;
 #pragma unroll
         for (int k = 0; k < 3; ++k) { A.P.acc[k][o] = acc[k]; A.P.jrk[k][o] = jrk[k]; }
         A.P.pot[o] = pot;

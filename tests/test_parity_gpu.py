@@ -20,7 +20,7 @@ def cluster():
     g6.g6x_set_npipes(256)
 
 
-KERNELS = [1, 2]          # 1 = checked reference kernel, 2 = fast kernel (FFMA2 + TMA)
+KERNELS = [0, 1, 2]       # 0 = automatic (small-block kernel for n_i <= 16), 1 = checked reference kernel, 2 = fast kernel (FFMA2 + TMA)
 
 
 # ------------------------------------------------------------------ C1: every particle
@@ -199,6 +199,44 @@ def test_eps2_zero_and_coincident_particles(cluster, oracle):
     d = np.linalg.norm(x - x[20], axis=1); d[20] = np.inf
     if d.min() == 0.5:
         assert got["nn_index"][20] == 400 == ref["nn_index"][20]
+
+
+# ------------------------------------------------------------------ small-block kernel (lanes over j, predictor fused)
+@pytest.mark.parametrize("n,ni,small", [(5000, 1, 16), (5000, 7, 16), (5000, 16, 16), (1000, 64, 64), (300, 33, 64), (40000, 3, 16)])
+def test_small_block_kernel_fused_predictor(cluster, oracle, n, ni, small):
+    """n_i <= `small`: one pass over the raw j-store, Eq. 1-2 evaluated on the fly, t_i != t_j, the
+    block's own particles present as j; must agree with the oracle and with the two-kernel path."""
+    x, v, m, _ = inputs.config("C2", n=n)
+    eps2 = 1e-8
+    rng = np.random.default_rng(ni)
+    idx = (rng.permutation(n) + 7).astype(np.int32)
+    tj, dtj, a0, j0 = inputs.taylor_state(n, 100 + ni, dt_max=2.0**-6)
+    load_j(x, v, m, index=idx, t=tj, acc=a0, jerk=j0)
+    ti = 2.0**-8
+    g6.g6_set_ti(0, ti)
+    xo, vo = oracle.predict(ti, tj, x, v, a0, j0)
+    block = np.sort(rng.choice(n, ni, replace=False))
+    ref = oracle.force(idx[block], xo[block], vo[block], idx, xo, vo, m, eps2)
+    g6.g6x_set_option(0, "small", small)
+    got = g6.force_host(0, idx[block], xo[block], vo[block], eps2, n)
+    tm = g6.g6x_get_timers(0)
+    assert tm["jsplits"] == (n + 255) // 256               # one partial result per j-tile: the small kernel ran
+    again = g6.force_host(0, idx[block], xo[block], vo[block], eps2, n)
+    for k in got:
+        assert np.array_equal(got[k], again[k]), k          # bit-reproducible
+    g6.g6x_set_option(0, "kernel", 2)                        # the two-kernel path: predictor, then the fast kernel
+    two = g6.force_host(0, idx[block], xo[block], vo[block], eps2, n)
+    g6.g6x_set_option(0, "kernel", 0)
+    g6.g6x_set_option(0, "small", 16)
+    if ni >= 16:
+        check_forces(got, ref, f"small n={n} ni={ni}")
+    assert rel_err(got["acc"], ref["acc"]).max() <= 1e-5 and rel_err(got["jerk"], ref["jerk"]).max() <= 1e-4
+    assert rel_err(got["pot"], ref["pot"]).max() <= 1e-6
+    check_nn(got["nn_index"], ref, idx, xo[block], xo)
+    assert rel_err(got["acc"], two["acc"]).max() < 2e-6 and np.array_equal(got["nn_index"], two["nn_index"])
+    # a second call at the same time reuses nothing stale: predicted positions read back are current
+    xp, vp = g6.g6x_get_predicted(0, 0, n)
+    assert np.abs(xp - xo).max() < 1e-7
 
 
 # ------------------------------------------------------------------ P11: Eq. 3 bit for bit
