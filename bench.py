@@ -123,6 +123,61 @@ def cpu_oracle_rate(x, v, m, eps2, idx, target_s, seed=7):
     return rows * float(n) / dt, rows, dt, orc.threads()
 
 
+NI_SWEEP = (1, 16, 256, 4096, 65536)
+
+
+def ni_sweep(g6, inputs, torch, dev, stream, flush, x, v, idx_all, n, eps2, peaks, reps=10):
+    """C4's block-step regime (BASELINE.json configs[3]): random active blocks of n_i particles
+    against all N_j, one block step = predictor over all j (t_i changes every step) + force +
+    combine.  Device times from CUDA events on the launching stream; `cold` = L2 flushed before
+    every step, `warm` = back to back (the j-store and the predicted tiles stay in the 126 MB L2).
+    Algorithmic bytes per step: 76 B/j when the predictor is fused into the
+    force pass, else 76 + 40 (predictor) + 40 (force read) = 156 B/j."""
+    f64 = torch.float64
+    hbm = float(peaks.get("hbm_gbs", 6650.0))
+    sm_max = float(peaks.get("sm_max_mhz", SM_MAX_MHZ_FALLBACK))
+    peak_inst = SM_COUNT * FP32_LANES_PER_SM * sm_max * 1e6
+    rows = []
+    for ni in NI_SWEEP:
+        if ni > n:
+            continue
+        block = inputs.active_subset(n, ni, 4040 + ni)
+        to = lambda a, dt=f64: torch.from_numpy(np.ascontiguousarray(a)).to(dev, dt)
+        d_xi, d_vi, d_ii = to(x[block]), to(v[block]), to(idx_all[block], torch.int32)
+        d_acc = torch.empty(ni, 3, dtype=f64, device=dev); d_jerk = torch.empty_like(d_acc)
+        d_pot = torch.empty(ni, dtype=f64, device=dev); d_nn = torch.empty(ni, dtype=torch.int32, device=dev)
+        d_r2 = torch.empty_like(d_pot)
+        res = {}
+        for mode in ("cold", "warm"):
+            tot, frc, prd, cmb = [], [], [], []
+            for k in range(reps + 3):
+                if mode == "cold":
+                    flush.zero_()
+                g6.g6_set_ti(0, (k % 2) * 2.0 ** -30)            # a new block time: the predictor runs again
+                e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                g6.g6x_calc_dev(0, n, ni, d_ii, d_xi, d_vi, eps2, d_acc, d_jerk, d_pot, d_nn, d_r2)
+                e1.record(stream)
+                torch.cuda.synchronize()
+                tm = g6.g6x_get_timers(0)
+                if k >= 3:
+                    tot.append(e0.elapsed_time(e1) * 1e3); frc.append(tm["force_us"]); prd.append(tm["predict_us"]); cmb.append(tm["combine_us"])
+            res[mode] = dict(step_us=float(np.median(tot)), force_us=float(np.median(frc)), predict_us=float(np.median(prd)),
+                             combine_us=float(np.median(cmb)), jsplits=tm["jsplits"], ctas=tm["force_ctas"])
+        fused = ni <= g6.g6x_get_option(0, "small")
+        bytes_step = n * (76 if fused else 156)
+        c = res["cold"]
+        rows.append({"n_i": ni, "cold": res["cold"], "warm": res["warm"], "fused_predictor": bool(fused),
+                     "interactions_per_s_cold": ni * float(n) / (c["step_us"] * 1e-6),
+                     "interactions_per_s_warm": ni * float(n) / (res["warm"]["step_us"] * 1e-6),
+                     "algorithmic_bytes_per_step": bytes_step,
+                     "hbm_gbs_cold": bytes_step / (c["step_us"] * 1e-6) / 1e9,
+                     "hbm_frac_cold": bytes_step / (c["step_us"] * 1e-6) / 1e9 / hbm,
+                     "fp32_frac_force_kernel_cold": FP32_INSTR_PER_INTERACTION * ni * float(n) / (c["force_us"] * 1e-6) / peak_inst})
+    g6.g6_set_ti(0, 0.0)
+    return rows
+
+
 def run_reference(args):
     """--impl reference: the oracle, timed on the host cores on a bounded sample per step."""
     rank = int(os.environ.get("RANK", "0"))
@@ -170,6 +225,7 @@ def main():
     ap.add_argument("--ref-seconds", type=float, default=8.0, help="CPU work per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the C4 n_i sweep (block-step regime)")
     ap.add_argument("--newton", type=int, default=None, help="override the library default (1 = rsqrt + one Newton step)")
     args = ap.parse_args()
     if args.warmup < 3:
@@ -290,6 +346,10 @@ def main():
                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                "note": "host arrays in, host arrays out (library stages through its own pinned buffers); includes the L2 flush"}
 
+    sweep = None
+    if rank == 0 and world == 1 and not args.no_sweep:
+        sweep = ni_sweep(g6, inputs, torch, dev, stream, flush, x, v, idx, n, eps2, measured_peaks()[0])
+
     if rank == 0:
         peaks, peaks_src = measured_peaks()
         sm_max = float(peaks.get("sm_max_mhz", SM_MAX_MHZ_FALLBACK))
@@ -322,6 +382,8 @@ def main():
                "wall_s_timed_region": wall}
         if e2e:
             out["e2e"] = e2e
+        if sweep is not None:
+            out["ni_sweep"] = sweep
         if not args.no_cpu_baseline and world == 1:
             rate, rows, dt, cores = cpu_oracle_rate(x, v, m, eps2, idx, args.cpu_seconds)
             out["cpu_baseline"] = {"value": rate, "unit": "interactions/s", "cores": cores, "kind": "oracle",

@@ -104,7 +104,11 @@ __device__ __forceinline__ void pair2(IPart &I, const float2 xh, const float2 yh
     const float2 dvz = add2(vz, I.nv[2]);
     const float2 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
     const float2 s2 = add2(r2, eps2);
+#if defined(G6_ABLATE) && (G6_ABLATE & 2)
+    float2 rinv = mul2(s2, dup(0.5f));
+#else
     float2 rinv = make_float2(rsqrt_approx(s2.x), rsqrt_approx(s2.y));
+#endif
     if (NEWTON) {
         // y <- y - (y/2)(s2 y^2 - 1)
         const float2 e = fma2(s2, mul2(rinv, rinv), dup(-1.0f));
@@ -251,8 +255,10 @@ k_force_fast(ForceArgs A)
                                       make_float2(f[3].z, f[3].w), make_float2(f[4].z, f[4].w), make_float2(f[5].z, f[5].w),
                                       make_float2(f[6].z, f[6].w), make_float2(f[7].z, f[7].w), make_float2(f[8].z, f[8].w),
                                       make_float2(f[9].z, f[9].w), eps2, rb);
+#if !(defined(G6_ABLATE) && (G6_ABLATE & 1))
                         I[q].rmin = fminf(fminf(ra.x, ra.y), I[q].rmin);
                         I[q].rmin = fminf(fminf(rb.x, rb.y), I[q].rmin);
+#endif
                     }
                 }
 #pragma unroll
