@@ -261,6 +261,7 @@ def main():
 
     g6.g6_open(0)
     g6.g6x_set_npipes(1 << 21)
+    g6.g6x_set_option(0, "timers", 1)                # per-phase CUDA events on the library's stream (off by default)
     if args.newton is not None:
         g6.g6x_set_option(0, "newton", args.newton)
     newton = g6.g6x_get_option(0, "newton")

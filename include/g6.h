@@ -165,9 +165,11 @@ int g6x_get_timers(int clusterid, double us[8]);
  *   "newton"  1 = one Newton step after rsqrt.approx, 0 = none
  *   "jsplit"  0 = automatic; S > 0 forces S j-splits
  *   "kernel"  0 = automatic; 1 = checked reference kernel everywhere; 2 = fast kernel
- *   "timers"  1 (default) record CUDA events per phase
+ *   "timers"  1 = record CUDA events per phase for g6x_get_timers; 0 (default, or env G6_TIMERS) = none:
+ *             the event records cost ~10 us per force call, a third of a small block step
  *   "variant" 0 = automatic; threads*8 + i_per_thread forces a fast-kernel shape (e.g. 128*8+2)
- *   "small"   largest n_i served by the small-block kernel (lanes over j, predictor fused); default 16, 0 = off
+ *   "small"   largest n_i served by the block-step kernel (one launch: j update + predictor + force +
+ *             combine, lanes over j); default 32, at most 64, 0 = off
  * Returns G6_ERR_ARG for an unknown key or value. */
 int g6x_set_option(int clusterid, const char *key, int value);
 int g6x_get_option(int clusterid, const char *key, int *value);

@@ -18,7 +18,7 @@
 #include "g6_device.cuh"
 #include "g6_force_ref.cuh"
 #include "g6_force_fast.cuh"
-#include "g6_force_small.cuh"
+#include "g6_block_step.cuh"
 
 using namespace g6;
 
@@ -42,6 +42,7 @@ struct Cluster {
     int capacity = 0;        // addresses
     int n_stored = 0;        // highest address set + 1
     JStore js{};
+    unsigned int *d_counter = nullptr;   // arrival ticket of the block-step kernel
     float *pred = nullptr;   // predicted tiles
     int *tile_imin = nullptr, *tile_imax = nullptr;
     bool pred_valid = false;
@@ -67,6 +68,7 @@ struct Cluster {
     char *h_iblk = nullptr, *hd_iblk = nullptr, *d_iblk = nullptr;
     char *h_res = nullptr, *hd_res = nullptr, *d_res = nullptr;
     bool res_on_host = false;   // last call's results were written straight into h_res
+    bool iblk_on_device = false;   // last host call left a copy of the i-block in d_iblk
 
     // partial results
     Partials part{};
@@ -88,7 +90,7 @@ struct Cluster {
     int last_ctas = 0, last_S = 0;
 
     // options
-    int opt_ds = 1, opt_newton = 1, opt_jsplit = 0, opt_kernel = 0, opt_timers = 1, opt_variant = 0, opt_small = 16;
+    int opt_ds = 1, opt_newton = 1, opt_jsplit = 0, opt_kernel = 0, opt_timers = 0, opt_variant = 0, opt_small = 32;
 };
 
 Cluster g_cl[MAX_CLUSTERS];
@@ -238,8 +240,7 @@ int ensure_rec(Cluster &c, int n)
 void release(Cluster &c)
 {
     if (c.stream) cudaStreamSynchronize(c.stream);
-    for (int k = 0; k < 3; ++k) { dfree(c.js.x[k]); dfree(c.js.v[k]); dfree(c.js.a2[k]); dfree(c.js.j6[k]); }
-    dfree(c.js.t); dfree(c.js.m); dfree(c.js.idx);
+    dfree(c.js.raw); dfree(c.d_counter);
     dfree(c.pred); dfree(c.tile_imin); dfree(c.tile_imax);
     for (int b = 0; b < 2; ++b) { hfree(c.h_rec[b]); if (c.ev_rec[b]) cudaEventDestroy(c.ev_rec[b]); }
     dfree(c.d_rec);
@@ -341,13 +342,21 @@ int choose_jsplit(int n_itiles, int ntiles, int slots, int ni)
 }
 
 // force + combine (steps a-4, a-5) on device-resident i-blocks; all asynchronous
+// small active blocks take the fused block-step kernel unless an experiment switch pins another path
+bool use_block_step(const Cluster &c, int ni)
+{
+    return ni <= c.opt_small && c.opt_kernel != 1 && c.opt_kernel != 2 && c.opt_jsplit == 0;
+}
+
+struct HostBlock { const double *xi, *vi; const int *index; };   // host copy of the i-block (small blocks travel in kernel parameters)
+
 int run_force(Cluster &c, int nj, int ni, const int *d_index, const double *d_xi, const double *d_vi,
               double eps2, double *d_acc, double *d_jerk, double *d_pot, int *d_nn_index, double *d_nn_r2,
-              cudaEvent_t ev_pred_done, cudaEvent_t ev_force_done)
+              cudaEvent_t ev_pred_done, cudaEvent_t ev_force_done, const HostBlock *hb)
 {
     ForceArgs A{};
     A.pred = c.pred;
-    A.jidx = c.js.idx;
+    A.jraw = c.js.raw;
     A.tile_imin = c.tile_imin;
     A.tile_imax = c.tile_imax;
     A.nj = nj;
@@ -359,37 +368,57 @@ int run_force(Cluster &c, int nj, int ni, const int *d_index, const double *d_xi
     A.eps2 = (float)eps2;
     A.ds = c.opt_ds;
 
-    // small active blocks: lanes over j, predictor fused in (g6_force_small.cuh)
-    if (ni <= c.opt_small && c.opt_kernel != 1 && c.opt_kernel != 2 && c.opt_jsplit == 0) {
-        SmallArgs B{};
-        B.js = c.js;
+    // small active blocks: the whole block step in one kernel (g6_block_step.cuh)
+    if (use_block_step(c, ni)) {
+        // a-1: changed j-particles ride in the kernel parameters when they fit and lie inside the j-range
+        const int maxi_need = std::max(ni, hb ? c.n_rec : 0);
+        bool inline_upd = hb && c.n_rec > 0 && c.n_rec <= BS_MAX_I;
+        if (inline_upd)
+            for (int k = 0; k < c.n_rec; ++k)
+                if (c.h_rec[c.rec_cur][k].addr >= A.ntiles * JT) { inline_upd = false; break; }
+        if (c.n_rec > 0 && !inline_upd) {
+            int rc = flush_j(c);
+            if (rc) return rc;
+        }
+        const bool big = (inline_upd ? maxi_need : ni) > 16;
+        const int per_sm = big ? bs_ctas_per_sm<BS_MAX_I>() : bs_ctas_per_sm<16>();
+        const int G = std::max(1, std::min(A.ntiles, c.n_sm * per_sm));
+        int rc = ensure_partials(c, (size_t)G * ni);
+        if (rc) return rc;
+        BsArgs B{};
+        B.raw = c.js.raw;
         B.ti = c.ti;
-        B.pred = c.pred;
-        B.fused = pred_is_current(c) ? 0 : 1;
         B.nj = nj;
         B.ntiles = A.ntiles;
-        B.i_index = d_index; B.xi = d_xi; B.vi = d_vi;
         B.ni = ni;
+        B.n_upd = inline_upd ? c.n_rec : 0;
         B.eps2 = A.eps2;
         B.ds = c.opt_ds;
-        const int S = A.ntiles;
-        int rc = ensure_partials(c, (size_t)S * ni);
-        if (rc) return rc;
+        B.inline_i = hb ? 1 : 0;
+        B.i_index = d_index; B.xi = d_xi; B.vi = d_vi;
         B.P = c.part;
         B.P.stride_s = 1;
-        B.P.stride_i = S;
-        const int blocks = (A.ntiles + 3) / 4;
+        B.P.stride_i = G;
+        B.counter = c.d_counter;
+        B.acc = d_acc; B.jerk = d_jerk; B.pot = d_pot; B.nn_index = d_nn_index; B.nn_r2 = d_nn_r2;
         if (ev_pred_done) CK(cudaEventRecord(ev_pred_done, c.stream));     // predictor fused: no separate phase
-        if (c.opt_newton) k_force_small<true><<<blocks, 128, 0, c.stream>>>(B);
-        else k_force_small<false><<<blocks, 128, 0, c.stream>>>(B);
-        CK(cudaGetLastError());
+        const JRecord *upd = inline_upd ? c.h_rec[c.rec_cur] : nullptr;
+        rc = big ? bs_launch_t<BS_MAX_I>(B, c.opt_newton != 0, G, hb ? hb->xi : nullptr, hb ? hb->vi : nullptr, hb ? hb->index : nullptr, upd, c.stream)
+                 : bs_launch_t<16>(B, c.opt_newton != 0, G, hb ? hb->xi : nullptr, hb ? hb->vi : nullptr, hb ? hb->index : nullptr, upd, c.stream);
+        if (rc) return fail(c, G6_ERR_CUDA, "block-step kernel launch failed: %s", cudaGetErrorString((cudaError_t)rc));
+        if (inline_upd) {      // the records were copied into the launch: the staging slots are free again
+            for (int k = 0; k < c.n_rec; ++k) c.slot_of_addr[c.h_rec[c.rec_cur][k].addr] = -1;
+            c.n_rec = 0;
+            c.pred_valid = false;
+        }
         if (ev_force_done) CK(cudaEventRecord(ev_force_done, c.stream));
-        if (S > 256) k_combine_block<<<ni, 128, 0, c.stream>>>(B.P, S, ni, c.js.idx, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2);
-        else k_combine_wide<<<(ni + 3) / 4, 128, 0, c.stream>>>(B.P, S, ni, c.js.idx, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2);
-        CK(cudaGetLastError());
-        c.last_ctas = blocks;
-        c.last_S = S;
+        c.last_ctas = G;
+        c.last_S = G;
         return G6_OK;
+    }
+    if (c.n_rec > 0) {         // callers of the sweep path have normally flushed already
+        int rcf = flush_j(c);
+        if (rcf) return rcf;
     }
     int rcp = run_predict(c);
     if (rcp) return rcp;
@@ -423,8 +452,8 @@ int run_force(Cluster &c, int nj, int ni, const int *d_index, const double *d_xi
         CK(cudaGetLastError());
     }
     if (ev_force_done) CK(cudaEventRecord(ev_force_done, c.stream));
-    if (wide) k_combine_wide<<<(ni + 3) / 4, 128, 0, c.stream>>>(A.P, S, ni, c.js.idx, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2);
-    else k_combine<<<(ni + 255) / 256, 256, 0, c.stream>>>(A.P, S, ni, c.js.idx, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2);
+    if (wide) k_combine_wide<<<(ni + 3) / 4, 128, 0, c.stream>>>(A.P, S, ni, c.js.raw, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2);
+    else k_combine<<<(ni + 255) / 256, 256, 0, c.stream>>>(A.P, S, ni, c.js.raw, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2);
     CK(cudaGetLastError());
     c.last_ctas = n_itiles * S;
     c.last_S = S;
@@ -494,16 +523,17 @@ int g6_open(int clusterid)
     int rc = [&]() -> int {
         CK(cudaStreamCreateWithFlags(&c.own_stream, cudaStreamNonBlocking));
         c.stream = c.own_stream;
-        for (int k = 0; k < 3; ++k) {
-            CK(dalloc(c.js.x[k], n)); CK(dalloc(c.js.v[k], n)); CK(dalloc(c.js.a2[k], n)); CK(dalloc(c.js.j6[k], n));
-        }
-        CK(dalloc(c.js.t, n)); CK(dalloc(c.js.m, n)); CK(dalloc(c.js.idx, n));
+        CK(dalloc(c.js.raw, n / JT * RAW_TILE_BYTES));
+        CK(cudaMemsetAsync(c.js.raw, 0, n / JT * RAW_TILE_BYTES, c.stream));
+        CK(dalloc(c.d_counter, 1));
+        CK(cudaMemsetAsync(c.d_counter, 0, sizeof(unsigned int), c.stream));
         CK(dalloc(c.pred, n * NF));
         CK(dalloc(c.tile_imin, n / JT)); CK(dalloc(c.tile_imax, n / JT));
         for (auto &ev : c.ev) CK(cudaEventCreate(&ev));
         for (auto &ev : c.ev_rec) CK(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
         int r = fast_kernel_init();
-        if (r) return fail(c, G6_ERR_CUDA, "fast kernel attribute setup failed: %s", cudaGetErrorString((cudaError_t)r));
+        if (!r) r = bs_kernel_init();
+        if (r) return fail(c, G6_ERR_CUDA, "kernel attribute setup failed: %s", cudaGetErrorString((cudaError_t)r));
         return G6_OK;
     }();
     if (rc != G6_OK) { release(c); return rc; }
@@ -516,6 +546,7 @@ int g6_open(int clusterid)
     c.open = true;
     c.opt_newton = env_int("G6_NEWTON", 1) ? 1 : 0;
     c.opt_kernel = env_int("G6_KERNEL", 0);
+    c.opt_timers = env_int("G6_TIMERS", 0) ? 1 : 0;
     snprintf(c.err, sizeof(c.err), "no error");
     return G6_OK;
 }
@@ -621,7 +652,7 @@ int g6x_calc_dev(int clusterid, int nj, int ni, const int *d_index, const double
     const bool tm = c.opt_timers != 0;
     if (tm) { CK(cudaEventRecord(c.ev[0], c.stream)); CK(cudaEventRecord(c.ev[1], c.stream)); }
     rc = run_force(c, nj, ni, d_index, d_xi, d_vi, eps2, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2, tm ? c.ev[2] : nullptr,
-                   tm ? c.ev[3] : nullptr);
+                   tm ? c.ev[3] : nullptr, nullptr);
     if (rc) return rc;
     if (tm) { CK(cudaEventRecord(c.ev[4], c.stream)); CK(cudaEventRecord(c.ev[5], c.stream)); }
     c.ev_valid = tm;
@@ -643,25 +674,44 @@ int g6calc_firsthalf(int clusterid, int nj, int ni, const int index[], const dou
     if (rc) return rc;
     const bool tm = c.opt_timers != 0;
     if (tm) CK(cudaEventRecord(c.ev[0], c.stream));
-    // a-3: i block to pinned staging (the only per-step H2D payload) ...
-    {
-        const IView hv = iview(c.h_iblk, ni);
-        memcpy((void *)hv.xi, xi, sizeof(double) * 3 * ni);
-        memcpy((void *)hv.vi, vi, sizeof(double) * 3 * ni);
-        memcpy((void *)hv.idx, index, sizeof(int) * ni);
-    }
-    // ... and, together with a-1 (changed j particles), on to the device
-    rc = stage_inputs(c, true, ni);
-    if (rc) return rc;
-    if (tm) CK(cudaEventRecord(c.ev[1], c.stream));
-    // a-2 (inside run_force: separate predictor kernel, or fused into the small-block force kernel), a-4, a-5;
-    // small blocks: the combine kernel writes the results straight into mapped host memory (a-6)
+    const bool bs = use_block_step(c, ni);
     const bool zc_out = ni <= ZC_MAX_I;
-    const IView dv = iview(c.d_iblk, ni);
     const RView out = rview(zc_out ? c.hd_res : c.d_res, ni);
-    rc = run_force(c, nj, ni, dv.idx, dv.xi, dv.vi, eps2, out.acc, out.jerk, out.pot, out.nnidx, out.nnr2, tm ? c.ev[2] : nullptr,
-                   tm ? c.ev[3] : nullptr);
-    if (rc) return rc;
+    if (bs) {
+        // small block: the i-block and the changed j-particles travel inside the kernel launch
+        // (copied from the caller's arrays by the launch itself); results come back through mapped memory
+        if (tm) CK(cudaEventRecord(c.ev[1], c.stream));
+        const HostBlock hb{&xi[0][0], &vi[0][0], index};
+        {   // keep a host copy for the debug read-backs
+            const IView hv = iview(c.h_iblk, ni);
+            memcpy((void *)hv.xi, xi, sizeof(double) * 3 * ni);
+            memcpy((void *)hv.vi, vi, sizeof(double) * 3 * ni);
+            memcpy((void *)hv.idx, index, sizeof(int) * ni);
+        }
+        c.iblk_on_device = false;
+        rc = run_force(c, nj, ni, nullptr, nullptr, nullptr, eps2, out.acc, out.jerk, out.pot, out.nnidx, out.nnr2, tm ? c.ev[2] : nullptr,
+                       tm ? c.ev[3] : nullptr, &hb);
+        if (rc) return rc;
+    } else {
+        // a-3: i block to pinned staging (the only per-step H2D payload) ...
+        {
+            const IView hv = iview(c.h_iblk, ni);
+            memcpy((void *)hv.xi, xi, sizeof(double) * 3 * ni);
+            memcpy((void *)hv.vi, vi, sizeof(double) * 3 * ni);
+            memcpy((void *)hv.idx, index, sizeof(int) * ni);
+        }
+        // ... and, together with a-1 (changed j particles), on to the device
+        rc = stage_inputs(c, true, ni);
+        if (rc) return rc;
+        c.iblk_on_device = true;
+        if (tm) CK(cudaEventRecord(c.ev[1], c.stream));
+        // a-2 (separate predictor kernel), a-4, a-5; blocks up to ZC_MAX_I: the combine kernel writes the
+        // results straight into mapped host memory (a-6)
+        const IView dv = iview(c.d_iblk, ni);
+        rc = run_force(c, nj, ni, dv.idx, dv.xi, dv.vi, eps2, out.acc, out.jerk, out.pot, out.nnidx, out.nnr2, tm ? c.ev[2] : nullptr,
+                       tm ? c.ev[3] : nullptr, nullptr);
+        if (rc) return rc;
+    }
     if (tm) CK(cudaEventRecord(c.ev[4], c.stream));
     // a-6
     if (!zc_out) CK(cudaMemcpyAsync(c.h_res, c.d_res, res_bytes(ni), cudaMemcpyDeviceToHost, c.stream));
@@ -786,7 +836,7 @@ int g6x_set_option(int clusterid, const char *key, int value)
     int *slot = option_slot(c, key);
     if (!slot) return fail(c, G6_ERR_ARG, "unknown option '%s'", key ? key : "(null)");
     const bool is_flag = slot == &c.opt_ds || slot == &c.opt_newton || slot == &c.opt_timers;
-    if (value < 0 || (is_flag && value > 1) || (slot == &c.opt_kernel && value > 2) || (slot == &c.opt_jsplit && value > 65535) || (slot == &c.opt_small && value > SMALL_MAX_I) ||
+    if (value < 0 || (is_flag && value > 1) || (slot == &c.opt_kernel && value > 2) || (slot == &c.opt_jsplit && value > 65535) || (slot == &c.opt_small && value > BS_MAX_I) ||
         (slot == &c.opt_variant && value != 0 && fast_ctas_per_sm(FastVariant{value / 8, value % 8}) < 1))
         return fail(c, G6_ERR_ARG, "bad value %d for option '%s'", value, key);
     *slot = value;
@@ -845,6 +895,10 @@ int g6x_debug_dx(int clusterid, int n, const int ipipe[], const int jaddr[], flo
         CK(dalloc(d_ip, n)); CK(dalloc(d_ja, n)); CK(dalloc(d_out, 3 * (size_t)n));
         CK(cudaMemcpyAsync(d_ip, ipipe, sizeof(int) * n, cudaMemcpyHostToDevice, c.stream));
         CK(cudaMemcpyAsync(d_ja, jaddr, sizeof(int) * n, cudaMemcpyHostToDevice, c.stream));
+        if (!c.iblk_on_device) {
+            CK(cudaMemcpyAsync(c.d_iblk, c.h_iblk, iblk_bytes(c.last_ni), cudaMemcpyHostToDevice, c.stream));
+            c.iblk_on_device = true;
+        }
         k_debug_dx<<<(n + 127) / 128, 128, 0, c.stream>>>(n, d_ip, d_ja, iview(c.d_iblk, c.last_ni).xi, c.opt_ds, c.pred, d_out);
         CK(cudaGetLastError());
         CK(cudaMemcpyAsync(dx, d_out, sizeof(float) * 3 * n, cudaMemcpyDeviceToHost, c.stream));

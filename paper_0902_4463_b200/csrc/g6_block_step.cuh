@@ -1,0 +1,402 @@
+// g6_block_step.cuh -- ONE kernel for the small active blocks of block time steps (n_i <= 64):
+// j-store update + j-predictor + force + combine (steps a-1 .. a-5 of the path) in a single launch.
+//
+// For a handful of i-particles the step is bound by the one pass over the N_j stored particles
+// (76 B each) and by launch/copy latency, not by arithmetic.  The paper's idea for
+// small blocks (fewer i than threads => several threads share an i and split the
+// j) is taken to its limit and the whole block step is fused:
+//
+//  * persistent CTAs (2 per SM), CTA c owns the raw j-tiles c, c+G, c+2G, ...  A raw tile (256
+//    particles x 76 B, g6_device.cuh) is staged global -> shared by ONE TMA bulk copy
+//    (cp.async.bulk + mbarrier complete_tx) into a 3-stage ring, so ~58 KB per CTA are in flight
+//    without costing a register -- that is what keeps HBM busy while the warps compute.
+//  * a-1: the particles corrected in the previous step arrive INSIDE THE KERNEL PARAMETERS (no
+//    staging kernel, no PCIe read); the CTA that owns a particle's tile patches the staged copy
+//    and writes the record through to the j-store.  The i-block travels the same way.
+//  * a-2: the 128 threads predict the tile (Eq. 1-2, same routine as k_predict) into a
+//    double-buffered shared array; nothing predicted ever goes to HBM.
+//  * a-4: LANES OVER j: every lane holds 8 predicted j in registers; warp w loops over the
+//    i-particles w, w+4, ... (broadcast from shared memory) and evaluates its 8 pairs with the
+//    same packed FP32 arithmetic as the sweep kernel (double-single separations, Eq. 3); the 7
+//    sums of a (i, tile) are reduced over the warp by a transposing butterfly (9 shuffles instead
+//    of 35) and folded into fp64 accumulators in shared memory; the nearest neighbour by two
+//    warp-wide integer min-reductions (r2 bits, then address).
+//  * a-5: each CTA writes one partial per i; the LAST CTA to finish (atomic ticket) sums the G
+//    partials in CTA order -- deterministic -- and writes the results, possibly straight into
+//    mapped host memory (a-6).
+// Every pair is checked (address < nj, index_j != index_i, s2 > 0), so eps2 = 0 is served too.
+#pragma once
+#include "g6_force_fast.cuh"
+
+namespace g6 {
+
+constexpr int BS_THREADS = 128;
+constexpr int BS_NSTAGE = 3;
+constexpr int BS_MAX_I = 64;
+
+// i-block and changed j-particles carried by value in the kernel parameters
+template <int MAXI>
+struct BsInline {
+    double xi[MAXI][3];
+    double vi[MAXI][3];
+    int index[MAXI];
+    JRecord upd[MAXI];
+};
+
+struct BsArgs {
+    char *raw;                  // j-store (inline updates are written through)
+    double ti;
+    int nj, ntiles;
+    int ni, n_upd;
+    float eps2;
+    int ds;
+    int inline_i;               // 1: i-block from BsInline, 0: from the device-visible pointers below
+    const int *i_index;
+    const double *xi, *vi;
+    Partials P;                 // [i][cta]: stride_s = 1, stride_i = gridDim.x
+    unsigned int *counter;      // arrival ticket, zero before the launch, reset by the last CTA
+    double *acc, *jerk, *pot;   // results (device or mapped host memory)
+    int *nn_index;
+    double *nn_r2;
+};
+
+template <int MAXI>
+struct BsSmem {
+    alignas(128) char raw[BS_NSTAGE][RAW_TILE_BYTES];
+    alignas(16) float pred[2][NF][JT];
+    alignas(16) int pidx[2][JT];
+    double acc[MAXI][8];
+    float ipart[MAXI][9];
+    int iidx[MAXI];
+    float r2[MAXI];
+    int addr[MAXI];
+    int uaddr[MAXI];
+    alignas(8) uint64_t full[BS_NSTAGE];
+    int is_last;
+};
+
+// two consecutive j against one i, every pair checked.  `ok` in: address < nj && index differs.
+template <bool NEWTON>
+__device__ __forceinline__ void pair2_checked(IPart &I, const float2 xh, const float2 yh, const float2 zh, const float2 xl,
+                                              const float2 yl, const float2 zl, const float2 vx, const float2 vy, const float2 vz,
+                                              float2 m, const float2 eps2, bool ok0, bool ok1, float2 &r2_out)
+{
+    constexpr float INF = __builtin_huge_valf();
+    const float2 dx = add2(add2(xh, I.nxh[0]), add2(xl, I.nxl[0]));      // Eq. 3
+    const float2 dy = add2(add2(yh, I.nxh[1]), add2(yl, I.nxl[1]));
+    const float2 dz = add2(add2(zh, I.nxh[2]), add2(zl, I.nxl[2]));
+    const float2 dvx = add2(vx, I.nv[0]);
+    const float2 dvy = add2(vy, I.nv[1]);
+    const float2 dvz = add2(vz, I.nv[2]);
+    const float2 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+    float2 s2 = add2(r2, eps2);
+    ok0 = ok0 && (s2.x > 0.0f);                                          // DESIGN.md reading 5
+    ok1 = ok1 && (s2.y > 0.0f);
+    s2 = make_float2(ok0 ? s2.x : 1.0f, ok1 ? s2.y : 1.0f);
+    m = make_float2(ok0 ? m.x : 0.0f, ok1 ? m.y : 0.0f);
+    float2 rinv = make_float2(rsqrt_approx(s2.x), rsqrt_approx(s2.y));
+    if (NEWTON) {
+        const float2 e = fma2(s2, mul2(rinv, rinv), dup(-1.0f));
+        rinv = fma2(mul2(dup(-0.5f), rinv), e, rinv);
+    }
+    const float2 rinv2 = mul2(rinv, rinv);
+    const float2 mrinv = mul2(m, rinv);
+    const float2 mrinv3 = mul2(mrinv, rinv2);
+    const float2 rv = fma2(dz, dvz, fma2(dy, dvy, mul2(dx, dvx)));
+    const float2 alpha = mul2(dup(-3.0f), mul2(rv, rinv2));
+    I.p = add2(I.p, mrinv);
+    I.a[0] = fma2(mrinv3, dx, I.a[0]);
+    I.a[1] = fma2(mrinv3, dy, I.a[1]);
+    I.a[2] = fma2(mrinv3, dz, I.a[2]);
+    I.j[0] = fma2(mrinv3, fma2(alpha, dx, dvx), I.j[0]);
+    I.j[1] = fma2(mrinv3, fma2(alpha, dy, dvy), I.j[1]);
+    I.j[2] = fma2(mrinv3, fma2(alpha, dz, dvz), I.j[2]);
+    r2_out = make_float2(ok0 ? r2.x : INF, ok1 ? r2.y : INF);
+}
+
+// Sum 8 per-lane values over the 32 lanes of a warp with 9 shuffles: after the three exchange
+// steps lane L holds quantity q(L) = 4*bit4(L) + 2*bit3(L) + bit2(L), summed over the lanes that
+// share bits 1..0 of L... then two plain butterfly steps finish it.  Fixed tree => reproducible.
+__device__ __forceinline__ float transpose_reduce8(const float (&v)[8], int lane)
+{
+    const unsigned FULL = 0xffffffffu;
+    float w[4], u[2];
+    const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const float send = b4 ? v[k] : v[k + 4];
+        const float keep = b4 ? v[k + 4] : v[k];
+        w[k] = __fadd_rn(keep, __shfl_xor_sync(FULL, send, 16));
+    }
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+        const float send = b3 ? w[k] : w[k + 2];
+        const float keep = b3 ? w[k + 2] : w[k];
+        u[k] = __fadd_rn(keep, __shfl_xor_sync(FULL, send, 8));
+    }
+    const float send = b2 ? u[0] : u[1];
+    const float keep = b2 ? u[1] : u[0];
+    float t = __fadd_rn(keep, __shfl_xor_sync(FULL, send, 4));
+    t = __fadd_rn(t, __shfl_xor_sync(FULL, t, 2));
+    t = __fadd_rn(t, __shfl_xor_sync(FULL, t, 1));
+    return t;
+}
+
+template <int MAXI, bool NEWTON>
+__global__ void __launch_bounds__(BS_THREADS)
+k_block_step(const BsArgs A, const BsInline<MAXI> D)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    BsSmem<MAXI> &sm = *reinterpret_cast<BsSmem<MAXI> *>(smem_raw);
+    constexpr float INF = __builtin_huge_valf();
+    const unsigned FULL = 0xffffffffu;
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const int G = gridDim.x, cta = blockIdx.x;
+    const int nt = cta < A.ntiles ? (A.ntiles - cta + G - 1) / G : 0;     // my tiles: cta, cta+G, ...
+
+    if (tid == 0) {
+#pragma unroll
+        for (int k = 0; k < BS_NSTAGE; ++k) mbar_init(&sm.full[k], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (tid == 0) {
+#pragma unroll
+        for (int k = 0; k < BS_NSTAGE; ++k)
+            if (k < nt) {
+                mbar_expect_tx(&sm.full[k], RAW_TILE_BYTES);
+                tma_load_1d(sm.raw[k], A.raw + (size_t)(cta + k * G) * RAW_TILE_BYTES, RAW_TILE_BYTES, &sm.full[k]);
+            }
+    }
+    // i-block -> shared memory (double-single split here: the host hands fp64)
+    for (int k = tid; k < A.ni * 3; k += BS_THREADS) {
+        const int i = k / 3, c = k % 3;
+        const double x = A.inline_i ? D.xi[i][c] : A.xi[k];
+        const double v = A.inline_i ? D.vi[i][c] : A.vi[k];
+        float hi, lo;
+        ds_split(x, hi, lo);
+        sm.ipart[i][c] = hi;
+        sm.ipart[i][3 + c] = A.ds ? lo : 0.0f;
+        sm.ipart[i][6 + c] = (float)v;
+    }
+    for (int i = tid; i < MAXI; i += BS_THREADS) {
+        if (i < A.ni) sm.iidx[i] = A.inline_i ? D.index[i] : A.i_index[i];
+        sm.r2[i] = INF;
+        sm.addr[i] = 0x7fffffff;
+        sm.uaddr[i] = i < A.n_upd ? D.upd[i].addr : -1;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) sm.acc[i][q] = 0.0;
+    }
+    __syncthreads();
+
+    const float2 eps2 = dup(A.eps2);
+    for (int it = 0; it < nt; ++it) {
+        const int tile = cta + it * G;
+        const int st = it % BS_NSTAGE;
+        const int buf = it & 1;
+        mbar_wait(&sm.full[st], (uint32_t)(it / BS_NSTAGE) & 1u);
+        char *R = sm.raw[st];
+
+        // ---- a-1: particles corrected in the last step that live in this tile
+        if (A.n_upd > 0) {
+            if (tid < A.n_upd && sm.uaddr[tid] / JT == tile) {
+                const JRecord r = D.upd[tid];
+                store_record(R, r.addr % JT, r);
+                store_record(A.raw + (size_t)tile * RAW_TILE_BYTES, r.addr % JT, r);
+            }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            __syncthreads();
+        }
+        // ---- a-2: predict the tile (2 j per thread) into pred[buf]
+#pragma unroll
+        for (int h = 0; h < JT / BS_THREADS; ++h) {
+            const int l = tid + h * BS_THREADS;
+            float f[NF];
+            if (tile * JT + l < A.nj) {
+                const float dt = (float)(A.ti - raw_t(R, l));
+#pragma unroll
+                for (int k = 0; k < 3; ++k)
+                    predict_coord(dt, raw_x(R, k, l), raw_v(R, k, l), raw_a2(R, k, l), raw_j6(R, k, l), A.ds, f[F_XH + k], f[F_XL + k], f[F_V + k]);
+                f[F_M] = raw_m(R, l);
+                sm.pidx[buf][l] = raw_idx(R, l);
+            } else {
+#pragma unroll
+                for (int k = 0; k < NF; ++k) f[k] = 0.0f;
+                sm.pidx[buf][l] = 0;
+            }
+#pragma unroll
+            for (int k = 0; k < NF; ++k) sm.pred[buf][k][l] = f[k];
+        }
+        __syncthreads();
+        // the raw stage is consumed: refill it with the tile NSTAGE ahead
+        if (tid == 0 && it + BS_NSTAGE < nt) {
+            mbar_expect_tx(&sm.full[st], RAW_TILE_BYTES);
+            tma_load_1d(sm.raw[st], A.raw + (size_t)(tile + BS_NSTAGE * G) * RAW_TILE_BYTES, RAW_TILE_BYTES, &sm.full[st]);
+        }
+
+        // ---- a-4: my 8 j (4 lane + [0,4) and 128 + 4 lane + [0,4)) -> registers
+        float4 jf[NF][2];
+        int4 jx[2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+#pragma unroll
+            for (int k = 0; k < NF; ++k) jf[k][h] = reinterpret_cast<const float4 *>(sm.pred[buf][k])[32 * h + lane];
+            jx[h] = reinterpret_cast<const int4 *>(sm.pidx[buf])[32 * h + lane];
+        }
+        const int ja0 = tile * JT + 4 * lane;              // addresses ja0 .. ja0+3 and ja0+128 .. ja0+131
+        for (int i = w; i < A.ni; i += BS_THREADS / 32) {
+            IPart I;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                I.nxh[k] = dup(-sm.ipart[i][k]);
+                I.nxl[k] = dup(-sm.ipart[i][3 + k]);
+                I.nv[k] = dup(-sm.ipart[i][6 + k]);
+                I.a[k] = dup(0.0f);
+                I.j[k] = dup(0.0f);
+            }
+            I.p = dup(0.0f);
+            const int my = sm.iidx[i];
+            float2 r2m[4];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int ja = ja0 + 128 * h;
+                pair2_checked<NEWTON>(I, make_float2(jf[0][h].x, jf[0][h].y), make_float2(jf[1][h].x, jf[1][h].y), make_float2(jf[2][h].x, jf[2][h].y),
+                                      make_float2(jf[3][h].x, jf[3][h].y), make_float2(jf[4][h].x, jf[4][h].y), make_float2(jf[5][h].x, jf[5][h].y),
+                                      make_float2(jf[6][h].x, jf[6][h].y), make_float2(jf[7][h].x, jf[7][h].y), make_float2(jf[8][h].x, jf[8][h].y),
+                                      make_float2(jf[9][h].x, jf[9][h].y), eps2, (ja + 0 < A.nj) && (jx[h].x != my), (ja + 1 < A.nj) && (jx[h].y != my),
+                                      r2m[2 * h]);
+                pair2_checked<NEWTON>(I, make_float2(jf[0][h].z, jf[0][h].w), make_float2(jf[1][h].z, jf[1][h].w), make_float2(jf[2][h].z, jf[2][h].w),
+                                      make_float2(jf[3][h].z, jf[3][h].w), make_float2(jf[4][h].z, jf[4][h].w), make_float2(jf[5][h].z, jf[5][h].w),
+                                      make_float2(jf[6][h].z, jf[6][h].w), make_float2(jf[7][h].z, jf[7][h].w), make_float2(jf[8][h].z, jf[8][h].w),
+                                      make_float2(jf[9][h].z, jf[9][h].w), eps2, (ja + 2 < A.nj) && (jx[h].z != my), (ja + 3 < A.nj) && (jx[h].w != my),
+                                      r2m[2 * h + 1]);
+            }
+            // the 7 sums of this (i, tile): FP32 tree over the 256 j, then fp64 (reading 9)
+            const float v8[8] = {__fadd_rn(I.a[0].x, I.a[0].y), __fadd_rn(I.a[1].x, I.a[1].y), __fadd_rn(I.a[2].x, I.a[2].y),
+                                 __fadd_rn(I.j[0].x, I.j[0].y), __fadd_rn(I.j[1].x, I.j[1].y), __fadd_rn(I.j[2].x, I.j[2].y),
+                                 __fadd_rn(I.p.x, I.p.y), 0.0f};
+            const float tot = transpose_reduce8(v8, lane);
+            if ((lane & 3) == 0) sm.acc[i][lane >> 2] += (double)tot;
+            // nearest neighbour: min r2 over the warp (non-negative floats order like unsigned integers)
+            float lmin = fminf(fminf(r2m[0].x, r2m[0].y), fminf(r2m[1].x, r2m[1].y));
+            lmin = fminf(lmin, fminf(fminf(r2m[2].x, r2m[2].y), fminf(r2m[3].x, r2m[3].y)));
+            const unsigned gbits = __reduce_min_sync(FULL, __float_as_uint(lmin));
+            if (gbits < __float_as_uint(sm.r2[i])) {        // strict: earlier tiles (lower addresses) keep ties
+                int cand = 0x7fffffff;
+                if (__float_as_uint(r2m[3].y) == gbits) cand = ja0 + 128 + 3;
+                if (__float_as_uint(r2m[3].x) == gbits) cand = ja0 + 128 + 2;
+                if (__float_as_uint(r2m[2].y) == gbits) cand = ja0 + 128 + 1;
+                if (__float_as_uint(r2m[2].x) == gbits) cand = ja0 + 128 + 0;
+                if (__float_as_uint(r2m[1].y) == gbits) cand = ja0 + 3;
+                if (__float_as_uint(r2m[1].x) == gbits) cand = ja0 + 2;
+                if (__float_as_uint(r2m[0].y) == gbits) cand = ja0 + 1;
+                if (__float_as_uint(r2m[0].x) == gbits) cand = ja0 + 0;
+                const int gaddr = __reduce_min_sync(FULL, cand);
+                __syncwarp();
+                if (lane == 0) { sm.r2[i] = __uint_as_float(gbits); sm.addr[i] = gaddr; }
+            }
+            __syncwarp();
+        }
+    }
+    __syncthreads();
+
+    // ---- a-5, first half: one partial per (i, CTA)
+    for (int i = tid; i < A.ni; i += BS_THREADS) {
+        const size_t o = (size_t)cta * A.P.stride_s + (size_t)i * A.P.stride_i;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { A.P.acc[k][o] = sm.acc[i][k]; A.P.jrk[k][o] = sm.acc[i][3 + k]; }
+        A.P.pot[o] = -sm.acc[i][6];
+        const bool has = sm.addr[i] != 0x7fffffff;
+        A.P.nn_r2[o] = has ? sm.r2[i] : INF;
+        A.P.nn_addr[o] = has ? sm.addr[i] : -1;
+    }
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) {
+        const unsigned ticket = atomicAdd(A.counter, 1u);
+        sm.is_last = (ticket == (unsigned)G - 1u);
+    }
+    __syncthreads();
+    if (!sm.is_last) return;
+    __threadfence();
+
+    // ---- a-5, second half (last CTA only): sum the G partials of every i in CTA order
+    for (int i = w; i < A.ni; i += BS_THREADS / 32) {
+        double v[7] = {0, 0, 0, 0, 0, 0, 0};
+        float best = INF;
+        int baddr = 0x7fffffff;
+        for (int s = lane; s < G; s += 32) {
+            const size_t o = (size_t)s * A.P.stride_s + (size_t)i * A.P.stride_i;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) { v[k] += __ldcg(A.P.acc[k] + o); v[3 + k] += __ldcg(A.P.jrk[k] + o); }
+            v[6] += __ldcg(A.P.pot + o);
+            const float r2 = __ldcg(A.P.nn_r2 + o);
+            const int ad = __ldcg(A.P.nn_addr + o);
+            if (ad >= 0 && (r2 < best || (r2 == best && ad < baddr))) { best = r2; baddr = ad; }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+            for (int k = 0; k < 7; ++k) v[k] += __shfl_xor_sync(FULL, v[k], o);
+            const float r2 = __shfl_xor_sync(FULL, best, o);
+            const int ad = __shfl_xor_sync(FULL, baddr, o);
+            if (r2 < best || (r2 == best && ad < baddr)) { best = r2; baddr = ad; }
+        }
+        if (lane == 0) {
+#pragma unroll
+            for (int k = 0; k < 3; ++k) { A.acc[3 * (size_t)i + k] = v[k]; A.jerk[3 * (size_t)i + k] = v[3 + k]; }
+            A.pot[i] = v[6];
+            const bool has = baddr != 0x7fffffff;
+            if (A.nn_index) A.nn_index[i] = has ? j_index(A.raw, baddr) : -1;
+            if (A.nn_r2) A.nn_r2[i] = has ? (double)best : (double)INF;
+        }
+    }
+    if (tid == 0) *A.counter = 0u;
+}
+
+// ---------------------------------------------------------------- host side
+template <int MAXI>
+inline int bs_attr()
+{
+    const int bytes = (int)sizeof(BsSmem<MAXI>);
+    cudaError_t e = cudaFuncSetAttribute(k_block_step<MAXI, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e != cudaSuccess) return (int)e;
+    return (int)cudaFuncSetAttribute(k_block_step<MAXI, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+}
+
+inline int bs_kernel_init()
+{
+    int r;
+    if ((r = bs_attr<16>())) return r;
+    return bs_attr<BS_MAX_I>();
+}
+
+template <int MAXI>
+inline int bs_ctas_per_sm()
+{
+    static int n = 0;
+    if (!n) {
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_block_step<MAXI, true>, BS_THREADS, sizeof(BsSmem<MAXI>)) != cudaSuccess || n < 1) n = 1;
+    }
+    return n;
+}
+
+// `src`: the host-side i-block and update records to carry in the parameters (NULL pointers: none)
+template <int MAXI>
+inline int bs_launch_t(const BsArgs &A, bool newton, int grid, const double *xi, const double *vi, const int *index,
+                       const JRecord *upd, cudaStream_t st)
+{
+    static BsInline<MAXI> D;       // one host thread per library (g6.h); filled per call, copied by the launch
+    if (A.inline_i) {
+        memcpy(D.xi, xi, sizeof(double) * 3 * A.ni);
+        memcpy(D.vi, vi, sizeof(double) * 3 * A.ni);
+        memcpy(D.index, index, sizeof(int) * A.ni);
+    }
+    if (A.n_upd > 0) memcpy(D.upd, upd, sizeof(JRecord) * A.n_upd);
+    const size_t bytes = sizeof(BsSmem<MAXI>);
+    if (newton) k_block_step<MAXI, true><<<grid, BS_THREADS, bytes, st>>>(A, D);
+    else k_block_step<MAXI, false><<<grid, BS_THREADS, bytes, st>>>(A, D);
+    return (int)cudaGetLastError();
+}
+
+}  // namespace g6

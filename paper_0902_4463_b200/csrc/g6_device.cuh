@@ -11,18 +11,47 @@
 
 namespace g6 {
 
-// ---- j-particle store (raw Hermite state at t_j), structure of arrays --------------------
+// ---- j-particle store (raw Hermite state at t_j): tiles of JT particles, field-major in a tile --
 // "Only the position is stored in DP, whereas the rest of the terms are stored in SP".
-// 8*3 + 8 + 4*(3+3+3+1) + 4 = 76 bytes per particle.
+// Tile k = RAW_TILE_BYTES bytes at raw + k * RAW_TILE_BYTES:
+//   x[3][JT] f64 | t[JT] f64 | v[3][JT] f32 | a/2[3][JT] f32 | j/6[3][JT] f32 | m[JT] f32 | index[JT] i32
+// = 76 B per particle, 19 456 B per tile, 16-byte aligned: ONE 1-D TMA bulk copy stages the whole raw
+// tile in shared memory (block-step kernel, g6_block_step.cuh); consecutive lanes touching
+// consecutive j of one field are coalesced (predictor, scatter).
+constexpr int JT = 256;
+constexpr int RAW_X = 0;                       // byte offsets inside a raw tile
+constexpr int RAW_T = RAW_X + 3 * JT * 8;
+constexpr int RAW_V = RAW_T + JT * 8;
+constexpr int RAW_A2 = RAW_V + 3 * JT * 4;
+constexpr int RAW_J6 = RAW_A2 + 3 * JT * 4;
+constexpr int RAW_M = RAW_J6 + 3 * JT * 4;
+constexpr int RAW_IDX = RAW_M + JT * 4;
+constexpr int RAW_TILE_BYTES = RAW_IDX + JT * 4;
+static_assert(RAW_TILE_BYTES == 76 * JT && RAW_TILE_BYTES % 16 == 0, "raw tile layout");
+
 struct JStore {
-    double *x[3];   // position at t_j, fp64
-    double *t;      // t_j
-    float *v[3];    // velocity
-    float *a2[3];   // acc / 2      (GRAPE convention, kept as handed in)
-    float *j6[3];   // jerk / 6
-    float *m;       // mass
-    int *idx;       // caller's particle id
+    char *raw;   // capacity / JT raw tiles
 };
+
+// pointers to the fields of particle `a` (k = coordinate)
+__host__ __device__ __forceinline__ char *raw_tile(char *raw, int a) { return raw + (size_t)(a / JT) * RAW_TILE_BYTES; }
+__device__ __forceinline__ double &raw_x(char *tile, int k, int l) { return reinterpret_cast<double *>(tile + RAW_X)[k * JT + l]; }
+__device__ __forceinline__ double &raw_t(char *tile, int l) { return reinterpret_cast<double *>(tile + RAW_T)[l]; }
+__device__ __forceinline__ float &raw_v(char *tile, int k, int l) { return reinterpret_cast<float *>(tile + RAW_V)[k * JT + l]; }
+__device__ __forceinline__ float &raw_a2(char *tile, int k, int l) { return reinterpret_cast<float *>(tile + RAW_A2)[k * JT + l]; }
+__device__ __forceinline__ float &raw_j6(char *tile, int k, int l) { return reinterpret_cast<float *>(tile + RAW_J6)[k * JT + l]; }
+__device__ __forceinline__ float &raw_m(char *tile, int l) { return reinterpret_cast<float *>(tile + RAW_M)[l]; }
+__device__ __forceinline__ int &raw_idx(char *tile, int l) { return reinterpret_cast<int *>(tile + RAW_IDX)[l]; }
+// the caller's index of j address `a`
+__device__ __forceinline__ int j_index(const char *raw, int a)
+{
+    return __ldg(reinterpret_cast<const int *>(raw + (size_t)(a / JT) * RAW_TILE_BYTES + RAW_IDX) + (a % JT));
+}
+// the 256 indices of tile t (16-byte aligned)
+__device__ __forceinline__ const int *tile_indices(const char *raw, int t)
+{
+    return reinterpret_cast<const int *>(raw + (size_t)t * RAW_TILE_BYTES + RAW_IDX);
+}
 
 // one j-particle on its way host -> device (g6_set_j_particle staging); 80 bytes
 struct JRecord {
@@ -34,11 +63,25 @@ struct JRecord {
     int addr;
 };
 
+// write one record into slot l of a raw tile (global or shared memory)
+__device__ __forceinline__ void store_record(char *T, int l, const JRecord &r)
+{
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        raw_x(T, k, l) = r.x[k];
+        raw_v(T, k, l) = r.v[k];
+        raw_a2(T, k, l) = r.a2[k];
+        raw_j6(T, k, l) = r.j6[k];
+    }
+    raw_t(T, l) = r.t;
+    raw_m(T, l) = r.m;
+    raw_idx(T, l) = r.idx;
+}
+
 // ---- predicted j-particles: tiles of JT particles, field-major inside a tile --------------
 // tile k = floats [k*JT*NF, (k+1)*JT*NF): x_hi[JT] y_hi z_hi x_lo y_lo z_lo vx vy vz m.
 // One contiguous 10 KiB block per tile = one TMA bulk copy into shared memory; consecutive
 // lanes reading consecutive j are coalesced; LDS.128 yields four consecutive j of one field.
-constexpr int JT = 256;
 constexpr int NF = 10;
 constexpr int F_XH = 0, F_XL = 3, F_V = 6, F_M = 9;
 constexpr int TILE_FLOATS = JT * NF;
@@ -84,17 +127,19 @@ k_store_from_f64(JStore S, int addr0, int n, const int *__restrict__ index, cons
 {
     int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= n) return;
-    int a = addr0 + p;
+    const int a = addr0 + p;
+    char *T = raw_tile(S.raw, a);
+    const int l = a % JT;
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-        S.x[k][a] = x[3 * (size_t)p + k];
-        S.v[k][a] = (float)v[3 * (size_t)p + k];
-        S.a2[k][a] = (float)(acc[3 * (size_t)p + k] * 0.5);
-        S.j6[k][a] = (float)(jerk[3 * (size_t)p + k] / 6.0);
+        raw_x(T, k, l) = x[3 * (size_t)p + k];
+        raw_v(T, k, l) = (float)v[3 * (size_t)p + k];
+        raw_a2(T, k, l) = (float)(acc[3 * (size_t)p + k] * 0.5);
+        raw_j6(T, k, l) = (float)(jerk[3 * (size_t)p + k] / 6.0);
     }
-    S.t[a] = tj[p];
-    S.m[a] = (float)mass[p];
-    S.idx[a] = index[p];
+    raw_t(T, l) = tj[p];
+    raw_m(T, l) = (float)mass[p];
+    raw_idx(T, l) = index[p];
 }
 
 // ---- a-1 + a-3: scatter of the particles changed since the last force call, and the i block -----
@@ -108,17 +153,8 @@ k_stage(JStore S, const JRecord *__restrict__ rec, int n_rec, int n_i, const dou
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p < n_rec) {
         const JRecord r = rec[p];
-        const int a = r.addr;
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            S.x[k][a] = r.x[k];
-            S.v[k][a] = r.v[k];
-            S.a2[k][a] = r.a2[k];
-            S.j6[k][a] = r.j6[k];
-        }
-        S.t[a] = r.t;
-        S.m[a] = r.m;
-        S.idx[a] = r.idx;
+        char *T = raw_tile(S.raw, r.addr);
+        store_record(T, r.addr % JT, r);
     }
     if (p < n_i) {
 #pragma unroll
@@ -128,6 +164,19 @@ k_stage(JStore S, const JRecord *__restrict__ rec, int n_rec, int n_i, const dou
         }
         idx_dst[p] = idx_src[p];
     }
+}
+
+// Eq. 1-2 for one coordinate (reading 11): FP32 Horner increment, fp64 add to x0, DS re-split
+__device__ __forceinline__ void predict_coord(float dt, double x0, float v0, float a2, float j6, int ds,
+                                              float &xh, float &xl, float &vp)
+{
+    // dx = dt (v0 + dt (a0/2 + dt j0/6))
+    const float d = __fmul_rn(dt, __fmaf_rn(dt, __fmaf_rn(dt, j6, a2), v0));
+    const double xp = x0 + (double)d;
+    ds_split(xp, xh, xl);
+    if (!ds) xl = 0.0f;
+    // v_p = v0 + dt (a0 + dt j0/2) = v0 + dt (2 (a0/2) + 3 dt (j0/6))
+    vp = __fmaf_rn(dt, __fmaf_rn(__fmul_rn(3.0f, dt), j6, __fadd_rn(a2, a2)), v0);
 }
 
 // ---- a-2: predictor, one thread per j, one CTA per tile ------------------------------------
@@ -147,23 +196,13 @@ k_predict(JStore S, int n_stored, double ti, int ds, float *__restrict__ pred,
     float f[NF];
     int id_lo = INT32_MAX, id_hi = INT32_MIN;
     if (j < n_stored) {
-        const float dt = (float)(ti - S.t[j]);
-        const float dt3 = 3.0f * dt;
+        char *T = S.raw + (size_t)tile * RAW_TILE_BYTES;
+        const float dt = (float)(ti - raw_t(T, l));
 #pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            const float v0 = S.v[k][j], a2 = S.a2[k][j], j6 = S.j6[k][j];
-            // dx = dt (v0 + dt (a0/2 + dt j0/6))
-            const float d = __fmul_rn(dt, __fmaf_rn(dt, __fmaf_rn(dt, j6, a2), v0));
-            const double xp = S.x[k][j] + (double)d;
-            float hi, lo;
-            ds_split(xp, hi, lo);
-            f[F_XH + k] = hi;
-            f[F_XL + k] = ds ? lo : 0.0f;
-            // v_p = v0 + dt (a0 + dt j0/2) = v0 + dt (2 (a0/2) + 3 dt (j0/6))
-            f[F_V + k] = __fmaf_rn(dt, __fmaf_rn(dt3, j6, __fadd_rn(a2, a2)), v0);
-        }
-        f[F_M] = S.m[j];
-        id_lo = id_hi = S.idx[j];
+        for (int k = 0; k < 3; ++k)
+            predict_coord(dt, raw_x(T, k, l), raw_v(T, k, l), raw_a2(T, k, l), raw_j6(T, k, l), ds, f[F_XH + k], f[F_XL + k], f[F_V + k]);
+        f[F_M] = raw_m(T, l);
+        id_lo = id_hi = raw_idx(T, l);
     } else {
 #pragma unroll
         for (int k = 0; k < NF; ++k) f[k] = 0.0f;      // padding of the last tile: finite, massless
@@ -194,7 +233,7 @@ k_predict(JStore S, int n_stored, double ti, int ds, float *__restrict__ pred,
 // (PAPER.md:106).  Sums in fp64 in split order; nearest neighbour: smallest r2, ties -> lowest
 // split = lowest j address (reading 7); address -> caller's index.
 __global__ void __launch_bounds__(256)
-k_combine(Partials P, int S, int ni, const int *__restrict__ jidx,
+k_combine(Partials P, int S, int ni, const char *__restrict__ jraw,
           double *__restrict__ acc, double *__restrict__ jerk, double *__restrict__ pot,
           int *__restrict__ nn_index, double *__restrict__ nn_r2)
 {
@@ -215,7 +254,7 @@ k_combine(Partials P, int S, int ni, const int *__restrict__ jidx,
 #pragma unroll
     for (int k = 0; k < 3; ++k) { acc[3 * (size_t)i + k] = a[k]; jerk[3 * (size_t)i + k] = jk[k]; }
     pot[i] = ph;
-    if (nn_index) nn_index[i] = baddr >= 0 ? jidx[baddr] : -1;
+    if (nn_index) nn_index[i] = baddr >= 0 ? j_index(jraw, baddr) : -1;
     if (nn_r2) nn_r2[i] = baddr >= 0 ? (double)best : (double)__int_as_float(0x7f800000);
 }
 
@@ -224,7 +263,7 @@ k_combine(Partials P, int S, int ni, const int *__restrict__ jidx,
 // fixed by (S) alone, so results are bit-reproducible.  Nearest neighbour: (r2, address)
 // lexicographic minimum = smallest r2, ties -> smallest address.
 __global__ void __launch_bounds__(128)
-k_combine_wide(Partials P, int S, int ni, const int *__restrict__ jidx,
+k_combine_wide(Partials P, int S, int ni, const char *__restrict__ jraw,
                double *__restrict__ acc, double *__restrict__ jerk, double *__restrict__ pot,
                int *__restrict__ nn_index, double *__restrict__ nn_r2)
 {
@@ -256,7 +295,7 @@ k_combine_wide(Partials P, int S, int ni, const int *__restrict__ jidx,
         for (int k = 0; k < 3; ++k) { acc[3 * (size_t)i + k] = v[k]; jerk[3 * (size_t)i + k] = v[3 + k]; }
         pot[i] = v[6];
         const bool has = baddr != 0x7fffffff;
-        if (nn_index) nn_index[i] = has ? jidx[baddr] : -1;
+        if (nn_index) nn_index[i] = has ? j_index(jraw, baddr) : -1;
         if (nn_r2) nn_r2[i] = has ? (double)best : (double)__int_as_float(0x7f800000);
     }
 }
@@ -265,7 +304,7 @@ k_combine_wide(Partials P, int S, int ni, const int *__restrict__ jidx,
 // Thread t sums s = t, t+128, ... in order; fixed xor tree inside each warp; the four warp sums are
 // added in warp order by thread 0.
 __global__ void __launch_bounds__(128)
-k_combine_block(Partials P, int S, int ni, const int *__restrict__ jidx,
+k_combine_block(Partials P, int S, int ni, const char *__restrict__ jraw,
                 double *__restrict__ acc, double *__restrict__ jerk, double *__restrict__ pot,
                 int *__restrict__ nn_index, double *__restrict__ nn_r2)
 {
@@ -312,7 +351,7 @@ k_combine_block(Partials P, int S, int ni, const int *__restrict__ jidx,
         for (int k = 0; k < 3; ++k) { acc[3 * (size_t)i + k] = v[k]; jerk[3 * (size_t)i + k] = v[3 + k]; }
         pot[i] = v[6];
         const bool has = baddr != 0x7fffffff;
-        if (nn_index) nn_index[i] = has ? jidx[baddr] : -1;
+        if (nn_index) nn_index[i] = has ? j_index(jraw, baddr) : -1;
         if (nn_r2) nn_r2[i] = has ? (double)best : (double)__int_as_float(0x7f800000);
     }
 }

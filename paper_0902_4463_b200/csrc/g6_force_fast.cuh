@@ -267,7 +267,8 @@ k_force_fast(ForceArgs A)
             }
         } else {
             // checked tile: mask out j >= nj and index_j == index_i (mass -> 0, r2 -> +inf)
-            const int4 *JX = reinterpret_cast<const int4 *>(A.jidx + (size_t)t * JT);
+            const int *JI = tile_indices(A.jraw, t);
+            const int4 *JX = reinterpret_cast<const int4 *>(JI);
 #pragma unroll 1
             for (int l4 = 0; l4 < JT / 4; ++l4) {
                 float4 f[NF];
@@ -277,9 +278,9 @@ k_force_fast(ForceArgs A)
                 int4 jx = make_int4(0, 0, 0, 0);
                 if (j0 + 3 < A.nj) jx = __ldg(JX + l4);
                 else {
-                    if (j0 + 0 < A.nj) jx.x = __ldg(A.jidx + j0 + 0);
-                    if (j0 + 1 < A.nj) jx.y = __ldg(A.jidx + j0 + 1);
-                    if (j0 + 2 < A.nj) jx.z = __ldg(A.jidx + j0 + 2);
+                    if (j0 + 0 < A.nj) jx.x = __ldg(JI + 4 * l4 + 0);
+                    if (j0 + 1 < A.nj) jx.y = __ldg(JI + 4 * l4 + 1);
+                    if (j0 + 2 < A.nj) jx.z = __ldg(JI + 4 * l4 + 2);
                 }
 #pragma unroll
                 for (int q = 0; q < IT; ++q) {
@@ -346,7 +347,7 @@ k_force_fast(ForceArgs A)
                     const float dz = __fadd_rn(__fadd_rn(xs[2][l], I[q].nxh[2].x), __fadd_rn(xs[5][l], I[q].nxl[2].x));
                     r2[4 * h + l] = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
                     const int ja = j0 + 4 * h + l;
-                    jx[4 * h + l] = ja < A.nj ? __ldg(A.jidx + ja) : my[q];
+                    jx[4 * h + l] = ja < A.nj ? j_index(A.jraw, ja) : my[q];
                 }
             }
 #pragma unroll

@@ -12,7 +12,7 @@ namespace g6 {
 
 struct ForceArgs {
     const float *pred;        // predicted j tiles
-    const int *jidx;          // caller's index of every j address (JStore.idx)
+    const char *jraw;         // raw j-store tiles (for the caller's index of every j address)
     const int *tile_imin;     // per-tile index range (from the predictor)
     const int *tile_imax;
     int nj;                   // j addresses [0, nj)
@@ -67,7 +67,7 @@ k_force_ref(ForceArgs A)
         for (int k = tid; k < TILE_FLOATS; k += REF_THREADS) sj[k] = g[k];
         for (int k = tid; k < JT; k += REF_THREADS) {
             int ja = t * JT + k;
-            sidx[k] = ja < A.nj ? A.jidx[ja] : 0;
+            sidx[k] = ja < A.nj ? j_index(A.jraw, ja) : 0;
         }
         __syncthreads();
 

@@ -15,12 +15,13 @@ def cluster():
     build.build()
     g6.g6_open(0)
     g6.g6x_set_npipes(1 << 21)
+    g6.g6x_set_option(0, "timers", 1)          # off by default (two event records per phase cost ~10 us a step)
     yield 0
     g6.g6_close(0)
     g6.g6x_set_npipes(256)
 
 
-KERNELS = [0, 1, 2]       # 0 = automatic (small-block kernel for n_i <= 16), 1 = checked reference kernel, 2 = fast kernel (FFMA2 + TMA)
+KERNELS = [0, 1, 2]       # 0 = automatic (block-step kernel for n_i <= 32), 1 = checked reference kernel, 2 = fast kernel (FFMA2 + TMA)
 
 
 # ------------------------------------------------------------------ C1: every particle
@@ -201,7 +202,7 @@ def test_eps2_zero_and_coincident_particles(cluster, oracle):
         assert got["nn_index"][20] == 400 == ref["nn_index"][20]
 
 
-# ------------------------------------------------------------------ small-block kernel (lanes over j, predictor fused)
+# ------------------------------------------------------------------ block-step kernel (one launch: update + predictor + force + combine)
 @pytest.mark.parametrize("n,ni,small", [(5000, 1, 16), (5000, 7, 16), (5000, 16, 16), (1000, 64, 64), (300, 33, 64), (40000, 3, 16)])
 def test_small_block_kernel_fused_predictor(cluster, oracle, n, ni, small):
     """n_i <= `small`: one pass over the raw j-store, Eq. 1-2 evaluated on the fly, t_i != t_j, the
@@ -220,14 +221,14 @@ def test_small_block_kernel_fused_predictor(cluster, oracle, n, ni, small):
     g6.g6x_set_option(0, "small", small)
     got = g6.force_host(0, idx[block], xo[block], vo[block], eps2, n)
     tm = g6.g6x_get_timers(0)
-    assert tm["jsplits"] == (n + 255) // 256               # one partial result per j-tile: the small kernel ran
+    assert tm["jsplits"] == tm["force_ctas"] <= (n + 255) // 256   # one partial per persistent CTA: the block-step kernel ran
     again = g6.force_host(0, idx[block], xo[block], vo[block], eps2, n)
     for k in got:
         assert np.array_equal(got[k], again[k]), k          # bit-reproducible
     g6.g6x_set_option(0, "kernel", 2)                        # the two-kernel path: predictor, then the fast kernel
     two = g6.force_host(0, idx[block], xo[block], vo[block], eps2, n)
     g6.g6x_set_option(0, "kernel", 0)
-    g6.g6x_set_option(0, "small", 16)
+    g6.g6x_set_option(0, "small", 32)
     if ni >= 16:
         check_forces(got, ref, f"small n={n} ni={ni}")
     assert rel_err(got["acc"], ref["acc"]).max() <= 1e-5 and rel_err(got["jerk"], ref["jerk"]).max() <= 1e-4
@@ -237,6 +238,48 @@ def test_small_block_kernel_fused_predictor(cluster, oracle, n, ni, small):
     # a second call at the same time reuses nothing stale: predicted positions read back are current
     xp, vp = g6.g6x_get_predicted(0, 0, n)
     assert np.abs(xp - xo).max() < 1e-7
+
+
+@pytest.mark.parametrize("n,ni", [(5000, 1), (5000, 5), (3000, 16), (70000, 32), (900, 64)])
+def test_block_step_cycle_with_j_updates(cluster, oracle, n, ni):
+    """The production cycle (SURVEY.md call stack 1): g6_set_j_particle for the n_i particles corrected in the
+    last step, g6_set_ti, firsthalf/lasthalf of the next block.  With n_i <= 32 the changed records ride in
+    the launch of the block-step kernel (a-1 fused); they must act in THAT call, persist in the j-store
+    for later calls, and agree with the staged path (kernel = 2) bit for bit in what is stored."""
+    x, v, m, _ = inputs.config("C2", n=n)
+    eps2 = 1e-8
+    rng = np.random.default_rng(1000 + ni)
+    idx = rng.permutation(n).astype(np.int32)
+    tj, dtj, a0, j0 = inputs.taylor_state(n, 200 + ni, dt_max=2.0**-6)
+    load_j(x, v, m, index=idx, t=tj, acc=a0, jerk=j0)
+    g6.g6x_set_option(0, "small", 64)
+    t = 2.0**-8
+    for step in range(3):
+        # "correct" a block: new state at time t for ni particles (addresses spread over tiles, one in the last, ragged tile)
+        blk = np.sort(rng.choice(n - 1, ni - 1, replace=False)) if ni > 1 else np.array([], dtype=int)
+        blk = np.append(blk, n - 1).astype(int)
+        x[blk] += 1e-3 * rng.standard_normal((ni, 3)); v[blk] += 1e-3 * rng.standard_normal((ni, 3))
+        a0[blk] = rng.standard_normal((ni, 3)); j0[blk] = rng.standard_normal((ni, 3)); tj[blk] = t
+        for p in blk:
+            g6.g6_set_j_particle(0, int(p), int(idx[p]), tj[p], dtj[p], m[p], None, j0[p] / 6, a0[p] / 2, v[p], x[p])
+        t += 2.0**-9
+        g6.g6_set_ti(0, t)
+        xo, vo = oracle.predict(t, tj, x, v, a0, j0)
+        nxt = np.sort(rng.choice(n, ni, replace=False))
+        nxt[0] = blk[0]                                     # a just-updated particle is also active next
+        ref = oracle.force(idx[nxt], xo[nxt], vo[nxt], idx, xo, vo, m, eps2)
+        got = g6.force_host(0, idx[nxt], xo[nxt], vo[nxt], eps2, n)
+        assert rel_err(got["acc"], ref["acc"]).max() <= 1e-5 and rel_err(got["jerk"], ref["jerk"]).max() <= 1e-4
+        assert rel_err(got["pot"], ref["pot"]).max() <= 1e-6
+        check_nn(got["nn_index"], ref, idx, xo[nxt], xo)
+        # the j-store now holds the updates: the two-kernel path sees the same particles
+        g6.g6x_set_option(0, "kernel", 2)
+        two = g6.force_host(0, idx[nxt], xo[nxt], vo[nxt], eps2, n)
+        g6.g6x_set_option(0, "kernel", 0)
+        assert rel_err(got["acc"], two["acc"]).max() < 2e-6 and np.array_equal(got["nn_index"], two["nn_index"])
+        xp, vp = g6.g6x_get_predicted(0, 0, n)
+        assert np.abs(xp - xo).max() < 1e-7 and np.abs(vp - vo).max() < 1e-5
+    g6.g6x_set_option(0, "small", 32)
 
 
 # ------------------------------------------------------------------ P11: Eq. 3 bit for bit
