@@ -425,7 +425,8 @@ int run_force(Cluster &c, int nj, int ni, const int *d_index, const double *d_xi
     if (ev_pred_done) CK(cudaEventRecord(ev_pred_done, c.stream));
 
     // kernel choice: the fast kernel needs a normal FP32 eps2 > 0 (its unchecked tiles rely on s2 > 0)
-    const bool fast_ok = A.eps2 >= std::numeric_limits<float>::min() && std::isfinite(A.eps2);
+    // (the kernel works on eps2 / 3, which must stay a normal float too)
+    const bool fast_ok = A.eps2 >= 4.0f * std::numeric_limits<float>::min() && std::isfinite(A.eps2);
     const bool use_fast = (c.opt_kernel == 2 || c.opt_kernel == 0) && fast_ok && fast_available();
 
     const FastVariant fv = fast_pick(ni, c.n_sm, c.opt_variant);

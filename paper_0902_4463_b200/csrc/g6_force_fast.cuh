@@ -81,6 +81,8 @@ __device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a
 __device__ __forceinline__ float2 mul2(float2 a, float2 b) { return __fmul2_rn(a, b); }
 __device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
 
+constexpr float THIRD = 0.333333343267440796f;     // RN32(1/3)
+
 // per-i-particle register state
 struct IPart {
     float2 nxh[3], nxl[3], nv[3];   // NEGATED hi/lo position words and velocity, duplicated
@@ -88,12 +90,12 @@ struct IPart {
     float rmin;                     // min unsoftened r2 so far (over this CTA's j-range)
 };
 
-// One i-particle against two consecutive j-particles (packed lanes).  34 FMA-pipe packed
+// One i-particle against two consecutive j-particles (packed lanes).  33 FMA-pipe packed
 // instructions (+4 with the Newton step), 2 MUFU, 1 FMNMX3.  MASKED: m and r2 already masked.
 template <bool NEWTON>
 __device__ __forceinline__ void pair2(IPart &I, const float2 xh, const float2 yh, const float2 zh, const float2 xl,
                                       const float2 yl, const float2 zl, const float2 vx, const float2 vy, const float2 vz,
-                                      const float2 m, const float2 eps2, float2 &r2_out)
+                                      const float2 m, const float2 eps2_3, float2 &r2_out)
 {
     // Eq. 3: dx = (xj_hi - xi_hi) + (xj_lo - xi_lo)
     const float2 dx = add2(add2(xh, I.nxh[0]), add2(xl, I.nxl[0]));
@@ -103,7 +105,11 @@ __device__ __forceinline__ void pair2(IPart &I, const float2 xh, const float2 yh
     const float2 dvy = add2(vy, I.nv[1]);
     const float2 dvz = add2(vz, I.nv[2]);
     const float2 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
-    const float2 s2 = add2(r2, eps2);
+    // s2/3 instead of s2 (one FFMA2 either way): y = rsqrt(s2/3) = sqrt(3)/s, so y^2 = 3/s^2 already carries
+    // the factor 3 of the jerk's radial term and alpha = -(dx.dv) y^2 needs no separate multiply.  The sums
+    // come out scaled by 3^(1/2) (pot) and 3^(3/2) (acc, jerk); k_force_fast undoes that exactly (with the
+    // binary32 value of THIRD) in fp64 when it writes its partials.  3 THIRD - 1 = 3e-8 only touches alpha.
+    const float2 s2 = fma2(r2, dup(THIRD), eps2_3);          // eps2_3 = THIRD * eps^2
 #if defined(G6_ABLATE) && (G6_ABLATE & 2)
     float2 rinv = mul2(s2, dup(0.5f));
 #else
@@ -118,7 +124,8 @@ __device__ __forceinline__ void pair2(IPart &I, const float2 xh, const float2 yh
     const float2 mrinv = mul2(m, rinv);
     const float2 mrinv3 = mul2(mrinv, rinv2);
     const float2 rv = fma2(dz, dvz, fma2(dy, dvy, mul2(dx, dvx)));
-    const float2 alpha = mul2(dup(-3.0f), mul2(rv, rinv2));
+    const float2 w = mul2(rv, rinv2);
+    const float2 alpha = make_float2(-w.x, -w.y);           // folded into the FFMA2 operand modifier
     I.p = add2(I.p, mrinv);                       // +m/s; the sign is applied at the flush
     I.a[0] = fma2(mrinv3, dx, I.a[0]);
     I.a[1] = fma2(mrinv3, dy, I.a[1]);
@@ -197,7 +204,8 @@ k_force_fast(ForceArgs A)
             jrk[q][k] = 0;
         }
     }
-    const float2 eps2 = dup(A.eps2);
+    const float2 eps2 = dup(THIRD * A.eps2);                 // pair2 works on s2 / 3
+    const double kP = sqrt((double)THIRD), kA = (double)THIRD * kP;
 
     for (int it = 0; it < nt; ++it) {
         const int t = t0 + it;
@@ -356,8 +364,8 @@ k_force_fast(ForceArgs A)
         }
         const size_t o = (size_t)s * A.P.stride_s + (size_t)i * A.P.stride_i;
 #pragma unroll
-        for (int k = 0; k < 3; ++k) { A.P.acc[k][o] = acc[q][k]; A.P.jrk[k][o] = jrk[q][k]; }
-        A.P.pot[o] = pot[q];
+        for (int k = 0; k < 3; ++k) { A.P.acc[k][o] = kA * acc[q][k]; A.P.jrk[k][o] = kA * jrk[q][k]; }
+        A.P.pot[o] = kP * pot[q];
         A.P.nn_r2[o] = baddr >= 0 ? I[q].rmin : INF;
         A.P.nn_addr[o] = baddr;
     }
