@@ -59,10 +59,14 @@ int g6_open(int clusterid);
 /* Wait for outstanding work and free everything the cluster owns. */
 int g6_close(int clusterid);
 
-/* Largest ni accepted by one firsthalf/lasthalf pair.  The paper's value is 256
- * (PAPER.md:132 fn.7); that is the default.  env G6_NPIPES or g6x_set_npipes raise it (up to
- * 2^21) so that a whole sweep fits one call; larger blocks are tiled inside the library
- * (the paper's "segments"). */
+/* Largest ni accepted by one firsthalf/lasthalf pair.  The paper's library reports 256
+ * "pipelines" (PAPER.md:132 fn.7: one 256-thread block of i-particles on a G80); the number a
+ * host code should chunk its blocks by on a B200 is what fills the chip, 148 SMs x 3 resident
+ * CTAs x 256 i-particles, rounded up to a power of two: G6_DEFAULT_NPIPES.  A host code that
+ * chunks by g6_npipes() (as GRAPE-6 codes do) then hands over whole blocks; chunks of 256 cost
+ * one call latency each.  env G6_NPIPES or g6x_set_npipes change it (1 .. 2^21); larger
+ * blocks are tiled inside the library (the paper's "segments"). */
+#define G6_DEFAULT_NPIPES 131072
 int g6_npipes(void);
 
 /* Store / overwrite j-memory slot `address` (x, v, a, j and time per particle).

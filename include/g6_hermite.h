@@ -47,6 +47,10 @@ int g6h_get_state(g6h_system *s, double x[][3], double v[][3]);
  * 2^b <= n_i < 2^(b+1) (64 entries). */
 int g6h_get_stats(g6h_system *s, double stats[8], long long ni_hist_log2[64]);
 
+/* wall_s_log2[b] = wall seconds spent inside the g6 force calls of the block steps counted in
+ * ni_hist_log2[b] (64 entries): where the time of a block-step run goes, by block size. */
+int g6h_get_force_wall_hist(g6h_system *s, double wall_s_log2[64]);
+
 #ifdef __cplusplus
 }
 #endif

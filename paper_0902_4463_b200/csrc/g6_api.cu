@@ -28,7 +28,7 @@ constexpr int MAX_CLUSTERS = 4;
 constexpr int MAX_NPIPES = 1 << 21;
 constexpr int N_EVENTS = 6;
 
-int g_npipes = 0;   // 0 = not initialised yet (env G6_NPIPES or 256)
+int g_npipes = 0;   // 0 = not initialised yet (env G6_NPIPES or G6_DEFAULT_NPIPES)
 
 struct Cluster {
     bool open = false;
@@ -128,7 +128,7 @@ int env_int(const char *name, int dflt)
 
 void init_npipes()
 {
-    if (g_npipes == 0) g_npipes = std::min(std::max(env_int("G6_NPIPES", 256), 1), MAX_NPIPES);
+    if (g_npipes == 0) g_npipes = std::min(std::max(env_int("G6_NPIPES", G6_DEFAULT_NPIPES), 1), MAX_NPIPES);
 }
 
 template <class T>

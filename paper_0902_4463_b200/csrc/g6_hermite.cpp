@@ -30,7 +30,7 @@ struct g6h_system {
     std::vector<V3> xi, vi, a1, ad1;
     std::vector<double> pot;
     long long nblock = 0, npart = 0, hist[64] = {};
-    double inter = 0, wall = 0, wall_force = 0;
+    double inter = 0, wall = 0, wall_force = 0, wall_force_hist[64] = {};
 };
 
 namespace {
@@ -131,7 +131,8 @@ int g6h_evolve(g6h_system *sp, double t_end, long long max_block_steps)
         for (int k = 0; k < ni; ++k) predict_one(s, s.act[k], tn, s.xi[k], s.vi[k]);
         const auto f0 = Clock::now();
         rc = block_force(s, tn);
-        s.wall_force += secs(f0, Clock::now());
+        const double wf = secs(f0, Clock::now());
+        s.wall_force += wf;
         if (rc) break;
         for (int k = 0; k < ni; ++k) {
             const int p = s.act[k];
@@ -171,6 +172,7 @@ int g6h_evolve(g6h_system *sp, double t_end, long long max_block_steps)
         int b = 0;
         while ((1LL << (b + 1)) <= ni) ++b;
         s.hist[b] += 1;
+        s.wall_force_hist[b] += wf;
     }
     s.wall += secs(w0, Clock::now());
     return rc;
@@ -194,6 +196,13 @@ int g6h_get_stats(g6h_system *s, double stats[8], long long ni_hist_log2[64])
     stats[0] = (double)s->nblock; stats[1] = (double)s->npart; stats[2] = s->t; stats[3] = s->dt_min;
     stats[4] = s->inter; stats[5] = s->wall; stats[6] = s->wall_force; stats[7] = 0;
     if (ni_hist_log2) std::memcpy(ni_hist_log2, s->hist, sizeof(s->hist));
+    return 0;
+}
+
+int g6h_get_force_wall_hist(g6h_system *s, double wall_s_log2[64])
+{
+    if (!s || !wall_s_log2) return G6_ERR_ARG;
+    std::memcpy(wall_s_log2, s->wall_force_hist, sizeof(s->wall_force_hist));
     return 0;
 }
 

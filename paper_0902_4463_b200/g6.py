@@ -14,6 +14,9 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libg6b200.so")
 
+#: include/g6.h G6_DEFAULT_NPIPES
+DEFAULT_NPIPES = 131072
+
 #: every symbol include/g6.h declares (tests check that the library exports each of them)
 SYMBOLS = [
     "g6_open", "g6_close", "g6_npipes", "g6_set_j_particle", "g6_set_ti", "g6calc_firsthalf",
@@ -21,7 +24,7 @@ SYMBOLS = [
     "g6x_last_error", "g6x_set_npipes", "g6x_set_j_particles", "g6x_set_j_particles_dev", "g6x_calc_dev",
     "g6x_get_nearest", "g6x_set_stream", "g6x_synchronize", "g6x_get_timers", "g6x_set_option",
     "g6x_get_option", "g6x_get_predicted", "g6x_debug_dx", "g6x_version",
-    "g6h_create", "g6h_destroy", "g6h_evolve", "g6h_get_state", "g6h_get_stats",
+    "g6h_create", "g6h_destroy", "g6h_evolve", "g6h_get_state", "g6h_get_stats", "g6h_get_force_wall_hist",
 ]
 
 ERRORS = {0: "G6_OK", -1: "G6_ERR_NOT_OPEN", -2: "G6_ERR_CLUSTER", -3: "G6_ERR_ADDRESS", -4: "G6_ERR_NI",
@@ -274,8 +277,10 @@ class Hermite:
     def stats(self):
         st = np.zeros(8); hist = np.zeros(64, np.int64)
         _chk(lib().g6h_get_stats(C.c_void_p(self._h), _dp(st), hist.ctypes.data_as(C.POINTER(C.c_longlong))), self.clusterid)
+        wall = np.zeros(64)
+        _chk(lib().g6h_get_force_wall_hist(C.c_void_p(self._h), _dp(wall)), self.clusterid)
         return dict(n_block_steps=int(st[0]), n_particle_steps=int(st[1]), t=st[2], dt_min=st[3], interactions=st[4],
-                    wall_s=st[5], wall_force_s=st[6], ni_hist_log2=hist)
+                    wall_s=st[5], wall_force_s=st[6], ni_hist_log2=hist, force_wall_s_log2=wall)
 
     def close(self):
         if self._h:

@@ -49,7 +49,7 @@ def main():
            "block_steps_per_s": st["n_block_steps"] / max(st["wall_s"], 1e-9),
            "interactions_per_s": st["interactions"] / max(st["wall_s"], 1e-9),
            "gflops_60": 60 * st["interactions"] / max(st["wall_s"], 1e-9) / 1e9,
-           "ni_hist_log2": hist}
+           "ni_hist_log2": hist, "force_wall_s_log2": [round(float(w), 4) for w in st["force_wall_s_log2"][:24]]}
     if args.state_out:
         np.savez(args.state_out, x0=x, v0=v, m=m, x1=x1, v1=v1, eps2=eps2)
     print(json.dumps(out), flush=True)

@@ -50,7 +50,7 @@ def test_headers_have_no_torch_or_cxx_types():
 
 def test_version_and_error_codes(library):
     assert b"sm_100a" in library.g6x_version()
-    assert g6.g6_npipes() == 256                      # PAPER.md:132 fn.7
+    assert g6.g6_npipes() == g6.DEFAULT_NPIPES == 131072   # include/g6.h G6_DEFAULT_NPIPES (PAPER.md:132 fn.7 had 256 on a G80)
     assert library.g6_set_ti(ctypes.c_int(0), ctypes.c_double(0.0)) == -1        # G6_ERR_NOT_OPEN
     assert library.g6_open(ctypes.c_int(99)) == -2                               # G6_ERR_CLUSTER
     assert library.g6x_set_npipes(ctypes.c_int(0)) == -8

@@ -17,7 +17,7 @@ def cluster():
     g6.g6_open(0)
     yield 0
     g6.g6_close(0)
-    g6.g6x_set_npipes(256)
+    g6.g6x_set_npipes(g6.DEFAULT_NPIPES)
 
 
 def _energy(oracle, x, v, m, eps2):

@@ -18,7 +18,7 @@ def cluster():
     g6.g6x_set_option(0, "timers", 1)          # off by default (two event records per phase cost ~10 us a step)
     yield 0
     g6.g6_close(0)
-    g6.g6x_set_npipes(256)
+    g6.g6x_set_npipes(g6.DEFAULT_NPIPES)
 
 
 KERNELS = [0, 1, 2]       # 0 = automatic (block-step kernel for n_i <= 32), 1 = checked reference kernel, 2 = fast kernel (FFMA2 + TMA)
