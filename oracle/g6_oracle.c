@@ -26,6 +26,13 @@
  *                 a pair with s2 == 0 is skipped (reading 5); nearest neighbour = argmin of
  *                 the UNSOFTENED r2 = dx.dx, ties -> smallest j address (readings 6-8);
  *                 none -> address -1, index -1, r2 = +inf.
+ *   orc_neighbours  neighbour lists, PAPER.md:206 (section 4): "a neighbour lists functionality ...
+ *                 The maximum number of neighbours that a particle in a block can store is
+ *                 configured at compile time (default is 256)".  The paper says no more; the
+ *                 reading (reading 20) is the GRAPE-6 one: j is a neighbour of i when
+ *                 the UNSOFTENED r2 = |x_j - x_i|^2 < h2_i (strict), index_j != index_i; the
+ *                 list holds the j addresses in increasing order; count = all neighbours, the
+ *                 stored list is its first `maxlen` entries (count > maxlen = overflow).
  *   orc_energy    total kinetic and (softened) potential energy, the quantity the paper's
  *                 accuracy test monitors (dE/E).
  *   orc_ds_*      double-single numbers, PAPER.md:68-74, :86 fn.5, and the truncated
@@ -33,7 +40,9 @@
  *
  * Pins (tests/test_oracle_pins.py): two-body closed form, regular polygon, rigid rotation,
  * homologous expansion, Newton's third law, Plummer W = -1/2, 50-digit decimal brute force,
- * translation invariance, cubic-polynomial predictor, phi self-term, DS error bounds.
+ * translation invariance, cubic-polynomial predictor, phi self-term, DS error bounds;
+ * orc_neighbours: lattice shell counts (closed form), consistency with the nearest neighbour
+ * of orc_force, overflow rule.
  * No function in this file is "parity unpinned".
  */
 #include <math.h>
@@ -114,6 +123,29 @@ void orc_force(int ni, const int *index_i, const double (*xi)[3], const double (
         if (nn_addr)  nn_addr[i] = best_addr;
         if (nn_index) nn_index[i] = best_addr >= 0 ? index_j[best_addr] : -1;
         if (nn_r2)    nn_r2[i] = (double)best;
+    }
+}
+
+/* ---- neighbour lists (reading 20) -------------------------------- */
+void orc_neighbours(int ni, const int *index_i, const double (*xi)[3], const double *h2,
+                    int nj, const int *index_j, const double (*xj)[3],
+                    int maxlen, int *count, int *list_addr)
+{
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int i = 0; i < ni; ++i) {
+        int n = 0;
+        for (int j = 0; j < nj; ++j) {
+            if (index_j[j] == index_i[i]) continue;
+            real dx = (real)xj[j][0] - (real)xi[i][0];
+            real dy = (real)xj[j][1] - (real)xi[i][1];
+            real dz = (real)xj[j][2] - (real)xi[i][2];
+            real r2 = dx * dx + dy * dy + dz * dz;
+            if (r2 < (real)h2[i]) {
+                if (n < maxlen) list_addr[(size_t)i * maxlen + n] = j;
+                ++n;
+            }
+        }
+        count[i] = n;
     }
 }
 

@@ -93,6 +93,19 @@ def force(index_i, xi, vi, index_j, xj, vj, mj, eps2, long_double=False):
     return dict(acc=acc, jerk=jerk, pot=pot, nn_addr=nn_addr, nn_index=nn_index, nn_r2=nn_r2)
 
 
+def neighbours(index_i, xi, h2, index_j, xj, maxlen=256, long_double=False):
+    """Neighbour lists (orc_neighbours): (count[ni], list_addr[ni, maxlen]); entries past
+    min(count, maxlen) are -1.  j addresses in increasing order."""
+    ni, nj = len(index_i), len(index_j)
+    index_i = _i32(index_i); index_j = _i32(index_j)
+    xi = _f64(xi, (ni, 3)); xj = _f64(xj, (nj, 3)); h2 = _f64(h2, (ni,))
+    count = np.zeros(ni, np.int32); lst = np.full((ni, maxlen), -1, np.int32)
+    d, i = C.c_double, C.c_int
+    _lib(long_double).orc_neighbours(i(ni), _p(index_i, i), _p(xi, d), _p(h2, d), i(nj), _p(index_j, i), _p(xj, d),
+                                     i(maxlen), _p(count, i), _p(lst, i))
+    return count, lst
+
+
 def energy(x, v, m, eps2, long_double=False):
     """(T, W): kinetic and softened potential energy."""
     n = len(m)

@@ -384,3 +384,56 @@ def test_aarseth_step_closed_form(oracle):
     e = np.array([1.0, 0, 0])
     dt = oracle.aarseth_dt(eta, A * e, lam * A * e, lam**2 * A * e, lam**3 * A * e)
     assert abs(dt - np.sqrt(eta) / lam) < 1e-15
+
+
+# ---- P13: neighbour lists (reading 20) -------------------------------------
+def test_p13_neighbour_lists_lattice_shell_counts(oracle):
+    """On the integer lattice the number of points at squared distance n from a lattice point is
+    r3(n), the number of representations of n as a sum of three squares: 6, 12, 8, 6, 24, 24, 0, 12, 30
+    for n = 1..9 (number theory, e.g. OEIS A005875).  Strict '<': a point AT h2 is not a neighbour."""
+    g = np.arange(-4, 5)
+    X = np.array(np.meshgrid(g, g, g, indexing="ij"), dtype=float).reshape(3, -1).T + np.array([10.0, -7.0, 3.0])
+    n = len(X)
+    idx = np.arange(n, dtype=np.int32)
+    c = int(np.nonzero((X == np.array([10.0, -7.0, 3.0])).all(axis=1))[0][0])
+    r3 = [6, 12, 8, 6, 24, 24, 0, 12, 30]
+    want = np.cumsum(r3)
+    for k in range(9):
+        cnt, lst = oracle.neighbours(idx[c:c + 1], X[c:c + 1], [k + 1.5], idx, X, maxlen=256)
+        assert cnt[0] == want[k]
+        got = lst[0, :cnt[0]]
+        assert (np.diff(got) > 0).all() and c not in got                       # increasing addresses, self excluded by index
+        d2 = ((X[got] - X[c]) ** 2).sum(axis=1)
+        assert (d2 < k + 1.5).all()
+        cnt_eq, _ = oracle.neighbours(idx[c:c + 1], X[c:c + 1], [float(k + 1)], idx, X, maxlen=256)
+        assert cnt_eq[0] == (want[k - 1] if k else 0)                         # strict inequality
+    # same answer from the long-double build
+    cnt_l, lst_l = oracle.neighbours(idx[c:c + 1], X[c:c + 1], [6.5], idx, X, maxlen=256, long_double=True)
+    cnt_d, lst_d = oracle.neighbours(idx[c:c + 1], X[c:c + 1], [6.5], idx, X, maxlen=256)
+    assert cnt_l[0] == cnt_d[0] == 80 and (lst_l == lst_d).all()
+
+
+def test_p13_neighbour_lists_brute_force_overflow_and_nearest(oracle):
+    rng = np.random.default_rng(13)
+    n = 400
+    X = rng.normal(size=(n, 3)); V = rng.normal(size=(n, 3)); m = np.full(n, 1.0 / n)
+    idx = rng.permutation(n).astype(np.int32) + 1000                          # index != address
+    h2 = rng.uniform(0.05, 0.6, size=n)
+    cnt, lst = oracle.neighbours(idx, X, h2, idx, X, maxlen=8)
+    for i in range(n):                                                        # numpy brute force, pair by pair
+        d2 = ((X - X[i]) ** 2).sum(axis=1)
+        want = np.nonzero((d2 < h2[i]) & (idx != idx[i]))[0]
+        assert cnt[i] == len(want)
+        k = min(len(want), 8)
+        assert (lst[i, :k] == want[:k]).all() and (lst[i, k:] == -1).all()   # overflow: count keeps counting, list = first maxlen
+    assert (cnt > 8).any() and (cnt < 8).any()
+    # the nearest neighbour of orc_force heads the set: with h2 just above its distance the list is exactly that particle
+    f = oracle.force(idx, X, V, idx, X, V, m, 0.0)
+    cnt1, lst1 = oracle.neighbours(idx, X, f["nn_r2"] * (1 + 1e-12), idx, X, maxlen=4)
+    assert (cnt1 == 1).all() and (lst1[:, 0] == f["nn_addr"]).all()
+    cnt0, _ = oracle.neighbours(idx, X, f["nn_r2"], idx, X, maxlen=4)          # at the distance itself: nobody (strict)
+    assert (cnt0 == 0).all()
+    # same index, different address (an i-particle that is also stored as a j): excluded by INDEX, not position
+    Xs = X.copy(); Xs[7] += 0.01
+    cnt2, lst2 = oracle.neighbours(idx[7:8], Xs[7:8], [0.5], idx, X, maxlen=64)
+    assert 7 not in lst2[0, :cnt2[0]]
