@@ -92,8 +92,16 @@ int g6_set_ti(int clusterid, double ti);
  *
  *   acc_old, jerk6_old, phi_old   GRAPE fixed-point scaling hints: ignored, may be NULL
  *   eps2               softening length squared for this block, >= 0
- *   h2[ni]             neighbour-sphere radius squared (reserved for neighbour lists,
- *                      PAPER.md:206): ignored, may be NULL
+ *   h2[ni]             neighbour-sphere radius squared per i-particle, or NULL.  When given, the
+ *                      call also builds neighbour lists ("neighbour lists functionality";
+ *                      DESIGN.md reading 20): j is a neighbour of i when the UNSOFTENED
+ *                      |x_j - x_i|^2 < h2[i] (strict; compared in binary32 on the double-single
+ *                      separation, like the nearest neighbour) and index_j != index_i.  At most
+ *                      `nb_maxlen` (option, default G6_NB_MAXLEN = 256, the paper's default)
+ *                      neighbours are stored per i, those with the smallest j addresses; the count
+ *                      keeps running (count > nb_maxlen = overflow).  Read with
+ *                      g6_read_neighbour_list + g6_get_neighbour_list.  Blocks with lists take the
+ *                      sweep kernels at any ni (the fused small-block kernel builds none).
  * Copies the block to pinned staging, uploads j-particles changed since the last call, and
  * enqueues predictor -> force -> combine -> download.  Returns without waiting. */
 int g6calc_firsthalf(int clusterid, int nj, int ni, const int index[],
@@ -113,13 +121,19 @@ int g6calc_lasthalf2(int clusterid, int nj, int ni, const int index[],
                      const double xi[][3], const double vi[][3], double eps2, const double h2[],
                      double acc[][3], double jerk[][3], double pot[], int nnb_index[]);
 
-/* Make the neighbour results of the last completed force call readable.  Returns 0
- * (a positive value would mean list overflow once neighbour lists exist). */
+/* Make the neighbour results of the last completed host force call readable (copies the lists
+ * device -> host when the call had h2 != NULL).  Returns 0, or the POSITIVE number of i-particles
+ * whose list overflowed nb_maxlen (the caller then shrinks h2 and repeats, as GRAPE-6 codes do),
+ * or a negative error. */
+#define G6_NB_MAXLEN 256
 int g6_read_neighbour_list(int clusterid);
 
-/* Neighbour "list" of pipe `ipipe` (the ipipe-th i-particle of the last call).  In this
- * version the list is the single nearest neighbour: *n = 1 and list[0] = its index, or
- * *n = 0.  maxlen must be >= 1. */
+/* Neighbour list of pipe `ipipe` (the ipipe-th i-particle of the last host force call): the
+ * callers' INDICES of its neighbours in increasing j-address order, at most `maxlen` (>= 1) of
+ * them into list[], their number into *n.  Returns 0, or 1 when neighbours were dropped (the
+ * particle has more than nb_maxlen, or more than `maxlen`), or a negative error.
+ * If the force call had h2 == NULL the "list" is the single nearest neighbour: *n = 1 and
+ * list[0] = its index, or *n = 0. */
 int g6_get_neighbour_list(int clusterid, int ipipe, int maxlen, int *n, int list[]);
 
 /* ---- extensions ------------------------------------------------------------------------ */
@@ -148,6 +162,19 @@ int g6x_calc_dev(int clusterid, int nj, int ni, const int *d_index, const double
                  const double *d_vi, double eps2, double *d_acc, double *d_jerk, double *d_pot,
                  int *d_nn_index, double *d_nn_r2);
 
+/* g6x_calc_dev with neighbour lists: d_h2[ni] fp64 radii squared in; d_nb_count[ni] (all neighbours
+ * found, may exceed nb_maxlen) and d_nb_list[ni][nb_maxlen] (callers' indices, increasing j address;
+ * entries past min(count, nb_maxlen) are left untouched) out.  The three pointers are given
+ * together or all NULL (= g6x_calc_dev). */
+int g6x_calc_dev_nb(int clusterid, int nj, int ni, const int *d_index, const double *d_xi,
+                    const double *d_vi, double eps2, double *d_acc, double *d_jerk, double *d_pot,
+                    int *d_nn_index, double *d_nn_r2, const double *d_h2, int *d_nb_count, int *d_nb_list);
+
+/* All neighbour lists of the last host force call at once: count[ni] = neighbours found (may exceed
+ * what is stored), list[ni][maxlen] row-major = indices, padded with -1.  Returns like
+ * g6_read_neighbour_list (number of truncated rows).  G6_ERR_SEQUENCE if that call had h2 == NULL. */
+int g6x_get_neighbour_lists(int clusterid, int ni, int maxlen, int count[], int list[]);
+
 /* Nearest neighbour of each i of the last completed host force call: index (-1 if none) and
  * UNSOFTENED squared distance (+inf if none). */
 int g6x_get_nearest(int clusterid, int ni, int nn_index[], double nn_r2[]);
@@ -174,6 +201,8 @@ int g6x_get_timers(int clusterid, double us[8]);
  *   "variant" 0 = automatic; threads*8 + i_per_thread forces a fast-kernel shape (e.g. 128*8+2)
  *   "small"   largest n_i served by the block-step kernel (one launch: j update + predictor + force +
  *             combine, lanes over j); default 32, at most 64, 0 = off
+ *   "nb_maxlen" neighbours stored per i-particle (1 .. 4096, default G6_NB_MAXLEN = 256; compile-time
+ *             in the paper); changing it discards the lists of the last call
  * Returns G6_ERR_ARG for an unknown key or value. */
 int g6x_set_option(int clusterid, const char *key, int value);
 int g6x_get_option(int clusterid, const char *key, int *value);

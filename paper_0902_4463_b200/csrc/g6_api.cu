@@ -75,6 +75,18 @@ struct Cluster {
     void *part_block = nullptr;
     size_t part_elems = 0;
 
+    // neighbour lists: per-split lists, combined lists, host copies; all on demand
+    int *d_nb_pcnt = nullptr, *d_nb_plist = nullptr;   // [S][ni], [S][ni][maxlen]
+    size_t nb_part_rows = 0;                           // S * ni rows allocated
+    int *d_nb_cnt = nullptr, *d_nb_list = nullptr;     // [ni], [ni][maxlen]
+    int *h_nb_cnt = nullptr, *h_nb_list = nullptr;     // pinned
+    double *h_h2 = nullptr, *d_h2 = nullptr;           // neighbour radii of the i-block
+    int nb_cap = 0;                                    // ni the combined / host / h2 buffers hold
+    int nb_alloc_maxlen = 0;                           // maxlen the buffers were sized for
+    bool last_nb = false;                              // the last host force call built lists
+    bool nb_on_host = false;                           // ... and they have been copied to h_nb_*
+    int last_nb_maxlen = 0;
+
     // bulk-load staging (host fp64 arrays -> device)
     void *h_bulk = nullptr, *d_bulk = nullptr;
     size_t bulk_bytes = 0;
@@ -84,13 +96,14 @@ struct Cluster {
     bool pending = false;      // firsthalf issued, lasthalf not yet
     bool have_result = false;  // a host force call completed (neighbour / debug queries)
     int pend_nj = 0, pend_ni = 0;
+    bool pend_nb = false;
     int last_ni = 0;
     cudaEvent_t ev[N_EVENTS] = {};
     bool ev_valid = false;
     int last_ctas = 0, last_S = 0;
 
     // options
-    int opt_ds = 1, opt_newton = 1, opt_jsplit = 0, opt_kernel = 0, opt_timers = 0, opt_variant = 0, opt_small = 32;
+    int opt_ds = 1, opt_newton = 1, opt_jsplit = 0, opt_kernel = 0, opt_timers = 0, opt_variant = 0, opt_small = 32, opt_nb_maxlen = 256;
 };
 
 Cluster g_cl[MAX_CLUSTERS];
@@ -207,6 +220,59 @@ int ensure_partials(Cluster &c, size_t elems)
     return G6_OK;
 }
 
+void free_nb(Cluster &c)
+{
+    dfree(c.d_nb_pcnt); dfree(c.d_nb_plist); dfree(c.d_nb_cnt); dfree(c.d_nb_list); dfree(c.d_h2);
+    hfree(c.h_nb_cnt); hfree(c.h_nb_list); hfree(c.h_h2);
+    c.nb_part_rows = 0;
+    c.nb_cap = 0;
+    c.nb_alloc_maxlen = 0;
+    c.last_nb = c.nb_on_host = false;
+}
+
+// maxlen changed since the buffers were sized: drop them all
+int nb_check_maxlen(Cluster &c)
+{
+    if (c.opt_nb_maxlen != c.nb_alloc_maxlen) {
+        CK(cudaStreamSynchronize(c.stream));
+        free_nb(c);
+        c.nb_alloc_maxlen = c.opt_nb_maxlen;
+    }
+    return G6_OK;
+}
+
+// per-split lists of a force call with neighbour lists (rows = S * ni)
+int ensure_nb_part(Cluster &c, size_t rows)
+{
+    int rc = nb_check_maxlen(c);
+    if (rc) return rc;
+    if (rows <= c.nb_part_rows) return G6_OK;
+    CK(cudaStreamSynchronize(c.stream));
+    dfree(c.d_nb_pcnt); dfree(c.d_nb_plist);
+    c.nb_part_rows = 0;
+    CK(dalloc(c.d_nb_pcnt, rows)); CK(dalloc(c.d_nb_plist, rows * c.opt_nb_maxlen));
+    c.nb_part_rows = rows;
+    return G6_OK;
+}
+
+// combined lists, radii and their pinned host copies for a HOST force call on ni particles
+int ensure_nb_host(Cluster &c, int ni)
+{
+    int rc = nb_check_maxlen(c);
+    if (rc) return rc;
+    if (ni <= c.nb_cap) return G6_OK;
+    CK(cudaStreamSynchronize(c.stream));
+    dfree(c.d_nb_cnt); dfree(c.d_nb_list); dfree(c.d_h2);
+    hfree(c.h_nb_cnt); hfree(c.h_nb_list); hfree(c.h_h2);
+    c.nb_cap = 0;
+    c.last_nb = c.nb_on_host = false;
+    const size_t n = std::max(ni, 1024), ml = c.opt_nb_maxlen;
+    CK(dalloc(c.d_nb_cnt, n)); CK(dalloc(c.d_nb_list, n * ml)); CK(dalloc(c.d_h2, n));
+    CK(halloc(c.h_nb_cnt, n)); CK(halloc(c.h_nb_list, n * ml)); CK(halloc(c.h_h2, n));
+    c.nb_cap = (int)n;
+    return G6_OK;
+}
+
 int ensure_bulk(Cluster &c, size_t bytes)
 {
     if (bytes <= c.bulk_bytes) return G6_OK;
@@ -245,6 +311,7 @@ void release(Cluster &c)
     for (int b = 0; b < 2; ++b) { hfree(c.h_rec[b]); if (c.ev_rec[b]) cudaEventDestroy(c.ev_rec[b]); }
     dfree(c.d_rec);
     free_i(c);
+    free_nb(c);
     if (c.part_block) cudaFree(c.part_block);
     if (c.h_bulk) cudaFreeHost(c.h_bulk);
     if (c.d_bulk) cudaFree(c.d_bulk);
@@ -323,12 +390,12 @@ int run_predict(Cluster &c)
 // pick the number of j-splits S that minimises  waves(S) x (tiles per CTA + per-CTA overhead),
 // waves(S) = ceil(i-tiles x S / resident CTA slots).  Small blocks get S ~ slots (every SM busy at
 // n_i = 1); big sweeps get the S that makes the last wave full.  Partials are capped at 1 GiB.
-int choose_jsplit(int n_itiles, int ntiles, int slots, int ni)
+int choose_jsplit(int n_itiles, int ntiles, int slots, int ni, long long s_cap = 1LL << 30)
 {
     const double OVH = 0.4;        // CTA prologue + epilogue, in tile times
     const double COMBINE = 0.004;  // per extra split: partial traffic + combine work, in tile times
     long long smax = std::min<long long>(ntiles, (1LL << 30) / (72LL * std::max(ni, 1)));
-    smax = std::max<long long>(1, std::min<long long>(smax, 2LL * slots / std::max(n_itiles, 1) + 2));
+    smax = std::max<long long>(1, std::min<long long>(std::min(smax, s_cap), 2LL * slots / std::max(n_itiles, 1) + 2));
     int best = 1;
     double best_cost = 1e300;
     for (int S = 1; S <= smax; ++S) {
@@ -343,16 +410,18 @@ int choose_jsplit(int n_itiles, int ntiles, int slots, int ni)
 
 // force + combine (steps a-4, a-5) on device-resident i-blocks; all asynchronous
 // small active blocks take the fused block-step kernel unless an experiment switch pins another path
-bool use_block_step(const Cluster &c, int ni)
+bool use_block_step(const Cluster &c, int ni, bool nb = false)
 {
-    return ni <= c.opt_small && c.opt_kernel != 1 && c.opt_kernel != 2 && c.opt_jsplit == 0;
+    return !nb && ni <= c.opt_small && c.opt_kernel != 1 && c.opt_kernel != 2 && c.opt_jsplit == 0;
 }
 
 struct HostBlock { const double *xi, *vi; const int *index; };   // host copy of the i-block (small blocks travel in kernel parameters)
+// neighbour-list request of a force call: radii in, combined counts and lists out (all device memory)
+struct NbReq { const double *d_h2; int *d_cnt; int *d_list; };
 
 int run_force(Cluster &c, int nj, int ni, const int *d_index, const double *d_xi, const double *d_vi,
               double eps2, double *d_acc, double *d_jerk, double *d_pot, int *d_nn_index, double *d_nn_r2,
-              cudaEvent_t ev_pred_done, cudaEvent_t ev_force_done, const HostBlock *hb)
+              cudaEvent_t ev_pred_done, cudaEvent_t ev_force_done, const HostBlock *hb, const NbReq *nb = nullptr)
 {
     ForceArgs A{};
     A.pred = c.pred;
@@ -369,7 +438,7 @@ int run_force(Cluster &c, int nj, int ni, const int *d_index, const double *d_xi
     A.ds = c.opt_ds;
 
     // small active blocks: the whole block step in one kernel (g6_block_step.cuh)
-    if (use_block_step(c, ni)) {
+    if (use_block_step(c, ni, nb != nullptr)) {
         // a-1: changed j-particles ride in the kernel parameters when they fit and lie inside the j-range
         const int maxi_need = std::max(ni, hb ? c.n_rec : 0);
         bool inline_upd = hb && c.n_rec > 0 && c.n_rec <= BS_MAX_I;
@@ -429,15 +498,26 @@ int run_force(Cluster &c, int nj, int ni, const int *d_index, const double *d_xi
     const bool fast_ok = A.eps2 >= 4.0f * std::numeric_limits<float>::min() && std::isfinite(A.eps2);
     const bool use_fast = (c.opt_kernel == 2 || c.opt_kernel == 0) && fast_ok && fast_available();
 
-    const FastVariant fv = fast_pick(ni, c.n_sm, c.opt_variant);
+    FastVariant fv = fast_pick(ni, c.n_sm, c.opt_variant);
+    if (nb && !fast_has_nb(fv)) fv = fast_pick(ni, c.n_sm, 0);     // lists exist for the automatic shapes only
     const int itile = use_fast ? fv.threads * fv.it : REF_THREADS;
     const int n_itiles = (ni + itile - 1) / itile;
-    const int slots = c.n_sm * (use_fast ? fast_ctas_per_sm(fv) : 8);
-    int S = c.opt_jsplit > 0 ? c.opt_jsplit : choose_jsplit(n_itiles, A.ntiles, slots, ni);
+    const int slots = c.n_sm * (use_fast ? (nb ? fast_ctas_per_sm_nb(fv) : fast_ctas_per_sm(fv)) : 8);
+    // per-split neighbour lists are capped at 2 GiB
+    const long long s_cap = nb ? std::max(1LL, (1LL << 31) / (4LL * c.opt_nb_maxlen * ni)) : (1LL << 30);
+    int S = c.opt_jsplit > 0 ? (int)std::min<long long>(c.opt_jsplit, s_cap) : choose_jsplit(n_itiles, A.ntiles, slots, ni, s_cap);
     S = std::max(1, std::min(S, A.ntiles));
     A.S = S;
     int rc = ensure_partials(c, (size_t)S * ni);
     if (rc) return rc;
+    if (nb) {
+        rc = ensure_nb_part(c, (size_t)S * ni);
+        if (rc) return rc;
+        A.h2 = nb->d_h2;
+        A.nb_maxlen = c.opt_nb_maxlen;
+        A.nb_cnt = c.d_nb_pcnt;
+        A.nb_list = c.d_nb_plist;
+    }
     A.P = c.part;
     const bool wide = S > 8;                 // many splits: [i][s] layout, one warp per i combines
     A.P.stride_s = wide ? 1 : ni;
@@ -456,6 +536,10 @@ int run_force(Cluster &c, int nj, int ni, const int *d_index, const double *d_xi
     if (wide) k_combine_wide<<<(ni + 3) / 4, 128, 0, c.stream>>>(A.P, S, ni, c.js.raw, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2);
     else k_combine<<<(ni + 255) / 256, 256, 0, c.stream>>>(A.P, S, ni, c.js.raw, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2);
     CK(cudaGetLastError());
+    if (nb) {
+        k_combine_nb<<<(ni + 3) / 4, 128, 0, c.stream>>>(c.d_nb_pcnt, c.d_nb_plist, S, ni, c.opt_nb_maxlen, c.js.raw, nb->d_cnt, nb->d_list);
+        CK(cudaGetLastError());
+    }
     c.last_ctas = n_itiles * S;
     c.last_S = S;
     return G6_OK;
@@ -642,7 +726,18 @@ int g6_set_ti(int clusterid, double ti)
 int g6x_calc_dev(int clusterid, int nj, int ni, const int *d_index, const double *d_xi, const double *d_vi,
                  double eps2, double *d_acc, double *d_jerk, double *d_pot, int *d_nn_index, double *d_nn_r2)
 {
+    return g6x_calc_dev_nb(clusterid, nj, ni, d_index, d_xi, d_vi, eps2, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2,
+                           nullptr, nullptr, nullptr);
+}
+
+int g6x_calc_dev_nb(int clusterid, int nj, int ni, const int *d_index, const double *d_xi, const double *d_vi,
+                    double eps2, double *d_acc, double *d_jerk, double *d_pot, int *d_nn_index, double *d_nn_r2,
+                    const double *d_h2, int *d_nb_count, int *d_nb_list)
+{
     GET_CLUSTER(clusterid);
+    if ((d_h2 != nullptr) != (d_nb_count != nullptr) || (d_h2 != nullptr) != (d_nb_list != nullptr))
+        return fail(c, G6_ERR_ARG, "d_h2, d_nb_count and d_nb_list must be given together");
+    const NbReq nbr{d_h2, d_nb_count, d_nb_list};
     if (c.pending) return fail(c, G6_ERR_SEQUENCE, "g6x_calc_dev between firsthalf and lasthalf");
     int rc = flush_j(c);
     if (rc) return rc;
@@ -653,7 +748,7 @@ int g6x_calc_dev(int clusterid, int nj, int ni, const int *d_index, const double
     const bool tm = c.opt_timers != 0;
     if (tm) { CK(cudaEventRecord(c.ev[0], c.stream)); CK(cudaEventRecord(c.ev[1], c.stream)); }
     rc = run_force(c, nj, ni, d_index, d_xi, d_vi, eps2, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2, tm ? c.ev[2] : nullptr,
-                   tm ? c.ev[3] : nullptr, nullptr);
+                   tm ? c.ev[3] : nullptr, nullptr, d_h2 ? &nbr : nullptr);
     if (rc) return rc;
     if (tm) { CK(cudaEventRecord(c.ev[4], c.stream)); CK(cudaEventRecord(c.ev[5], c.stream)); }
     c.ev_valid = tm;
@@ -665,7 +760,7 @@ int g6calc_firsthalf(int clusterid, int nj, int ni, const int index[], const dou
                      double eps2, const double h2[])
 {
     GET_CLUSTER(clusterid);
-    (void)acc_old; (void)jerk6_old; (void)phi_old; (void)h2;
+    (void)acc_old; (void)jerk6_old; (void)phi_old;
     if (c.pending) return fail(c, G6_ERR_SEQUENCE, "g6calc_firsthalf called twice without g6calc_lasthalf");
     int rc = check_force_args(c, nj, ni);
     if (rc) return rc;
@@ -675,7 +770,17 @@ int g6calc_firsthalf(int clusterid, int nj, int ni, const int index[], const dou
     if (rc) return rc;
     const bool tm = c.opt_timers != 0;
     if (tm) CK(cudaEventRecord(c.ev[0], c.stream));
-    const bool bs = use_block_step(c, ni);
+    // neighbour lists when the caller passes radii
+    const bool want_nb = h2 != nullptr;
+    NbReq nbr{nullptr, nullptr, nullptr};
+    if (want_nb) {
+        rc = ensure_nb_host(c, ni);
+        if (rc) return rc;
+        memcpy(c.h_h2, h2, sizeof(double) * ni);
+        CK(cudaMemcpyAsync(c.d_h2, c.h_h2, sizeof(double) * ni, cudaMemcpyHostToDevice, c.stream));
+        nbr = NbReq{c.d_h2, c.d_nb_cnt, c.d_nb_list};
+    }
+    const bool bs = use_block_step(c, ni, want_nb);
     const bool zc_out = ni <= ZC_MAX_I;
     const RView out = rview(zc_out ? c.hd_res : c.d_res, ni);
     if (bs) {
@@ -710,7 +815,7 @@ int g6calc_firsthalf(int clusterid, int nj, int ni, const int index[], const dou
         // results straight into mapped host memory (a-6)
         const IView dv = iview(c.d_iblk, ni);
         rc = run_force(c, nj, ni, dv.idx, dv.xi, dv.vi, eps2, out.acc, out.jerk, out.pot, out.nnidx, out.nnr2, tm ? c.ev[2] : nullptr,
-                       tm ? c.ev[3] : nullptr, nullptr);
+                       tm ? c.ev[3] : nullptr, nullptr, want_nb ? &nbr : nullptr);
         if (rc) return rc;
     }
     if (tm) CK(cudaEventRecord(c.ev[4], c.stream));
@@ -722,6 +827,7 @@ int g6calc_firsthalf(int clusterid, int nj, int ni, const int index[], const dou
     c.pending = true;
     c.pend_nj = nj;
     c.pend_ni = ni;
+    c.pend_nb = want_nb;
     return G6_OK;
 }
 
@@ -743,6 +849,9 @@ int g6calc_lasthalf2(int clusterid, int nj, int ni, const int index[], const dou
     if (nnb_index) memcpy(nnb_index, r.nnidx, sizeof(int) * ni);
     c.have_result = true;
     c.last_ni = ni;
+    c.last_nb = c.pend_nb;
+    c.nb_on_host = false;
+    c.last_nb_maxlen = c.opt_nb_maxlen;
     return G6_OK;
 }
 
@@ -752,11 +861,30 @@ int g6calc_lasthalf(int clusterid, int nj, int ni, const int index[], const doub
     return g6calc_lasthalf2(clusterid, nj, ni, index, xi, vi, eps2, h2, acc, jerk, pot, nullptr);
 }
 
+// copy the combined lists of the last host force call to the host (once)
+static int nb_fetch(Cluster &c)
+{
+    if (c.nb_on_host) return G6_OK;
+    if (c.last_nb_maxlen != c.nb_alloc_maxlen || c.last_ni > c.nb_cap)
+        return fail(c, G6_ERR_SEQUENCE, "neighbour lists of the last force call are gone (nb_maxlen changed)");
+    const size_t ni = c.last_ni, ml = c.last_nb_maxlen;
+    CK(cudaMemcpyAsync(c.h_nb_cnt, c.d_nb_cnt, sizeof(int) * ni, cudaMemcpyDeviceToHost, c.stream));
+    CK(cudaMemcpyAsync(c.h_nb_list, c.d_nb_list, sizeof(int) * ni * ml, cudaMemcpyDeviceToHost, c.stream));
+    CK(cudaStreamSynchronize(c.stream));
+    c.nb_on_host = true;
+    return G6_OK;
+}
+
 int g6_read_neighbour_list(int clusterid)
 {
     GET_CLUSTER(clusterid);
     if (c.pending || !c.have_result) return fail(c, G6_ERR_SEQUENCE, "no completed force call to read neighbours of");
-    return 0;
+    if (!c.last_nb) return 0;
+    int rc = nb_fetch(c);
+    if (rc) return rc;
+    int over = 0;
+    for (int i = 0; i < c.last_ni; ++i) over += c.h_nb_cnt[i] > c.last_nb_maxlen;
+    return over;
 }
 
 int g6_get_neighbour_list(int clusterid, int ipipe, int maxlen, int *n, int list[])
@@ -765,10 +893,41 @@ int g6_get_neighbour_list(int clusterid, int ipipe, int maxlen, int *n, int list
     if (c.pending || !c.have_result) return fail(c, G6_ERR_SEQUENCE, "no completed force call");
     if (ipipe < 0 || ipipe >= c.last_ni) return fail(c, G6_ERR_ARG, "ipipe = %d outside [0, %d)", ipipe, c.last_ni);
     if (!n || !list || maxlen < 1) return fail(c, G6_ERR_ARG, "bad neighbour list buffer");
+    if (c.last_nb) {
+        int rc = nb_fetch(c);
+        if (rc) return rc;
+        const int cnt = c.h_nb_cnt[ipipe];
+        const int stored = std::min(cnt, c.last_nb_maxlen);
+        const int ncopy = std::min(stored, maxlen);
+        memcpy(list, c.h_nb_list + (size_t)ipipe * c.last_nb_maxlen, sizeof(int) * ncopy);
+        *n = ncopy;
+        return ncopy < cnt ? 1 : 0;
+    }
     const int nb = rview(c.h_res, c.last_ni).nnidx[ipipe];
     if (nb >= 0) { *n = 1; list[0] = nb; }
     else *n = 0;
     return G6_OK;
+}
+
+int g6x_get_neighbour_lists(int clusterid, int ni, int maxlen, int count[], int list[])
+{
+    GET_CLUSTER(clusterid);
+    if (c.pending || !c.have_result) return fail(c, G6_ERR_SEQUENCE, "no completed force call");
+    if (!c.last_nb) return fail(c, G6_ERR_SEQUENCE, "the last force call built no neighbour lists (h2 was NULL)");
+    if (ni != c.last_ni) return fail(c, G6_ERR_ARG, "ni = %d but the last call had %d", ni, c.last_ni);
+    if (!count || !list || maxlen < 1) return fail(c, G6_ERR_ARG, "bad neighbour list buffer");
+    int rc = nb_fetch(c);
+    if (rc) return rc;
+    int over = 0;
+    for (int i = 0; i < ni; ++i) {
+        const int cnt = c.h_nb_cnt[i];
+        const int ncopy = std::min(std::min(cnt, c.last_nb_maxlen), maxlen);
+        count[i] = cnt;
+        memcpy(list + (size_t)i * maxlen, c.h_nb_list + (size_t)i * c.last_nb_maxlen, sizeof(int) * ncopy);
+        for (int k = ncopy; k < maxlen; ++k) list[(size_t)i * maxlen + k] = -1;
+        over += ncopy < cnt;
+    }
+    return over;
 }
 
 int g6x_get_nearest(int clusterid, int ni, int nn_index[], double nn_r2[])
@@ -828,6 +987,7 @@ static int *option_slot(Cluster &c, const char *key)
     if (!strcmp(key, "timers")) return &c.opt_timers;
     if (!strcmp(key, "variant")) return &c.opt_variant;
     if (!strcmp(key, "small")) return &c.opt_small;
+    if (!strcmp(key, "nb_maxlen")) return &c.opt_nb_maxlen;
     return nullptr;
 }
 
@@ -838,6 +998,7 @@ int g6x_set_option(int clusterid, const char *key, int value)
     if (!slot) return fail(c, G6_ERR_ARG, "unknown option '%s'", key ? key : "(null)");
     const bool is_flag = slot == &c.opt_ds || slot == &c.opt_newton || slot == &c.opt_timers;
     if (value < 0 || (is_flag && value > 1) || (slot == &c.opt_kernel && value > 2) || (slot == &c.opt_jsplit && value > 65535) || (slot == &c.opt_small && value > BS_MAX_I) ||
+        (slot == &c.opt_nb_maxlen && (value < 1 || value > 4096)) ||
         (slot == &c.opt_variant && value != 0 && fast_ctas_per_sm(FastVariant{value / 8, value % 8}) < 1))
         return fail(c, G6_ERR_ARG, "bad value %d for option '%s'", value, key);
     *slot = value;

@@ -356,6 +356,32 @@ k_combine_block(Partials P, int S, int ni, const char *__restrict__ jraw,
     }
 }
 
+// ---- a-5 for neighbour lists: concatenate the per-split lists of every i ------
+// Split s covers an increasing address range and appends in address order, so the concatenation in
+// split order is the list in increasing j address; the first `maxlen` entries are kept, the count
+// is the total (count > maxlen = overflow, reading 20).  Addresses -> caller's indices.
+// One warp per i.
+__global__ void __launch_bounds__(128)
+k_combine_nb(const int *__restrict__ part_cnt, const int *__restrict__ part_list, int S, int ni, int maxlen,
+             const char *__restrict__ jraw, int *__restrict__ cnt, int *__restrict__ list)
+{
+    const int i = blockIdx.x * 4 + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (i >= ni) return;
+    int total = 0;
+    for (int s = 0; s < S; ++s) {
+        const int c = part_cnt[(size_t)s * ni + i];
+        const int stored = min(c, maxlen);
+        const int *src = part_list + ((size_t)s * ni + i) * maxlen;
+        for (int k = lane; k < stored; k += 32) {
+            const int pos = total + k;
+            if (pos < maxlen) list[(size_t)i * maxlen + pos] = j_index(jraw, src[k]);
+        }
+        total += c;
+    }
+    if (lane == 0) cnt[i] = total;
+}
+
 // ---- debug: the kernel's Eq.-3 separation for chosen (i, j) pairs (DESIGN.md pin P11) -------
 __global__ void k_debug_dx(int n, const int *__restrict__ ipipe, const int *__restrict__ jaddr,
                            const double *__restrict__ xi, int ds, const float *__restrict__ pred,

@@ -145,8 +145,12 @@ struct FastSmem {
     alignas(8) uint64_t empty[FAST_NSTAGE];
 };
 
-template <int THREADS, int IT, bool NEWTON>
-__global__ void __launch_bounds__(THREADS)
+// NB = true: also build the neighbour lists (r2 < h2_i, reading 20).  The
+// unchecked loop then keeps the minimum r2 of each 8-j step (as many FMNMX as before) and compares
+// it with max(h2_i, rmin): only a step that holds a neighbour or a new nearest neighbour leaves
+// the packed code, re-evaluates its 8 separations from shared memory and appends to the list.
+template <int THREADS, int IT, bool NEWTON, bool NB = false>
+__global__ void __launch_bounds__(THREADS, (NB && THREADS * IT == 256) ? 3 : 1)
 k_force_fast(ForceArgs A)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -182,6 +186,8 @@ k_force_fast(ForceArgs A)
     int my[IT];
     double acc[IT][3], jrk[IT][3], pot[IT];
     int bstep[IT];          // the 8-j step (global numbering: address / 8) in which rmin last improved
+    float h2f[IT], thr[IT]; // NB: neighbour radius^2 and max(h2, rmin), the step-minimum that needs a look
+    int nbc[IT];            // NB: neighbours found so far in this CTA's j-range
 #pragma unroll
     for (int q = 0; q < IT; ++q) {
         const int i = (blockIdx.x * IT + q) * THREADS + tid;
@@ -189,6 +195,9 @@ k_force_fast(ForceArgs A)
         bstep[q] = -1;
         pot[q] = 0;
         I[q].rmin = INF;
+        h2f[q] = (NB && i < A.ni) ? (float)A.h2[i] : 0.0f;
+        thr[q] = INF;
+        nbc[q] = 0;
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
             float hi = 0.0f, lo = 0.0f, vv = 0.0f;
@@ -263,15 +272,40 @@ k_force_fast(ForceArgs A)
                                       make_float2(f[3].z, f[3].w), make_float2(f[4].z, f[4].w), make_float2(f[5].z, f[5].w),
                                       make_float2(f[6].z, f[6].w), make_float2(f[7].z, f[7].w), make_float2(f[8].z, f[8].w),
                                       make_float2(f[9].z, f[9].w), eps2, rb);
+                        if (NB) {
+                            // before[] is reused as the running minimum of this step
+                            if (h == 0) before[q] = fminf(fminf(ra.x, ra.y), fminf(rb.x, rb.y));
+                            else before[q] = fminf(fminf(fminf(ra.x, ra.y), before[q]), fminf(rb.x, rb.y));
+                        } else {
 #if !(defined(G6_ABLATE) && (G6_ABLATE & 1))
-                        I[q].rmin = fminf(fminf(ra.x, ra.y), I[q].rmin);
-                        I[q].rmin = fminf(fminf(rb.x, rb.y), I[q].rmin);
+                            I[q].rmin = fminf(fminf(ra.x, ra.y), I[q].rmin);
+                            I[q].rmin = fminf(fminf(rb.x, rb.y), I[q].rmin);
 #endif
+                        }
                     }
                 }
 #pragma unroll
-                for (int q = 0; q < IT; ++q)
-                    if (I[q].rmin < before[q]) bstep[q] = t * (JT / 8) + s8;
+                for (int q = 0; q < IT; ++q) {
+                    if (!NB) {
+                        if (I[q].rmin < before[q]) bstep[q] = t * (JT / 8) + s8;
+                    } else if (before[q] < thr[q]) {
+                        // rare: this step holds a neighbour or a new nearest neighbour
+                        if (before[q] < I[q].rmin) { I[q].rmin = before[q]; bstep[q] = t * (JT / 8) + s8; }
+                        if (before[q] < h2f[q]) {
+                            const float *Tf = sm.tile[st] + 8 * s8;
+                            const int i = (blockIdx.x * IT + q) * THREADS + tid;
+#pragma unroll
+                            for (int l = 0; l < 8; ++l) {
+                                const float dx = __fadd_rn(__fadd_rn(Tf[(F_XH + 0) * JT + l], I[q].nxh[0].x), __fadd_rn(Tf[(F_XL + 0) * JT + l], I[q].nxl[0].x));
+                                const float dy = __fadd_rn(__fadd_rn(Tf[(F_XH + 1) * JT + l], I[q].nxh[1].x), __fadd_rn(Tf[(F_XL + 1) * JT + l], I[q].nxl[1].x));
+                                const float dz = __fadd_rn(__fadd_rn(Tf[(F_XH + 2) * JT + l], I[q].nxh[2].x), __fadd_rn(Tf[(F_XL + 2) * JT + l], I[q].nxl[2].x));
+                                const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+                                if (r2 < h2f[q]) nb_append(A, s, i, nbc[q], t * JT + 8 * s8 + l);
+                            }
+                        }
+                        thr[q] = fmaxf(h2f[q], I[q].rmin);
+                    }
+                }
             }
         } else {
             // checked tile: mask out j >= nj and index_j == index_i (mass -> 0, r2 -> +inf)
@@ -309,6 +343,14 @@ k_force_fast(ForceArgs A)
                     I[q].rmin = fminf(fminf(o0 ? ra.x : INF, o1 ? ra.y : INF), I[q].rmin);
                     I[q].rmin = fminf(fminf(o2 ? rb.x : INF, o3 ? rb.y : INF), I[q].rmin);
                     if (I[q].rmin < before) bstep[q] = j0 >> 3;
+                    if (NB) {
+                        const int i = (blockIdx.x * IT + q) * THREADS + tid;
+                        if (o0 && ra.x < h2f[q]) nb_append(A, s, i, nbc[q], j0 + 0);
+                        if (o1 && ra.y < h2f[q]) nb_append(A, s, i, nbc[q], j0 + 1);
+                        if (o2 && rb.x < h2f[q]) nb_append(A, s, i, nbc[q], j0 + 2);
+                        if (o3 && rb.y < h2f[q]) nb_append(A, s, i, nbc[q], j0 + 3);
+                        thr[q] = fmaxf(h2f[q], I[q].rmin);
+                    }
                 }
             }
         }
@@ -368,6 +410,7 @@ k_force_fast(ForceArgs A)
         A.P.pot[o] = kP * pot[q];
         A.P.nn_r2[o] = baddr >= 0 ? I[q].rmin : INF;
         A.P.nn_addr[o] = baddr;
+        if (NB) A.nb_cnt[(size_t)s * A.ni + i] = nbc[q];
     }
 }
 
@@ -385,6 +428,15 @@ inline int fast_attr()
     e = cudaFuncSetAttribute(k_force_fast<THREADS, IT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     return (int)e;
 }
+template <int THREADS, int IT>
+inline int fast_attr_nb()
+{
+    const int bytes = (int)sizeof(FastSmem<THREADS, IT>);
+    cudaError_t e = cudaFuncSetAttribute(k_force_fast<THREADS, IT, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e != cudaSuccess) return (int)e;
+    e = cudaFuncSetAttribute(k_force_fast<THREADS, IT, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    return (int)e;
+}
 
 inline int fast_kernel_init()
 {
@@ -398,6 +450,11 @@ inline int fast_kernel_init()
     if ((r = fast_attr<128, 4>())) return r;
     if ((r = fast_attr<64, 2>())) return r;
     if ((r = fast_attr<64, 4>())) return r;
+    // neighbour-list variants: the shapes fast_pick chooses
+    if ((r = fast_attr_nb<128, 2>())) return r;
+    if ((r = fast_attr_nb<128, 1>())) return r;
+    if ((r = fast_attr_nb<64, 1>())) return r;
+    if ((r = fast_attr_nb<32, 1>())) return r;
     return 0;
 }
 
@@ -422,9 +479,35 @@ inline int fast_launch_t(const ForceArgs &A, bool newton, int n_itiles, int S, c
     return (int)cudaGetLastError();
 }
 
+template <int THREADS, int IT>
+inline int fast_launch_nb_t(const ForceArgs &A, bool newton, int n_itiles, int S, cudaStream_t st)
+{
+    dim3 grid(n_itiles, S);
+    const size_t bytes = sizeof(FastSmem<THREADS, IT>);
+    if (newton) k_force_fast<THREADS, IT, true, true><<<grid, THREADS, bytes, st>>>(A);
+    else k_force_fast<THREADS, IT, false, true><<<grid, THREADS, bytes, st>>>(A);
+    return (int)cudaGetLastError();
+}
+
+// is (threads, it) one of the shapes built with neighbour lists?
+inline bool fast_has_nb(FastVariant v)
+{
+    const int key = v.threads * 8 + v.it;
+    return key == 128 * 8 + 2 || key == 128 * 8 + 1 || key == 64 * 8 + 1 || key == 32 * 8 + 1;
+}
+
 inline int launch_force_fast(const ForceArgs &A, bool newton, FastVariant v, int n_itiles, int S, cudaStream_t st)
 {
     const int key = v.threads * 8 + v.it;
+    if (A.h2) {
+        switch (key) {
+            case 128 * 8 + 2: return fast_launch_nb_t<128, 2>(A, newton, n_itiles, S, st);
+            case 128 * 8 + 1: return fast_launch_nb_t<128, 1>(A, newton, n_itiles, S, st);
+            case 64 * 8 + 1: return fast_launch_nb_t<64, 1>(A, newton, n_itiles, S, st);
+            case 32 * 8 + 1: return fast_launch_nb_t<32, 1>(A, newton, n_itiles, S, st);
+            default: return (int)cudaErrorInvalidValue;
+        }
+    }
     switch (key) {
         case 128 * 8 + 2: return fast_launch_t<128, 2>(A, newton, n_itiles, S, st);
         case 128 * 8 + 1: return fast_launch_t<128, 1>(A, newton, n_itiles, S, st);
@@ -440,12 +523,24 @@ inline int launch_force_fast(const ForceArgs &A, bool newton, FastVariant v, int
 }
 
 // resident CTAs per SM of a variant (for the j-split scheduler)
-template <int THREADS, int IT>
+template <int THREADS, int IT, bool NB = false>
 inline int fast_occ_t()
 {
     int n = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_force_fast<THREADS, IT, true>, THREADS, sizeof(FastSmem<THREADS, IT>)) != cudaSuccess) return 1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_force_fast<THREADS, IT, true, NB>, THREADS, sizeof(FastSmem<THREADS, IT>)) != cudaSuccess) return 1;
     return n > 0 ? n : 1;
+}
+inline int fast_ctas_per_sm_nb(FastVariant v)
+{
+    static int cache[4] = {0};
+    const int key = v.threads * 8 + v.it;
+    switch (key) {
+        case 128 * 8 + 2: return cache[0] ? cache[0] : (cache[0] = fast_occ_t<128, 2, true>());
+        case 128 * 8 + 1: return cache[1] ? cache[1] : (cache[1] = fast_occ_t<128, 1, true>());
+        case 64 * 8 + 1: return cache[2] ? cache[2] : (cache[2] = fast_occ_t<64, 1, true>());
+        case 32 * 8 + 1: return cache[3] ? cache[3] : (cache[3] = fast_occ_t<32, 1, true>());
+        default: return 1;
+    }
 }
 inline int fast_ctas_per_sm(FastVariant v)
 {

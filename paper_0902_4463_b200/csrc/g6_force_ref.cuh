@@ -25,7 +25,19 @@ struct ForceArgs {
     int ds;                   // 0: pure-FP32 positions (lo words dropped)
     int S;                    // number of j-splits (gridDim.y)
     Partials P;
+    // neighbour lists (reading 20); h2 == nullptr: none
+    const double *h2;         // [ni] neighbour-sphere radius squared
+    int nb_maxlen;            // entries stored per (split, i)
+    int *nb_cnt;              // [S][ni]          neighbours found by split s (may exceed nb_maxlen)
+    int *nb_list;             // [S][ni][maxlen]  their j addresses, increasing
 };
+
+// append j address `ja` to the list of (split s, i-particle i); `cnt` is the thread's running count
+__device__ __forceinline__ void nb_append(const ForceArgs &A, int s, int i, int &cnt, int ja)
+{
+    if (cnt < A.nb_maxlen) A.nb_list[((size_t)s * A.ni + i) * A.nb_maxlen + cnt] = ja;
+    ++cnt;
+}
 
 constexpr int REF_THREADS = 128;
 
@@ -60,6 +72,9 @@ k_force_ref(ForceArgs A)
     double acc[3] = {0, 0, 0}, jrk[3] = {0, 0, 0}, pot = 0;
     float best = __int_as_float(0x7f800000);
     int baddr = -1;
+    // neighbour sphere: unsoftened r2 < h2, compared in binary32 like the nearest neighbour (reading 20)
+    const float h2f = (active && A.h2) ? (float)A.h2[i] : 0.0f;
+    int nbc = 0;
 
     for (int t = t0; t < t1; ++t) {
         __syncthreads();
@@ -104,6 +119,7 @@ k_force_ref(ForceArgs A)
             j32[1] = __fmaf_rn(mrinv3, __fmaf_rn(alpha, dy, dvy), j32[1]);
             j32[2] = __fmaf_rn(mrinv3, __fmaf_rn(alpha, dz, dvz), j32[2]);
             if (ok && r2 < best) { best = r2; baddr = t * JT + l; }
+            if (ok && r2 < h2f) nb_append(A, s, i, nbc, t * JT + l);
         }
         // FP32 chains are at most JT pairs long; fold into fp64 (reading 9)
 #pragma unroll
@@ -118,6 +134,7 @@ k_force_ref(ForceArgs A)
         A.P.pot[o] = pot;
         A.P.nn_r2[o] = best;
         A.P.nn_addr[o] = baddr;
+        if (A.h2) A.nb_cnt[(size_t)s * A.ni + i] = nbc;
     }
 }
 

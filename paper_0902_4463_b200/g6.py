@@ -22,6 +22,7 @@ SYMBOLS = [
     "g6_open", "g6_close", "g6_npipes", "g6_set_j_particle", "g6_set_ti", "g6calc_firsthalf",
     "g6calc_lasthalf", "g6calc_lasthalf2", "g6_read_neighbour_list", "g6_get_neighbour_list",
     "g6x_last_error", "g6x_set_npipes", "g6x_set_j_particles", "g6x_set_j_particles_dev", "g6x_calc_dev",
+    "g6x_calc_dev_nb", "g6x_get_neighbour_lists",
     "g6x_get_nearest", "g6x_set_stream", "g6x_synchronize", "g6x_get_timers", "g6x_set_option",
     "g6x_get_option", "g6x_get_predicted", "g6x_debug_dx", "g6x_version",
     "g6h_create", "g6h_destroy", "g6h_evolve", "g6h_get_state", "g6h_get_stats", "g6h_get_force_wall_hist",
@@ -115,8 +116,9 @@ def g6_set_ti(clusterid, ti):
 
 def g6calc_firsthalf(clusterid, nj, ni, index, xi, vi, acc_old=None, jerk6_old=None, phi_old=None, eps2=0.0, h2=None):
     index = _i32(index, (ni,)); xi = _f64(xi, (ni, 3)); vi = _f64(vi, (ni, 3))
+    h2p = _dp(_f64(h2, (ni,))) if h2 is not None else None
     return _chk(lib().g6calc_firsthalf(C.c_int(clusterid), C.c_int(nj), C.c_int(ni), _ip(index), _dp(xi), _dp(vi),
-                                       None, None, None, C.c_double(eps2), None), clusterid)
+                                       None, None, None, C.c_double(eps2), h2p), clusterid)
 
 
 def g6calc_lasthalf(clusterid, nj, ni, index=None, xi=None, vi=None, eps2=0.0, h2=None):
@@ -144,6 +146,13 @@ def g6_get_neighbour_list(clusterid, ipipe, maxlen=1):
     lst = np.zeros(max(maxlen, 1), np.int32)
     _chk(lib().g6_get_neighbour_list(C.c_int(clusterid), C.c_int(ipipe), C.c_int(maxlen), C.byref(n), _ip(lst)), clusterid)
     return lst[: n.value].copy()
+
+
+def g6x_get_neighbour_lists(clusterid, ni, maxlen):
+    """Returns (count[ni], list[ni, maxlen] padded with -1, number of truncated rows)."""
+    count = np.empty(ni, np.int32); lst = np.empty((ni, maxlen), np.int32)
+    over = _chk(lib().g6x_get_neighbour_lists(C.c_int(clusterid), C.c_int(ni), C.c_int(maxlen), _ip(count), _ip(lst)), clusterid)
+    return count, lst, over
 
 
 # ---- extensions ----------------------------------------------------------------------------------
@@ -197,6 +206,16 @@ def g6x_calc_dev(clusterid, nj, ni, d_index, d_xi, d_vi, eps2, d_acc, d_jerk, d_
                                    _dev(d_pot, f, ni), _dev(d_nn_index, i, ni), _dev(d_nn_r2, f, ni)), clusterid)
 
 
+def g6x_calc_dev_nb(clusterid, nj, ni, d_index, d_xi, d_vi, eps2, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2, d_h2, d_nb_count, d_nb_list):
+    import torch
+    f, i = torch.float64, torch.int32
+    return _chk(lib().g6x_calc_dev_nb(C.c_int(clusterid), C.c_int(nj), C.c_int(ni), _dev(d_index, i, ni), _dev(d_xi, f, 3 * ni),
+                                      _dev(d_vi, f, 3 * ni), C.c_double(eps2), _dev(d_acc, f, 3 * ni), _dev(d_jerk, f, 3 * ni),
+                                      _dev(d_pot, f, ni), _dev(d_nn_index, i, ni), _dev(d_nn_r2, f, ni), _dev(d_h2, f, ni),
+                                      _dev(d_nb_count, i, ni), _dev(d_nb_list, i, d_nb_list.numel() if d_nb_list is not None else 0)),
+                clusterid)
+
+
 def g6x_get_nearest(clusterid, ni):
     idx = np.empty(ni, np.int32); r2 = np.empty(ni)
     _chk(lib().g6x_get_nearest(C.c_int(clusterid), C.c_int(ni), _ip(idx), _dp(r2)), clusterid)
@@ -244,10 +263,10 @@ def g6x_debug_dx(clusterid, ipipe, jaddr):
 
 
 # ---- convenience (still only calls the functions above) ------------------------------------------
-def force_host(clusterid, index, xi, vi, eps2, nj):
+def force_host(clusterid, index, xi, vi, eps2, nj, h2=None):
     """firsthalf + lasthalf2 + nearest-neighbour distances through HOST buffers."""
     ni = len(index)
-    g6calc_firsthalf(clusterid, nj, ni, index, xi, vi, eps2=eps2)
+    g6calc_firsthalf(clusterid, nj, ni, index, xi, vi, eps2=eps2, h2=h2)
     acc, jerk, pot, nn = g6calc_lasthalf2(clusterid, nj, ni, eps2=eps2)
     _, r2 = g6x_get_nearest(clusterid, ni)
     return dict(acc=acc, jerk=jerk, pot=pot, nn_index=nn, nn_r2=r2)

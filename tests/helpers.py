@@ -55,3 +55,43 @@ def check_forces(got, ref, what=""):
     assert ej.max() <= TOL_JERK_MAX, (what, stats)
     assert ep.max() <= TOL_POT_MAX, (what, stats)
     return stats
+
+
+TOL_NB = 1e-6          # neighbour lists: membership exact except pairs with |r2 - h2| <= TOL_NB h2
+
+
+def check_neighbours(got_count, got_list, orc_count, orc_list, index_j, xi, xj, h2, maxlen, tol=TOL_NB):
+    """Neighbour lists of the CUDA path (callers' indices, -1 padded rows) against the oracle's
+    (j addresses, NOT truncated: call the oracle with a maxlen above every count).  The sphere
+    test r2 < h2 is taken in binary32 on the GPU and in fp64 by the oracle, so a pair whose fp64
+    r2 is within `tol` (relative) of h2 may fall on either side; everything else must agree:
+    compare what is unique, check that the rest is valid.  Lists must be in increasing j address
+    and, on overflow, hold the neighbours with the smallest addresses.  Returns the number of
+    borderline disagreements."""
+    addr_of = {int(ix): a for a, ix in enumerate(index_j)}
+    n_border = 0
+    for i in range(len(got_count)):
+        row = got_list[i]
+        G = [addr_of[int(ix)] for ix in row[row >= 0]]
+        assert all(a < b for a, b in zip(G, G[1:])), f"i={i}: list not in increasing j address: {G[:8]}..."
+        assert len(G) == min(int(got_count[i]), maxlen), (i, len(G), int(got_count[i]), maxlen)
+        assert int(orc_count[i]) <= orc_list.shape[1], "oracle list truncated: raise its maxlen"
+        O = [int(a) for a in orc_list[i, : orc_count[i]]]
+
+        def border(a):
+            r2 = float(np.sum((xj[a] - xi[i]) ** 2))
+            return abs(r2 - h2[i]) <= tol * h2[i]
+
+        if got_count[i] <= maxlen and orc_count[i] <= maxlen:
+            sym = set(G) ^ set(O)
+        else:
+            # overflow: stored entries are valid, and no neighbour below the last stored address is missing
+            last = G[-1] if len(G) == maxlen else np.inf
+            sym = (set(G) - set(O)) | {a for a in O if a < last and a not in set(G)}
+            r2 = np.sum((xj - xi[i]) ** 2, axis=1)
+            nb = int(np.sum(np.abs(r2 - h2[i]) <= tol * h2[i]))
+            assert abs(int(got_count[i]) - int(orc_count[i])) <= nb, (i, int(got_count[i]), int(orc_count[i]), nb)
+        for a in sym:
+            assert border(a), f"i={i}: j address {a} in one list only and not borderline (h2={h2[i]!r})"
+        n_border += len(sym)
+    return n_border

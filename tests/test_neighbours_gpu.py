@@ -1,0 +1,152 @@
+"""GPU parity of the neighbour lists (reading 20):
+the CUDA path through the C ABI against oracle.neighbours on the same seeded inputs."""
+import numpy as np
+import pytest
+
+from paper_0902_4463_b200 import g6, inputs
+from helpers import check_forces, check_neighbours, check_nn, load_j
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture()
+def cluster():
+    from paper_0902_4463_b200 import build
+    build.build()
+    g6.g6_open(0)
+    g6.g6x_set_npipes(1 << 21)
+    yield 0
+    g6.g6_close(0)
+    g6.g6x_set_npipes(g6.DEFAULT_NPIPES)
+
+
+def radii(x, idx_i, seed, lo=0.2, hi=3.0):
+    """h2 per i-particle: (lo..hi x the local mean spacing)^2, so that counts run from 0 to some tens"""
+    rng = np.random.default_rng(seed)
+    n = len(x)
+    r = np.linalg.norm(x[idx_i], axis=1)
+    a = 3 * np.pi / 16
+    rho = 3 / (4 * np.pi * a ** 3) * (1 + (r / a) ** 2) ** -2.5 * n        # Plummer number density
+    return (rng.uniform(lo, hi, len(idx_i)) * rho ** (-1.0 / 3)) ** 2
+
+
+def run(idx_i, xi, vi, eps2, nj, h2, maxlen):
+    got = g6.force_host(0, idx_i, xi, vi, eps2, nj, h2=h2)
+    over = g6.g6_read_neighbour_list(0)
+    cnt, lst, over2 = g6.g6x_get_neighbour_lists(0, len(idx_i), maxlen)
+    assert over == int(np.sum(cnt > maxlen)) == over2
+    return got, cnt, lst
+
+
+@pytest.mark.parametrize("kernel", [0, 1, 2])
+@pytest.mark.parametrize("jsplit", [0, 1, 3])
+def test_c1_lists_every_particle(cluster, oracle, kernel, jsplit):
+    x, v, m, eps2 = inputs.config("C1")
+    n = len(m)
+    idx = load_j(x, v, m)
+    h2 = radii(x, idx, 5)
+    g6.g6x_set_option(0, "kernel", kernel); g6.g6x_set_option(0, "jsplit", jsplit)
+    g6.g6_set_ti(0, 0.0)
+    got, cnt, lst = run(idx, x, v, eps2, n, h2, 256)
+    oc, ol = oracle.neighbours(idx, x, h2, idx, x, maxlen=1024)
+    assert oc.max() > 20 and (oc == 0).any()              # the recipe spans empty and well-filled lists
+    nb = check_neighbours(cnt, lst, oc, ol, idx, x, x, h2, 256)
+    # forces and nearest neighbour are unchanged by the list building
+    ref = oracle.force(idx, x, v, idx, x, v, m, eps2)
+    check_forces(got, ref, "C1 with lists"); check_nn(got["nn_index"], ref, idx, x, x)
+    # the GRAPE-6 per-pipe call returns the same rows
+    for i in (0, 5, 1023):
+        row = g6.g6_get_neighbour_list(0, i, 256)
+        assert list(row) == list(lst[i][lst[i] >= 0])
+    print("C1 lists kernel", kernel, "jsplit", jsplit, "mean count", cnt.mean(), "max", cnt.max(), "borderline", nb)
+
+
+@pytest.mark.parametrize("kernel", [1, 2])
+def test_overflow_rule(cluster, oracle, kernel):
+    x, v, m, eps2 = inputs.config("C1", n=3000)
+    n = len(m)
+    idx = load_j(x, v, m)
+    h2 = radii(x, idx, 6, lo=1.0, hi=4.0)
+    g6.g6x_set_option(0, "kernel", kernel); g6.g6x_set_option(0, "nb_maxlen", 8)
+    g6.g6_set_ti(0, 0.0)
+    got, cnt, lst = run(idx, x, v, eps2, n, h2, 8)
+    oc, ol = oracle.neighbours(idx, x, h2, idx, x, maxlen=n)
+    assert (oc > 8).sum() > 100 and (oc <= 8).sum() > 100
+    check_neighbours(cnt, lst, oc, ol, idx, x, x, h2, 8)
+    assert g6.g6_read_neighbour_list(0) == int((cnt > 8).sum()) > 0
+    # per-pipe call: 1 = neighbours dropped
+    i = int(np.argmax(cnt))
+    n_out = g6.lib().g6_get_neighbour_list
+    import ctypes as C
+    nn = C.c_int(0); buf = (C.c_int * 8)()
+    assert n_out(0, i, 8, C.byref(nn), buf) == 1 and nn.value == 8
+    g6.g6x_set_option(0, "nb_maxlen", 256)
+
+
+@pytest.mark.parametrize("n,ni", [(4097, 130), (1000, 1), (257, 257), (5000, 3), (70000, 40)])
+def test_ragged_small_blocks_and_extremes(cluster, oracle, n, ni):
+    x, v, m, eps2 = inputs.config("C1", n=n)
+    idx = load_j(x, v, m)
+    sel = inputs.active_subset(n, ni, 99 + ni)
+    h2 = radii(x, sel, 7)
+    h2[0] = 0.0                    # nothing is inside an empty sphere
+    if ni > 2:
+        h2[1] = 1e6                # everything but the particle itself is inside this one: overflow
+    g6.g6_set_ti(0, 0.0)
+    got, cnt, lst = run(idx[sel], x[sel], v[sel], eps2, n, h2, 256)
+    oc, ol = oracle.neighbours(idx[sel], x[sel], h2, idx, x, maxlen=max(n, 256))
+    check_neighbours(cnt, lst, oc, ol, idx, x[sel], x, h2, 256)
+    assert cnt[0] == 0
+    if ni > 2:
+        assert cnt[1] == n - 1
+    ref = oracle.force(idx[sel], x[sel], v[sel], idx, x, v, m, eps2)
+    check_forces(got, ref, f"lists n={n} ni={ni}"); check_nn(got["nn_index"], ref, idx, x[sel], x)
+
+
+def test_lists_with_ti_not_tj_and_foreign_indices(cluster, oracle):
+    """i-particles that are also j-particles, predicted to a later time on both sides: the self pair
+    must stay out of the list although its separation is not zero (reading 4)."""
+    n, ni = 6000, 200
+    x, v, m, eps2 = inputs.config("C1", n=n)
+    tj, dtj, a0, j0 = inputs.taylor_state(n, 31)
+    index = (np.arange(n, dtype=np.int32) * 7 + 3).astype(np.int32)           # ids are not addresses
+    g6.g6x_set_j_particles(0, 0, index, tj, m, j0, a0, v, x)
+    ti = 0.0625
+    g6.g6_set_ti(0, ti)
+    xp, vp = oracle.predict(ti, tj, x, v, a0, j0)
+    sel = inputs.active_subset(n, ni, 12)
+    h2 = radii(x, sel, 8, lo=0.5, hi=2.5)
+    got, cnt, lst = run(index[sel], xp[sel], vp[sel], eps2, n, h2, 256)
+    oc, ol = oracle.neighbours(index[sel], xp[sel], h2, index, xp, maxlen=n)
+    # predicted positions differ by the FP32 Taylor increment: widen the borderline band accordingly
+    check_neighbours(cnt, lst, oc, ol, index, xp[sel], xp, h2, 256, tol=1e-4)
+    for k in range(ni):
+        assert index[sel[k]] not in lst[k]
+
+
+def test_c4_size_device_entry_sampled_block(cluster, oracle):
+    """BASELINE.json's full size (N = 2^20) in the launch shape bench.py times: a 4096-block through
+    g6x_calc_dev_nb, every row against the oracle."""
+    import torch
+    x, v, m, eps2 = inputs.config("C4")
+    n = len(m)
+    idx = np.arange(n, dtype=np.int32)
+    dev = torch.device("cuda:0")
+    t = lambda a, dt=torch.float64: torch.from_numpy(np.ascontiguousarray(a)).to(dev, dt)
+    z3 = torch.zeros(n, 3, dtype=torch.float64, device=dev)
+    g6.g6x_set_j_particles_dev(0, 0, n, t(idx, torch.int32), torch.zeros(n, dtype=torch.float64, device=dev), t(m), z3, z3, t(v), t(x))
+    g6.g6_set_ti(0, 0.0)
+    ni = 4096
+    sel = inputs.active_subset(n, ni, 4040 + ni)
+    h2 = radii(x, sel, 9, lo=0.3, hi=3.5)
+    acc = torch.empty(ni, 3, dtype=torch.float64, device=dev); jerk = torch.empty_like(acc)
+    pot = torch.empty(ni, dtype=torch.float64, device=dev); nn = torch.empty(ni, dtype=torch.int32, device=dev); r2 = torch.empty_like(pot)
+    cnt = torch.zeros(ni, dtype=torch.int32, device=dev); lst = torch.full((ni, 256), -1, dtype=torch.int32, device=dev)
+    g6.g6x_calc_dev_nb(0, n, ni, t(idx[sel], torch.int32), t(x[sel]), t(v[sel]), eps2, acc, jerk, pot, nn, r2, t(h2), cnt, lst)
+    g6.g6x_synchronize(0)
+    oc, ol = oracle.neighbours(idx[sel], x[sel], h2, idx, x, maxlen=8192)
+    nb = check_neighbours(cnt.cpu().numpy(), lst.cpu().numpy(), oc, ol, idx, x[sel], x, h2, 256)
+    ref = oracle.force(idx[sel], x[sel], v[sel], idx, x, v, m, eps2)
+    got = dict(acc=acc.cpu().numpy(), jerk=jerk.cpu().numpy(), pot=pot.cpu().numpy())
+    check_forces(got, ref, "C4 4096-block with lists")
+    print("C4 lists: mean count", oc.mean(), "max", oc.max(), "borderline", nb)
