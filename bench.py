@@ -150,18 +150,27 @@ def ni_sweep(g6, inputs, torch, dev, stream, flush, x, v, idx_all, n, eps2, peak
         res = {}
         for mode in ("cold", "warm"):
             tot, frc, prd, cmb = [], [], [], []
-            for k in range(reps + 3):
-                if mode == "cold":
-                    flush.zero_()
-                g6.g6_set_ti(0, (k % 2) * 2.0 ** -30)            # a new block time: the predictor runs again
-                e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
-                e0.record(stream)
-                g6.g6x_calc_dev(0, n, ni, d_ii, d_xi, d_vi, eps2, d_acc, d_jerk, d_pot, d_nn, d_r2)
-                e1.record(stream)
-                torch.cuda.synchronize()
-                tm = g6.g6x_get_timers(0)
-                if k >= 3:
-                    tot.append(e0.elapsed_time(e1) * 1e3); frc.append(tm["force_us"]); prd.append(tm["predict_us"]); cmb.append(tm["combine_us"])
+            # pass 1: the library's per-phase events (they cost ~10 us of stream time per call); pass 2: timers off,
+            # the step as a host code sees it (CUDA events around the call on the launching stream)
+            for timers in (1, 0):
+                g6.g6x_set_option(0, "timers", timers)
+                for k in range(reps + 3):
+                    if mode == "cold":
+                        flush.zero_()
+                    g6.g6_set_ti(0, (k % 2) * 2.0 ** -30)            # a new block time: the predictor runs again
+                    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+                    e0.record(stream)
+                    g6.g6x_calc_dev(0, n, ni, d_ii, d_xi, d_vi, eps2, d_acc, d_jerk, d_pot, d_nn, d_r2)
+                    e1.record(stream)
+                    torch.cuda.synchronize()
+                    if k < 3:
+                        continue
+                    if timers:
+                        tm = g6.g6x_get_timers(0)
+                        frc.append(tm["force_us"]); prd.append(tm["predict_us"]); cmb.append(tm["combine_us"])
+                    else:
+                        tot.append(e0.elapsed_time(e1) * 1e3)
+            g6.g6x_set_option(0, "timers", 1)
             res[mode] = dict(step_us=float(np.median(tot)), force_us=float(np.median(frc)), predict_us=float(np.median(prd)),
                              combine_us=float(np.median(cmb)), jsplits=tm["jsplits"], ctas=tm["force_ctas"])
         fused = ni <= g6.g6x_get_option(0, "small")

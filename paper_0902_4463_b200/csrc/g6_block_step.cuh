@@ -6,21 +6,27 @@
 // small blocks (fewer i than threads => several threads share an i and split the
 // j) is taken to its limit and the whole block step is fused:
 //
-//  * persistent CTAs (2 per SM), CTA c owns the raw j-tiles c, c+G, c+2G, ...  A raw tile (256
-//    particles x 76 B, g6_device.cuh) is staged global -> shared by ONE TMA bulk copy
-//    (cp.async.bulk + mbarrier complete_tx) into a 3-stage ring, so ~58 KB per CTA are in flight
-//    without costing a register -- that is what keeps HBM busy while the warps compute.
+//  * one persistent CTA of 8 warps per SM; CTA c owns the raw j-tiles c, c+G, c+2G, ...  A raw tile
+//    (256 particles x 76 B, g6_device.cuh) is staged global -> shared by ONE TMA bulk copy
+//    (cp.async.bulk + mbarrier complete_tx) into a ring of 9-11 slots that fills the SM's shared
+//    memory, so ~100-200 KB per SM are in flight without costing a register -- that is what keeps
+//    HBM busy while the warps compute.
+//  * THE WARPS ARE THE WORKERS: tile number `it` of the CTA is handled by warp it % 8 alone --
+//    no __syncthreads in the loop, one mbarrier per slot, and the warp that has read a slot into
+//    registers re-issues the copy of the tile NS ahead into it at once.  (With a block-wide
+//    predict / barrier / compute sequence all warps load, then all compute, and HBM idles half
+//    the time: measured 28 us per step at N_j = 2^20 whether or not the j-store sat in L2.)
 //  * a-1: the particles corrected in the previous step arrive INSIDE THE KERNEL PARAMETERS (no
-//    staging kernel, no PCIe read); the CTA that owns a particle's tile patches the staged copy
+//    staging kernel, no PCIe read); the warp that owns a particle's tile patches the staged copy
 //    and writes the record through to the j-store.  The i-block travels the same way.
-//  * a-2: the 128 threads predict the tile (Eq. 1-2, same routine as k_predict) into a
-//    double-buffered shared array; nothing predicted ever goes to HBM.
-//  * a-4: LANES OVER j: every lane holds 8 predicted j in registers; warp w loops over the
-//    i-particles w, w+4, ... (broadcast from shared memory) and evaluates its 8 pairs with the
-//    same packed FP32 arithmetic as the sweep kernel (double-single separations, Eq. 3); the 7
-//    sums of a (i, tile) are reduced over the warp by a transposing butterfly (9 shuffles instead
-//    of 35) and folded into fp64 accumulators in shared memory; the nearest neighbour by two
-//    warp-wide integer min-reductions (r2 bits, then address).
+//  * a-2: LANES OVER j: every lane predicts 8 j of the tile (Eq. 1-2, same routine as k_predict)
+//    straight into registers; nothing predicted ever goes to shared memory or HBM.
+//  * a-4: the warp loops over all i-particles of the block (broadcast from shared memory) and
+//    evaluates its 8 pairs per lane with the same packed FP32 arithmetic as the sweep kernel
+//    (double-single separations, Eq. 3); the 7 sums of a (i, tile) are reduced over the warp by a
+//    transposing butterfly (9 shuffles instead of 35) and folded into the warp's fp64 accumulators
+//    in shared memory; the nearest neighbour by two warp-wide integer min-reductions (r2 bits,
+//    then address).  At the end the 8 warps' sums are added in warp order.
 //  * a-5: each CTA writes one partial per i; the LAST CTA to finish (atomic ticket) sums the G
 //    partials in CTA order -- deterministic -- and writes the results, possibly straight into
 //    mapped host memory (a-6).
@@ -30,8 +36,9 @@
 
 namespace g6 {
 
-constexpr int BS_THREADS = 128;
-constexpr int BS_NSTAGE = 3;
+constexpr int BS_THREADS = 384;
+// raw-tile slots of the shared-memory ring (one CTA per SM owns all of its shared memory)
+__host__ __device__ constexpr int bs_nslots(int maxi) { return maxi <= 16 ? 10 : 8; }
 constexpr int BS_MAX_I = 64;
 
 // i-block and changed j-particles carried by value in the kernel parameters
@@ -62,18 +69,18 @@ struct BsArgs {
 
 template <int MAXI>
 struct BsSmem {
-    alignas(128) char raw[BS_NSTAGE][RAW_TILE_BYTES];
-    alignas(16) float pred[2][NF][JT];
-    alignas(16) int pidx[2][JT];
-    double acc[MAXI][8];
+    alignas(128) char raw[bs_nslots(MAXI)][RAW_TILE_BYTES];   // ring of raw tiles: tile `it` of the CTA lives in slot it % NS
+    double acc[BS_THREADS / 32][MAXI][8];                     // per-warp fp64 sums of every i
+    float r2[BS_THREADS / 32][MAXI];                          // per-warp nearest neighbour of every i
+    int addr[BS_THREADS / 32][MAXI];
     float ipart[MAXI][9];
     int iidx[MAXI];
-    float r2[MAXI];
-    int addr[MAXI];
     int uaddr[MAXI];
-    alignas(8) uint64_t full[BS_NSTAGE];
+    alignas(8) uint64_t full[bs_nslots(MAXI)];
+    volatile int armed[bs_nslots(MAXI)];                      // CTA tile number whose copy was last issued into the slot
     int is_last;
 };
+static_assert(sizeof(BsSmem<16>) <= 232448 && sizeof(BsSmem<64>) <= 232448, "block-step shared memory");
 
 // two consecutive j against one i, every pair checked.  `ok` in: address < nj && index differs.
 template <bool NEWTON>
@@ -149,20 +156,22 @@ k_block_step(const BsArgs A, const BsInline<MAXI> D)
     extern __shared__ __align__(128) unsigned char smem_raw[];
     BsSmem<MAXI> &sm = *reinterpret_cast<BsSmem<MAXI> *>(smem_raw);
     constexpr float INF = __builtin_huge_valf();
+    constexpr int NW = BS_THREADS / 32;
     const unsigned FULL = 0xffffffffu;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int G = gridDim.x, cta = blockIdx.x;
-    const int nt = cta < A.ntiles ? (A.ntiles - cta + G - 1) / G : 0;     // my tiles: cta, cta+G, ...
+    // The CTA (one per SM) owns the raw tiles cta, cta + G, ...; tile number `it` of that sequence is staged
+    // in ring slot it % NS and worked on by warp it % NW alone: the warps never wait for one another inside
+    // the loop (no __syncthreads), and NS > NW slots keep copies in flight while every warp computes.
+    constexpr int NS = bs_nslots(MAXI);
+    const int nt = cta < A.ntiles ? (A.ntiles - cta + G - 1) / G : 0;
 
     if (tid == 0) {
 #pragma unroll
-        for (int k = 0; k < BS_NSTAGE; ++k) mbar_init(&sm.full[k], 1);
+        for (int k = 0; k < NS; ++k) { mbar_init(&sm.full[k], 1); sm.armed[k] = k; }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    __syncthreads();
-    if (tid == 0) {
 #pragma unroll
-        for (int k = 0; k < BS_NSTAGE; ++k)
+        for (int k = 0; k < NS; ++k)
             if (k < nt) {
                 mbar_expect_tx(&sm.full[k], RAW_TILE_BYTES);
                 tma_load_1d(sm.raw[k], A.raw + (size_t)(cta + k * G) * RAW_TILE_BYTES, RAW_TILE_BYTES, &sm.full[k]);
@@ -181,70 +190,84 @@ k_block_step(const BsArgs A, const BsInline<MAXI> D)
     }
     for (int i = tid; i < MAXI; i += BS_THREADS) {
         if (i < A.ni) sm.iidx[i] = A.inline_i ? D.index[i] : A.i_index[i];
-        sm.r2[i] = INF;
-        sm.addr[i] = 0x7fffffff;
         sm.uaddr[i] = i < A.n_upd ? D.upd[i].addr : -1;
 #pragma unroll
-        for (int q = 0; q < 8; ++q) sm.acc[i][q] = 0.0;
+        for (int q = 0; q < NW; ++q) {
+            sm.r2[q][i] = INF;
+            sm.addr[q][i] = 0x7fffffff;
+#pragma unroll
+            for (int k = 0; k < 8; ++k) sm.acc[q][i][k] = 0.0;
+        }
     }
     __syncthreads();
 
     const float2 eps2 = dup(A.eps2);
-    for (int it = 0; it < nt; ++it) {
+    for (int it = w; it < nt; it += NW) {
         const int tile = cta + it * G;
-        const int st = it % BS_NSTAGE;
-        const int buf = it & 1;
-        mbar_wait(&sm.full[st], (uint32_t)(it / BS_NSTAGE) & 1u);
-        char *R = sm.raw[st];
+        const int slot = it % NS;
+        char *R = sm.raw[slot];
+        // the copy of THIS tile must have been issued before its phase is waited for (a parity wait
+        // cannot tell phase p+1 from the completed phase p-1)
+        if (it >= NS) {
+            uint32_t spins = 0;
+            while (sm.armed[slot] != it) { if (++spins > (1u << 26)) __trap(); }
+            __threadfence_block();
+        }
+        mbar_wait(&sm.full[slot], (uint32_t)(it / NS) & 1u);
 
-        // ---- a-1: particles corrected in the last step that live in this tile
+        // ---- a-1: particles corrected in the last step that live in this tile: patch the staged copy
+        // and write the record through to the j-store
         if (A.n_upd > 0) {
-            if (tid < A.n_upd && sm.uaddr[tid] / JT == tile) {
-                const JRecord r = D.upd[tid];
-                store_record(R, r.addr % JT, r);
-                store_record(A.raw + (size_t)tile * RAW_TILE_BYTES, r.addr % JT, r);
-            }
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            __syncthreads();
+            for (int u = lane; u < A.n_upd; u += 32)
+                if (sm.uaddr[u] / JT == tile) {
+                    const JRecord r = D.upd[u];
+                    store_record(R, r.addr % JT, r);
+                    store_record(A.raw + (size_t)tile * RAW_TILE_BYTES, r.addr % JT, r);
+                }
+            __syncwarp();
         }
-        // ---- a-2: predict the tile (2 j per thread) into pred[buf]
-#pragma unroll
-        for (int h = 0; h < JT / BS_THREADS; ++h) {
-            const int l = tid + h * BS_THREADS;
-            float f[NF];
-            if (tile * JT + l < A.nj) {
-                const float dt = (float)(A.ti - raw_t(R, l));
-#pragma unroll
-                for (int k = 0; k < 3; ++k)
-                    predict_coord(dt, raw_x(R, k, l), raw_v(R, k, l), raw_a2(R, k, l), raw_j6(R, k, l), A.ds, f[F_XH + k], f[F_XL + k], f[F_V + k]);
-                f[F_M] = raw_m(R, l);
-                sm.pidx[buf][l] = raw_idx(R, l);
-            } else {
-#pragma unroll
-                for (int k = 0; k < NF; ++k) f[k] = 0.0f;
-                sm.pidx[buf][l] = 0;
-            }
-#pragma unroll
-            for (int k = 0; k < NF; ++k) sm.pred[buf][k][l] = f[k];
-        }
-        __syncthreads();
-        // the raw stage is consumed: refill it with the tile NSTAGE ahead
-        if (tid == 0 && it + BS_NSTAGE < nt) {
-            mbar_expect_tx(&sm.full[st], RAW_TILE_BYTES);
-            tma_load_1d(sm.raw[st], A.raw + (size_t)(tile + BS_NSTAGE * G) * RAW_TILE_BYTES, RAW_TILE_BYTES, &sm.full[st]);
-        }
-
-        // ---- a-4: my 8 j (4 lane + [0,4) and 128 + 4 lane + [0,4)) -> registers
+        // ---- a-2: predict my 8 j (4 lane + [0,4) and 128 + 4 lane + [0,4)) straight into registers
+        // (Eq. 1-2, same routine as k_predict); nothing predicted ever goes to memory
         float4 jf[NF][2];
         int4 jx[2];
+        const int ja0 = tile * JT + 4 * lane;
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
+            const int l0 = 4 * lane + 128 * h;
+            float f[4][NF];
+            int id[4];
 #pragma unroll
-            for (int k = 0; k < NF; ++k) jf[k][h] = reinterpret_cast<const float4 *>(sm.pred[buf][k])[32 * h + lane];
-            jx[h] = reinterpret_cast<const int4 *>(sm.pidx[buf])[32 * h + lane];
+            for (int e = 0; e < 4; ++e) {
+                const int l = l0 + e;
+                if (tile * JT + l < A.nj) {
+                    const float dt = (float)(A.ti - raw_t(R, l));
+#pragma unroll
+                    for (int k = 0; k < 3; ++k)
+                        predict_coord(dt, raw_x(R, k, l), raw_v(R, k, l), raw_a2(R, k, l), raw_j6(R, k, l), A.ds, f[e][F_XH + k], f[e][F_XL + k], f[e][F_V + k]);
+                    f[e][F_M] = raw_m(R, l);
+                    id[e] = raw_idx(R, l);
+                } else {
+#pragma unroll
+                    for (int k = 0; k < NF; ++k) f[e][k] = 0.0f;
+                    id[e] = 0;
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < NF; ++k) jf[k][h] = make_float4(f[0][k], f[1][k], f[2][k], f[3][k]);
+            jx[h] = make_int4(id[0], id[1], id[2], id[3]);
         }
-        const int ja0 = tile * JT + 4 * lane;              // addresses ja0 .. ja0+3 and ja0+128 .. ja0+131
-        for (int i = w; i < A.ni; i += BS_THREADS / 32) {
+        // the slot is consumed: refill it with the tile NS ahead while the forces are computed
+        __syncwarp();
+        if (lane == 0 && it + NS < nt) {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            mbar_expect_tx(&sm.full[slot], RAW_TILE_BYTES);
+            tma_load_1d(R, A.raw + (size_t)(tile + NS * G) * RAW_TILE_BYTES, RAW_TILE_BYTES, &sm.full[slot]);
+            __threadfence_block();
+            sm.armed[slot] = it + NS;
+        }
+
+        // ---- a-4: every i-particle of the block against my 8 j
+        for (int i = 0; i < A.ni; ++i) {
             IPart I;
 #pragma unroll
             for (int k = 0; k < 3; ++k) {
@@ -276,12 +299,12 @@ k_block_step(const BsArgs A, const BsInline<MAXI> D)
                                  __fadd_rn(I.j[0].x, I.j[0].y), __fadd_rn(I.j[1].x, I.j[1].y), __fadd_rn(I.j[2].x, I.j[2].y),
                                  __fadd_rn(I.p.x, I.p.y), 0.0f};
             const float tot = transpose_reduce8(v8, lane);
-            if ((lane & 3) == 0) sm.acc[i][lane >> 2] += (double)tot;
+            if ((lane & 3) == 0) sm.acc[w][i][lane >> 2] += (double)tot;
             // nearest neighbour: min r2 over the warp (non-negative floats order like unsigned integers)
             float lmin = fminf(fminf(r2m[0].x, r2m[0].y), fminf(r2m[1].x, r2m[1].y));
             lmin = fminf(lmin, fminf(fminf(r2m[2].x, r2m[2].y), fminf(r2m[3].x, r2m[3].y)));
             const unsigned gbits = __reduce_min_sync(FULL, __float_as_uint(lmin));
-            if (gbits < __float_as_uint(sm.r2[i])) {        // strict: earlier tiles (lower addresses) keep ties
+            if (gbits < __float_as_uint(sm.r2[w][i])) {     // strict: my earlier tiles (lower addresses) keep ties
                 int cand = 0x7fffffff;
                 if (__float_as_uint(r2m[3].y) == gbits) cand = ja0 + 128 + 3;
                 if (__float_as_uint(r2m[3].x) == gbits) cand = ja0 + 128 + 2;
@@ -293,22 +316,35 @@ k_block_step(const BsArgs A, const BsInline<MAXI> D)
                 if (__float_as_uint(r2m[0].x) == gbits) cand = ja0 + 0;
                 const int gaddr = __reduce_min_sync(FULL, cand);
                 __syncwarp();
-                if (lane == 0) { sm.r2[i] = __uint_as_float(gbits); sm.addr[i] = gaddr; }
+                if (lane == 0) { sm.r2[w][i] = __uint_as_float(gbits); sm.addr[w][i] = gaddr; }
             }
             __syncwarp();
         }
     }
     __syncthreads();
 
-    // ---- a-5, first half: one partial per (i, CTA)
+    // ---- a-5, first half: one partial per (i, CTA): the warps' sums in warp order
     for (int i = tid; i < A.ni; i += BS_THREADS) {
         const size_t o = (size_t)cta * A.P.stride_s + (size_t)i * A.P.stride_i;
+        double v[7];
 #pragma unroll
-        for (int k = 0; k < 3; ++k) { A.P.acc[k][o] = sm.acc[i][k]; A.P.jrk[k][o] = sm.acc[i][3 + k]; }
-        A.P.pot[o] = -sm.acc[i][6];
-        const bool has = sm.addr[i] != 0x7fffffff;
-        A.P.nn_r2[o] = has ? sm.r2[i] : INF;
-        A.P.nn_addr[o] = has ? sm.addr[i] : -1;
+        for (int k = 0; k < 7; ++k) v[k] = sm.acc[0][i][k];
+        float best = sm.r2[0][i];
+        int baddr = sm.addr[0][i];
+#pragma unroll
+        for (int q = 1; q < NW; ++q) {
+#pragma unroll
+            for (int k = 0; k < 7; ++k) v[k] += sm.acc[q][i][k];
+            const float r2 = sm.r2[q][i];
+            const int ad = sm.addr[q][i];
+            if (r2 < best || (r2 == best && ad < baddr)) { best = r2; baddr = ad; }
+        }
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { A.P.acc[k][o] = v[k]; A.P.jrk[k][o] = v[3 + k]; }
+        A.P.pot[o] = -v[6];
+        const bool has = baddr != 0x7fffffff;
+        A.P.nn_r2[o] = has ? best : INF;
+        A.P.nn_addr[o] = has ? baddr : -1;
     }
     __threadfence();
     __syncthreads();

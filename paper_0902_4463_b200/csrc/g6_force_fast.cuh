@@ -82,6 +82,9 @@ __device__ __forceinline__ float2 mul2(float2 a, float2 b) { return __fmul2_rn(a
 __device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
 
 constexpr float THIRD = 0.333333343267440796f;     // RN32(1/3)
+constexpr float FOUR_THIRDS = 1.33333337306976318f; // RN32(4/3)
+// pair2 works on sigma = SC s2 (s2 = r2 + eps2) so that the y it ends up with satisfies y^2 = 3 / s2 (see pair2)
+template <bool NEWTON> __host__ __device__ constexpr float pair_scale() { return NEWTON ? FOUR_THIRDS : THIRD; }
 
 // per-i-particle register state
 struct IPart {
@@ -91,7 +94,7 @@ struct IPart {
 };
 
 // One i-particle against two consecutive j-particles (packed lanes).  33 FMA-pipe packed
-// instructions (+4 with the Newton step), 2 MUFU, 1 FMNMX3.  MASKED: m and r2 already masked.
+// instructions (+3 with the Newton step), 2 MUFU, 1 FMNMX3.  MASKED: m and r2 already masked.
 template <bool NEWTON>
 __device__ __forceinline__ void pair2(IPart &I, const float2 xh, const float2 yh, const float2 zh, const float2 xl,
                                       const float2 yl, const float2 zl, const float2 vx, const float2 vy, const float2 vz,
@@ -105,20 +108,24 @@ __device__ __forceinline__ void pair2(IPart &I, const float2 xh, const float2 yh
     const float2 dvy = add2(vy, I.nv[1]);
     const float2 dvz = add2(vz, I.nv[2]);
     const float2 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
-    // s2/3 instead of s2 (one FFMA2 either way): y = rsqrt(s2/3) = sqrt(3)/s, so y^2 = 3/s^2 already carries
-    // the factor 3 of the jerk's radial term and alpha = -(dx.dv) y^2 needs no separate multiply.  The sums
-    // come out scaled by 3^(1/2) (pot) and 3^(3/2) (acc, jerk); k_force_fast undoes that exactly (with the
-    // binary32 value of THIRD) in fp64 when it writes its partials.  3 THIRD - 1 = 3e-8 only touches alpha.
-    const float2 s2 = fma2(r2, dup(THIRD), eps2_3);          // eps2_3 = THIRD * eps^2
+    // sigma = SC s2 instead of s2 (one FFMA2 either way), SC chosen so that the y used below has y^2 = 3 / s2:
+    // y^2 then already carries the factor 3 of the jerk's radial term and alpha = -(dx.dv) y^2 needs no separate
+    // multiply.  The sums come out scaled by y s (pot) and (y s)^3 (acc, jerk); k_force_fast undoes that exactly
+    // (with the binary32 value of SC) in fp64 when it writes its partials.  3 - y^2 s2 = 3e-8 only touches alpha.
+    //   no Newton step: SC = 1/3,  y = rsqrt(sigma) = sqrt(3) / s
+    //   Newton step   : SC = 4/3,  y0 = rsqrt(sigma);  y = y0 (3 - sigma y0^2) = TWICE the Newton-Raphson iterate
+    //                   y0 (3 - sigma y0^2) / 2, i.e. 2 / sqrt(sigma) = sqrt(3) / s: the halving is never done,
+    //                   the step costs 3 packed instructions (FMUL2, FFMA2, FMUL2) instead of 4.
+    const float2 s2 = fma2(r2, dup(pair_scale<NEWTON>()), eps2_3);          // eps2_3 = SC * eps^2
 #if defined(G6_ABLATE) && (G6_ABLATE & 2)
     float2 rinv = mul2(s2, dup(0.5f));
 #else
     float2 rinv = make_float2(rsqrt_approx(s2.x), rsqrt_approx(s2.y));
 #endif
     if (NEWTON) {
-        // y <- y - (y/2)(s2 y^2 - 1)
-        const float2 e = fma2(s2, mul2(rinv, rinv), dup(-1.0f));
-        rinv = fma2(mul2(dup(-0.5f), rinv), e, rinv);
+        const float2 ns2 = make_float2(-s2.x, -s2.y);       // folded into the FFMA2 operand modifier
+        const float2 u = fma2(ns2, mul2(rinv, rinv), dup(3.0f));
+        rinv = mul2(rinv, u);
     }
     const float2 rinv2 = mul2(rinv, rinv);
     const float2 mrinv = mul2(m, rinv);
@@ -150,7 +157,7 @@ struct FastSmem {
 // it with max(h2_i, rmin): only a step that holds a neighbour or a new nearest neighbour leaves
 // the packed code, re-evaluates its 8 separations from shared memory and appends to the list.
 template <int THREADS, int IT, bool NEWTON, bool NB = false>
-__global__ void __launch_bounds__(THREADS, (NB && THREADS * IT == 256) ? 3 : 1)
+__global__ void __launch_bounds__(THREADS, (NB && THREADS * IT == 256) ? 3 : 0)
 k_force_fast(ForceArgs A)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -213,8 +220,9 @@ k_force_fast(ForceArgs A)
             jrk[q][k] = 0;
         }
     }
-    const float2 eps2 = dup(THIRD * A.eps2);                 // pair2 works on s2 / 3
-    const double kP = sqrt((double)THIRD), kA = (double)THIRD * kP;
+    const float2 eps2 = dup(pair_scale<NEWTON>() * A.eps2);  // pair2 works on sigma = SC s2
+    // y s = 1 / kP: sqrt(3) nominally; exactly 1 / sqrt(SC) without and 2 / sqrt(SC) with the Newton step
+    const double kP = NEWTON ? 0.5 * sqrt((double)FOUR_THIRDS) : sqrt((double)THIRD), kA = kP * kP * kP;
 
     for (int it = 0; it < nt; ++it) {
         const int t = t0 + it;
