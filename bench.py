@@ -187,6 +187,43 @@ def ni_sweep(g6, inputs, torch, dev, stream, flush, x, v, idx_all, n, eps2, peak
     return rows
 
 
+def neighbour_list_cost(g6, inputs, torch, dev, x, v, idx_all, n, eps2, ni=65536, reps=3):
+    """What building neighbour lists costs (the paper: "a few tens of percent"): the same
+    65536-block against all N_j with and without lists; h2_i = (2 x the local mean spacing)^2 of the
+    Plummer model, i.e. ~30 neighbours per particle."""
+    f64 = torch.float64
+    ni = min(ni, n)
+    block = inputs.active_subset(n, ni, 4040 + ni)
+    to = lambda a, dt=f64: torch.from_numpy(np.ascontiguousarray(a)).to(dev, dt)
+    a = 3 * np.pi / 16
+    r = np.linalg.norm(x[block], axis=1)
+    rho = 3 / (4 * np.pi * a ** 3) * (1 + (r / a) ** 2) ** -2.5 * n
+    h2 = (2.0 * rho ** (-1.0 / 3)) ** 2
+    d_xi, d_vi, d_ii, d_h2 = to(x[block]), to(v[block]), to(idx_all[block], torch.int32), to(h2)
+    d_acc = torch.empty(ni, 3, dtype=f64, device=dev); d_jerk = torch.empty_like(d_acc)
+    d_pot = torch.empty(ni, dtype=f64, device=dev); d_nn = torch.empty(ni, dtype=torch.int32, device=dev); d_r2 = torch.empty_like(d_pot)
+    maxlen = g6.g6x_get_option(0, "nb_maxlen")
+    d_cnt = torch.zeros(ni, dtype=torch.int32, device=dev); d_lst = torch.empty(ni, maxlen, dtype=torch.int32, device=dev)
+    g6.g6_set_ti(0, 0.0)
+    out = {}
+    for name in ("without", "with"):
+        ts = []
+        for k in range(reps + 1):
+            if name == "with":
+                g6.g6x_calc_dev_nb(0, n, ni, d_ii, d_xi, d_vi, eps2, d_acc, d_jerk, d_pot, d_nn, d_r2, d_h2, d_cnt, d_lst)
+            else:
+                g6.g6x_calc_dev(0, n, ni, d_ii, d_xi, d_vi, eps2, d_acc, d_jerk, d_pot, d_nn, d_r2)
+            torch.cuda.synchronize()
+            tm = g6.g6x_get_timers(0)
+            if k > 0:
+                ts.append(tm["force_us"] + tm["combine_us"])
+        out[name] = float(np.median(ts))
+    cnt = d_cnt.cpu().numpy()
+    return {"n_i": ni, "force_plus_combine_us_without": out["without"], "force_plus_combine_us_with": out["with"],
+            "cost": out["with"] / out["without"] - 1.0, "mean_neighbours": float(cnt.mean()), "max_neighbours": int(cnt.max()),
+            "overflowed": int((cnt > maxlen).sum()), "nb_maxlen": maxlen}
+
+
 def run_reference(args):
     """--impl reference: the oracle, timed on the host cores on a bounded sample per step."""
     rank = int(os.environ.get("RANK", "0"))
@@ -357,8 +394,15 @@ def main():
                "note": "host arrays in, host arrays out (library stages through its own pinned buffers); includes the L2 flush"}
 
     sweep = None
+    nb_cost = None
+    ceilings = None
     if rank == 0 and world == 1 and not args.no_sweep:
         sweep = ni_sweep(g6, inputs, torch, dev, stream, flush, x, v, idx, n, eps2, measured_peaks()[0])
+        nb_cost = neighbour_list_cost(g6, inputs, torch, dev, x, v, idx, n, eps2)
+    if rank == 0:
+        # what the FP32 pipes sustain for register-sourced instructions (g6x_probe_fp32_peak, include/g6.h), measured live
+        ceilings = {name: max(g6.g6x_probe_fp32_peak(0, mode, c) for c in (3, 4, 8))
+                    for mode, name in ((0, "scalar_ffma"), (1, "ffma2_two_reused_operands"), (2, "fadd2_fmul2_ffma2_mix"), (3, "ffma2_three_distinct_sources"))}
 
     if rank == 0:
         peaks, peaks_src = measured_peaks()
@@ -378,6 +422,8 @@ def main():
                     "flops47_tflops": FLOP47 * inter_per_launch / (f_us * 1e-6) / 1e12,
                     "frac_at_measured_clock": (ach_inst / (SM_COUNT * FP32_LANES_PER_SM * clocks["sm_mhz"] * 1e6)) if clocks.get("sm_mhz") else None,
                     "kernel_share_of_step": f_us * args.steps / (ms_total * 1e3) if world == 1 else None,
+                    "measured_issue_ceiling_frac_of_peak": {k: v / peak_inst for k, v in ceilings.items()},
+                    "pipe_busy_equivalent": (FP32_INSTR_PER_INTERACTION + 3 * int(newton)) / FP32_INSTR_PER_INTERACTION * ach_inst / peak_inst,
                     "predictor_gbs": (n * (76 + 40)) / (float(np.mean(pred_us)) * 1e-6) / 1e9,
                     "hbm_peak_gbs": peaks.get("hbm_gbs")}
         out = {"metric": METRIC, "value": value, "unit": "interactions/s", "n_gpus": world, "steps": args.steps,
@@ -394,6 +440,8 @@ def main():
             out["e2e"] = e2e
         if sweep is not None:
             out["ni_sweep"] = sweep
+        if nb_cost is not None:
+            out["neighbour_lists"] = nb_cost
         if not args.no_cpu_baseline and world == 1:
             rate, rows, dt, cores = cpu_oracle_rate(x, v, m, eps2, idx, args.cpu_seconds)
             out["cpu_baseline"] = {"value": rate, "unit": "interactions/s", "cores": cores, "kind": "oracle",

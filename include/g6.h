@@ -215,6 +215,29 @@ int g6x_get_predicted(int clusterid, int addr0, int n, double xp[][3], double vp
  * the last host force call, j address jaddr[k]).  For the bit-exactness pin of DESIGN.md. */
 int g6x_debug_dx(int clusterid, int n, const int ipipe[], const int jaddr[], float dx[][3]);
 
+/* ---- multi-GPU j-split ("n/Q j-particles per GPU", the same i-particles on every GPU) ----
+ * Each process (one per GPU) loads its slice of the j-particles -- increasing address ranges by rank --
+ * and calls g6x_calc_dev on the SAME i-block; the partial acc/jerk/pot are then SUMMED over the
+ * processes and the nearest neighbour is the MINIMUM (ties -> lowest rank = lowest addresses).  The
+ * collectives themselves (two allreduces on device buffers: MIN on int64 keys, then SUM on fp64) are the
+ * caller's (NCCL through torch.distributed in paper_0902_4463_b200/sharding.py); these three calls are the
+ * device-side halves of the nearest-neighbour exchange.  All pointers are DEVICE pointers, work is
+ * asynchronous on the cluster's stream.  Neighbour lists are not exchanged.
+ *   pack    d_key[i] = (binary32 bits of d_nn_r2[i]) << 32 | rank, INT64_MAX when d_nn_index[i] < 0
+ *   select  d_index_f64[i] = d_nn_index[i] if this rank holds the minimum d_key_min[i], else 0
+ *   unpack  final d_nn_index / d_nn_r2 (either may be NULL) from the reduced keys and the summed index */
+int g6x_jsplit_pack_dev(int clusterid, int ni, int rank, const double *d_nn_r2, const int *d_nn_index, long long *d_key);
+int g6x_jsplit_select_dev(int clusterid, int ni, int rank, const long long *d_key_min, const int *d_nn_index, double *d_index_f64);
+int g6x_jsplit_unpack_dev(int clusterid, int ni, const long long *d_key_min, const double *d_index_sum, int *d_nn_index, double *d_nn_r2);
+
+/* Measurement aid (not part of the path): FP32 lane-instructions per second (an FMA counts once) that
+ * this device sustains for register-sourced instructions in independent chains, `ctas_per_sm` CTAs of
+ * 128 threads per SM (1..16).  mode 0: scalar FFMA; 1: packed FFMA2 with two loop-constant operands;
+ * 2: FADD2 / FMUL2 / FFMA2 in turn (the instruction kinds of the pair kernel); 3: FFMA2 with three
+ * distinct changing sources.  bench.py reports the force kernel against the nominal
+ * SMs x 128 lanes x clock AND against this measured issue ceiling. */
+int g6x_probe_fp32_peak(int clusterid, int mode, int ctas_per_sm, double *lane_instr_per_s);
+
 /* Library build information: a static string (arch, variant flags). */
 const char *g6x_version(void);
 

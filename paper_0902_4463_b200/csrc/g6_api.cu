@@ -19,6 +19,7 @@
 #include "g6_force_ref.cuh"
 #include "g6_force_fast.cuh"
 #include "g6_block_step.cuh"
+#include "g6_probe.cuh"
 
 using namespace g6;
 
@@ -1038,6 +1039,48 @@ int g6x_get_predicted(int clusterid, int addr0, int n, double xp[][3], double vp
             vp[p][k] = (double)t[(F_V + k) * JT];
         }
     }
+    return G6_OK;
+}
+
+int g6x_jsplit_pack_dev(int clusterid, int ni, int rank, const double *d_nn_r2, const int *d_nn_index, long long *d_key)
+{
+    GET_CLUSTER(clusterid);
+    if (ni < 1 || rank < 0 || !d_nn_r2 || !d_nn_index || !d_key) return fail(c, G6_ERR_ARG, "bad j-split pack arguments");
+    k_jsplit_pack<<<(ni + 255) / 256, 256, 0, c.stream>>>(ni, rank, d_nn_r2, d_nn_index, d_key);
+    CK(cudaGetLastError());
+    return G6_OK;
+}
+
+int g6x_jsplit_select_dev(int clusterid, int ni, int rank, const long long *d_key_min, const int *d_nn_index, double *d_index_f64)
+{
+    GET_CLUSTER(clusterid);
+    if (ni < 1 || rank < 0 || !d_key_min || !d_nn_index || !d_index_f64) return fail(c, G6_ERR_ARG, "bad j-split select arguments");
+    k_jsplit_select<<<(ni + 255) / 256, 256, 0, c.stream>>>(ni, rank, d_key_min, d_nn_index, d_index_f64);
+    CK(cudaGetLastError());
+    return G6_OK;
+}
+
+int g6x_jsplit_unpack_dev(int clusterid, int ni, const long long *d_key_min, const double *d_index_sum, int *d_nn_index, double *d_nn_r2)
+{
+    GET_CLUSTER(clusterid);
+    if (ni < 1 || !d_key_min || !d_index_sum) return fail(c, G6_ERR_ARG, "bad j-split unpack arguments");
+    k_jsplit_unpack<<<(ni + 255) / 256, 256, 0, c.stream>>>(ni, d_key_min, d_index_sum, d_nn_index, d_nn_r2);
+    CK(cudaGetLastError());
+    return G6_OK;
+}
+
+int g6x_probe_fp32_peak(int clusterid, int mode, int ctas_per_sm, double *lane_instr_per_s)
+{
+    GET_CLUSTER(clusterid);
+    if (c.pending) return fail(c, G6_ERR_SEQUENCE, "force call pending");
+    if (mode < 0 || mode > 3 || ctas_per_sm < 1 || ctas_per_sm > 16 || !lane_instr_per_s) return fail(c, G6_ERR_ARG, "bad probe arguments");
+    float *d_out = nullptr;
+    CK(cudaStreamSynchronize(c.stream));
+    CK(dalloc(d_out, (size_t)c.n_sm * ctas_per_sm * PROBE_THREADS));
+    const double r = probe_fp32(mode, c.n_sm, c.stream, d_out, ctas_per_sm);
+    dfree(d_out);
+    if (r < 0) return fail(c, G6_ERR_CUDA, "FP32 probe failed: %s", cudaGetErrorString(cudaGetLastError()));
+    *lane_instr_per_s = r;
     return G6_OK;
 }
 

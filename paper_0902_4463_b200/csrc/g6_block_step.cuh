@@ -226,35 +226,34 @@ k_block_step(const BsArgs A, const BsInline<MAXI> D)
                 }
             __syncwarp();
         }
-        // ---- a-2: predict my 8 j (4 lane + [0,4) and 128 + 4 lane + [0,4)) straight into registers
-        // (Eq. 1-2, same routine as k_predict); nothing predicted ever goes to memory
-        float4 jf[NF][2];
-        int4 jx[2];
-        const int ja0 = tile * JT + 4 * lane;
+        // ---- a-2: predict my 8 j straight into registers (Eq. 1-2, same routine as k_predict); nothing
+        // predicted ever goes to memory.  Lane l owns the pairs {2l, 2l+1} + 64 g, g = 0..3: one conflict-free
+        // vector load per field and pair (double2 / float2 / int2, consecutive lanes on consecutive addresses)
+        float2 jf[NF][4];
+        int2 jx[4];
+        const int ja0 = tile * JT + 2 * lane;                 // my pairs: ja0 + 64 g + {0, 1}
+        const bool ragged = tile * JT + JT > A.nj;            // only the last tile of the j-range
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const int l0 = 4 * lane + 128 * h;
-            float f[4][NF];
-            int id[4];
+        for (int g = 0; g < 4; ++g) {
+            const int l0 = 2 * lane + 64 * g;
+            const double2 tj = *reinterpret_cast<const double2 *>(R + RAW_T + 8 * l0);
+            const float2 dt = make_float2((float)(A.ti - tj.x), (float)(A.ti - tj.y));
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                const int l = l0 + e;
-                if (tile * JT + l < A.nj) {
-                    const float dt = (float)(A.ti - raw_t(R, l));
-#pragma unroll
-                    for (int k = 0; k < 3; ++k)
-                        predict_coord(dt, raw_x(R, k, l), raw_v(R, k, l), raw_a2(R, k, l), raw_j6(R, k, l), A.ds, f[e][F_XH + k], f[e][F_XL + k], f[e][F_V + k]);
-                    f[e][F_M] = raw_m(R, l);
-                    id[e] = raw_idx(R, l);
-                } else {
-#pragma unroll
-                    for (int k = 0; k < NF; ++k) f[e][k] = 0.0f;
-                    id[e] = 0;
-                }
+            for (int k = 0; k < 3; ++k) {
+                const double2 x0 = *reinterpret_cast<const double2 *>(R + RAW_X + 8 * (k * JT + l0));
+                const float2 v0 = *reinterpret_cast<const float2 *>(R + RAW_V + 4 * (k * JT + l0));
+                const float2 a2 = *reinterpret_cast<const float2 *>(R + RAW_A2 + 4 * (k * JT + l0));
+                const float2 j6 = *reinterpret_cast<const float2 *>(R + RAW_J6 + 4 * (k * JT + l0));
+                predict_coord(dt.x, x0.x, v0.x, a2.x, j6.x, A.ds, jf[F_XH + k][g].x, jf[F_XL + k][g].x, jf[F_V + k][g].x);
+                predict_coord(dt.y, x0.y, v0.y, a2.y, j6.y, A.ds, jf[F_XH + k][g].y, jf[F_XL + k][g].y, jf[F_V + k][g].y);
             }
+            jf[F_M][g] = *reinterpret_cast<const float2 *>(R + RAW_M + 4 * l0);
+            jx[g] = *reinterpret_cast<const int2 *>(R + RAW_IDX + 4 * l0);
+            if (ragged) {                                     // addresses >= nj: finite and massless
+                const bool in0 = ja0 + 64 * g < A.nj, in1 = ja0 + 64 * g + 1 < A.nj;
 #pragma unroll
-            for (int k = 0; k < NF; ++k) jf[k][h] = make_float4(f[0][k], f[1][k], f[2][k], f[3][k]);
-            jx[h] = make_int4(id[0], id[1], id[2], id[3]);
+                for (int k = 0; k < NF; ++k) jf[k][g] = make_float2(in0 ? jf[k][g].x : 0.0f, in1 ? jf[k][g].y : 0.0f);
+            }
         }
         // the slot is consumed: refill it with the tile NS ahead while the forces are computed
         __syncwarp();
@@ -281,18 +280,10 @@ k_block_step(const BsArgs A, const BsInline<MAXI> D)
             const int my = sm.iidx[i];
             float2 r2m[4];
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const int ja = ja0 + 128 * h;
-                pair2_checked<NEWTON>(I, make_float2(jf[0][h].x, jf[0][h].y), make_float2(jf[1][h].x, jf[1][h].y), make_float2(jf[2][h].x, jf[2][h].y),
-                                      make_float2(jf[3][h].x, jf[3][h].y), make_float2(jf[4][h].x, jf[4][h].y), make_float2(jf[5][h].x, jf[5][h].y),
-                                      make_float2(jf[6][h].x, jf[6][h].y), make_float2(jf[7][h].x, jf[7][h].y), make_float2(jf[8][h].x, jf[8][h].y),
-                                      make_float2(jf[9][h].x, jf[9][h].y), eps2, (ja + 0 < A.nj) && (jx[h].x != my), (ja + 1 < A.nj) && (jx[h].y != my),
-                                      r2m[2 * h]);
-                pair2_checked<NEWTON>(I, make_float2(jf[0][h].z, jf[0][h].w), make_float2(jf[1][h].z, jf[1][h].w), make_float2(jf[2][h].z, jf[2][h].w),
-                                      make_float2(jf[3][h].z, jf[3][h].w), make_float2(jf[4][h].z, jf[4][h].w), make_float2(jf[5][h].z, jf[5][h].w),
-                                      make_float2(jf[6][h].z, jf[6][h].w), make_float2(jf[7][h].z, jf[7][h].w), make_float2(jf[8][h].z, jf[8][h].w),
-                                      make_float2(jf[9][h].z, jf[9][h].w), eps2, (ja + 2 < A.nj) && (jx[h].z != my), (ja + 3 < A.nj) && (jx[h].w != my),
-                                      r2m[2 * h + 1]);
+            for (int g = 0; g < 4; ++g) {
+                const int ja = ja0 + 64 * g;
+                pair2_checked<NEWTON>(I, jf[0][g], jf[1][g], jf[2][g], jf[3][g], jf[4][g], jf[5][g], jf[6][g], jf[7][g], jf[8][g], jf[9][g], eps2,
+                                      (ja < A.nj) && (jx[g].x != my), (ja + 1 < A.nj) && (jx[g].y != my), r2m[g]);
             }
             // the 7 sums of this (i, tile): FP32 tree over the 256 j, then fp64 (reading 9)
             const float v8[8] = {__fadd_rn(I.a[0].x, I.a[0].y), __fadd_rn(I.a[1].x, I.a[1].y), __fadd_rn(I.a[2].x, I.a[2].y),
@@ -306,14 +297,11 @@ k_block_step(const BsArgs A, const BsInline<MAXI> D)
             const unsigned gbits = __reduce_min_sync(FULL, __float_as_uint(lmin));
             if (gbits < __float_as_uint(sm.r2[w][i])) {     // strict: my earlier tiles (lower addresses) keep ties
                 int cand = 0x7fffffff;
-                if (__float_as_uint(r2m[3].y) == gbits) cand = ja0 + 128 + 3;
-                if (__float_as_uint(r2m[3].x) == gbits) cand = ja0 + 128 + 2;
-                if (__float_as_uint(r2m[2].y) == gbits) cand = ja0 + 128 + 1;
-                if (__float_as_uint(r2m[2].x) == gbits) cand = ja0 + 128 + 0;
-                if (__float_as_uint(r2m[1].y) == gbits) cand = ja0 + 3;
-                if (__float_as_uint(r2m[1].x) == gbits) cand = ja0 + 2;
-                if (__float_as_uint(r2m[0].y) == gbits) cand = ja0 + 1;
-                if (__float_as_uint(r2m[0].x) == gbits) cand = ja0 + 0;
+#pragma unroll
+                for (int g = 3; g >= 0; --g) {               // descending, so the smallest address is kept
+                    if (__float_as_uint(r2m[g].y) == gbits) cand = ja0 + 64 * g + 1;
+                    if (__float_as_uint(r2m[g].x) == gbits) cand = ja0 + 64 * g;
+                }
                 const int gaddr = __reduce_min_sync(FULL, cand);
                 __syncwarp();
                 if (lane == 0) { sm.r2[w][i] = __uint_as_float(gbits); sm.addr[w][i] = gaddr; }

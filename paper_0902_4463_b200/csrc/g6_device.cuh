@@ -382,6 +382,47 @@ k_combine_nb(const int *__restrict__ part_cnt, const int *__restrict__ part_list
     if (lane == 0) cnt[i] = total;
 }
 
+// ---- multi-GPU j-split (section 2.4): the exchange step's device-side halves ----------
+// Every GPU holds N_j / Q of the j-particles (increasing address ranges by rank) and computes partial
+// forces on the SAME i-block; the partial (a, adot, phi) are summed and the nearest neighbour is the
+// minimum over the GPUs.  The paper sums on the host; here the two reductions are collectives on
+// device buffers (NCCL allreduce): MIN on a 64-bit key, then SUM on [8][ni] fp64.
+//   key = (bits of the binary32 r2) << 32 | rank      (non-negative floats order like integers; ties ->
+//         lowest rank = lowest address range, reading 7);  no neighbour -> INT64_MAX
+__global__ void __launch_bounds__(256)
+k_jsplit_pack(int ni, int rank, const double *__restrict__ nn_r2, const int *__restrict__ nn_index, long long *__restrict__ key)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= ni) return;
+    const long long none = 0x7fffffffffffffffLL;
+    const float r2 = (float)nn_r2[i];               // exact: the kernels produce r2 in binary32
+    key[i] = nn_index[i] < 0 ? none : (((long long)__float_as_uint(r2) << 32) | (long long)(unsigned)rank);
+}
+
+// after the MIN: the winning rank contributes its neighbour's index (as fp64, exact) to the SUM buffer
+__global__ void __launch_bounds__(256)
+k_jsplit_select(int ni, int rank, const long long *__restrict__ key_min, const int *__restrict__ nn_index, double *__restrict__ index_f64)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= ni) return;
+    const long long k = key_min[i];
+    const bool mine = k != 0x7fffffffffffffffLL && (int)(k & 0xffffffffLL) == rank;
+    index_f64[i] = mine ? (double)nn_index[i] : 0.0;
+}
+
+// after the SUM: final nearest neighbour of every i
+__global__ void __launch_bounds__(256)
+k_jsplit_unpack(int ni, const long long *__restrict__ key_min, const double *__restrict__ index_sum, int *__restrict__ nn_index,
+                double *__restrict__ nn_r2)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= ni) return;
+    const long long k = key_min[i];
+    const bool has = k != 0x7fffffffffffffffLL;
+    if (nn_index) nn_index[i] = has ? (int)index_sum[i] : -1;
+    if (nn_r2) nn_r2[i] = has ? (double)__uint_as_float((unsigned)(k >> 32)) : (double)__int_as_float(0x7f800000);
+}
+
 // ---- debug: the kernel's Eq.-3 separation for chosen (i, j) pairs (DESIGN.md pin P11) -------
 __global__ void k_debug_dx(int n, const int *__restrict__ ipipe, const int *__restrict__ jaddr,
                            const double *__restrict__ xi, int ds, const float *__restrict__ pred,

@@ -22,9 +22,9 @@ SYMBOLS = [
     "g6_open", "g6_close", "g6_npipes", "g6_set_j_particle", "g6_set_ti", "g6calc_firsthalf",
     "g6calc_lasthalf", "g6calc_lasthalf2", "g6_read_neighbour_list", "g6_get_neighbour_list",
     "g6x_last_error", "g6x_set_npipes", "g6x_set_j_particles", "g6x_set_j_particles_dev", "g6x_calc_dev",
-    "g6x_calc_dev_nb", "g6x_get_neighbour_lists",
+    "g6x_calc_dev_nb", "g6x_get_neighbour_lists", "g6x_jsplit_pack_dev", "g6x_jsplit_select_dev", "g6x_jsplit_unpack_dev",
     "g6x_get_nearest", "g6x_set_stream", "g6x_synchronize", "g6x_get_timers", "g6x_set_option",
-    "g6x_get_option", "g6x_get_predicted", "g6x_debug_dx", "g6x_version",
+    "g6x_get_option", "g6x_get_predicted", "g6x_debug_dx", "g6x_probe_fp32_peak", "g6x_version",
     "g6h_create", "g6h_destroy", "g6h_evolve", "g6h_get_state", "g6h_get_stats", "g6h_get_force_wall_hist",
 ]
 
@@ -260,6 +260,31 @@ def g6x_debug_dx(clusterid, ipipe, jaddr):
     _chk(lib().g6x_debug_dx(C.c_int(clusterid), C.c_int(n), _ip(ipipe), _ip(jaddr),
                             dx.ctypes.data_as(C.POINTER(C.c_float))), clusterid)
     return dx
+
+
+def g6x_jsplit_pack_dev(clusterid, ni, rank, d_nn_r2, d_nn_index, d_key):
+    import torch
+    return _chk(lib().g6x_jsplit_pack_dev(C.c_int(clusterid), C.c_int(ni), C.c_int(rank), _dev(d_nn_r2, torch.float64, ni),
+                                          _dev(d_nn_index, torch.int32, ni), _dev(d_key, torch.int64, ni)), clusterid)
+
+
+def g6x_jsplit_select_dev(clusterid, ni, rank, d_key_min, d_nn_index, d_index_f64):
+    import torch
+    return _chk(lib().g6x_jsplit_select_dev(C.c_int(clusterid), C.c_int(ni), C.c_int(rank), _dev(d_key_min, torch.int64, ni),
+                                            _dev(d_nn_index, torch.int32, ni), _dev(d_index_f64, torch.float64, ni)), clusterid)
+
+
+def g6x_jsplit_unpack_dev(clusterid, ni, d_key_min, d_index_sum, d_nn_index, d_nn_r2):
+    import torch
+    return _chk(lib().g6x_jsplit_unpack_dev(C.c_int(clusterid), C.c_int(ni), _dev(d_key_min, torch.int64, ni),
+                                            _dev(d_index_sum, torch.float64, ni), _dev(d_nn_index, torch.int32, ni),
+                                            _dev(d_nn_r2, torch.float64, ni)), clusterid)
+
+
+def g6x_probe_fp32_peak(clusterid, mode, ctas_per_sm=4):
+    r = C.c_double(0.0)
+    _chk(lib().g6x_probe_fp32_peak(C.c_int(clusterid), C.c_int(mode), C.c_int(ctas_per_sm), C.byref(r)), clusterid)
+    return r.value
 
 
 # ---- convenience (still only calls the functions above) ------------------------------------------
