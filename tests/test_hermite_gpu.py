@@ -102,7 +102,8 @@ def test_c2_full_run_vs_oracle_driven(cluster, oracle):
         dE = (_energy(oracle, xg, vg, m, eps2) - E0) / abs(E0)
         rep[f"library_newton{newton}"] = {"dE_over_E": dE, "block_steps": st["n_block_steps"], "particle_steps": st["n_particle_steps"],
                                           "interactions": st["interactions"], "wall_s": wall, "wall_force_calls_s": st["wall_force_s"],
-                                          "dt_min": st["dt_min"], "ni_hist_log2": [int(c) for c in st["ni_hist_log2"][:20]]}
+                                          "dt_min": st["dt_min"], "ni_hist_log2": [int(c) for c in st["ni_hist_log2"][:20]],
+                                          "force_wall_s_log2": [round(float(c), 4) for c in st["force_wall_s_log2"][:20]]}
         print(json.dumps({f"library_newton{newton}": rep[f"library_newton{newton}"]}), flush=True)
     t0 = time.perf_counter()
     ro = oracle.hermite(x, v, m, eps2, eta, t_end)
