@@ -349,14 +349,31 @@ k_block_step(const BsArgs A, const BsInline<MAXI> D)
         double v[7] = {0, 0, 0, 0, 0, 0, 0};
         float best = INF;
         int baddr = 0x7fffffff;
-        for (int s = lane; s < G; s += 32) {
-            const size_t o = (size_t)s * A.P.stride_s + (size_t)i * A.P.stride_i;
+        // all loads of a chunk of 5 x 32 partials are issued before the first is used (one L2 round trip instead
+        // of five); the lane still adds its partials s = lane, lane + 32, ... in that order
+        for (int s0 = 0; s0 < G; s0 += 160) {
+            double t[5][7];
+            float r2[5];
+            int ad[5];
 #pragma unroll
-            for (int k = 0; k < 3; ++k) { v[k] += __ldcg(A.P.acc[k] + o); v[3 + k] += __ldcg(A.P.jrk[k] + o); }
-            v[6] += __ldcg(A.P.pot + o);
-            const float r2 = __ldcg(A.P.nn_r2 + o);
-            const int ad = __ldcg(A.P.nn_addr + o);
-            if (ad >= 0 && (r2 < best || (r2 == best && ad < baddr))) { best = r2; baddr = ad; }
+            for (int q = 0; q < 5; ++q) {
+                const int sq = s0 + lane + 32 * q;
+                const bool in = sq < G;
+                const size_t o = (size_t)(in ? sq : 0) * A.P.stride_s + (size_t)i * A.P.stride_i;
+#pragma unroll
+                for (int k = 0; k < 3; ++k) { t[q][k] = in ? __ldcg(A.P.acc[k] + o) : 0.0; t[q][3 + k] = in ? __ldcg(A.P.jrk[k] + o) : 0.0; }
+                t[q][6] = in ? __ldcg(A.P.pot + o) : 0.0;
+                r2[q] = in ? __ldcg(A.P.nn_r2 + o) : INF;
+                ad[q] = in ? __ldcg(A.P.nn_addr + o) : -1;
+            }
+#pragma unroll
+            for (int q = 0; q < 5; ++q) {
+                if (s0 + lane + 32 * q < G) {
+#pragma unroll
+                    for (int k = 0; k < 7; ++k) v[k] += t[q][k];
+                    if (ad[q] >= 0 && (r2[q] < best || (r2[q] == best && ad[q] < baddr))) { best = r2[q]; baddr = ad[q]; }
+                }
+            }
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {

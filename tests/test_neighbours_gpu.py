@@ -150,3 +150,44 @@ def test_c4_size_device_entry_sampled_block(cluster, oracle):
     got = dict(acc=acc.cpu().numpy(), jerk=jerk.cpu().numpy(), pot=pot.cpu().numpy())
     check_forces(got, ref, "C4 4096-block with lists")
     print("C4 lists: mean count", oc.mean(), "max", oc.max(), "borderline", nb)
+
+
+def test_neighbour_abi_errors_and_maxlen_change(cluster, oracle):
+    import ctypes as C
+    x, v, m, eps2 = inputs.config("C1", n=600)
+    n = len(m)
+    idx = load_j(x, v, m)
+    g6.g6_set_ti(0, 0.0)
+    # a call without h2 builds no lists: the bulk getter refuses, the per-pipe getter returns the nearest neighbour
+    got = g6.force_host(0, idx, x, v, eps2, n)
+    assert g6.g6_read_neighbour_list(0) == 0
+    with pytest.raises(g6.G6Error) as e:
+        g6.g6x_get_neighbour_lists(0, n, 16)
+    assert e.value.code == -6
+    assert list(g6.g6_get_neighbour_list(0, 3, 4)) == [got["nn_index"][3]]
+    # bad option values
+    for bad in (0, 5000):
+        with pytest.raises(g6.G6Error) as e:
+            g6.g6x_set_option(0, "nb_maxlen", bad)
+        assert e.value.code == -8
+    # the three neighbour pointers of the device entry go together
+    import torch
+    d = torch.zeros(8, dtype=torch.float64, device="cuda:0")
+    L = g6.lib()
+    rc = L.g6x_calc_dev_nb(0, n, 1, C.c_void_p(d.data_ptr()), C.c_void_p(d.data_ptr()), C.c_void_p(d.data_ptr()), C.c_double(eps2),
+                           C.c_void_p(d.data_ptr()), C.c_void_p(d.data_ptr()), C.c_void_p(d.data_ptr()), None, None,
+                           C.c_void_p(d.data_ptr()), None, None)
+    assert rc == -8
+    # lists, then a different nb_maxlen: the old lists are gone (error), a new call works with the new length
+    h2 = radii(x, idx, 3, lo=1.0, hi=2.0)
+    run(idx, x, v, eps2, n, h2, 256)
+    g6.g6x_set_option(0, "nb_maxlen", 4)
+    got2, cnt, lst = run(idx, x, v, eps2, n, h2, 4)
+    oc, ol = oracle.neighbours(idx, x, h2, idx, x, maxlen=n)
+    check_neighbours(cnt, lst, oc, ol, idx, x, x, h2, 4)
+    # caller's buffer shorter than the stored list: truncated, return value 1
+    i = int(np.argmax(cnt))
+    nn = C.c_int(0); buf = (C.c_int * 2)()
+    assert L.g6_get_neighbour_list(0, i, 2, C.byref(nn), buf) == 1 and nn.value == 2
+    assert [buf[0], buf[1]] == list(lst[i][:2])
+    g6.g6x_set_option(0, "nb_maxlen", 256)
