@@ -138,6 +138,16 @@ def ni_sweep(g6, inputs, torch, dev, stream, flush, x, v, idx_all, n, eps2, peak
     sm_max = float(peaks.get("sm_max_mhz", SM_MAX_MHZ_FALLBACK))
     peak_inst = SM_COUNT * FP32_LANES_PER_SM * sm_max * 1e6
     rows = []
+    # floor of a block step at small n_i: a kernel that only reads the j-store once (same bytes, L2 flushed)
+    bare = []
+    for k in range(reps + 3):
+        flush.zero_()
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(stream); g6.g6x_probe_read_jstore(0, n); e1.record(stream)
+        torch.cuda.synchronize()
+        if k >= 3:
+            bare.append(e0.elapsed_time(e1) * 1e3)
+    bare_us = float(np.median(bare))
     for ni in NI_SWEEP:
         if ni > n:
             continue
@@ -180,6 +190,7 @@ def ni_sweep(g6, inputs, torch, dev, stream, flush, x, v, idx_all, n, eps2, peak
                      "interactions_per_s_cold": ni * float(n) / (c["step_us"] * 1e-6),
                      "interactions_per_s_warm": ni * float(n) / (res["warm"]["step_us"] * 1e-6),
                      "algorithmic_bytes_per_step": bytes_step,
+                     "bare_read_us": bare_us, "step_over_bare_read": c["step_us"] / bare_us,
                      "hbm_gbs_cold": bytes_step / (c["step_us"] * 1e-6) / 1e9,
                      "hbm_frac_cold": bytes_step / (c["step_us"] * 1e-6) / 1e9 / hbm,
                      "fp32_frac_force_kernel_cold": FP32_INSTR_PER_INTERACTION * ni * float(n) / (c["force_us"] * 1e-6) / peak_inst})

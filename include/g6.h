@@ -238,6 +238,12 @@ int g6x_jsplit_unpack_dev(int clusterid, int ni, const long long *d_key_min, con
  * SMs x 128 lanes x clock AND against this measured issue ceiling. */
 int g6x_probe_fp32_peak(int clusterid, int mode, int ctas_per_sm, double *lane_instr_per_s);
 
+/* Measurement aid (not part of the path): enqueue, on the cluster's stream, a kernel that does nothing but
+ * READ the raw j-store of addresses [0, nj) once (76 B per particle).  Timed by the caller with events on
+ * that stream, it is the floor for one block step at small n_i, which must make the same pass
+ * (bench.py `ni_sweep[].bare_read_us`). */
+int g6x_probe_read_jstore(int clusterid, int nj);
+
 /* Library build information: a static string (arch, variant flags). */
 const char *g6x_version(void);
 

@@ -611,8 +611,8 @@ int g6_open(int clusterid)
         c.stream = c.own_stream;
         CK(dalloc(c.js.raw, n / JT * RAW_TILE_BYTES));
         CK(cudaMemsetAsync(c.js.raw, 0, n / JT * RAW_TILE_BYTES, c.stream));
-        CK(dalloc(c.d_counter, 1));
-        CK(cudaMemsetAsync(c.d_counter, 0, sizeof(unsigned int), c.stream));
+        CK(dalloc(c.d_counter, 2));     // [0] ticket of the block-step kernel, [1] sink of the read probe
+        CK(cudaMemsetAsync(c.d_counter, 0, 2 * sizeof(unsigned int), c.stream));
         CK(dalloc(c.pred, n * NF));
         CK(dalloc(c.tile_imin, n / JT)); CK(dalloc(c.tile_imax, n / JT));
         for (auto &ev : c.ev) CK(cudaEventCreate(&ev));
@@ -1081,6 +1081,17 @@ int g6x_probe_fp32_peak(int clusterid, int mode, int ctas_per_sm, double *lane_i
     dfree(d_out);
     if (r < 0) return fail(c, G6_ERR_CUDA, "FP32 probe failed: %s", cudaGetErrorString(cudaGetLastError()));
     *lane_instr_per_s = r;
+    return G6_OK;
+}
+
+int g6x_probe_read_jstore(int clusterid, int nj)
+{
+    GET_CLUSTER(clusterid);
+    if (c.pending) return fail(c, G6_ERR_SEQUENCE, "force call pending");
+    if (nj < 1 || nj > c.capacity) return fail(c, G6_ERR_NJ, "nj = %d outside [1, capacity]", nj);
+    const size_t n16 = (size_t)((nj + JT - 1) / JT) * RAW_TILE_BYTES / 16;
+    k_probe_read<<<c.n_sm * 8, 256, 0, c.stream>>>(reinterpret_cast<const float4 *>(c.js.raw), n16, reinterpret_cast<float *>(c.d_counter + 1));
+    CK(cudaGetLastError());
     return G6_OK;
 }
 

@@ -67,6 +67,17 @@ struct BsArgs {
     double *nn_r2;
 };
 
+__device__ __forceinline__ int ld_acquire_cta(const volatile int *p)
+{
+    int v;
+    asm volatile("ld.acquire.cta.shared.s32 %0, [%1];" : "=r"(v) : "r"(smem_u32(const_cast<const int *>(p))) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_cta(volatile int *p, int v)
+{
+    asm volatile("st.release.cta.shared.s32 [%0], %1;" ::"r"(smem_u32(const_cast<int *>(p))), "r"(v) : "memory");
+}
+
 template <int MAXI>
 struct BsSmem {
     alignas(128) char raw[bs_nslots(MAXI)][RAW_TILE_BYTES];   // ring of raw tiles: tile `it` of the CTA lives in slot it % NS
@@ -210,8 +221,7 @@ k_block_step(const BsArgs A, const BsInline<MAXI> D)
         // cannot tell phase p+1 from the completed phase p-1)
         if (it >= NS) {
             uint32_t spins = 0;
-            while (sm.armed[slot] != it) { if (++spins > (1u << 26)) __trap(); }
-            __threadfence_block();
+            while (ld_acquire_cta(&sm.armed[slot]) != it) { if (++spins > (1u << 26)) __trap(); }
         }
         mbar_wait(&sm.full[slot], (uint32_t)(it / NS) & 1u);
 
@@ -244,8 +254,12 @@ k_block_step(const BsArgs A, const BsInline<MAXI> D)
                 const float2 v0 = *reinterpret_cast<const float2 *>(R + RAW_V + 4 * (k * JT + l0));
                 const float2 a2 = *reinterpret_cast<const float2 *>(R + RAW_A2 + 4 * (k * JT + l0));
                 const float2 j6 = *reinterpret_cast<const float2 *>(R + RAW_J6 + 4 * (k * JT + l0));
+#if defined(G6_ABLATE) && (G6_ABLATE & 4)      // experiment: no predictor arithmetic (positions truncated to binary32)
+                jf[F_XH + k][g] = make_float2((float)x0.x, (float)x0.y); jf[F_XL + k][g] = make_float2(dt.x * a2.x, dt.y * j6.y); jf[F_V + k][g] = v0;
+#else
                 predict_coord(dt.x, x0.x, v0.x, a2.x, j6.x, A.ds, jf[F_XH + k][g].x, jf[F_XL + k][g].x, jf[F_V + k][g].x);
                 predict_coord(dt.y, x0.y, v0.y, a2.y, j6.y, A.ds, jf[F_XH + k][g].y, jf[F_XL + k][g].y, jf[F_V + k][g].y);
+#endif
             }
             jf[F_M][g] = *reinterpret_cast<const float2 *>(R + RAW_M + 4 * l0);
             jx[g] = *reinterpret_cast<const int2 *>(R + RAW_IDX + 4 * l0);
@@ -258,15 +272,19 @@ k_block_step(const BsArgs A, const BsInline<MAXI> D)
         // the slot is consumed: refill it with the tile NS ahead while the forces are computed
         __syncwarp();
         if (lane == 0 && it + NS < nt) {
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            if (A.n_upd > 0) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // a-1 wrote the slot through the generic proxy
             mbar_expect_tx(&sm.full[slot], RAW_TILE_BYTES);
             tma_load_1d(R, A.raw + (size_t)(tile + NS * G) * RAW_TILE_BYTES, RAW_TILE_BYTES, &sm.full[slot]);
-            __threadfence_block();
-            sm.armed[slot] = it + NS;
+            st_release_cta(&sm.armed[slot], it + NS);
         }
 
         // ---- a-4: every i-particle of the block against my 8 j
+#if defined(G6_ABLATE) && (G6_ABLATE & 8)      // experiment: no force evaluation (the predicted j are only touched)
+        if (jf[0][0].x == 123.456f && jf[9][3].y == 1.0f) sm.r2[w][0] = jf[3][1].x + jf[7][2].y;
+        for (int i = A.ni; i < A.ni; ++i) {
+#else
         for (int i = 0; i < A.ni; ++i) {
+#endif
             IPart I;
 #pragma unroll
             for (int k = 0; k < 3; ++k) {

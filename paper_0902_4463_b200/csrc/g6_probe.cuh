@@ -68,4 +68,19 @@ inline double probe_fp32(int mode, int n_sm, cudaStream_t st, float *d_out, int 
     return best;
 }
 
+// the cheapest possible pass over `n16` 16-byte words: what a kernel that only READS the j-store costs
+__global__ void __launch_bounds__(256)
+k_probe_read(const float4 *__restrict__ p, size_t n16, float *out)
+{
+    float s = 0.0f;
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t st = (size_t)gridDim.x * blockDim.x;
+    for (; i + 3 * st < n16; i += 4 * st) {
+        const float4 a = __ldcs(p + i), b = __ldcs(p + i + st), c = __ldcs(p + i + 2 * st), d = __ldcs(p + i + 3 * st);
+        s += a.x + b.y + c.z + d.w;
+    }
+    for (; i < n16; i += st) s += __ldcs(p + i).x;
+    if (s == 123.456f) out[0] = s;          // keeps the loads alive
+}
+
 }  // namespace g6

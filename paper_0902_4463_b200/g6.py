@@ -24,7 +24,7 @@ SYMBOLS = [
     "g6x_last_error", "g6x_set_npipes", "g6x_set_j_particles", "g6x_set_j_particles_dev", "g6x_calc_dev",
     "g6x_calc_dev_nb", "g6x_get_neighbour_lists", "g6x_jsplit_pack_dev", "g6x_jsplit_select_dev", "g6x_jsplit_unpack_dev",
     "g6x_get_nearest", "g6x_set_stream", "g6x_synchronize", "g6x_get_timers", "g6x_set_option",
-    "g6x_get_option", "g6x_get_predicted", "g6x_debug_dx", "g6x_probe_fp32_peak", "g6x_version",
+    "g6x_get_option", "g6x_get_predicted", "g6x_debug_dx", "g6x_probe_fp32_peak", "g6x_probe_read_jstore", "g6x_version",
     "g6h_create", "g6h_destroy", "g6h_evolve", "g6h_get_state", "g6h_get_stats", "g6h_get_force_wall_hist",
 ]
 
@@ -285,6 +285,10 @@ def g6x_probe_fp32_peak(clusterid, mode, ctas_per_sm=4):
     r = C.c_double(0.0)
     _chk(lib().g6x_probe_fp32_peak(C.c_int(clusterid), C.c_int(mode), C.c_int(ctas_per_sm), C.byref(r)), clusterid)
     return r.value
+
+
+def g6x_probe_read_jstore(clusterid, nj):
+    return _chk(lib().g6x_probe_read_jstore(C.c_int(clusterid), C.c_int(nj)), clusterid)
 
 
 # ---- convenience (still only calls the functions above) ------------------------------------------
