@@ -51,6 +51,29 @@ int g6h_get_stats(g6h_system *s, double stats[8], long long ni_hist_log2[64]);
  * ni_hist_log2[b] (64 entries): where the time of a block-step run goes, by block size. */
 int g6h_get_force_wall_hist(g6h_system *s, double wall_s_log2[64]);
 
+/* ---- device-resident variant -----------------------------------------------
+ * The same integrator with the particle state kept in device memory and the O(n_i) steps -- block
+ * selection, prediction of the i-particles, corrector, step choice, j-store update --
+ * run as CUDA kernels; the force is the library's own path.  Per block step the host waits once, for
+ * (n_i, t_next).  The paper leaves these steps on the CPU because GRAPE host codes did.
+ * Same formulas as above, fp64 (the device contracts a*b+c into FMAs, so results agree with g6h_* to
+ * rounding, not bit for bit).  Same argument and error conventions; n <= the cluster's capacity. */
+typedef struct g6hd_system g6hd_system;
+
+g6hd_system *g6hd_create(int clusterid, int n, const double x[][3], const double v[][3], const double m[],
+                         double eps2, double eta, double eta_start, double dt_max);
+void g6hd_destroy(g6hd_system *s);
+int g6hd_evolve(g6hd_system *s, double t_end, long long max_block_steps);
+/* as g6h_get_state (Eq. 1-2 predictions to the system time, evaluated on the device) */
+int g6hd_get_state(g6hd_system *s, double x[][3], double v[][3]);
+/* stats[0..5] as g6h_get_stats ([6], [7] unused) */
+int g6hd_get_stats(g6hd_system *s, double stats[8], long long ni_hist_log2[64]);
+/* Raw per-particle Hermite state (each at its own time t[p]); any pointer may be NULL.  For parity tests. */
+int g6hd_get_particles(g6hd_system *s, double x[][3], double v[][3], double a[][3], double adot[][3], double t[], double dt[]);
+/* The last block step's i-block: *ni particles, their addresses, predicted x/v and the forces the corrector
+ * used (any array may be NULL; G6_ERR_ARG if *ni > maxn).  For parity tests of the corrector kernel. */
+int g6hd_get_last_block(g6hd_system *s, int maxn, int *ni, int act[], double xi[][3], double vi[][3], double acc[][3], double jerk[][3]);
+
 #ifdef __cplusplus
 }
 #endif

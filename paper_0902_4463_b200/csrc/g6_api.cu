@@ -574,7 +574,7 @@ int g6x_set_npipes(int npipes)
 
 const char *g6x_version(void)
 {
-    return "libg6b200 0.1 (sm_100a; FP32 + double-single separations; kernels: ref, fast[FFMA2+TMA])";
+    return "libg6b200 0.2 (sm_100a; FP32 + double-single separations; kernels: ref, fast[FFMA2+TMA, neighbour lists], block-step[TMA ring]; j-split exchange)";
 }
 
 const char *g6x_last_error(int clusterid)
@@ -1126,3 +1126,6 @@ int g6x_debug_dx(int clusterid, int n, const int ipipe[], const int jaddr[], flo
 }
 
 }  // extern "C"
+
+// device-resident Hermite integrator (g6hd_*, include/g6_hermite.h): needs the internals above
+#include "g6_hermite_dev_api.cuh"

@@ -1,0 +1,254 @@
+// g6_hermite_dev.cuh -- device-resident 4th-order Hermite block-step integrator:
+// the block selection, the prediction of the i-particles, the corrector and the step choice run on the
+// GPU, so that per block step only two numbers (n_i and the block time) cross to the host, instead of the
+// i-block, the forces and n_i calls of g6_set_j_particle.  The paper keeps these O(n_i) steps on the CPU
+// (Fig. 1) because the GRAPE host codes did; it names the force as the only O(N n_i) part
+// (PAPER.md:49).  Formulas: DESIGN.md reading 16 (Makino & Aarseth 1992 / Aarseth 1985, cited at
+// PAPER.md:31, :156), the same as the host driver g6_hermite.cpp, in fp64.
+//
+//   k_hd_select   t_next = min_p (t_p + dt_p); the active block = all p with t_p + dt_p == t_next, in
+//                 increasing address order; Eq. 1-2 prediction of those i-particles in
+//                 fp64 ("similarly implemented on the CPU" -- here on the device)
+//   force         the library's own path (run_force: block-step kernel or predictor + sweep kernel)
+//   k_hd_correct  corrector, Aarseth step, power-of-two quantisation, new j-store record
+#pragma once
+#include "g6_device.cuh"
+
+namespace g6 {
+
+struct HdState {
+    double *x, *v, *a, *ad;     // [n][3] at each particle's own time t
+    double *m, *t, *dt;         // [n]
+    int n;
+};
+
+// per-step scratch written by k_hd_select
+struct HdBlock {
+    int *act;                   // [n] active addresses, increasing
+    double *xi, *vi;            // [n][3] predicted i-particles
+    double *bmin;               // [nblocks] per-thread-block minimum of t + dt
+    int *bcnt;                  // [nblocks] particles of the block attaining it
+    unsigned int *ticket;
+    int *h_ni;                  // mapped host memory: n_i of the block ...
+    double *h_tnext;            // ... and its time
+    int *d_ni;                  // device copy of n_i (read by k_hd_correct)
+    double *d_tnext;
+};
+
+constexpr int HD_THREADS = 256;
+constexpr int HD_PER_BLOCK = 1024;      // particles per thread block of k_hd_select
+
+__device__ __forceinline__ double hd_block_min(double v, double *sm)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double r = sm[0];
+#pragma unroll
+    for (int w = 1; w < HD_THREADS / 32; ++w) r = fmin(r, sm[w]);
+    __syncthreads();
+    return r;
+}
+
+// Eq. 1-2 in fp64 for particle p at time tn
+__device__ __forceinline__ void hd_predict(const HdState &S, int p, double tn, double *xp, double *vp)
+{
+    const double h = tn - S.t[p], h2 = h * h / 2, h3 = h * h * h / 6;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const double x = S.x[3 * (size_t)p + k], v = S.v[3 * (size_t)p + k], a = S.a[3 * (size_t)p + k], ad = S.ad[3 * (size_t)p + k];
+        xp[k] = x + v * h + a * h2 + ad * h3;
+        vp[k] = v + a * h + ad * h2;
+    }
+}
+
+// One launch selects the next block.  Every thread block reduces its HD_PER_BLOCK particles to
+// (min of t + dt, how many attain it); the LAST thread block to finish (atomic ticket) takes the global
+// minimum and writes, block by block in address order, the active list and the predicted i-particles.
+// Small blocks touch a few thread blocks' particles again; a block of all N particles makes the last
+// thread block walk all N (a fraction of a per cent of the force time it precedes).
+__global__ void __launch_bounds__(HD_THREADS)
+k_hd_select(HdState S, HdBlock B)
+{
+    __shared__ double smin[HD_THREADS / 32];
+    __shared__ int scnt[HD_THREADS / 32];
+    __shared__ int s_last, s_base;
+    const int tid = threadIdx.x, b = blockIdx.x, nb = gridDim.x;
+    const int p0 = b * HD_PER_BLOCK;
+    double tn[HD_PER_BLOCK / HD_THREADS];
+    double lmin = __longlong_as_double(0x7ff0000000000000LL);
+#pragma unroll
+    for (int q = 0; q < HD_PER_BLOCK / HD_THREADS; ++q) {
+        const int p = p0 + q * HD_THREADS + tid;
+        tn[q] = p < S.n ? S.t[p] + S.dt[p] : __longlong_as_double(0x7ff0000000000000LL);
+        lmin = fmin(lmin, tn[q]);
+    }
+    const double bm = hd_block_min(lmin, smin);
+    int c = 0;
+#pragma unroll
+    for (int q = 0; q < HD_PER_BLOCK / HD_THREADS; ++q) c += tn[q] == bm;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+    if ((tid & 31) == 0) scnt[tid >> 5] = c;
+    __syncthreads();
+    if (tid == 0) {
+        int tot = 0;
+        for (int w = 0; w < HD_THREADS / 32; ++w) tot += scnt[w];
+        B.bmin[b] = bm;
+        B.bcnt[b] = tot;
+        __threadfence();
+        s_last = atomicAdd(B.ticket, 1u) == (unsigned)nb - 1u;
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+
+    // ---- last thread block: global minimum, then the ordered active list
+    double g = __longlong_as_double(0x7ff0000000000000LL);
+    for (int k = tid; k < nb; k += HD_THREADS) g = fmin(g, __ldcg(B.bmin + k));
+    const double tnext = hd_block_min(g, smin);
+    if (tid == 0) s_base = 0;
+    __syncthreads();
+    for (int k = 0; k < nb; ++k) {
+        if (__ldcg(B.bmin + k) != tnext) continue;          // uniform over the thread block
+        const int base = s_base;
+        const int cntk = __ldcg(B.bcnt + k);
+        // ordered compaction of thread block k's particles: HD_PER_BLOCK / HD_THREADS rounds of a block-wide scan
+        int off = base;
+        for (int q = 0; q < HD_PER_BLOCK / HD_THREADS; ++q) {
+            const int p = k * HD_PER_BLOCK + q * HD_THREADS + tid;
+            const bool on = p < S.n && S.t[p] + S.dt[p] == tnext;
+            const unsigned bal = __ballot_sync(0xffffffffu, on);
+            if ((tid & 31) == 0) scnt[tid >> 5] = __popc(bal);
+            __syncthreads();
+            int before = 0, total = 0;
+#pragma unroll
+            for (int w = 0; w < HD_THREADS / 32; ++w) {
+                const int cw = scnt[w];
+                before += w < (tid >> 5) ? cw : 0;
+                total += cw;
+            }
+            if (on) {
+                const int slot = off + before + __popc(bal & ((1u << (tid & 31)) - 1u));
+                B.act[slot] = p;
+                hd_predict(S, p, tnext, B.xi + 3 * (size_t)slot, B.vi + 3 * (size_t)slot);
+            }
+            off += total;
+            __syncthreads();
+        }
+        if (tid == 0) s_base = base + cntk;
+        __syncthreads();
+    }
+    if (tid == 0) {
+        *B.d_ni = s_base;
+        *B.d_tnext = tnext;
+        *B.h_tnext = tnext;
+        __threadfence_system();
+        *B.h_ni = s_base;
+        *B.ticket = 0u;
+    }
+}
+
+// smallest power-of-two step <= cap that does not exceed `want` (the host driver's pow2_floor)
+__device__ __forceinline__ double hd_pow2_floor(double want, double cap)
+{
+    double d = cap;
+    while (d > want && d > 1e-300) d *= 0.5;
+    return d;
+}
+
+__device__ __forceinline__ double hd_norm3(const double *a) { return sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]); }
+
+// write particle p's Hermite state into the raw j-store (what g6_set_j_particle + k_stage do on the host path)
+__device__ __forceinline__ void hd_store_j(char *raw, const HdState &S, int p)
+{
+    char *T = raw_tile(raw, p);
+    const int l = p % JT;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        raw_x(T, k, l) = S.x[3 * (size_t)p + k];
+        raw_v(T, k, l) = (float)S.v[3 * (size_t)p + k];
+        raw_a2(T, k, l) = (float)(S.a[3 * (size_t)p + k] / 2);
+        raw_j6(T, k, l) = (float)(S.ad[3 * (size_t)p + k] / 6);
+    }
+    raw_t(T, l) = S.t[p];
+    raw_m(T, l) = (float)S.m[p];
+    raw_idx(T, l) = p;
+}
+
+// first call: forces at t = 0 are in (a1, ad1) for ALL particles -> state, first steps, j-store
+__global__ void __launch_bounds__(HD_THREADS)
+k_hd_init(HdState S, const double *__restrict__ a1, const double *__restrict__ ad1, double eta_start, double dt_max, char *raw,
+          unsigned long long *dt_min_bits)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= S.n) return;
+    double a[3], ad[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { a[k] = a1[3 * (size_t)p + k]; ad[k] = ad1[3 * (size_t)p + k]; S.a[3 * (size_t)p + k] = a[k]; S.ad[3 * (size_t)p + k] = ad[k]; }
+    const double na = hd_norm3(a), nad = hd_norm3(ad);
+    const double d = hd_pow2_floor(nad > 0 ? eta_start * na / nad : dt_max, dt_max);
+    S.dt[p] = d;
+    S.t[p] = 0.0;
+    atomicMin(dt_min_bits, (unsigned long long)__double_as_longlong(d));
+    hd_store_j(raw, S, p);
+}
+
+// corrector + Aarseth step for the n_i particles of the block (reading 16); one thread per particle
+__global__ void __launch_bounds__(HD_THREADS)
+k_hd_correct(HdState S, HdBlock B, const double *__restrict__ a1, const double *__restrict__ ad1, double eta, double dt_max,
+             char *raw, unsigned long long *dt_min_bits)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int ni = *B.d_ni;
+    if (k >= ni) return;
+    const double tn = *B.d_tnext;
+    const int p = B.act[k];
+    const double h = S.dt[p], h2 = h * h, h3 = h2 * h, h4 = h3 * h, h5 = h4 * h;
+    double a2n[3], a3[3], an[3], adn[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const double a0 = S.a[3 * (size_t)p + c], ad0 = S.ad[3 * (size_t)p + c];
+        an[c] = a1[3 * (size_t)k + c];
+        adn[c] = ad1[3 * (size_t)k + c];
+        const double da = a0 - an[c];
+        const double a2 = (-6 * da - h * (4 * ad0 + 2 * adn[c])) / h2;
+        a3[c] = (12 * da + 6 * h * (ad0 + adn[c])) / h3;
+        S.x[3 * (size_t)p + c] = B.xi[3 * (size_t)k + c] + h4 * a2 / 24 + h5 * a3[c] / 120;
+        S.v[3 * (size_t)p + c] = B.vi[3 * (size_t)k + c] + h3 * a2 / 6 + h4 * a3[c] / 24;
+        a2n[c] = a2 + h * a3[c];
+        S.a[3 * (size_t)p + c] = an[c];
+        S.ad[3 * (size_t)p + c] = adn[c];
+    }
+    S.t[p] = tn;
+    const double na = hd_norm3(an), nad = hd_norm3(adn), n2 = hd_norm3(a2n), n3 = hd_norm3(a3);
+    const double den = nad * n3 + n2 * n2;
+    const double want = den > 0 ? sqrt(eta * (na * n2 + nad * nad) / den) : dt_max;
+    double d = h;
+    if (want < d) {
+        while (d > want) d *= 0.5;
+    } else if (want >= 2 * d && 2 * d <= dt_max && fmod(tn, 2 * d) == 0.0) {
+        d *= 2;
+    }
+    S.dt[p] = d;
+    atomicMin(dt_min_bits, (unsigned long long)__double_as_longlong(d));
+    hd_store_j(raw, S, p);
+}
+
+__global__ void k_hd_iota(int *act, int n)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p < n) act[p] = p;
+}
+
+// Eq. 1-2 of every particle to the time tn (state read-out)
+__global__ void __launch_bounds__(HD_THREADS)
+k_hd_predict_all(HdState S, double tn, double *__restrict__ xo, double *__restrict__ vo)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= S.n) return;
+    hd_predict(S, p, tn, xo + 3 * (size_t)p, vo + 3 * (size_t)p);
+}
+
+}  // namespace g6

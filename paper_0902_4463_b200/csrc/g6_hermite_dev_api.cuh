@@ -1,0 +1,225 @@
+// g6_hermite_dev_api.cuh -- host side of the device-resident Hermite integrator (include/g6_hermite.h, g6hd_*).
+// Included at the end of g6_api.cu: it drives the library's own force path (run_force) on device-resident
+// i-blocks and keeps the whole particle state in HBM.  Per block step the host waits once, for (n_i, t_next).
+#pragma once
+#include "../../include/g6_hermite.h"
+#include "g6_hermite_dev.cuh"
+
+#include <chrono>
+
+struct g6hd_system {
+    int cl = 0, n = 0;
+    double eps2 = 0, eta = 0, dt_max = 0, t = 0;
+    HdState S{};
+    HdBlock B{};
+    double *a1 = nullptr, *ad1 = nullptr, *pot = nullptr;      // forces of the current block [n][3], [n]
+    unsigned long long *dt_min_bits = nullptr;                // smallest step used so far (bits of a positive double)
+    int *h_ni = nullptr;                                       // mapped host memory
+    double *h_tnext = nullptr;
+    cudaEvent_t ev = nullptr;
+    int last_ni = 0;
+    long long nblock = 0, npart = 0, hist[64] = {};
+    double inter = 0, wall = 0;
+};
+
+namespace {
+
+void hd_free(g6hd_system *s)
+{
+    if (!s) return;
+    cudaFree(s->S.x); cudaFree(s->S.v); cudaFree(s->S.a); cudaFree(s->S.ad); cudaFree(s->S.m); cudaFree(s->S.t); cudaFree(s->S.dt);
+    cudaFree(s->B.act); cudaFree(s->B.xi); cudaFree(s->B.vi); cudaFree(s->B.bmin); cudaFree(s->B.bcnt); cudaFree(s->B.ticket);
+    cudaFree(s->B.d_ni); cudaFree(s->B.d_tnext);
+    cudaFree(s->a1); cudaFree(s->ad1); cudaFree(s->pot); cudaFree(s->dt_min_bits);
+    if (s->h_ni) cudaFreeHost(s->h_ni);
+    if (s->h_tnext) cudaFreeHost(s->h_tnext);
+    if (s->ev) cudaEventDestroy(s->ev);
+    delete s;
+}
+
+// force on the device-resident i-block (act, xi, vi)[0, ni) at time tn -> a1, ad1, pot; chunks of g6_npipes()
+int hd_force(Cluster &c, g6hd_system &s, int ni, double tn)
+{
+    c.ti = tn;
+    init_npipes();
+    for (int i0 = 0; i0 < ni; i0 += g_npipes) {
+        const int cnt = std::min(g_npipes, ni - i0);
+        int rc = run_force(c, s.n, cnt, s.B.act + i0, s.B.xi + 3 * (size_t)i0, s.B.vi + 3 * (size_t)i0, s.eps2, s.a1 + 3 * (size_t)i0,
+                           s.ad1 + 3 * (size_t)i0, s.pot + i0, nullptr, nullptr, nullptr, nullptr, nullptr);
+        if (rc) return rc;
+    }
+    return G6_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+g6hd_system *g6hd_create(int clusterid, int n, const double x[][3], const double v[][3], const double m[],
+                         double eps2, double eta, double eta_start, double dt_max)
+{
+    if (clusterid < 0 || clusterid >= MAX_CLUSTERS) return nullptr;
+    Cluster &c = g_cl[clusterid];
+    if (!c.open) { fail(c, G6_ERR_NOT_OPEN, "cluster %d is not open", clusterid); return nullptr; }
+    if (n < 1 || n > c.capacity || !x || !v || !m || !(eta > 0) || !(dt_max > 0) || !(eps2 >= 0) || c.pending) {
+        fail(c, G6_ERR_ARG, "bad g6hd_create arguments (n = %d, capacity %d)", n, c.capacity);
+        return nullptr;
+    }
+    g6hd_system *s = new (std::nothrow) g6hd_system;
+    if (!s) return nullptr;
+    s->cl = clusterid; s->n = n; s->eps2 = eps2; s->eta = eta; s->dt_max = dt_max;
+    s->S.n = n;
+    const size_t n3 = 3 * (size_t)n;
+    const int nb = (n + HD_PER_BLOCK - 1) / HD_PER_BLOCK;
+    int rc = [&]() -> int {
+        CK(dalloc(s->S.x, n3)); CK(dalloc(s->S.v, n3)); CK(dalloc(s->S.a, n3)); CK(dalloc(s->S.ad, n3));
+        CK(dalloc(s->S.m, n)); CK(dalloc(s->S.t, n)); CK(dalloc(s->S.dt, n));
+        CK(dalloc(s->B.act, n)); CK(dalloc(s->B.xi, n3)); CK(dalloc(s->B.vi, n3));
+        CK(dalloc(s->B.bmin, nb)); CK(dalloc(s->B.bcnt, nb)); CK(dalloc(s->B.ticket, 1)); CK(dalloc(s->B.d_ni, 1)); CK(dalloc(s->B.d_tnext, 1));
+        CK(dalloc(s->a1, n3)); CK(dalloc(s->ad1, n3)); CK(dalloc(s->pot, n)); CK(dalloc(s->dt_min_bits, 1));
+        CK(cudaHostAlloc((void **)&s->h_ni, sizeof(int), cudaHostAllocMapped));
+        CK(cudaHostAlloc((void **)&s->h_tnext, sizeof(double), cudaHostAllocMapped));
+        CK(cudaHostGetDevicePointer((void **)&s->B.h_ni, s->h_ni, 0));
+        CK(cudaHostGetDevicePointer((void **)&s->B.h_tnext, s->h_tnext, 0));
+        CK(cudaEventCreateWithFlags(&s->ev, cudaEventDisableTiming));
+        CK(cudaMemsetAsync(s->B.ticket, 0, sizeof(unsigned int), c.stream));
+        const unsigned long long big = 0x7ff0000000000000ULL;
+        CK(cudaMemcpyAsync(s->dt_min_bits, &big, sizeof(big), cudaMemcpyHostToDevice, c.stream));
+        CK(cudaMemcpyAsync(s->S.x, x, n3 * sizeof(double), cudaMemcpyHostToDevice, c.stream));
+        CK(cudaMemcpyAsync(s->S.v, v, n3 * sizeof(double), cudaMemcpyHostToDevice, c.stream));
+        CK(cudaMemcpyAsync(s->S.m, m, n * sizeof(double), cudaMemcpyHostToDevice, c.stream));
+        CK(cudaMemsetAsync(s->S.a, 0, n3 * sizeof(double), c.stream));
+        CK(cudaMemsetAsync(s->S.ad, 0, n3 * sizeof(double), c.stream));
+        CK(cudaMemsetAsync(s->S.t, 0, n * sizeof(double), c.stream));
+        CK(cudaMemsetAsync(s->S.dt, 0, n * sizeof(double), c.stream));
+        CK(cudaStreamSynchronize(c.stream));           // the caller's arrays may be pageable
+        // t = 0: every particle is its own i-particle; a = adot = 0 makes the prediction the identity
+        int r = flush_j(c);
+        if (r) return r;
+        k_hd_init<<<(n + HD_THREADS - 1) / HD_THREADS, HD_THREADS, 0, c.stream>>>(s->S, s->S.a, s->S.ad, eta_start, dt_max, c.js.raw, s->dt_min_bits);
+        CK(cudaGetLastError());                        // loads the j-store (the steps it sets are overwritten below)
+        c.n_stored = std::max(c.n_stored, n);
+        c.pred_valid = false;
+        k_hd_predict_all<<<(n + HD_THREADS - 1) / HD_THREADS, HD_THREADS, 0, c.stream>>>(s->S, 0.0, s->B.xi, s->B.vi);
+        CK(cudaGetLastError());
+        k_hd_iota<<<(n + HD_THREADS - 1) / HD_THREADS, HD_THREADS, 0, c.stream>>>(s->B.act, n);      // the first block is everybody
+        CK(cudaGetLastError());
+        r = hd_force(c, *s, n, 0.0);
+        if (r) return r;
+        CK(cudaMemcpyAsync(s->dt_min_bits, &big, sizeof(big), cudaMemcpyHostToDevice, c.stream));
+        k_hd_init<<<(n + HD_THREADS - 1) / HD_THREADS, HD_THREADS, 0, c.stream>>>(s->S, s->a1, s->ad1, eta_start, dt_max, c.js.raw, s->dt_min_bits);
+        CK(cudaGetLastError());
+        c.pred_valid = false;
+        CK(cudaStreamSynchronize(c.stream));
+        return G6_OK;
+    }();
+    if (rc != G6_OK) { hd_free(s); return nullptr; }
+    return s;
+}
+
+void g6hd_destroy(g6hd_system *s)
+{
+    if (s && s->cl >= 0 && s->cl < MAX_CLUSTERS && g_cl[s->cl].open) cudaStreamSynchronize(g_cl[s->cl].stream);
+    hd_free(s);
+}
+
+int g6hd_evolve(g6hd_system *sp, double t_end, long long max_block_steps)
+{
+    if (!sp) return G6_ERR_ARG;
+    g6hd_system &s = *sp;
+    GET_CLUSTER(s.cl);
+    if (c.pending) return fail(c, G6_ERR_SEQUENCE, "force call pending");
+    const auto w0 = std::chrono::steady_clock::now();
+    const int nb = (s.n + HD_PER_BLOCK - 1) / HD_PER_BLOCK;
+    long long done = 0;
+    while (s.t < t_end && (max_block_steps <= 0 || done < max_block_steps)) {
+        k_hd_select<<<nb, HD_THREADS, 0, c.stream>>>(s.S, s.B);
+        CK(cudaGetLastError());
+        CK(cudaEventRecord(s.ev, c.stream));
+        CK(cudaEventSynchronize(s.ev));                 // the one host wait of the block step
+        const int ni = *(volatile int *)s.h_ni;
+        const double tn = *(volatile double *)s.h_tnext;
+        if (ni < 1 || ni > s.n || !(tn > s.t)) return fail(c, G6_ERR_CUDA, "block selection returned ni = %d, t = %g", ni, tn);
+        int rc = hd_force(c, s, ni, tn);
+        if (rc) return rc;
+        k_hd_correct<<<(ni + HD_THREADS - 1) / HD_THREADS, HD_THREADS, 0, c.stream>>>(s.S, s.B, s.a1, s.ad1, s.eta, s.dt_max, c.js.raw, s.dt_min_bits);
+        CK(cudaGetLastError());
+        c.pred_valid = false;                           // the corrector rewrote j-store records
+        s.t = tn;
+        s.last_ni = ni;
+        ++s.nblock; ++done;
+        s.npart += ni;
+        s.inter += (double)ni * (double)s.n;
+        int b = 0;
+        while ((1LL << (b + 1)) <= ni) ++b;
+        s.hist[b] += 1;
+    }
+    CK(cudaStreamSynchronize(c.stream));
+    s.wall += std::chrono::duration<double>(std::chrono::steady_clock::now() - w0).count();
+    return G6_OK;
+}
+
+int g6hd_get_state(g6hd_system *sp, double x[][3], double v[][3])
+{
+    if (!sp || !x || !v) return G6_ERR_ARG;
+    g6hd_system &s = *sp;
+    GET_CLUSTER(s.cl);
+    // B.xi / B.vi are free between block steps
+    k_hd_predict_all<<<(s.n + HD_THREADS - 1) / HD_THREADS, HD_THREADS, 0, c.stream>>>(s.S, s.t, s.B.xi, s.B.vi);
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(x, s.B.xi, 3 * (size_t)s.n * sizeof(double), cudaMemcpyDeviceToHost, c.stream));
+    CK(cudaMemcpyAsync(v, s.B.vi, 3 * (size_t)s.n * sizeof(double), cudaMemcpyDeviceToHost, c.stream));
+    CK(cudaStreamSynchronize(c.stream));
+    return G6_OK;
+}
+
+int g6hd_get_particles(g6hd_system *sp, double x[][3], double v[][3], double a[][3], double adot[][3], double t[], double dt[])
+{
+    if (!sp) return G6_ERR_ARG;
+    g6hd_system &s = *sp;
+    GET_CLUSTER(s.cl);
+    const size_t b3 = 3 * (size_t)s.n * sizeof(double), b1 = (size_t)s.n * sizeof(double);
+    CK(cudaStreamSynchronize(c.stream));
+    if (x) CK(cudaMemcpy(x, s.S.x, b3, cudaMemcpyDeviceToHost));
+    if (v) CK(cudaMemcpy(v, s.S.v, b3, cudaMemcpyDeviceToHost));
+    if (a) CK(cudaMemcpy(a, s.S.a, b3, cudaMemcpyDeviceToHost));
+    if (adot) CK(cudaMemcpy(adot, s.S.ad, b3, cudaMemcpyDeviceToHost));
+    if (t) CK(cudaMemcpy(t, s.S.t, b1, cudaMemcpyDeviceToHost));
+    if (dt) CK(cudaMemcpy(dt, s.S.dt, b1, cudaMemcpyDeviceToHost));
+    return G6_OK;
+}
+
+int g6hd_get_last_block(g6hd_system *sp, int maxn, int *ni, int act[], double xi[][3], double vi[][3], double acc[][3], double jerk[][3])
+{
+    if (!sp || !ni) return G6_ERR_ARG;
+    g6hd_system &s = *sp;
+    GET_CLUSTER(s.cl);
+    *ni = s.last_ni;
+    if (s.last_ni > maxn) return fail(c, G6_ERR_ARG, "last block has %d particles, buffer holds %d", s.last_ni, maxn);
+    const size_t b3 = 3 * (size_t)s.last_ni * sizeof(double);
+    CK(cudaStreamSynchronize(c.stream));
+    if (act) CK(cudaMemcpy(act, s.B.act, s.last_ni * sizeof(int), cudaMemcpyDeviceToHost));
+    if (xi) CK(cudaMemcpy(xi, s.B.xi, b3, cudaMemcpyDeviceToHost));
+    if (vi) CK(cudaMemcpy(vi, s.B.vi, b3, cudaMemcpyDeviceToHost));
+    if (acc) CK(cudaMemcpy(acc, s.a1, b3, cudaMemcpyDeviceToHost));
+    if (jerk) CK(cudaMemcpy(jerk, s.ad1, b3, cudaMemcpyDeviceToHost));
+    return G6_OK;
+}
+
+int g6hd_get_stats(g6hd_system *sp, double stats[8], long long ni_hist_log2[64])
+{
+    if (!sp || !stats) return G6_ERR_ARG;
+    g6hd_system &s = *sp;
+    GET_CLUSTER(s.cl);
+    unsigned long long bits = 0;
+    CK(cudaStreamSynchronize(c.stream));
+    CK(cudaMemcpy(&bits, s.dt_min_bits, sizeof(bits), cudaMemcpyDeviceToHost));
+    double dmin;
+    memcpy(&dmin, &bits, sizeof(dmin));
+    stats[0] = (double)s.nblock; stats[1] = (double)s.npart; stats[2] = s.t; stats[3] = dmin;
+    stats[4] = s.inter; stats[5] = s.wall; stats[6] = 0; stats[7] = 0;
+    if (ni_hist_log2) memcpy(ni_hist_log2, s.hist, sizeof(s.hist));
+    return G6_OK;
+}
+
+}  // extern "C"

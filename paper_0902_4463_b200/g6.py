@@ -26,6 +26,7 @@ SYMBOLS = [
     "g6x_get_nearest", "g6x_set_stream", "g6x_synchronize", "g6x_get_timers", "g6x_set_option",
     "g6x_get_option", "g6x_get_predicted", "g6x_debug_dx", "g6x_probe_fp32_peak", "g6x_probe_read_jstore", "g6x_version",
     "g6h_create", "g6h_destroy", "g6h_evolve", "g6h_get_state", "g6h_get_stats", "g6h_get_force_wall_hist",
+    "g6hd_create", "g6hd_destroy", "g6hd_evolve", "g6hd_get_state", "g6hd_get_stats", "g6hd_get_particles", "g6hd_get_last_block",
 ]
 
 ERRORS = {0: "G6_OK", -1: "G6_ERR_NOT_OPEN", -2: "G6_ERR_CLUSTER", -3: "G6_ERR_ADDRESS", -4: "G6_ERR_NI",
@@ -54,6 +55,7 @@ def lib():
         L.g6x_last_error.restype = C.c_char_p
         L.g6x_version.restype = C.c_char_p
         L.g6h_create.restype = C.c_void_p
+        L.g6hd_create.restype = C.c_void_p
         _lib = L
     return _lib
 
@@ -333,6 +335,62 @@ class Hermite:
     def close(self):
         if self._h:
             lib().g6h_destroy(C.c_void_p(self._h))
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class HermiteDev:
+    """The device-resident Hermite block-step integrator (g6hd_* functions, include/g6_hermite.h): block
+    selection, i-prediction, corrector and step choice are CUDA kernels; argument marshalling only here."""
+
+    def __init__(self, clusterid, x, v, m, eps2, eta, eta_start=0.01, dt_max=0.125):
+        n = len(m)
+        x = _f64(x, (n, 3)); v = _f64(v, (n, 3)); m = _f64(m, (n,))
+        self.n, self.clusterid = n, clusterid
+        self._h = lib().g6hd_create(C.c_int(clusterid), C.c_int(n), _dp(x), _dp(v), _dp(m), C.c_double(eps2),
+                                    C.c_double(eta), C.c_double(eta_start), C.c_double(dt_max))
+        if not self._h:
+            raise G6Error(-8, "g6hd_create failed: " + g6x_last_error(clusterid))
+
+    def evolve(self, t_end, max_block_steps=0):
+        return _chk(lib().g6hd_evolve(C.c_void_p(self._h), C.c_double(t_end), C.c_longlong(max_block_steps)), self.clusterid)
+
+    def state(self):
+        x = np.empty((self.n, 3)); v = np.empty((self.n, 3))
+        _chk(lib().g6hd_get_state(C.c_void_p(self._h), _dp(x), _dp(v)), self.clusterid)
+        return x, v
+
+    def particles(self):
+        """raw Hermite state, each particle at its own time: dict x, v, a, adot [n,3], t, dt [n]"""
+        n = self.n
+        o = dict(x=np.empty((n, 3)), v=np.empty((n, 3)), a=np.empty((n, 3)), adot=np.empty((n, 3)), t=np.empty(n), dt=np.empty(n))
+        _chk(lib().g6hd_get_particles(C.c_void_p(self._h), _dp(o["x"]), _dp(o["v"]), _dp(o["a"]), _dp(o["adot"]), _dp(o["t"]), _dp(o["dt"])),
+             self.clusterid)
+        return o
+
+    def last_block(self):
+        """the last block step's i-block: dict act[ni], xi, vi, acc, jerk [ni,3]"""
+        n = self.n
+        ni = C.c_int(0)
+        act = np.empty(n, np.int32); xi = np.empty((n, 3)); vi = np.empty((n, 3)); acc = np.empty((n, 3)); jerk = np.empty((n, 3))
+        _chk(lib().g6hd_get_last_block(C.c_void_p(self._h), C.c_int(n), C.byref(ni), _ip(act), _dp(xi), _dp(vi), _dp(acc), _dp(jerk)), self.clusterid)
+        k = ni.value
+        return dict(act=act[:k].copy(), xi=xi[:k].copy(), vi=vi[:k].copy(), acc=acc[:k].copy(), jerk=jerk[:k].copy())
+
+    def stats(self):
+        st = np.zeros(8); hist = np.zeros(64, np.int64)
+        _chk(lib().g6hd_get_stats(C.c_void_p(self._h), _dp(st), hist.ctypes.data_as(C.POINTER(C.c_longlong))), self.clusterid)
+        return dict(n_block_steps=int(st[0]), n_particle_steps=int(st[1]), t=st[2], dt_min=st[3], interactions=st[4],
+                    wall_s=st[5], ni_hist_log2=hist)
+
+    def close(self):
+        if self._h:
+            lib().g6hd_destroy(C.c_void_p(self._h))
             self._h = None
 
     def __del__(self):

@@ -34,8 +34,8 @@ def test_every_declared_symbol_is_exported(library):
     # and the Python binding mirrors the same names
     assert sorted(set(g6.SYMBOLS)) == declared
     for name in declared:
-        if name.startswith("g6h_"):
-            continue                      # wrapped by the g6.Hermite class
+        if name.startswith("g6h_") or name.startswith("g6hd_"):
+            continue                      # wrapped by the g6.Hermite / g6.HermiteDev classes
         assert hasattr(g6, name), f"binding lacks {name}"
 
 

@@ -105,6 +105,17 @@ def test_c2_full_run_vs_oracle_driven(cluster, oracle):
                                           "dt_min": st["dt_min"], "ni_hist_log2": [int(c) for c in st["ni_hist_log2"][:20]],
                                           "force_wall_s_log2": [round(float(c), 4) for c in st["force_wall_s_log2"][:20]]}
         print(json.dumps({f"library_newton{newton}": rep[f"library_newton{newton}"]}), flush=True)
+    g6.g6x_set_option(0, "newton", 1)
+    t0 = time.perf_counter()
+    hd = g6.HermiteDev(0, x, v, m, eps2, eta)
+    hd.evolve(t_end)
+    xd, vd = hd.state(); sd = hd.stats(); hd.close()
+    wall = time.perf_counter() - t0
+    dE = (_energy(oracle, xd, vd, m, eps2) - E0) / abs(E0)
+    rep["device_resident_newton1"] = {"dE_over_E": dE, "block_steps": sd["n_block_steps"], "particle_steps": sd["n_particle_steps"],
+                                      "interactions": sd["interactions"], "wall_s": wall, "wall_evolve_s": sd["wall_s"], "dt_min": sd["dt_min"],
+                                      "ni_hist_log2": [int(c) for c in sd["ni_hist_log2"][:20]]}
+    print(json.dumps({"device_resident_newton1": rep["device_resident_newton1"]}), flush=True)
     t0 = time.perf_counter()
     ro = oracle.hermite(x, v, m, eps2, eta, t_end)
     wall = time.perf_counter() - t0
@@ -116,3 +127,79 @@ def test_c2_full_run_vs_oracle_driven(cluster, oracle):
     os.makedirs("gpurun_out", exist_ok=True)
     json.dump(rep, open("gpurun_out/c2_report.json", "w"), indent=1)
     assert abs(rep["library_newton1"]["dE_over_E"]) <= 2 * abs(dE_o) + 2e-8
+    assert abs(rep["device_resident_newton1"]["dE_over_E"]) <= 2 * abs(dE_o) + 2e-8
+
+
+# ------------------------------------------------------------------ device-resident integrator (NEXT-3, g6hd_*)
+def test_device_corrector_and_selection_against_oracle(cluster, oracle):
+    """One block step at a time: the block the device selects is the set of particles with the smallest
+    t + dt, in address order; its i-particles are Eq. 1-2 predictions (oracle.predict); the corrector kernel's
+    new x, v equal oracle.hermite_correct and the new step follows oracle.aarseth_dt and the power-of-two
+    rule, given the forces the device used."""
+    n = 3000
+    x, v, m, _ = inputs.config("C2", n=n)
+    eps2, eta, dt_max = 1e-4 ** 2, 0.01, 0.125
+    h = g6.HermiteDev(0, x, v, m, eps2, eta)
+    before = h.particles()
+    assert np.all(before["t"] == 0) and np.all(before["dt"] <= dt_max) and np.all(np.log2(before["dt"]) % 1 == 0)
+    seen = 0
+    for step in range(40):
+        tn_all = before["t"] + before["dt"]
+        tnext = tn_all.min()
+        want_act = np.nonzero(tn_all == tnext)[0]
+        h.evolve(1.0, max_block_steps=1)
+        blk = h.last_block()
+        after = h.particles()
+        assert np.array_equal(blk["act"], want_act.astype(np.int32))
+        act = blk["act"]
+        xp, vp = oracle.predict(tnext, before["t"][act], before["x"][act], before["v"][act], before["a"][act], before["adot"][act])
+        assert np.allclose(blk["xi"], xp, rtol=1e-14, atol=1e-15) and np.allclose(blk["vi"], vp, rtol=1e-13, atol=1e-15)
+        for k, p in enumerate(act):
+            hh = before["dt"][p]
+            x1, v1, a2n, a3 = oracle.hermite_correct(hh, blk["xi"][k], blk["vi"][k], before["a"][p], before["adot"][p], blk["acc"][k], blk["jerk"][k])
+            assert np.allclose(after["x"][p], x1, rtol=1e-14, atol=1e-16) and np.allclose(after["v"][p], v1, rtol=1e-13, atol=1e-15)
+            assert np.array_equal(after["a"][p], blk["acc"][k]) and np.array_equal(after["adot"][p], blk["jerk"][k])
+            assert after["t"][p] == tnext
+            want = oracle.aarseth_dt(eta, blk["acc"][k], blk["jerk"][k], a2n, a3, dt_max)
+            d = hh
+            if want < d:
+                while d > want:
+                    d *= 0.5
+            elif want >= 2 * d and 2 * d <= dt_max and np.fmod(tnext, 2 * d) == 0.0:
+                d *= 2
+            # a wish within rounding of a power of two may fall on either side of it
+            assert after["dt"][p] == d or abs(want / after["dt"][p] - 1) < 1e-12 or abs(want / (2 * after["dt"][p]) - 1) < 1e-12, (p, want, d, after["dt"][p])
+        untouched = np.setdiff1d(np.arange(n), act)
+        for key in ("x", "v", "a", "adot", "t", "dt"):
+            assert np.array_equal(after[key][untouched], before[key][untouched])
+        seen += len(act)
+        before = after
+    # the forces the device used are the library's: check one block against the oracle on the predicted system
+    st = h.stats()
+    assert st["n_block_steps"] == 40 and st["n_particle_steps"] == seen
+    h.close()
+
+
+@pytest.mark.parametrize("n,t_end", [(512, 0.25), (5000, 0.03125)])
+def test_device_driven_vs_host_driven_vs_oracle_driven(cluster, oracle, n, t_end):
+    x, v, m, _ = inputs.config("C2", n=n)
+    eps2, eta = 1e-4 ** 2, 0.01
+    E0 = _energy(oracle, x, v, m, eps2)
+    ro = oracle.hermite(x, v, m, eps2, eta, t_end)
+    dE_o = abs(_energy(oracle, ro.x, ro.v, m, eps2) - E0) / abs(E0)
+    hd = g6.HermiteDev(0, x, v, m, eps2, eta)
+    hd.evolve(t_end)
+    xd, vd = hd.state(); sd = hd.stats(); hd.close()
+    hh = g6.Hermite(0, x, v, m, eps2, eta)
+    hh.evolve(t_end)
+    xh, vh = hh.state(); sh = hh.stats(); hh.close()
+    dE_d = abs(_energy(oracle, xd, vd, m, eps2) - E0) / abs(E0)
+    print(f"N={n} t={t_end}: dE/E device-driven {dE_d:.3e}, oracle-driven {dE_o:.3e}; block steps device {sd['n_block_steps']} host {sh['n_block_steps']} "
+          f"oracle {ro.n_block_steps}; particle steps {sd['n_particle_steps']} / {sh['n_particle_steps']} / {ro.n_particle_steps}")
+    assert sd["t"] == t_end
+    assert dE_d <= 2 * dE_o + 2e-8
+    assert abs(sd["n_particle_steps"] - ro.n_particle_steps) <= 0.03 * ro.n_particle_steps
+    assert abs(sd["n_particle_steps"] - sh["n_particle_steps"]) <= 0.01 * sh["n_particle_steps"]
+    assert sd["ni_hist_log2"].sum() == sd["n_block_steps"]
+    assert np.median(np.linalg.norm(xd - ro.x, axis=1)) < 1e-6
+    assert np.median(np.linalg.norm(xd - xh, axis=1)) < 1e-7
