@@ -25,9 +25,11 @@ struct HdState {
 // per-step scratch written by k_hd_select
 struct HdBlock {
     int *act;                   // [n] active addresses, increasing
+    int *cand;                  // [nblocks * HD_PER_BLOCK] per-thread-block candidates (particles at the block minimum)
     double *xi, *vi;            // [n][3] predicted i-particles
     double *bmin;               // [nblocks] per-thread-block minimum of t + dt
     int *bcnt;                  // [nblocks] particles of the block attaining it
+    int *boff;                  // [nblocks] where the block's candidates go in the active list, -1: not in this block step
     unsigned int *ticket;
     int *h_ni;                  // mapped host memory: n_i of the block ...
     double *h_tnext;            // ... and its time
@@ -63,99 +65,19 @@ __device__ __forceinline__ void hd_predict(const HdState &S, int p, double tn, d
     }
 }
 
-// One launch selects the next block.  Every thread block reduces its HD_PER_BLOCK particles to
-// (min of t + dt, how many attain it); the LAST thread block to finish (atomic ticket) takes the global
-// minimum and writes, block by block in address order, the active list and the predicted i-particles.
-// Small blocks touch a few thread blocks' particles again; a block of all N particles makes the last
-// thread block walk all N (a fraction of a per cent of the force time it precedes).
-__global__ void __launch_bounds__(HD_THREADS)
-k_hd_select(HdState S, HdBlock B)
-{
-    __shared__ double smin[HD_THREADS / 32];
-    __shared__ int scnt[HD_THREADS / 32];
-    __shared__ int s_last, s_base;
-    const int tid = threadIdx.x, b = blockIdx.x, nb = gridDim.x;
-    const int p0 = b * HD_PER_BLOCK;
-    double tn[HD_PER_BLOCK / HD_THREADS];
-    double lmin = __longlong_as_double(0x7ff0000000000000LL);
-#pragma unroll
-    for (int q = 0; q < HD_PER_BLOCK / HD_THREADS; ++q) {
-        const int p = p0 + q * HD_THREADS + tid;
-        tn[q] = p < S.n ? S.t[p] + S.dt[p] : __longlong_as_double(0x7ff0000000000000LL);
-        lmin = fmin(lmin, tn[q]);
-    }
-    const double bm = hd_block_min(lmin, smin);
-    int c = 0;
-#pragma unroll
-    for (int q = 0; q < HD_PER_BLOCK / HD_THREADS; ++q) c += tn[q] == bm;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
-    if ((tid & 31) == 0) scnt[tid >> 5] = c;
-    __syncthreads();
-    if (tid == 0) {
-        int tot = 0;
-        for (int w = 0; w < HD_THREADS / 32; ++w) tot += scnt[w];
-        B.bmin[b] = bm;
-        B.bcnt[b] = tot;
-        __threadfence();
-        s_last = atomicAdd(B.ticket, 1u) == (unsigned)nb - 1u;
-    }
-    __syncthreads();
-    if (!s_last) return;
-    __threadfence();
-
-    // ---- last thread block: global minimum, then the ordered active list
-    double g = __longlong_as_double(0x7ff0000000000000LL);
-    for (int k = tid; k < nb; k += HD_THREADS) g = fmin(g, __ldcg(B.bmin + k));
-    const double tnext = hd_block_min(g, smin);
-    if (tid == 0) s_base = 0;
-    __syncthreads();
-    for (int k = 0; k < nb; ++k) {
-        if (__ldcg(B.bmin + k) != tnext) continue;          // uniform over the thread block
-        const int base = s_base;
-        const int cntk = __ldcg(B.bcnt + k);
-        // ordered compaction of thread block k's particles: HD_PER_BLOCK / HD_THREADS rounds of a block-wide scan
-        int off = base;
-        for (int q = 0; q < HD_PER_BLOCK / HD_THREADS; ++q) {
-            const int p = k * HD_PER_BLOCK + q * HD_THREADS + tid;
-            const bool on = p < S.n && S.t[p] + S.dt[p] == tnext;
-            const unsigned bal = __ballot_sync(0xffffffffu, on);
-            if ((tid & 31) == 0) scnt[tid >> 5] = __popc(bal);
-            __syncthreads();
-            int before = 0, total = 0;
-#pragma unroll
-            for (int w = 0; w < HD_THREADS / 32; ++w) {
-                const int cw = scnt[w];
-                before += w < (tid >> 5) ? cw : 0;
-                total += cw;
-            }
-            if (on) {
-                const int slot = off + before + __popc(bal & ((1u << (tid & 31)) - 1u));
-                B.act[slot] = p;
-                hd_predict(S, p, tnext, B.xi + 3 * (size_t)slot, B.vi + 3 * (size_t)slot);
-            }
-            off += total;
-            __syncthreads();
-        }
-        if (tid == 0) s_base = base + cntk;
-        __syncthreads();
-    }
-    if (tid == 0) {
-        *B.d_ni = s_base;
-        *B.d_tnext = tnext;
-        *B.h_tnext = tnext;
-        __threadfence_system();
-        *B.h_ni = s_base;
-        *B.ticket = 0u;
-    }
-}
-
 // smallest power-of-two step <= cap that does not exceed `want` (the host driver's pow2_floor)
 __device__ __forceinline__ double hd_pow2_floor(double want, double cap)
 {
     double d = cap;
     while (d > want && d > 1e-300) d *= 0.5;
     return d;
+}
+
+// is t a multiple of the power-of-two step d?  (t / d is exact; fmod in fp64 is a long loop on the device)
+__device__ __forceinline__ bool hd_is_multiple(double t, double d)
+{
+    const double q = t / d;
+    return q == rint(q);
 }
 
 __device__ __forceinline__ double hd_norm3(const double *a) { return sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]); }
@@ -177,6 +99,184 @@ __device__ __forceinline__ void hd_store_j(char *raw, const HdState &S, int p)
     raw_idx(T, l) = p;
 }
 
+// corrector + Aarseth step + power-of-two rule + new j-store record for entry k of the block (reading 16)
+struct HdCorr {
+    const double *a1, *ad1;     // forces of the block, [n_i][3]
+    double eta, dt_max;
+    char *raw;                  // the library's j-store
+    unsigned long long *dt_min_bits;
+};
+
+__device__ __forceinline__ void hd_correct_one(const HdState &S, const HdBlock &B, const HdCorr &C, int k, double tn)
+{
+    const int p = B.act[k];
+    const double h = S.dt[p], h2 = h * h, h3 = h2 * h, h4 = h3 * h, h5 = h4 * h;
+    double a2n[3], a3[3], an[3], adn[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const double a0 = S.a[3 * (size_t)p + c], ad0 = S.ad[3 * (size_t)p + c];
+        an[c] = C.a1[3 * (size_t)k + c];
+        adn[c] = C.ad1[3 * (size_t)k + c];
+        const double da = a0 - an[c];
+        const double a2 = (-6 * da - h * (4 * ad0 + 2 * adn[c])) / h2;
+        a3[c] = (12 * da + 6 * h * (ad0 + adn[c])) / h3;
+        S.x[3 * (size_t)p + c] = B.xi[3 * (size_t)k + c] + h4 * a2 / 24 + h5 * a3[c] / 120;
+        S.v[3 * (size_t)p + c] = B.vi[3 * (size_t)k + c] + h3 * a2 / 6 + h4 * a3[c] / 24;
+        a2n[c] = a2 + h * a3[c];
+        S.a[3 * (size_t)p + c] = an[c];
+        S.ad[3 * (size_t)p + c] = adn[c];
+    }
+    S.t[p] = tn;
+    const double na = hd_norm3(an), nad = hd_norm3(adn), n2 = hd_norm3(a2n), n3 = hd_norm3(a3);
+    const double den = nad * n3 + n2 * n2;
+    const double want = den > 0 ? sqrt(C.eta * (na * n2 + nad * nad) / den) : C.dt_max;
+    double d = h;
+    if (want < d) {
+        while (d > want) d *= 0.5;
+    } else if (want >= 2 * d && 2 * d <= C.dt_max && hd_is_multiple(tn, 2 * d)) {
+        d *= 2;
+    }
+    S.dt[p] = d;
+    atomicMin(C.dt_min_bits, (unsigned long long)__double_as_longlong(d));
+    hd_store_j(C.raw, S, p);
+}
+
+// One launch finishes the previous block step (phase 0) and selects the next block.  Phase 1, every thread block: reduce its HD_PER_BLOCK particles to the
+// minimum of t + dt and write the particles that attain it, in address order, to its segment of `cand`.
+// Phase 2, the LAST thread block to finish (atomic ticket): global minimum over the per-block minima (held in
+// shared memory), prefix sum of the counts of the thread blocks that attain it, then the active list = the
+// concatenation of their candidate segments, with the fp64 prediction of each i-particle.
+constexpr int HD_GATHER_INLINE = 32;
+constexpr int HD_MAX_BLOCKS = 2048;     // x HD_PER_BLOCK = 2^21 particles, the library's largest capacity
+
+__global__ void __launch_bounds__(HD_THREADS)
+k_hd_select(HdState S, HdBlock B, HdCorr C, int correct_first)
+{
+    __shared__ double smin[HD_THREADS / 32];
+    __shared__ int scnt[HD_THREADS / 32];
+    __shared__ int s_last;
+    __shared__ double s_bmin[HD_MAX_BLOCKS];
+    __shared__ int s_cnt[HD_MAX_BLOCKS], s_off[HD_MAX_BLOCKS];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, b = blockIdx.x, nb = gridDim.x;
+    const int p0 = b * HD_PER_BLOCK;
+    const double INF = __longlong_as_double(0x7ff0000000000000LL);
+    // Phase 0 (correct_first): the corrector of the PREVIOUS block step, owner computes -- this thread block's
+    // own particles of that block are entries [boff[b], boff[b] + bcnt[b]) of its active list (written by the
+    // previous launch), so no other thread block touches the t, dt this one is about to read.
+    if (correct_first) {
+        const int base = B.boff[b];
+        if (base >= 0) {
+            const int cntb = B.bcnt[b];
+            const double tprev = *B.d_tnext;
+            for (int u = tid; u < cntb; u += HD_THREADS) hd_correct_one(S, B, C, base + u, tprev);
+        }
+        __syncthreads();
+    }
+    double tn[HD_PER_BLOCK / HD_THREADS];
+    double lmin = INF;
+#pragma unroll
+    for (int q = 0; q < HD_PER_BLOCK / HD_THREADS; ++q) {
+        const int p = p0 + q * HD_THREADS + tid;
+        tn[q] = p < S.n ? S.t[p] + S.dt[p] : INF;
+        lmin = fmin(lmin, tn[q]);
+    }
+    const double bm = hd_block_min(lmin, smin);
+    // ordered compaction of the particles at the block minimum (order = address = (q, tid))
+    int off = 0;
+#pragma unroll
+    for (int q = 0; q < HD_PER_BLOCK / HD_THREADS; ++q) {
+        const bool on = tn[q] == bm;
+        const unsigned bal = __ballot_sync(0xffffffffu, on);
+        if (lane == 0) scnt[wid] = __popc(bal);
+        __syncthreads();
+        int before = 0, total = 0;
+#pragma unroll
+        for (int w = 0; w < HD_THREADS / 32; ++w) {
+            const int cw = scnt[w];
+            before += w < wid ? cw : 0;
+            total += cw;
+        }
+        if (on) B.cand[p0 + off + before + __popc(bal & ((1u << lane) - 1u))] = p0 + q * HD_THREADS + tid;
+        off += total;
+        __syncthreads();
+    }
+    if (tid == 0) {
+        B.bmin[b] = bm;
+        B.bcnt[b] = off;
+    }
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) s_last = atomicAdd(B.ticket, 1u) == (unsigned)nb - 1u;
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+
+    // ---- last thread block
+    double g = INF;
+    for (int k = tid; k < nb; k += HD_THREADS) {
+        const double v = __ldcg(B.bmin + k);
+        s_bmin[k] = v;
+        s_cnt[k] = __ldcg(B.bcnt + k);
+        g = fmin(g, v);
+    }
+    const double tnext = hd_block_min(g, smin);          // (its barriers also publish s_bmin / s_cnt)
+    int ni = 0;
+    if (wid == 0) {                                       // warp 0: offsets of the thread blocks at the minimum, in order
+        for (int c0 = 0; c0 < nb; c0 += 32) {
+            const int k = c0 + lane;
+            const bool hit = k < nb && s_bmin[k] == tnext;
+            const int c = hit ? s_cnt[k] : 0;
+            int inc = c;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int u = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += u;
+            }
+            if (k < nb) { s_off[k] = hit ? ni + inc - c : -1; B.boff[k] = s_off[k]; }
+            ni += __shfl_sync(0xffffffffu, inc, 31);
+        }
+        if (lane == 0) scnt[0] = ni;
+    }
+    __syncthreads();
+    ni = scnt[0];
+    // small blocks are gathered and predicted right here; for large ones the host, which is told n_i anyway,
+    // launches k_hd_gather over all thread blocks (HD_GATHER_INLINE)
+    for (int k = 0; k < (ni <= HD_GATHER_INLINE ? nb : 0); ++k) {
+        const int base = s_off[k];
+        if (base < 0) continue;                           // uniform over the thread block
+        const int cntk = s_cnt[k];
+        for (int u = tid; u < cntk; u += HD_THREADS) {
+            const int p = __ldcg(B.cand + k * HD_PER_BLOCK + u);
+            B.act[base + u] = p;
+            hd_predict(S, p, tnext, B.xi + 3 * (size_t)(base + u), B.vi + 3 * (size_t)(base + u));
+        }
+    }
+    if (tid == 0) {
+        *B.d_ni = ni;
+        *B.d_tnext = tnext;
+        *B.h_tnext = tnext;
+        __threadfence_system();
+        *B.h_ni = ni;
+        *B.ticket = 0u;
+    }
+}
+
+// large blocks: thread block k moves its candidates to their place in the active list and predicts them
+__global__ void __launch_bounds__(HD_THREADS)
+k_hd_gather(HdState S, HdBlock B)
+{
+    const int k = blockIdx.x;
+    const int base = B.boff[k];
+    if (base < 0) return;
+    const int cntk = B.bcnt[k];
+    const double tnext = *B.d_tnext;
+    for (int u = threadIdx.x; u < cntk; u += HD_THREADS) {
+        const int p = B.cand[k * HD_PER_BLOCK + u];
+        B.act[base + u] = p;
+        hd_predict(S, p, tnext, B.xi + 3 * (size_t)(base + u), B.vi + 3 * (size_t)(base + u));
+    }
+}
+
 // first call: forces at t = 0 are in (a1, ad1) for ALL particles -> state, first steps, j-store
 __global__ void __launch_bounds__(HD_THREADS)
 k_hd_init(HdState S, const double *__restrict__ a1, const double *__restrict__ ad1, double eta_start, double dt_max, char *raw,
@@ -195,45 +295,13 @@ k_hd_init(HdState S, const double *__restrict__ a1, const double *__restrict__ a
     hd_store_j(raw, S, p);
 }
 
-// corrector + Aarseth step for the n_i particles of the block (reading 16); one thread per particle
+// the corrector alone (the pending block at the end of g6hd_evolve); one thread per particle
 __global__ void __launch_bounds__(HD_THREADS)
-k_hd_correct(HdState S, HdBlock B, const double *__restrict__ a1, const double *__restrict__ ad1, double eta, double dt_max,
-             char *raw, unsigned long long *dt_min_bits)
+k_hd_correct(HdState S, HdBlock B, HdCorr C)
 {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    const int ni = *B.d_ni;
-    if (k >= ni) return;
-    const double tn = *B.d_tnext;
-    const int p = B.act[k];
-    const double h = S.dt[p], h2 = h * h, h3 = h2 * h, h4 = h3 * h, h5 = h4 * h;
-    double a2n[3], a3[3], an[3], adn[3];
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        const double a0 = S.a[3 * (size_t)p + c], ad0 = S.ad[3 * (size_t)p + c];
-        an[c] = a1[3 * (size_t)k + c];
-        adn[c] = ad1[3 * (size_t)k + c];
-        const double da = a0 - an[c];
-        const double a2 = (-6 * da - h * (4 * ad0 + 2 * adn[c])) / h2;
-        a3[c] = (12 * da + 6 * h * (ad0 + adn[c])) / h3;
-        S.x[3 * (size_t)p + c] = B.xi[3 * (size_t)k + c] + h4 * a2 / 24 + h5 * a3[c] / 120;
-        S.v[3 * (size_t)p + c] = B.vi[3 * (size_t)k + c] + h3 * a2 / 6 + h4 * a3[c] / 24;
-        a2n[c] = a2 + h * a3[c];
-        S.a[3 * (size_t)p + c] = an[c];
-        S.ad[3 * (size_t)p + c] = adn[c];
-    }
-    S.t[p] = tn;
-    const double na = hd_norm3(an), nad = hd_norm3(adn), n2 = hd_norm3(a2n), n3 = hd_norm3(a3);
-    const double den = nad * n3 + n2 * n2;
-    const double want = den > 0 ? sqrt(eta * (na * n2 + nad * nad) / den) : dt_max;
-    double d = h;
-    if (want < d) {
-        while (d > want) d *= 0.5;
-    } else if (want >= 2 * d && 2 * d <= dt_max && fmod(tn, 2 * d) == 0.0) {
-        d *= 2;
-    }
-    S.dt[p] = d;
-    atomicMin(dt_min_bits, (unsigned long long)__double_as_longlong(d));
-    hd_store_j(raw, S, p);
+    if (k >= *B.d_ni) return;
+    hd_correct_one(S, B, C, k, *B.d_tnext);
 }
 
 __global__ void k_hd_iota(int *act, int n)

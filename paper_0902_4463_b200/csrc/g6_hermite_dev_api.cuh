@@ -18,8 +18,13 @@ struct g6hd_system {
     double *h_tnext = nullptr;
     cudaEvent_t ev = nullptr;
     int last_ni = 0;
+    bool pending = false;                                      // the last block's forces are computed, its corrector has not run yet
     long long nblock = 0, npart = 0, hist[64] = {};
     double inter = 0, wall = 0;
+    // env G6_HD_PROFILE=1: device time of the three phases of every block step (CUDA events; slows the loop down)
+    bool profile = false;
+    cudaEvent_t pe[4] = {};
+    double phase_us[3][64] = {};
 };
 
 namespace {
@@ -28,12 +33,13 @@ void hd_free(g6hd_system *s)
 {
     if (!s) return;
     cudaFree(s->S.x); cudaFree(s->S.v); cudaFree(s->S.a); cudaFree(s->S.ad); cudaFree(s->S.m); cudaFree(s->S.t); cudaFree(s->S.dt);
-    cudaFree(s->B.act); cudaFree(s->B.xi); cudaFree(s->B.vi); cudaFree(s->B.bmin); cudaFree(s->B.bcnt); cudaFree(s->B.ticket);
+    cudaFree(s->B.act); cudaFree(s->B.cand); cudaFree(s->B.xi); cudaFree(s->B.vi); cudaFree(s->B.bmin); cudaFree(s->B.bcnt); cudaFree(s->B.boff); cudaFree(s->B.ticket);
     cudaFree(s->B.d_ni); cudaFree(s->B.d_tnext);
     cudaFree(s->a1); cudaFree(s->ad1); cudaFree(s->pot); cudaFree(s->dt_min_bits);
     if (s->h_ni) cudaFreeHost(s->h_ni);
     if (s->h_tnext) cudaFreeHost(s->h_tnext);
     if (s->ev) cudaEventDestroy(s->ev);
+    for (auto &e : s->pe) if (e) cudaEventDestroy(e);
     delete s;
 }
 
@@ -48,6 +54,19 @@ int hd_force(Cluster &c, g6hd_system &s, int ni, double tn)
                            s.ad1 + 3 * (size_t)i0, s.pot + i0, nullptr, nullptr, nullptr, nullptr, nullptr);
         if (rc) return rc;
     }
+    return G6_OK;
+}
+
+HdCorr hd_corr(const Cluster &c, const g6hd_system &s) { return HdCorr{s.a1, s.ad1, s.eta, s.dt_max, c.js.raw, s.dt_min_bits}; }
+
+// run the corrector of the last block step now (it normally rides in the next k_hd_select)
+int hd_finish(Cluster &c, g6hd_system &s)
+{
+    if (!s.pending) return G6_OK;
+    k_hd_correct<<<(s.last_ni + HD_THREADS - 1) / HD_THREADS, HD_THREADS, 0, c.stream>>>(s.S, s.B, hd_corr(c, s));
+    CK(cudaGetLastError());
+    c.pred_valid = false;
+    s.pending = false;
     return G6_OK;
 }
 
@@ -74,14 +93,16 @@ g6hd_system *g6hd_create(int clusterid, int n, const double x[][3], const double
     int rc = [&]() -> int {
         CK(dalloc(s->S.x, n3)); CK(dalloc(s->S.v, n3)); CK(dalloc(s->S.a, n3)); CK(dalloc(s->S.ad, n3));
         CK(dalloc(s->S.m, n)); CK(dalloc(s->S.t, n)); CK(dalloc(s->S.dt, n));
-        CK(dalloc(s->B.act, n)); CK(dalloc(s->B.xi, n3)); CK(dalloc(s->B.vi, n3));
-        CK(dalloc(s->B.bmin, nb)); CK(dalloc(s->B.bcnt, nb)); CK(dalloc(s->B.ticket, 1)); CK(dalloc(s->B.d_ni, 1)); CK(dalloc(s->B.d_tnext, 1));
+        CK(dalloc(s->B.act, n)); CK(dalloc(s->B.cand, (size_t)nb * HD_PER_BLOCK)); CK(dalloc(s->B.xi, n3)); CK(dalloc(s->B.vi, n3));
+        CK(dalloc(s->B.bmin, nb)); CK(dalloc(s->B.bcnt, nb)); CK(dalloc(s->B.boff, nb)); CK(dalloc(s->B.ticket, 1)); CK(dalloc(s->B.d_ni, 1)); CK(dalloc(s->B.d_tnext, 1));
         CK(dalloc(s->a1, n3)); CK(dalloc(s->ad1, n3)); CK(dalloc(s->pot, n)); CK(dalloc(s->dt_min_bits, 1));
         CK(cudaHostAlloc((void **)&s->h_ni, sizeof(int), cudaHostAllocMapped));
         CK(cudaHostAlloc((void **)&s->h_tnext, sizeof(double), cudaHostAllocMapped));
         CK(cudaHostGetDevicePointer((void **)&s->B.h_ni, s->h_ni, 0));
         CK(cudaHostGetDevicePointer((void **)&s->B.h_tnext, s->h_tnext, 0));
         CK(cudaEventCreateWithFlags(&s->ev, cudaEventDisableTiming));
+        s->profile = env_int("G6_HD_PROFILE", 0) != 0;
+        if (s->profile) for (auto &e : s->pe) CK(cudaEventCreate(&e));
         CK(cudaMemsetAsync(s->B.ticket, 0, sizeof(unsigned int), c.stream));
         const unsigned long long big = 0x7ff0000000000000ULL;
         CK(cudaMemcpyAsync(s->dt_min_bits, &big, sizeof(big), cudaMemcpyHostToDevice, c.stream));
@@ -133,18 +154,36 @@ int g6hd_evolve(g6hd_system *sp, double t_end, long long max_block_steps)
     const int nb = (s.n + HD_PER_BLOCK - 1) / HD_PER_BLOCK;
     long long done = 0;
     while (s.t < t_end && (max_block_steps <= 0 || done < max_block_steps)) {
-        k_hd_select<<<nb, HD_THREADS, 0, c.stream>>>(s.S, s.B);
+        if (s.profile) CK(cudaEventRecord(s.pe[0], c.stream));
+        k_hd_select<<<nb, HD_THREADS, 0, c.stream>>>(s.S, s.B, hd_corr(c, s), s.pending ? 1 : 0);
         CK(cudaGetLastError());
+        c.pred_valid = false;                           // phase 0 rewrote j-store records
+        s.pending = false;
+        if (s.profile) CK(cudaEventRecord(s.pe[1], c.stream));
         CK(cudaEventRecord(s.ev, c.stream));
         CK(cudaEventSynchronize(s.ev));                 // the one host wait of the block step
         const int ni = *(volatile int *)s.h_ni;
         const double tn = *(volatile double *)s.h_tnext;
         if (ni < 1 || ni > s.n || !(tn > s.t)) return fail(c, G6_ERR_CUDA, "block selection returned ni = %d, t = %g", ni, tn);
+        if (ni > HD_GATHER_INLINE) {
+            k_hd_gather<<<nb, HD_THREADS, 0, c.stream>>>(s.S, s.B);
+            CK(cudaGetLastError());
+        }
         int rc = hd_force(c, s, ni, tn);
         if (rc) return rc;
-        k_hd_correct<<<(ni + HD_THREADS - 1) / HD_THREADS, HD_THREADS, 0, c.stream>>>(s.S, s.B, s.a1, s.ad1, s.eta, s.dt_max, c.js.raw, s.dt_min_bits);
-        CK(cudaGetLastError());
-        c.pred_valid = false;                           // the corrector rewrote j-store records
+        s.pending = true;                               // its corrector is phase 0 of the next k_hd_select
+        if (s.profile) {
+            CK(cudaEventRecord(s.pe[2], c.stream));
+            CK(cudaEventRecord(s.pe[3], c.stream));
+            CK(cudaEventSynchronize(s.pe[3]));
+            int bb = 0;
+            while ((1LL << (bb + 1)) <= ni) ++bb;
+            for (int q = 0; q < 3; ++q) {
+                float ms = 0;
+                CK(cudaEventElapsedTime(&ms, s.pe[q], s.pe[q + 1]));
+                s.phase_us[q][bb] += 1e3 * ms;
+            }
+        }
         s.t = tn;
         s.last_ni = ni;
         ++s.nblock; ++done;
@@ -153,6 +192,10 @@ int g6hd_evolve(g6hd_system *sp, double t_end, long long max_block_steps)
         int b = 0;
         while ((1LL << (b + 1)) <= ni) ++b;
         s.hist[b] += 1;
+    }
+    {
+        int rcf = hd_finish(c, s);
+        if (rcf) return rcf;
     }
     CK(cudaStreamSynchronize(c.stream));
     s.wall += std::chrono::duration<double>(std::chrono::steady_clock::now() - w0).count();
@@ -218,6 +261,11 @@ int g6hd_get_stats(g6hd_system *sp, double stats[8], long long ni_hist_log2[64])
     memcpy(&dmin, &bits, sizeof(dmin));
     stats[0] = (double)s.nblock; stats[1] = (double)s.npart; stats[2] = s.t; stats[3] = dmin;
     stats[4] = s.inter; stats[5] = s.wall; stats[6] = 0; stats[7] = 0;
+    if (s.profile)
+        for (int b = 0; b < 64; ++b)
+            if (s.hist[b])
+                fprintf(stderr, "g6hd profile: n_i in [2^%d, 2^%d): %lld block steps, select %.1f us, force (from the host wait to its last kernel) %.1f us, correct %.1f us per step\n",
+                        b, b + 1, s.hist[b], s.phase_us[0][b] / s.hist[b], s.phase_us[1][b] / s.hist[b], s.phase_us[2][b] / s.hist[b]);
     if (ni_hist_log2) memcpy(ni_hist_log2, s.hist, sizeof(s.hist));
     return G6_OK;
 }
