@@ -160,10 +160,11 @@ __device__ __forceinline__ float transpose_reduce8(const float (&v)[8], int lane
     return t;
 }
 
+// `Dp`: the inline i-block / j updates of the launch (nullptr when there are none: device-resident callers)
 template <int MAXI, bool NEWTON>
-__global__ void __launch_bounds__(BS_THREADS)
-k_block_step(const BsArgs A, const BsInline<MAXI> D)
+__device__ __forceinline__ void block_step_body(const BsArgs &A0, const BsInline<MAXI> *Dp)
 {
+    const BsArgs &A = A0;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     BsSmem<MAXI> &sm = *reinterpret_cast<BsSmem<MAXI> *>(smem_raw);
     constexpr float INF = __builtin_huge_valf();
@@ -191,8 +192,8 @@ k_block_step(const BsArgs A, const BsInline<MAXI> D)
     // i-block -> shared memory (double-single split here: the host hands fp64)
     for (int k = tid; k < A.ni * 3; k += BS_THREADS) {
         const int i = k / 3, c = k % 3;
-        const double x = A.inline_i ? D.xi[i][c] : A.xi[k];
-        const double v = A.inline_i ? D.vi[i][c] : A.vi[k];
+        const double x = A.inline_i ? Dp->xi[i][c] : A.xi[k];
+        const double v = A.inline_i ? Dp->vi[i][c] : A.vi[k];
         float hi, lo;
         ds_split(x, hi, lo);
         sm.ipart[i][c] = hi;
@@ -200,8 +201,8 @@ k_block_step(const BsArgs A, const BsInline<MAXI> D)
         sm.ipart[i][6 + c] = (float)v;
     }
     for (int i = tid; i < MAXI; i += BS_THREADS) {
-        if (i < A.ni) sm.iidx[i] = A.inline_i ? D.index[i] : A.i_index[i];
-        sm.uaddr[i] = i < A.n_upd ? D.upd[i].addr : -1;
+        if (i < A.ni) sm.iidx[i] = A.inline_i ? Dp->index[i] : A.i_index[i];
+        sm.uaddr[i] = i < A.n_upd ? Dp->upd[i].addr : -1;
 #pragma unroll
         for (int q = 0; q < NW; ++q) {
             sm.r2[q][i] = INF;
@@ -230,7 +231,7 @@ k_block_step(const BsArgs A, const BsInline<MAXI> D)
         if (A.n_upd > 0) {
             for (int u = lane; u < A.n_upd; u += 32)
                 if (sm.uaddr[u] / JT == tile) {
-                    const JRecord r = D.upd[u];
+                    const JRecord r = Dp->upd[u];
                     store_record(R, r.addr % JT, r);
                     store_record(A.raw + (size_t)tile * RAW_TILE_BYTES, r.addr % JT, r);
                 }
@@ -413,6 +414,21 @@ k_block_step(const BsArgs A, const BsInline<MAXI> D)
     if (tid == 0) *A.counter = 0u;
 }
 
+template <int MAXI, bool NEWTON>
+__global__ void __launch_bounds__(BS_THREADS)
+k_block_step(const BsArgs A, const __grid_constant__ BsInline<MAXI> D)
+{
+    block_step_body<MAXI, NEWTON>(A, &D);
+}
+
+// the same kernel without the inline payload (i-block in device memory, no j updates): 2-8 KB fewer launch parameters
+template <int MAXI, bool NEWTON>
+__global__ void __launch_bounds__(BS_THREADS)
+k_block_step_dev(const BsArgs A)
+{
+    block_step_body<MAXI, NEWTON>(A, nullptr);
+}
+
 // ---------------------------------------------------------------- host side
 template <int MAXI>
 inline int bs_attr()
@@ -420,7 +436,11 @@ inline int bs_attr()
     const int bytes = (int)sizeof(BsSmem<MAXI>);
     cudaError_t e = cudaFuncSetAttribute(k_block_step<MAXI, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     if (e != cudaSuccess) return (int)e;
-    return (int)cudaFuncSetAttribute(k_block_step<MAXI, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    e = cudaFuncSetAttribute(k_block_step<MAXI, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e != cudaSuccess) return (int)e;
+    e = cudaFuncSetAttribute(k_block_step_dev<MAXI, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e != cudaSuccess) return (int)e;
+    return (int)cudaFuncSetAttribute(k_block_step_dev<MAXI, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
 }
 
 inline int bs_kernel_init()
@@ -453,6 +473,11 @@ inline int bs_launch_t(const BsArgs &A, bool newton, int grid, const double *xi,
     }
     if (A.n_upd > 0) memcpy(D.upd, upd, sizeof(JRecord) * A.n_upd);
     const size_t bytes = sizeof(BsSmem<MAXI>);
+    if (!A.inline_i && A.n_upd == 0) {          // nothing to carry: the launch without the inline payload
+        if (newton) k_block_step_dev<MAXI, true><<<grid, BS_THREADS, bytes, st>>>(A);
+        else k_block_step_dev<MAXI, false><<<grid, BS_THREADS, bytes, st>>>(A);
+        return (int)cudaGetLastError();
+    }
     if (newton) k_block_step<MAXI, true><<<grid, BS_THREADS, bytes, st>>>(A, D);
     else k_block_step<MAXI, false><<<grid, BS_THREADS, bytes, st>>>(A, D);
     return (int)cudaGetLastError();
