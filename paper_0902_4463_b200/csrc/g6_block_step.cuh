@@ -465,7 +465,7 @@ template <int MAXI>
 inline int bs_launch_t(const BsArgs &A, bool newton, int grid, const double *xi, const double *vi, const int *index,
                        const JRecord *upd, cudaStream_t st)
 {
-    static BsInline<MAXI> D;       // one host thread per library (g6.h); filled per call, copied by the launch
+    static thread_local BsInline<MAXI> D;   // one host thread per cluster (g6.h); filled per call, copied by the launch
     if (A.inline_i) {
         memcpy(D.xi, xi, sizeof(double) * 3 * A.ni);
         memcpy(D.vi, vi, sizeof(double) * 3 * A.ni);
