@@ -463,6 +463,7 @@ inline int fast_kernel_init()
     if ((r = fast_attr_nb<128, 1>())) return r;
     if ((r = fast_attr_nb<64, 1>())) return r;
     if ((r = fast_attr_nb<32, 1>())) return r;
+    if ((r = fast_attr_nb<256, 1>())) return r;
     return 0;
 }
 
@@ -473,7 +474,10 @@ inline FastVariant fast_pick(int ni, int n_sm, int force)
     if (force > 0) return FastVariant{force / 8, force % 8};
     if (ni <= 32) return FastVariant{32, 1};
     if (ni <= 64) return FastVariant{64, 1};
-    if (ni <= 128 * n_sm) return FastVariant{128, 1};
+    if (ni < 256) return FastVariant{128, 1};
+    // measured at N_j = 2^20: 8 warps sharing one staged j-tile beat 4 by 6-7 % for
+    // blocks of 256 .. 4096; on full sweeps 128 x 2 and 256 x 1 are equal
+    if (ni <= 128 * n_sm) return FastVariant{256, 1};
     return FastVariant{128, 2};
 }
 
@@ -501,7 +505,7 @@ inline int fast_launch_nb_t(const ForceArgs &A, bool newton, int n_itiles, int S
 inline bool fast_has_nb(FastVariant v)
 {
     const int key = v.threads * 8 + v.it;
-    return key == 128 * 8 + 2 || key == 128 * 8 + 1 || key == 64 * 8 + 1 || key == 32 * 8 + 1;
+    return key == 128 * 8 + 2 || key == 128 * 8 + 1 || key == 64 * 8 + 1 || key == 32 * 8 + 1 || key == 256 * 8 + 1;
 }
 
 inline int launch_force_fast(const ForceArgs &A, bool newton, FastVariant v, int n_itiles, int S, cudaStream_t st)
@@ -513,6 +517,7 @@ inline int launch_force_fast(const ForceArgs &A, bool newton, FastVariant v, int
             case 128 * 8 + 1: return fast_launch_nb_t<128, 1>(A, newton, n_itiles, S, st);
             case 64 * 8 + 1: return fast_launch_nb_t<64, 1>(A, newton, n_itiles, S, st);
             case 32 * 8 + 1: return fast_launch_nb_t<32, 1>(A, newton, n_itiles, S, st);
+            case 256 * 8 + 1: return fast_launch_nb_t<256, 1>(A, newton, n_itiles, S, st);
             default: return (int)cudaErrorInvalidValue;
         }
     }
@@ -540,9 +545,10 @@ inline int fast_occ_t()
 }
 inline int fast_ctas_per_sm_nb(FastVariant v)
 {
-    static int cache[4] = {0};
+    static int cache[5] = {0};
     const int key = v.threads * 8 + v.it;
     switch (key) {
+        case 256 * 8 + 1: return cache[4] ? cache[4] : (cache[4] = fast_occ_t<256, 1, true>());
         case 128 * 8 + 2: return cache[0] ? cache[0] : (cache[0] = fast_occ_t<128, 2, true>());
         case 128 * 8 + 1: return cache[1] ? cache[1] : (cache[1] = fast_occ_t<128, 1, true>());
         case 64 * 8 + 1: return cache[2] ? cache[2] : (cache[2] = fast_occ_t<64, 1, true>());
