@@ -399,7 +399,7 @@ int choose_jsplit(int n_itiles, int ntiles, int slots, int ni, long long s_cap =
     const double TAIL = 0.06;      // CTAs of the last wave do not finish together: a fraction of one CTA's length is lost
     const double COMBINE = 0.004;  // per extra split: partial traffic + combine work, in tile times
     long long smax = std::min<long long>(ntiles, (1LL << 30) / (72LL * std::max(ni, 1)));
-    smax = std::max<long long>(1, std::min<long long>(std::min(smax, s_cap), 4LL * slots / std::max(n_itiles, 1) + 2));
+    smax = std::max<long long>(1, std::min<long long>(std::min(smax, s_cap), std::max(8LL, 4LL * slots / std::max(n_itiles, 1) + 2)));
     int best = 1;
     double best_cost = 1e300;
     for (int S = 1; S <= smax; ++S) {
