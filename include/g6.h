@@ -100,8 +100,7 @@ int g6_set_ti(int clusterid, double ti);
  *                      `nb_maxlen` (option, default G6_NB_MAXLEN = 256, the paper's default)
  *                      neighbours are stored per i, those with the smallest j addresses; the count
  *                      keeps running (count > nb_maxlen = overflow).  Read with
- *                      g6_read_neighbour_list + g6_get_neighbour_list.  Blocks with lists take the
- *                      sweep kernels at any ni (the fused small-block kernel builds none).
+ *                      g6_read_neighbour_list + g6_get_neighbour_list.
  * Copies the block to pinned staging, uploads j-particles changed since the last call, and
  * enqueues predictor -> force -> combine -> download.  Returns without waiting. */
 int g6calc_firsthalf(int clusterid, int nj, int ni, const int index[],
@@ -203,6 +202,8 @@ int g6x_get_timers(int clusterid, double us[8]);
  *             combine, lanes over j); default 32, at most 64, 0 = off
  *   "nb_maxlen" neighbours stored per i-particle (1 .. 4096, default G6_NB_MAXLEN = 256; compile-time
  *             in the paper); changing it discards the lists of the last call
+ *   "last_kernel" (g6x_get_option only) the force kernel the last call took: 1 checked reference kernel,
+ *             2 fast sweep kernel, 3 block-step kernel
  * Returns G6_ERR_ARG for an unknown key or value. */
 int g6x_set_option(int clusterid, const char *key, int value);
 int g6x_get_option(int clusterid, const char *key, int *value);

@@ -79,6 +79,8 @@ struct Cluster {
     // neighbour lists: per-split lists, combined lists, host copies; all on demand
     int *d_nb_pcnt = nullptr, *d_nb_plist = nullptr;   // [S][ni], [S][ni][maxlen]
     size_t nb_part_rows = 0;                           // S * ni rows allocated
+    int *d_nb_wcnt = nullptr, *d_nb_wlist = nullptr;   // block-step kernel: per-warp lists [ni][warps], [warps][ni][maxlen]
+    size_t nb_w_rows = 0;                              // warps * ni rows allocated
     int *d_nb_cnt = nullptr, *d_nb_list = nullptr;     // [ni], [ni][maxlen]
     int *h_nb_cnt = nullptr, *h_nb_list = nullptr;     // pinned
     double *h_h2 = nullptr, *d_h2 = nullptr;           // neighbour radii of the i-block
@@ -102,6 +104,7 @@ struct Cluster {
     cudaEvent_t ev[N_EVENTS] = {};
     bool ev_valid = false;
     int last_ctas = 0, last_S = 0;
+    int last_kernel = 0;       // force kernel of the last call: 1 checked reference, 2 fast sweep kernel, 3 block-step kernel
 
     // options
     int opt_ds = 1, opt_newton = 1, opt_jsplit = 0, opt_kernel = 0, opt_timers = 0, opt_variant = 0, opt_small = 32, opt_nb_maxlen = 256;
@@ -224,8 +227,10 @@ int ensure_partials(Cluster &c, size_t elems)
 void free_nb(Cluster &c)
 {
     dfree(c.d_nb_pcnt); dfree(c.d_nb_plist); dfree(c.d_nb_cnt); dfree(c.d_nb_list); dfree(c.d_h2);
+    dfree(c.d_nb_wcnt); dfree(c.d_nb_wlist);
     hfree(c.h_nb_cnt); hfree(c.h_nb_list); hfree(c.h_h2);
     c.nb_part_rows = 0;
+    c.nb_w_rows = 0;
     c.nb_cap = 0;
     c.nb_alloc_maxlen = 0;
     c.last_nb = c.nb_on_host = false;
@@ -253,6 +258,20 @@ int ensure_nb_part(Cluster &c, size_t rows)
     c.nb_part_rows = 0;
     CK(dalloc(c.d_nb_pcnt, rows)); CK(dalloc(c.d_nb_plist, rows * c.opt_nb_maxlen));
     c.nb_part_rows = rows;
+    return G6_OK;
+}
+
+// per-warp lists of the block-step kernel (rows = warps of the grid * ni)
+int ensure_nb_warp(Cluster &c, size_t rows)
+{
+    int rc = nb_check_maxlen(c);
+    if (rc) return rc;
+    if (rows <= c.nb_w_rows) return G6_OK;
+    CK(cudaStreamSynchronize(c.stream));
+    dfree(c.d_nb_wcnt); dfree(c.d_nb_wlist);
+    c.nb_w_rows = 0;
+    CK(dalloc(c.d_nb_wcnt, rows)); CK(dalloc(c.d_nb_wlist, rows * c.opt_nb_maxlen));
+    c.nb_w_rows = rows;
     return G6_OK;
 }
 
@@ -416,7 +435,8 @@ int choose_jsplit(int n_itiles, int ntiles, int slots, int ni, long long s_cap =
 // small active blocks take the fused block-step kernel unless an experiment switch pins another path
 bool use_block_step(const Cluster &c, int ni, bool nb = false)
 {
-    return !nb && ni <= c.opt_small && c.opt_kernel != 1 && c.opt_kernel != 2 && c.opt_jsplit == 0;
+    // with neighbour lists the kernel's last-CTA merge holds one list per warp in shared memory
+    return (!nb || c.opt_nb_maxlen <= BS_NB_SCRATCH) && ni <= c.opt_small && c.opt_kernel != 1 && c.opt_kernel != 2 && c.opt_jsplit == 0;
 }
 
 struct HostBlock { const double *xi, *vi; const int *index; };   // host copy of the i-block (small blocks travel in kernel parameters)
@@ -474,6 +494,16 @@ int run_force(Cluster &c, int nj, int ni, const int *d_index, const double *d_xi
         B.P.stride_i = G;
         B.counter = c.d_counter;
         B.acc = d_acc; B.jerk = d_jerk; B.pot = d_pot; B.nn_index = d_nn_index; B.nn_r2 = d_nn_r2;
+        if (nb) {
+            rc = ensure_nb_warp(c, (size_t)G * (BS_THREADS / 32) * ni);
+            if (rc) return rc;
+            B.h2 = nb->d_h2;
+            B.nb_maxlen = c.opt_nb_maxlen;
+            B.nb_wcnt = c.d_nb_wcnt;
+            B.nb_wlist = c.d_nb_wlist;
+            B.nb_cnt = nb->d_cnt;
+            B.nb_list = nb->d_list;
+        }
         if (ev_pred_done) CK(cudaEventRecord(ev_pred_done, c.stream));     // predictor fused: no separate phase
         const JRecord *upd = inline_upd ? c.h_rec[c.rec_cur] : nullptr;
         rc = big ? bs_launch_t<BS_MAX_I>(B, c.opt_newton != 0, G, hb ? hb->xi : nullptr, hb ? hb->vi : nullptr, hb ? hb->index : nullptr, upd, c.stream)
@@ -487,6 +517,7 @@ int run_force(Cluster &c, int nj, int ni, const int *d_index, const double *d_xi
         if (ev_force_done) CK(cudaEventRecord(ev_force_done, c.stream));
         c.last_ctas = G;
         c.last_S = G;
+        c.last_kernel = 3;
         return G6_OK;
     }
     if (c.n_rec > 0) {         // callers of the sweep path have normally flushed already
@@ -546,6 +577,7 @@ int run_force(Cluster &c, int nj, int ni, const int *d_index, const double *d_xi
     }
     c.last_ctas = n_itiles * S;
     c.last_S = S;
+    c.last_kernel = use_fast ? 2 : 1;
     return G6_OK;
 }
 
@@ -800,7 +832,7 @@ int g6calc_firsthalf(int clusterid, int nj, int ni, const int index[], const dou
         }
         c.iblk_on_device = false;
         rc = run_force(c, nj, ni, nullptr, nullptr, nullptr, eps2, out.acc, out.jerk, out.pot, out.nnidx, out.nnr2, tm ? c.ev[2] : nullptr,
-                       tm ? c.ev[3] : nullptr, &hb);
+                       tm ? c.ev[3] : nullptr, &hb, want_nb ? &nbr : nullptr);
         if (rc) return rc;
     } else {
         // a-3: i block to pinned staging (the only per-step H2D payload) ...
@@ -1012,6 +1044,7 @@ int g6x_set_option(int clusterid, const char *key, int value)
 int g6x_get_option(int clusterid, const char *key, int *value)
 {
     GET_CLUSTER(clusterid);
+    if (key && value && !strcmp(key, "last_kernel")) { *value = c.last_kernel; return G6_OK; }
     int *slot = option_slot(c, key);
     if (!slot || !value) return fail(c, G6_ERR_ARG, "unknown option '%s'", key ? key : "(null)");
     *value = *slot;

@@ -40,6 +40,7 @@ constexpr int BS_THREADS = 384;
 // raw-tile slots of the shared-memory ring (one CTA per SM owns all of its shared memory)
 __host__ __device__ constexpr int bs_nslots(int maxi) { return maxi <= 16 ? 10 : 8; }
 constexpr int BS_MAX_I = 64;
+constexpr int BS_NB_SCRATCH = 1024;     // addresses per warp in the last CTA's neighbour-list merge: the largest nb_maxlen served
 
 // i-block and changed j-particles carried by value in the kernel parameters
 template <int MAXI>
@@ -65,6 +66,14 @@ struct BsArgs {
     double *acc, *jerk, *pot;   // results (device or mapped host memory)
     int *nn_index;
     double *nn_r2;
+    // neighbour lists (reading 20); h2 == nullptr: none.  Every warp of the grid keeps its own
+    // list per i-particle (it meets its tiles in increasing address order); the last CTA merges them by address.
+    const double *h2;           // [ni] neighbour-sphere radius squared
+    int nb_maxlen;
+    int *nb_wcnt;               // [ni][G * NW]          neighbours found by warp (cta * NW + w), may exceed nb_maxlen
+    int *nb_wlist;              // [G * NW][ni][maxlen]  their j addresses, increasing
+    int *nb_cnt;                // [ni]          out: all neighbours found
+    int *nb_list;               // [ni][maxlen]  out: callers' indices, increasing j address, the smallest addresses on overflow
 };
 
 __device__ __forceinline__ int ld_acquire_cta(const volatile int *p)
@@ -85,6 +94,8 @@ struct BsSmem {
     float r2[BS_THREADS / 32][MAXI];                          // per-warp nearest neighbour of every i
     int addr[BS_THREADS / 32][MAXI];
     float ipart[MAXI][9];
+    float h2[MAXI];                                           // neighbour radii (binary32, like r2)
+    int nbcnt[BS_THREADS / 32][MAXI];                         // per-warp running neighbour counts
     int iidx[MAXI];
     int uaddr[MAXI];
     alignas(8) uint64_t full[bs_nslots(MAXI)];
@@ -203,8 +214,10 @@ __device__ __forceinline__ void block_step_body(const BsArgs &A0, const BsInline
     for (int i = tid; i < MAXI; i += BS_THREADS) {
         if (i < A.ni) sm.iidx[i] = A.inline_i ? Dp->index[i] : A.i_index[i];
         sm.uaddr[i] = i < A.n_upd ? Dp->upd[i].addr : -1;
+        sm.h2[i] = (A.h2 && i < A.ni) ? (float)A.h2[i] : 0.0f;
 #pragma unroll
         for (int q = 0; q < NW; ++q) {
+            sm.nbcnt[q][i] = 0;
             sm.r2[q][i] = INF;
             sm.addr[q][i] = 0x7fffffff;
 #pragma unroll
@@ -314,6 +327,25 @@ __device__ __forceinline__ void block_step_body(const BsArgs &A0, const BsInline
             float lmin = fminf(fminf(r2m[0].x, r2m[0].y), fminf(r2m[1].x, r2m[1].y));
             lmin = fminf(lmin, fminf(fminf(r2m[2].x, r2m[2].y), fminf(r2m[3].x, r2m[3].y)));
             const unsigned gbits = __reduce_min_sync(FULL, __float_as_uint(lmin));
+            // neighbour list: pairs with r2 < h2_i (masked pairs carry r2 = +inf), appended in address order
+            // = (g, lane, x before y); rare, so the whole warp leaves the common path only when some lane has a hit
+            if (A.h2 && gbits < __float_as_uint(sm.h2[i])) {
+                const float h2i = sm.h2[i];
+                int cnt = sm.nbcnt[w][i];
+                int *dst = A.nb_wlist + ((size_t)(cta * NW + w) * A.ni + i) * A.nb_maxlen;
+                const unsigned lt = (1u << lane) - 1u;
+#pragma unroll
+                for (int g = 0; g < 4; ++g) {
+                    const bool hx = r2m[g].x < h2i, hy = r2m[g].y < h2i;
+                    const unsigned mx = __ballot_sync(FULL, hx), my_ = __ballot_sync(FULL, hy);
+                    const int px = cnt + __popc(mx & lt) + __popc(my_ & lt);
+                    if (hx && px < A.nb_maxlen) dst[px] = ja0 + 64 * g;
+                    if (hy && px + (hx ? 1 : 0) < A.nb_maxlen) dst[px + (hx ? 1 : 0)] = ja0 + 64 * g + 1;
+                    cnt += __popc(mx) + __popc(my_);
+                }
+                __syncwarp();
+                if (lane == 0) sm.nbcnt[w][i] = cnt;
+            }
             if (gbits < __float_as_uint(sm.r2[w][i])) {     // strict: my earlier tiles (lower addresses) keep ties
                 int cand = 0x7fffffff;
 #pragma unroll
@@ -353,6 +385,11 @@ __device__ __forceinline__ void block_step_body(const BsArgs &A0, const BsInline
         A.P.nn_r2[o] = has ? best : INF;
         A.P.nn_addr[o] = has ? baddr : -1;
     }
+    if (A.h2)
+        for (int k = tid; k < A.ni * NW; k += BS_THREADS) {
+            const int i = k / NW, q = k % NW;
+            A.nb_wcnt[(size_t)i * (G * NW) + cta * NW + q] = sm.nbcnt[q][i];
+        }
     __threadfence();
     __syncthreads();
     if (tid == 0) {
@@ -409,6 +446,68 @@ __device__ __forceinline__ void block_step_body(const BsArgs &A0, const BsInline
             const bool has = baddr != 0x7fffffff;
             if (A.nn_index) A.nn_index[i] = has ? j_index(A.raw, baddr) : -1;
             if (A.nn_r2) A.nn_r2[i] = has ? (double)best : (double)INF;
+        }
+    }
+    // ---- neighbour lists (last CTA): merge the per-warp lists of every i by j address.  One warp per i; the shared-memory
+    // ring is idle now and serves as scratch (BS_NB_SCRATCH addresses per warp >= nb_maxlen, enforced by the host).
+    if (A.h2) {
+        const int NSEG = G * NW;
+        int *scratch = reinterpret_cast<int *>(&sm.raw[0][0]) + w * BS_NB_SCRATCH;
+        for (int i = w; i < A.ni; i += NW) {
+            const int *wc = A.nb_wcnt + (size_t)i * NSEG;
+            int tot = 0;
+            for (int sg = lane; sg < NSEG; sg += 32) tot += __ldcg(wc + sg);
+            tot = __reduce_add_sync(FULL, tot);
+            // T: entries with address < T are kept.  No overflow: everything.  Overflow: the nb_maxlen smallest addresses,
+            // found by bisection on the address (every per-warp list is sorted and holds its own nb_maxlen smallest).
+            int T = 0x7fffffff;
+            if (tot > A.nb_maxlen) {
+                int lo = 0, hi = A.ntiles * JT;
+                while (hi - lo > 1) {
+                    const int mid = lo + (hi - lo) / 2;
+                    int below = 0;
+                    for (int sg = lane; sg < NSEG; sg += 32) {
+                        const int c = min(__ldcg(wc + sg), A.nb_maxlen);
+                        if (c > 0) {
+                            const int *L = A.nb_wlist + ((size_t)sg * A.ni + i) * A.nb_maxlen;
+                            int a = 0, b = c;                       // first entry >= mid
+                            while (a < b) { const int m = (a + b) >> 1; if (__ldcg(L + m) < mid) a = m + 1; else b = m; }
+                            below += a;
+                        }
+                    }
+                    below = __reduce_add_sync(FULL, below);
+                    if (below >= A.nb_maxlen) hi = mid; else lo = mid;
+                }
+                T = hi;
+            }
+            // gather the kept entries of all segments into the scratch (order irrelevant), then rank-sort by address
+            int base = 0;
+            for (int s0 = 0; s0 < NSEG; s0 += 32) {
+                const int sg = s0 + lane;
+                const int c = sg < NSEG ? min(__ldcg(wc + sg), A.nb_maxlen) : 0;
+                const int *L = A.nb_wlist + ((size_t)(sg < NSEG ? sg : 0) * A.ni + i) * A.nb_maxlen;
+                int keep = 0;
+                while (keep < c && __ldcg(L + keep) < T) ++keep;
+                int inc = keep;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int u = __shfl_up_sync(FULL, inc, o);
+                    if (lane >= o) inc += u;
+                }
+                const int at = base + inc - keep;
+                for (int k = 0; k < keep; ++k) scratch[at + k] = __ldcg(L + k);
+                base += __shfl_sync(FULL, inc, 31);
+            }
+            __syncwarp();
+            const int nkeep = base;                               // = min(tot, nb_maxlen)
+            for (int e = lane; e < nkeep; e += 32) {
+                const int v = scratch[e];
+                int rank = 0;
+                for (int k = 0; k < nkeep; ++k) rank += scratch[k] < v;
+                A.nb_list[(size_t)i * A.nb_maxlen + rank] = j_index(A.raw, v);
+            }
+            if (lane == 0) A.nb_cnt[i] = tot;
+            __syncwarp();
         }
     }
     if (tid == 0) *A.counter = 0u;

@@ -191,3 +191,36 @@ def test_neighbour_abi_errors_and_maxlen_change(cluster, oracle):
     assert L.g6_get_neighbour_list(0, i, 2, C.byref(nn), buf) == 1 and nn.value == 2
     assert [buf[0], buf[1]] == list(lst[i][:2])
     g6.g6x_set_option(0, "nb_maxlen", 256)
+
+
+@pytest.mark.parametrize("n,ni,small", [(5000, 1, 32), (5000, 7, 32), (3000, 16, 32), (70000, 32, 32), (900, 64, 64), (300, 33, 64)])
+def test_small_blocks_lists_from_the_block_step_kernel(cluster, oracle, n, ni, small):
+    """n_i <= `small`: lists come from the fused block-step kernel (per-warp lists merged by address in its last CTA);
+    the same call with the kernel switched off (sweep path) must give identical lists."""
+    x, v, m, eps2 = inputs.config("C1", n=n)
+    tj, dtj, a0, j0 = inputs.taylor_state(n, 41)
+    index = (np.arange(n, dtype=np.int32) * 3 + 1).astype(np.int32)
+    g6.g6x_set_j_particles(0, 0, index, tj, m, j0, a0, v, x)
+    ti = 0.03125
+    g6.g6_set_ti(0, ti)
+    xp, vp = oracle.predict(ti, tj, x, v, a0, j0)
+    sel = inputs.active_subset(n, ni, 7 + ni)
+    h2 = radii(x, sel, 10, lo=0.5, hi=3.0)
+    if ni > 2:
+        h2[1] = 1e6                                # overflow: everybody is a neighbour
+    h2[0] = 0.0
+    g6.g6x_set_option(0, "small", small)
+    got, cnt, lst = run(index[sel], xp[sel], vp[sel], eps2, n, h2, 256)
+    assert g6.g6x_get_option(0, "last_kernel") == 3          # the block-step kernel served it
+    oc, ol = oracle.neighbours(index[sel], xp[sel], h2, index, xp, maxlen=max(n, 256))
+    check_neighbours(cnt, lst, oc, ol, index, xp[sel], xp, h2, 256, tol=1e-4)
+    assert cnt[0] == 0
+    if ni > 2:
+        assert cnt[1] == n - 1 and (lst[1] >= 0).sum() == min(256, n - 1)
+    ref = oracle.force(index[sel], xp[sel], vp[sel], index, xp, vp, m, eps2)
+    assert np.abs(got["pot"] - ref["pot"]).max() / np.abs(ref["pot"]).max() < 1e-5
+    g6.g6x_set_option(0, "small", 0)               # the sweep kernels on the same call
+    got2, cnt2, lst2 = run(index[sel], xp[sel], vp[sel], eps2, n, h2, 256)
+    assert g6.g6x_get_option(0, "last_kernel") == 2
+    assert np.array_equal(cnt, cnt2) and np.array_equal(lst, lst2)
+    g6.g6x_set_option(0, "small", 32)
