@@ -427,7 +427,7 @@ def main():
                     "unit": "TFLOP/s", "frac": ach_inst / peak_inst,
                     # dram__bytes_read.sum + dram__bytes_write.sum of one launch of this kernel at N = 2^20, from the ncu --set full
                     # capture profiles/r01_force_fast_1M_ncu_full.txt (bytes per launch; only valid for the headline workload)
-                    "traffic": 282398720 if (n == 1048576 and world == 1) else None,
+                    "traffic": 1028230400 if (n == 1048576 and world == 1) else None,
                     "how": ("FP32-pipe issue-slot equivalent: 33 algorithmic FP32 lane-instructions per interaction (SURVEY 8(d)) x "
                             "interactions per launch / mean force-kernel time (CUDA events on the launching stream, live in this run); "
                             f"peak = 148 SM x 128 lanes x {sm_max:.0f} MHz ({peaks_src} max SM clock) x 2"),
