@@ -408,7 +408,7 @@ int run_predict(Cluster &c)
 
 // i/j-split scheduler (PAPER.md:82 "j-particles distributed evenly among the P MPs", :104 generalised):
 // pick the number of j-splits S that minimises  waves(S) x (tiles per CTA + per-CTA overhead) + tail,
-// waves(S) = ceil(i-tiles x S / resident CTA slots), over up to ~4 waves.  Small blocks get S ~ slots (every
+// waves(S) = ceil(i-tiles x S / resident CTA slots), S up to ~4 waves or CTAs of >= 64 tiles, whichever allows more.  Small blocks get S ~ slots (every
 // SM busy at n_i = 1); big sweeps get the S that makes the last wave full; in between, whole numbers of
 // waves of shorter CTAs (measured at N_j = 2^20, 256 x 1 threads: n_i = 1024 at 1 / 2 / 4 / 8 waves ->
 // 0.67 / 0.716 / 0.723 / 0.716 of the FP32 peak; 1.5 or 1.7 waves cost 5-10 %).  Partials are capped at 1 GiB.
@@ -418,7 +418,7 @@ int choose_jsplit(int n_itiles, int ntiles, int slots, int ni, long long s_cap =
     const double TAIL = 0.06;      // CTAs of the last wave do not finish together: a fraction of one CTA's length is lost
     const double COMBINE = 0.004;  // per extra split: partial traffic + combine work, in tile times
     long long smax = std::min<long long>(ntiles, (1LL << 30) / (72LL * std::max(ni, 1)));
-    smax = std::max<long long>(1, std::min<long long>(std::min(smax, s_cap), std::max(8LL, 4LL * slots / std::max(n_itiles, 1) + 2)));
+    smax = std::max<long long>(1, std::min<long long>(std::min(smax, s_cap), std::max<long long>(std::max(8, ntiles / 64), 4LL * slots / std::max(n_itiles, 1) + 2)));
     int best = 1;
     double best_cost = 1e300;
     for (int S = 1; S <= smax; ++S) {
