@@ -2,7 +2,7 @@
 4th-order Hermite with block time steps (eta = 0.01, power-of-two steps), driven through the
 GRAPE-6 calling sequence of libg6b200 (Fig. 1).
 
-    python -m paper_0902_4463_b200.hermite_run [--n 32768] [--t-end 1.0] [--eta 0.01] [--newton 1]
+    python -m paper_0902_4463_b200.hermite_run [--n 32768] [--t-end 1.0] [--eta 0.01] [--newton 1] [--driver host|device]
 
 Prints one JSON line: block-step statistics, the n_i histogram, wall-clock rates and (with
 --state-out) writes the final state for an independent energy check.  The energy itself is the
@@ -25,6 +25,8 @@ def main():
     ap.add_argument("--t-end", type=float, default=1.0)
     ap.add_argument("--eta", type=float, default=0.01)
     ap.add_argument("--newton", type=int, default=None)
+    ap.add_argument("--driver", default="host", choices=["host", "device"],
+                    help="host: g6h_* (host corrector, GRAPE-6 calling sequence); device: g6hd_* (corrector and block selection on the GPU)")
     ap.add_argument("--state-out", default=None, help=".npz file for the initial and final state")
     args = ap.parse_args()
     build.build()
@@ -33,7 +35,7 @@ def main():
     if args.newton is not None:
         g6.g6x_set_option(0, "newton", args.newton)
     t0 = time.perf_counter()
-    h = g6.Hermite(0, x, v, m, eps2, args.eta)
+    h = (g6.HermiteDev if args.driver == "device" else g6.Hermite)(0, x, v, m, eps2, args.eta)
     t_init = time.perf_counter() - t0
     h.evolve(args.t_end)
     x1, v1 = h.state()
@@ -41,7 +43,8 @@ def main():
     h.close()
     g6.g6_close(0)
     hist = [int(c) for c in st["ni_hist_log2"][:24]]
-    out = {"config": "C2", "n": len(m), "eps2": eps2, "eta": args.eta, "t_end": st["t"],
+    st.setdefault("wall_force_s", float("nan")); st.setdefault("force_wall_s_log2", np.zeros(64))
+    out = {"config": "C2", "driver": args.driver, "n": len(m), "eps2": eps2, "eta": args.eta, "t_end": st["t"],
            "block_steps": st["n_block_steps"], "particle_steps": st["n_particle_steps"],
            "mean_block_size": st["n_particle_steps"] / max(1, st["n_block_steps"]),
            "interactions": st["interactions"], "dt_min": st["dt_min"],
