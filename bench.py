@@ -235,6 +235,35 @@ def neighbour_list_cost(g6, inputs, torch, dev, x, v, idx_all, n, eps2, ni=65536
             "overflowed": int((cnt > maxlen).sum()), "nb_maxlen": maxlen}
 
 
+def c3_sweep(g6, inputs, torch, dev, peaks, reps=5):
+    """BASELINE.json configs[2] (C3): full force sweep at N = 131072, device-resident, L2-resident j-store
+    (a side figure; the headline is C4).  Replaces the j-store contents: call last."""
+    f64 = torch.float64
+    x, v, m, eps2 = inputs.config("C3")
+    n = len(m)
+    to = lambda a, dt=f64: torch.from_numpy(np.ascontiguousarray(a)).to(dev, dt)
+    d_x, d_v, d_m, d_idx = to(x), to(v), to(m), to(np.arange(n, dtype=np.int32), torch.int32)
+    z3 = torch.zeros(n, 3, dtype=f64, device=dev); zt = torch.zeros(n, dtype=f64, device=dev)
+    acc = torch.empty(n, 3, dtype=f64, device=dev); jerk = torch.empty_like(acc); pot = torch.empty(n, dtype=f64, device=dev)
+    nn = torch.empty(n, dtype=torch.int32, device=dev); r2 = torch.empty_like(pot)
+    ts, fs = [], []
+    for k in range(reps + 2):
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(torch.cuda.current_stream())
+        g6.g6x_set_j_particles_dev(0, 0, n, d_idx, zt, d_m, z3, z3, d_v, d_x)
+        g6.g6_set_ti(0, 0.0)
+        g6.g6x_calc_dev(0, n, n, d_idx, d_x, d_v, eps2, acc, jerk, pot, nn, r2)
+        e1.record(torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        if k >= 2:
+            ts.append(e0.elapsed_time(e1)); fs.append(g6.g6x_get_timers(0)["force_us"])
+    ms, f_us = float(np.median(ts)), float(np.median(fs))
+    peak_inst = SM_COUNT * FP32_LANES_PER_SM * float(peaks.get("sm_max_mhz", SM_MAX_MHZ_FALLBACK)) * 1e6
+    return {"workload": f"C3: N={n} equal-mass Plummer, eps=1e-4, full sweep", "ms_per_step": ms, "interactions_per_s": float(n) * n / (ms * 1e-3),
+            "gflops_60": FLOP_PAPER * float(n) * n / (ms * 1e-3) / 1e9, "force_kernel_ms": f_us / 1e3,
+            "fp32_frac_force_kernel": FP32_INSTR_PER_INTERACTION * float(n) * n / (f_us * 1e-6) / peak_inst}
+
+
 def run_reference(args):
     """--impl reference: the oracle, timed on the host cores on a bounded sample per step."""
     rank = int(os.environ.get("RANK", "0"))
@@ -405,11 +434,13 @@ def main():
                "note": "host arrays in, host arrays out (library stages through its own pinned buffers); includes the L2 flush"}
 
     sweep = None
+    c3 = None
     nb_cost = None
     ceilings = None
     if rank == 0 and world == 1 and not args.no_sweep:
         sweep = ni_sweep(g6, inputs, torch, dev, stream, flush, x, v, idx, n, eps2, measured_peaks()[0])
         nb_cost = neighbour_list_cost(g6, inputs, torch, dev, x, v, idx, n, eps2)
+        c3 = c3_sweep(g6, inputs, torch, dev, measured_peaks()[0]) if args.n is None else None
     if rank == 0:
         # what the FP32 pipes sustain for register-sourced instructions (g6x_probe_fp32_peak, include/g6.h), measured live
         ceilings = {name: max(g6.g6x_probe_fp32_peak(0, mode, c) for c in (3, 4, 8))
@@ -456,6 +487,8 @@ def main():
             out["ni_sweep"] = sweep
         if nb_cost is not None:
             out["neighbour_lists"] = nb_cost
+        if c3 is not None:
+            out["c3_sweep"] = c3
         if not args.no_cpu_baseline and world == 1:
             rate, rows, dt, cores = cpu_oracle_rate(x, v, m, eps2, idx, args.cpu_seconds)
             out["cpu_baseline"] = {"value": rate, "unit": "interactions/s", "cores": cores, "kind": "oracle",
