@@ -203,3 +203,22 @@ def test_device_driven_vs_host_driven_vs_oracle_driven(cluster, oracle, n, t_end
     assert sd["ni_hist_log2"].sum() == sd["n_block_steps"]
     assert np.median(np.linalg.norm(xd - ro.x, axis=1)) < 1e-6
     assert np.median(np.linalg.norm(xd - xh, axis=1)) < 1e-7
+
+
+@pytest.mark.parametrize("n", [1, 2, 1025, 2049])
+def test_device_driver_edge_sizes_match_host_driver(cluster, oracle, n):
+    """sizes around the selection kernel's 1024-particle thread blocks, and the degenerate N = 1, 2"""
+    x, v, m, _ = inputs.config("C2", n=max(n, 2))
+    x, v, m = x[:n], v[:n], m[:n] / m[:n].sum()
+    eps2, eta, t_end = 1e-2 ** 2, 0.02, 0.125
+    hd = g6.HermiteDev(0, x, v, m, eps2, eta)
+    hd.evolve(t_end)
+    xd, vd = hd.state(); sd = hd.stats(); hd.close()
+    hh = g6.Hermite(0, x, v, m, eps2, eta)
+    hh.evolve(t_end)
+    xh, vh = hh.state(); sh = hh.stats(); hh.close()
+    assert sd["t"] == t_end == sh["t"]
+    assert abs(sd["n_particle_steps"] - sh["n_particle_steps"]) <= 0.01 * sh["n_particle_steps"] + 1
+    assert np.abs(xd - xh).max() < 1e-7 and np.abs(vd - vh).max() < 1e-6
+    if n == 1:          # a lone particle feels nothing: straight line
+        assert np.allclose(xd, x + v * t_end, rtol=0, atol=1e-15)
