@@ -407,3 +407,24 @@ def test_overwriting_a_j_particle_takes_effect(cluster, oracle):
     got = g6.force_host(0, idx[:50], x[:50], v[:50], eps2, 500)
     ref = oracle.force(idx[:50], x[:50], v[:50], idx, x2, v, m2, eps2)
     check_forces(got, ref, "after overwrite")
+
+
+def test_maximum_capacity(cluster, oracle):
+    """The largest j-store the library holds by default (2^21 addresses): every address in use, the last one included;
+    a 512-block through the sweep kernels and a 7-block through the block-step kernel against the oracle; one address
+    past the end is refused."""
+    n = 1 << 21
+    x, v, m, eps2 = inputs.config("C4", n=n)
+    idx = load_j(x, v, m)
+    g6.g6_set_ti(0, 0.0)
+    E = g6.G6Error
+    with pytest.raises(E) as e: g6.g6_set_j_particle(0, n, 0, 0.0, 0.0, 1.0, None, x[0], x[0], x[0], x[0])
+    assert e.value.code == -3
+    for ni, kernel in ((512, 2), (7, 3)):
+        sel = inputs.active_subset(n, ni, 77 + ni)
+        sel[-1] = n - 1                                   # the last address is an i-particle too
+        got = g6.force_host(0, idx[sel], x[sel], v[sel], eps2, n)
+        assert g6.g6x_get_option(0, "last_kernel") == kernel
+        ref = oracle.force(idx[sel], x[sel], v[sel], idx, x, v, m, eps2)
+        check_forces(got, ref, f"capacity n_i={ni}")
+        check_nn(got["nn_index"], ref, idx, x[sel], x)
