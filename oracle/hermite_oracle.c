@@ -18,6 +18,9 @@
  *       a multiple of 2 dt and 2 dt <= dt_max;
  *   start: dt = eta_start |a| / |adot| rounded down to a power of two, <= dt_max.
  *
+ * orc_hermite_shared: the same with ONE step for all particles (reading 21), pinned by: identical to the block scheme
+ * on a configuration whose particles all ask for the same step (rotating polygon), step counts, energy conservation.
+ *
  * Plain fp64, one block step after the other, the whole system re-predicted every step.
  * Uses orc_force of g6_oracle.c for the forces (same oracle, same pins).  Pinned by
  * tests/test_oracle_pins.py: a circular binary returns to its start after one period, the
@@ -81,9 +84,12 @@ double orc_aarseth_dt(double eta, const double *a1, const double *ad1, const dou
  * Stops at t_end (a multiple of dt_max, where every particle is synchronised) or after
  * max_block_steps block steps if that is > 0 (then the state is NOT synchronised:
  * x, v are returned as predicted to the last block time). */
-int orc_hermite(int n, double (*x)[3], double (*v)[3], const double *m,
-                double eps2, double eta, double eta_start, double dt_max, double t_end,
-                long long max_block_steps, long long *ni_hist_log2, double *stats)
+/* shared != 0: the shared-time-step variant ("shared or block time steps"; reading 21): every
+ * particle is advanced every step with one common step; after the corrector each particle applies the rule above to the
+ * common step and the new common step is the smallest result (likewise at the start). */
+static int hermite_impl(int n, double (*x)[3], double (*v)[3], const double *m,
+                        double eps2, double eta, double eta_start, double dt_max, double t_end,
+                        long long max_block_steps, long long *ni_hist_log2, double *stats, int shared)
 {
     double (*a)[3] = malloc(sizeof(double[3]) * n), (*ad)[3] = malloc(sizeof(double[3]) * n);
     double (*xp)[3] = malloc(sizeof(double[3]) * n), (*vp)[3] = malloc(sizeof(double[3]) * n);
@@ -104,6 +110,7 @@ int orc_hermite(int n, double (*x)[3], double (*v)[3], const double *m,
         dt[p] = pow2_floor(want, dt_max);
         if (dt[p] < dt_min) dt_min = dt[p];
     }
+    if (shared) for (int p = 0; p < n; ++p) dt[p] = dt_min;
 
     long long nblock = 0, npart = 0;
     double inter = 0.0, tnow = 0.0;
@@ -143,6 +150,11 @@ int orc_hermite(int n, double (*x)[3], double (*v)[3], const double *m,
             dt[p] = d;
             if (d < dt_min) dt_min = d;
         }
+        if (shared) {
+            double dcommon = dt[act[0]];
+            for (int k = 1; k < ni; ++k) if (dt[act[k]] < dcommon) dcommon = dt[act[k]];
+            for (int k = 0; k < ni; ++k) dt[act[k]] = dcommon;
+        }
         tnow = tn;
         ++nblock;
         npart += ni;
@@ -162,4 +174,18 @@ int orc_hermite(int n, double (*x)[3], double (*v)[3], const double *m,
     free(a); free(ad); free(xp); free(vp); free(xi); free(vi); free(a1); free(ad1);
     free(pot); free(t); free(dt); free(index); free(act); free(iidx);
     return 0;
+}
+
+int orc_hermite(int n, double (*x)[3], double (*v)[3], const double *m,
+                double eps2, double eta, double eta_start, double dt_max, double t_end,
+                long long max_block_steps, long long *ni_hist_log2, double *stats)
+{
+    return hermite_impl(n, x, v, m, eps2, eta, eta_start, dt_max, t_end, max_block_steps, ni_hist_log2, stats, 0);
+}
+
+int orc_hermite_shared(int n, double (*x)[3], double (*v)[3], const double *m,
+                       double eps2, double eta, double eta_start, double dt_max, double t_end,
+                       long long max_block_steps, long long *ni_hist_log2, double *stats)
+{
+    return hermite_impl(n, x, v, m, eps2, eta, eta_start, dt_max, t_end, max_block_steps, ni_hist_log2, stats, 1);
 }

@@ -139,17 +139,18 @@ class HermiteResult(dict):
     __getattr__ = dict.__getitem__
 
 
-def hermite(x, v, m, eps2, eta, t_end, dt_max=0.125, eta_start=0.01, max_steps=0):
-    """Oracle-driven 4th-order Hermite block-step integration (oracle/hermite_oracle.c).
-    Returns the final synchronised state and step statistics."""
+def hermite(x, v, m, eps2, eta, t_end, dt_max=0.125, eta_start=0.01, max_steps=0, shared=False):
+    """Oracle-driven 4th-order Hermite block-step integration (oracle/hermite_oracle.c); shared=True:
+    one common step for all particles.  Returns the final synchronised state and step statistics."""
     n = len(m)
     x = _f64(x, (n, 3)).copy(); v = _f64(v, (n, 3)).copy(); m = _f64(m, (n,))
     hist = np.zeros(64, np.int64)
     stats = np.zeros(8, np.float64)
     d = C.c_double
     lib = _lib()
-    lib.orc_hermite.restype = C.c_int
-    rc = lib.orc_hermite(C.c_int(n), _p(x, d), _p(v, d), _p(m, d), d(float(eps2)), d(float(eta)),
+    fn = lib.orc_hermite_shared if shared else lib.orc_hermite
+    fn.restype = C.c_int
+    rc = fn(C.c_int(n), _p(x, d), _p(v, d), _p(m, d), d(float(eps2)), d(float(eta)),
                          d(float(eta_start)), d(float(dt_max)), d(float(t_end)),
                          C.c_longlong(int(max_steps)), _p(hist, C.c_longlong), _p(stats, d))
     if rc != 0:

@@ -304,6 +304,39 @@ k_hd_correct(HdState S, HdBlock B, HdCorr C)
     hd_correct_one(S, B, C, k, *B.d_tnext);
 }
 
+// ---- shared-time-step variant ("shared or block time steps"; reading 21) --------------------
+// every particle takes every step with one common step = the smallest of the per-particle wishes
+__global__ void __launch_bounds__(HD_THREADS)
+k_hd_min_dt(HdState S, unsigned long long *bits)
+{
+    __shared__ double smin[HD_THREADS / 32];
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    const double d = hd_block_min(p < S.n ? S.dt[p] : __longlong_as_double(0x7ff0000000000000LL), smin);
+    if (threadIdx.x == 0) atomicMin(bits, (unsigned long long)__double_as_longlong(d));
+}
+
+// the common step to every particle; the block is everybody, predicted to t + h
+__global__ void __launch_bounds__(HD_THREADS)
+k_hd_shared_apply(HdState S, HdBlock B, const unsigned long long *bits)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= S.n) return;
+    const double h = __longlong_as_double((long long)*bits);
+    const double tn = S.t[p] + h;
+    S.dt[p] = h;
+    B.act[p] = p;
+    hd_predict(S, p, tn, B.xi + 3 * (size_t)p, B.vi + 3 * (size_t)p);
+    if (p == 0) {
+        *B.d_ni = S.n;
+        *B.d_tnext = tn;
+        *B.h_tnext = tn;
+        __threadfence_system();
+        *B.h_ni = S.n;
+    }
+}
+
+__global__ void k_hd_set_u64(unsigned long long *p, unsigned long long v) { *p = v; }
+
 __global__ void k_hd_iota(int *act, int n)
 {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;

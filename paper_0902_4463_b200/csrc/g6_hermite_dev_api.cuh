@@ -18,6 +18,8 @@ struct g6hd_system {
     double *h_tnext = nullptr;
     cudaEvent_t ev = nullptr;
     int last_ni = 0;
+    bool shared = false;                                       // one common step for all particles (reading 21)
+    unsigned long long *shared_bits = nullptr;                 // the common step of the next shared step (bits of a double)
     bool pending = false;                                      // the last block's forces are computed, its corrector has not run yet
     long long nblock = 0, npart = 0, hist[64] = {};
     double inter = 0, wall = 0;
@@ -35,7 +37,7 @@ void hd_free(g6hd_system *s)
     cudaFree(s->S.x); cudaFree(s->S.v); cudaFree(s->S.a); cudaFree(s->S.ad); cudaFree(s->S.m); cudaFree(s->S.t); cudaFree(s->S.dt);
     cudaFree(s->B.act); cudaFree(s->B.cand); cudaFree(s->B.xi); cudaFree(s->B.vi); cudaFree(s->B.bmin); cudaFree(s->B.bcnt); cudaFree(s->B.boff); cudaFree(s->B.ticket);
     cudaFree(s->B.d_ni); cudaFree(s->B.d_tnext);
-    cudaFree(s->a1); cudaFree(s->ad1); cudaFree(s->pot); cudaFree(s->dt_min_bits);
+    cudaFree(s->a1); cudaFree(s->ad1); cudaFree(s->pot); cudaFree(s->dt_min_bits); cudaFree(s->shared_bits);
     if (s->h_ni) cudaFreeHost(s->h_ni);
     if (s->h_tnext) cudaFreeHost(s->h_tnext);
     if (s->ev) cudaEventDestroy(s->ev);
@@ -95,7 +97,7 @@ g6hd_system *g6hd_create(int clusterid, int n, const double x[][3], const double
         CK(dalloc(s->S.m, n)); CK(dalloc(s->S.t, n)); CK(dalloc(s->S.dt, n));
         CK(dalloc(s->B.act, n)); CK(dalloc(s->B.cand, (size_t)nb * HD_PER_BLOCK)); CK(dalloc(s->B.xi, n3)); CK(dalloc(s->B.vi, n3));
         CK(dalloc(s->B.bmin, nb)); CK(dalloc(s->B.bcnt, nb)); CK(dalloc(s->B.boff, nb)); CK(dalloc(s->B.ticket, 1)); CK(dalloc(s->B.d_ni, 1)); CK(dalloc(s->B.d_tnext, 1));
-        CK(dalloc(s->a1, n3)); CK(dalloc(s->ad1, n3)); CK(dalloc(s->pot, n)); CK(dalloc(s->dt_min_bits, 1));
+        CK(dalloc(s->a1, n3)); CK(dalloc(s->ad1, n3)); CK(dalloc(s->pot, n)); CK(dalloc(s->dt_min_bits, 1)); CK(dalloc(s->shared_bits, 1));
         CK(cudaHostAlloc((void **)&s->h_ni, sizeof(int), cudaHostAllocMapped));
         CK(cudaHostAlloc((void **)&s->h_tnext, sizeof(double), cudaHostAllocMapped));
         CK(cudaHostGetDevicePointer((void **)&s->B.h_ni, s->h_ni, 0));
@@ -153,7 +155,32 @@ int g6hd_evolve(g6hd_system *sp, double t_end, long long max_block_steps)
     const auto w0 = std::chrono::steady_clock::now();
     const int nb = (s.n + HD_PER_BLOCK - 1) / HD_PER_BLOCK;
     long long done = 0;
-    while (s.t < t_end && (max_block_steps <= 0 || done < max_block_steps)) {
+    while (s.shared && s.t < t_end && (max_block_steps <= 0 || done < max_block_steps)) {
+        // shared steps: corrector of the previous step for everybody, common step = smallest wish, everybody predicted
+        int rcf = hd_finish(c, s);
+        if (rcf) return rcf;
+        const int g = (s.n + HD_THREADS - 1) / HD_THREADS;
+        k_hd_set_u64<<<1, 1, 0, c.stream>>>(s.shared_bits, 0x7ff0000000000000ULL);
+        k_hd_min_dt<<<g, HD_THREADS, 0, c.stream>>>(s.S, s.shared_bits);
+        k_hd_shared_apply<<<g, HD_THREADS, 0, c.stream>>>(s.S, s.B, s.shared_bits);
+        CK(cudaGetLastError());
+        CK(cudaEventRecord(s.ev, c.stream));
+        CK(cudaEventSynchronize(s.ev));
+        const double tn = *(volatile double *)s.h_tnext;
+        if (!(tn > s.t)) return fail(c, G6_ERR_CUDA, "shared step returned t = %g", tn);
+        int rc = hd_force(c, s, s.n, tn);
+        if (rc) return rc;
+        s.pending = true;
+        s.t = tn;
+        s.last_ni = s.n;
+        ++s.nblock; ++done;
+        s.npart += s.n;
+        s.inter += (double)s.n * (double)s.n;
+        int b = 0;
+        while ((1LL << (b + 1)) <= s.n) ++b;
+        s.hist[b] += 1;
+    }
+    while (!s.shared && s.t < t_end && (max_block_steps <= 0 || done < max_block_steps)) {
         if (s.profile) CK(cudaEventRecord(s.pe[0], c.stream));
         k_hd_select<<<nb, HD_THREADS, 0, c.stream>>>(s.S, s.B, hd_corr(c, s), s.pending ? 1 : 0);
         CK(cudaGetLastError());
@@ -199,6 +226,17 @@ int g6hd_evolve(g6hd_system *sp, double t_end, long long max_block_steps)
     }
     CK(cudaStreamSynchronize(c.stream));
     s.wall += std::chrono::duration<double>(std::chrono::steady_clock::now() - w0).count();
+    return G6_OK;
+}
+
+int g6hd_set_shared_steps(g6hd_system *sp, int on)
+{
+    if (!sp) return G6_ERR_ARG;
+    g6hd_system &s = *sp;
+    GET_CLUSTER(s.cl);
+    int rc = hd_finish(c, s);           // (never pending between calls; kept for safety)
+    if (rc) return rc;
+    s.shared = on != 0;
     return G6_OK;
 }
 

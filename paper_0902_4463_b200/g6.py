@@ -26,7 +26,7 @@ SYMBOLS = [
     "g6x_get_nearest", "g6x_set_stream", "g6x_synchronize", "g6x_get_timers", "g6x_set_option",
     "g6x_get_option", "g6x_get_predicted", "g6x_debug_dx", "g6x_probe_fp32_peak", "g6x_probe_read_jstore", "g6x_version",
     "g6h_create", "g6h_destroy", "g6h_evolve", "g6h_get_state", "g6h_get_stats", "g6h_get_force_wall_hist",
-    "g6hd_create", "g6hd_destroy", "g6hd_evolve", "g6hd_get_state", "g6hd_get_stats", "g6hd_get_particles", "g6hd_get_last_block",
+    "g6hd_create", "g6hd_destroy", "g6hd_evolve", "g6hd_get_state", "g6hd_get_stats", "g6hd_get_particles", "g6hd_get_last_block", "g6hd_set_shared_steps",
 ]
 
 ERRORS = {0: "G6_OK", -1: "G6_ERR_NOT_OPEN", -2: "G6_ERR_CLUSTER", -3: "G6_ERR_ADDRESS", -4: "G6_ERR_NI",
@@ -364,6 +364,9 @@ class HermiteDev:
         x = np.empty((self.n, 3)); v = np.empty((self.n, 3))
         _chk(lib().g6hd_get_state(C.c_void_p(self._h), _dp(x), _dp(v)), self.clusterid)
         return x, v
+
+    def set_shared_steps(self, on=True):
+        return _chk(lib().g6hd_set_shared_steps(C.c_void_p(self._h), C.c_int(1 if on else 0)), self.clusterid)
 
     def particles(self):
         """raw Hermite state, each particle at its own time: dict x, v, a, adot [n,3], t, dt [n]"""

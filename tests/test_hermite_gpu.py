@@ -222,3 +222,37 @@ def test_device_driver_edge_sizes_match_host_driver(cluster, oracle, n):
     assert np.abs(xd - xh).max() < 1e-7 and np.abs(vd - vh).max() < 1e-6
     if n == 1:          # a lone particle feels nothing: straight line
         assert np.allclose(xd, x + v * t_end, rtol=0, atol=1e-15)
+
+
+@pytest.mark.parametrize("n,t_end", [(512, 0.0625), (3000, 0.015625)])
+def test_device_shared_time_steps_vs_oracle(cluster, oracle, n, t_end):
+    """shared-time-step variant (reading 21) on the device against the oracle's: every particle takes every
+    step, the same sequence of common steps (FP32 forces may shift a step or two), the same energy behaviour"""
+    x, v, m, _ = inputs.config("C2", n=n)
+    eps2, eta = 1e-3 ** 2, 0.01
+    E0 = _energy(oracle, x, v, m, eps2)
+    ro = oracle.hermite(x, v, m, eps2, eta, t_end, shared=True)
+    dE_o = abs(_energy(oracle, ro.x, ro.v, m, eps2) - E0) / abs(E0)
+    hd = g6.HermiteDev(0, x, v, m, eps2, eta)
+    hd.set_shared_steps(True)
+    hd.evolve(t_end)
+    pt = hd.particles()
+    xd, vd = hd.state(); sd = hd.stats()
+    dE_d = abs(_energy(oracle, xd, vd, m, eps2) - E0) / abs(E0)
+    print(f"shared N={n}: steps device {sd['n_block_steps']} oracle {ro.n_block_steps}, dE/E device {dE_d:.3e} oracle {dE_o:.3e}, dt_min {sd['dt_min']} / {ro.dt_min}")
+    assert sd["t"] == t_end == ro.t
+    assert np.all(pt["t"] == t_end) and len(np.unique(pt["dt"])) <= n        # everybody at the same time
+    assert sd["n_particle_steps"] == n * sd["n_block_steps"]
+    b = int(np.log2(n))
+    assert sd["ni_hist_log2"][b] == sd["n_block_steps"]
+    # the common step is the SMALLEST wish: one particle near a power-of-two boundary moves the whole system, so FP32
+    # forces shift the step sequence more than in the block scheme
+    assert abs(sd["n_block_steps"] - ro.n_block_steps) <= 0.1 * ro.n_block_steps + 2
+    assert sd["dt_min"] in (ro.dt_min, ro.dt_min / 2, ro.dt_min * 2)
+    assert dE_d <= 2 * dE_o + 2e-8
+    assert np.median(np.linalg.norm(xd - ro.x, axis=1)) < 1e-7
+    # back to block steps: the run continues and stays synchronised at multiples of dt_max
+    hd.set_shared_steps(False)
+    hd.evolve(0.125)
+    assert hd.stats()["t"] == 0.125 and hd.stats()["n_particle_steps"] < n * hd.stats()["n_block_steps"]
+    hd.close()

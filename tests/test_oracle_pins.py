@@ -437,3 +437,33 @@ def test_p13_neighbour_lists_brute_force_overflow_and_nearest(oracle):
     Xs = X.copy(); Xs[7] += 0.01
     cnt2, lst2 = oracle.neighbours(idx[7:8], Xs[7:8], [0.5], idx, X, maxlen=64)
     assert 7 not in lst2[0, :cnt2[0]]
+
+
+def test_hermite_oracle_shared_steps(oracle):
+    """Shared-time-step variant (reading 21; "shared or block time steps").
+    (i) A square of equal masses on a circular orbit: the four particles are images of one another under 90-degree
+    rotations, which only permute and negate coordinates, so they ask for bit-identical steps and the shared scheme
+    must reproduce the (pinned) block scheme bit for bit.  (ii) On a cluster every particle takes every step, the
+    common step is never larger than the block scheme's smallest, and the energy is conserved at least as well."""
+    R, mass = 1.0, 0.25
+    x = np.array([[R, 0, 0], [0, R, 0], [-R, 0, 0], [0, -R, 0]], float)
+    a = mass / R ** 2 * 0.25 * sum(1 / np.sin(np.pi * k / 4) for k in range(1, 4))      # polygon closed form (pin P2)
+    vc = np.sqrt(a * R)
+    v = np.array([[0, vc, 0], [-vc, 0, 0], [0, -vc, 0], [vc, 0, 0]], float)
+    m = np.full(4, mass)
+    rb = oracle.hermite(x, v, m, 0.0, 0.01, 0.5)
+    rs = oracle.hermite(x, v, m, 0.0, 0.01, 0.5, shared=True)
+    assert np.array_equal(rb.x, rs.x) and np.array_equal(rb.v, rs.v)
+    assert rb.n_block_steps == rs.n_block_steps and rs.n_particle_steps == 4 * rs.n_block_steps
+    assert np.allclose(np.linalg.norm(rs.x, axis=1), R, rtol=1e-7)                        # still on the circle
+    # (ii)
+    x, v, m, eps2 = inputs.config("C1", n=64)
+    E0 = sum(oracle.energy(x, v, m, eps2))
+    rb = oracle.hermite(x, v, m, eps2, 0.01, 0.125)
+    rs = oracle.hermite(x, v, m, eps2, 0.01, 0.125, shared=True)
+    assert rs.t == 0.125 and rs.n_particle_steps == 64 * rs.n_block_steps
+    assert rs.ni_hist_log2[6] == rs.n_block_steps and rs.ni_hist_log2.sum() == rs.n_block_steps
+    assert rs.dt_min <= rb.dt_min and rs.n_particle_steps > rb.n_particle_steps
+    dEs = abs(sum(oracle.energy(rs.x, rs.v, m, eps2)) - E0) / abs(E0)
+    dEb = abs(sum(oracle.energy(rb.x, rb.v, m, eps2)) - E0) / abs(E0)
+    assert dEs < 1e-7 and dEs <= 2 * dEb + 1e-12, (dEs, dEb)
