@@ -224,3 +224,40 @@ def test_small_blocks_lists_from_the_block_step_kernel(cluster, oracle, n, ni, s
     assert g6.g6x_get_option(0, "last_kernel") == 2
     assert np.array_equal(cnt, cnt2) and np.array_equal(lst, lst2)
     g6.g6x_set_option(0, "small", 32)
+
+
+@pytest.mark.parametrize("n,ni", [(5000, 5), (3000, 16), (40000, 32)])
+def test_production_cycle_with_lists_and_inline_j_updates(cluster, oracle, n, ni):
+    """The Hermite cycle with neighbour lists: g6_set_j_particle for the corrected particles (they ride in the launch of the
+    block-step kernel), then firsthalf with h2 / lasthalf / read_neighbour_list; lists see the UPDATED positions and agree
+    with the sweep kernels' lists for the same call."""
+    from helpers import rel_err
+    x, v, m, _ = inputs.config("C2", n=n)
+    eps2 = 1e-8
+    rng = np.random.default_rng(500 + ni)
+    idx = rng.permutation(n).astype(np.int32)
+    tj, dtj, a0, j0 = inputs.taylor_state(n, 300 + ni, dt_max=2.0**-6)
+    load_j(x, v, m, index=idx, t=tj, acc=a0, jerk=j0)
+    t = 2.0**-8
+    for step in range(3):
+        blk = np.append(np.sort(rng.choice(n - 1, ni - 1, replace=False)), n - 1).astype(int)
+        x[blk] += 1e-3 * rng.standard_normal((ni, 3)); v[blk] += 1e-3 * rng.standard_normal((ni, 3))
+        a0[blk] = rng.standard_normal((ni, 3)); j0[blk] = rng.standard_normal((ni, 3)); tj[blk] = t
+        for p in blk:
+            g6.g6_set_j_particle(0, int(p), int(idx[p]), tj[p], dtj[p], m[p], None, j0[p] / 6, a0[p] / 2, v[p], x[p])
+        t += 2.0**-9
+        g6.g6_set_ti(0, t)
+        xo, vo = oracle.predict(t, tj, x, v, a0, j0)
+        nxt = np.sort(rng.choice(n, ni, replace=False))
+        nxt[0] = blk[0]
+        h2 = radii(x, nxt, 600 + step, lo=0.5, hi=2.5)
+        got, cnt, lst = run(idx[nxt], xo[nxt], vo[nxt], eps2, n, h2, 256)
+        assert g6.g6x_get_option(0, "last_kernel") == 3
+        oc, ol = oracle.neighbours(idx[nxt], xo[nxt], h2, idx, xo, maxlen=n)
+        check_neighbours(cnt, lst, oc, ol, idx, xo[nxt], xo, h2, 256, tol=1e-4)
+        ref = oracle.force(idx[nxt], xo[nxt], vo[nxt], idx, xo, vo, m, eps2)
+        assert rel_err(got["acc"], ref["acc"]).max() <= 1e-5 and rel_err(got["pot"], ref["pot"]).max() <= 1e-6
+        g6.g6x_set_option(0, "kernel", 2)
+        got2, cnt2, lst2 = run(idx[nxt], xo[nxt], vo[nxt], eps2, n, h2, 256)
+        g6.g6x_set_option(0, "kernel", 0)
+        assert np.array_equal(cnt, cnt2) and np.array_equal(lst, lst2)
