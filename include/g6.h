@@ -199,7 +199,9 @@ int g6x_get_timers(int clusterid, double us[8]);
  *             the event records cost ~10 us per force call, a third of a small block step
  *   "variant" 0 = automatic; threads*8 + i_per_thread forces a fast-kernel shape (e.g. 128*8+2)
  *   "small"   largest n_i served by the block-step kernel (one launch: j update + predictor + force +
- *             combine, lanes over j); default 32, at most 64, 0 = off
+ *             combine, lanes over j); at most 64, 0 = off.  Until it is set the library uses its own rule,
+ *             the measured crossover with the three-launch sweep path: 24 below 65536 j-particles, 32 below
+ *             262144, 48 above (g6x_get_option reports 32 then)
  *   "nb_maxlen" neighbours stored per i-particle (1 .. 4096, default G6_NB_MAXLEN = 256; compile-time
  *             in the paper); changing it discards the lists of the last call
  *   "last_kernel" (g6x_get_option only) the force kernel the last call took: 1 checked reference kernel,

@@ -108,6 +108,7 @@ struct Cluster {
 
     // options
     int opt_ds = 1, opt_newton = 1, opt_jsplit = 0, opt_kernel = 0, opt_timers = 0, opt_variant = 0, opt_small = 32, opt_nb_maxlen = 256;
+    bool small_explicit = false;   // option "small" was set by the caller (else the N_j-dependent rule of small_limit)
 };
 
 Cluster g_cl[MAX_CLUSTERS];
@@ -433,10 +434,20 @@ int choose_jsplit(int n_itiles, int ntiles, int slots, int ni, long long s_cap =
 
 // force + combine (steps a-4, a-5) on device-resident i-blocks; all asynchronous
 // small active blocks take the fused block-step kernel unless an experiment switch pins another path
-bool use_block_step(const Cluster &c, int ni, bool nb = false)
+// Largest block the block-step kernel serves.  Its time grows by ~2.0 us per i-particle per 2^20 j, the sweep path's
+// (predictor + sweep kernel + combine: three launches) starts higher and grows slower; measured crossover n_i = 28 at
+// N_j = 32768 and ~56 at N_j = 2^20.  Option "small" set by the caller overrides the rule.
+int small_limit(const Cluster &c, int nj)
+{
+    if (c.small_explicit) return c.opt_small;
+    const int ntiles = (nj + JT - 1) / JT;
+    return ntiles >= 1024 ? 48 : (ntiles >= 256 ? 32 : 24);
+}
+
+bool use_block_step(const Cluster &c, int ni, int nj, bool nb = false)
 {
     // with neighbour lists the kernel's last-CTA merge holds one list per warp in shared memory
-    return (!nb || c.opt_nb_maxlen <= BS_NB_SCRATCH) && ni <= c.opt_small && c.opt_kernel != 1 && c.opt_kernel != 2 && c.opt_jsplit == 0;
+    return (!nb || c.opt_nb_maxlen <= BS_NB_SCRATCH) && ni <= small_limit(c, nj) && c.opt_kernel != 1 && c.opt_kernel != 2 && c.opt_jsplit == 0;
 }
 
 struct HostBlock { const double *xi, *vi; const int *index; };   // host copy of the i-block (small blocks travel in kernel parameters)
@@ -462,7 +473,7 @@ int run_force(Cluster &c, int nj, int ni, const int *d_index, const double *d_xi
     A.ds = c.opt_ds;
 
     // small active blocks: the whole block step in one kernel (g6_block_step.cuh)
-    if (use_block_step(c, ni, nb != nullptr)) {
+    if (use_block_step(c, ni, nj, nb != nullptr)) {
         // a-1: changed j-particles ride in the kernel parameters when they fit and lie inside the j-range
         const int maxi_need = std::max(ni, hb ? c.n_rec : 0);
         bool inline_upd = hb && c.n_rec > 0 && c.n_rec <= BS_MAX_I;
@@ -816,7 +827,7 @@ int g6calc_firsthalf(int clusterid, int nj, int ni, const int index[], const dou
         CK(cudaMemcpyAsync(c.d_h2, c.h_h2, sizeof(double) * ni, cudaMemcpyHostToDevice, c.stream));
         nbr = NbReq{c.d_h2, c.d_nb_cnt, c.d_nb_list};
     }
-    const bool bs = use_block_step(c, ni, want_nb);
+    const bool bs = use_block_step(c, ni, nj, want_nb);
     const bool zc_out = ni <= ZC_MAX_I;
     const RView out = rview(zc_out ? c.hd_res : c.d_res, ni);
     if (bs) {
@@ -1038,6 +1049,7 @@ int g6x_set_option(int clusterid, const char *key, int value)
         (slot == &c.opt_variant && value != 0 && fast_ctas_per_sm(FastVariant{value / 8, value % 8}) < 1))
         return fail(c, G6_ERR_ARG, "bad value %d for option '%s'", value, key);
     *slot = value;
+    if (slot == &c.opt_small) c.small_explicit = true;
     return G6_OK;
 }
 

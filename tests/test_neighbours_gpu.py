@@ -238,6 +238,7 @@ def test_production_cycle_with_lists_and_inline_j_updates(cluster, oracle, n, ni
     idx = rng.permutation(n).astype(np.int32)
     tj, dtj, a0, j0 = inputs.taylor_state(n, 300 + ni, dt_max=2.0**-6)
     load_j(x, v, m, index=idx, t=tj, acc=a0, jerk=j0)
+    g6.g6x_set_option(0, "small", 32)
     t = 2.0**-8
     for step in range(3):
         blk = np.append(np.sort(rng.choice(n - 1, ni - 1, replace=False)), n - 1).astype(int)
