@@ -22,6 +22,20 @@ struct HdState {
     int n;
 };
 
+// what the host waits for, written with ONE 16-byte store to mapped host memory (one PCIe write: never torn)
+struct alignas(16) HdNote {
+    double tnext;
+    int ni;
+    unsigned int seq;
+};
+
+__device__ __forceinline__ void hd_notify(HdNote *h, double tnext, int ni, unsigned int seq)
+{
+    const unsigned long long lo = (unsigned long long)__double_as_longlong(tnext);
+    const unsigned long long hi = (unsigned long long)(unsigned)ni | ((unsigned long long)seq << 32);
+    asm volatile("st.global.v2.u64 [%0], {%1, %2};" ::"l"(h), "l"(lo), "l"(hi) : "memory");
+}
+
 // per-step scratch written by k_hd_select
 struct HdBlock {
     int *act;                   // [n] active addresses, increasing
@@ -31,8 +45,8 @@ struct HdBlock {
     int *bcnt;                  // [nblocks] particles of the block attaining it
     int *boff;                  // [nblocks] where the block's candidates go in the active list, -1: not in this block step
     unsigned int *ticket;
-    int *h_ni;                  // mapped host memory: n_i of the block ...
-    double *h_tnext;            // ... and its time
+    HdNote *h_note;             // mapped host memory: (t_next, n_i, sequence number) of the block, one 16-byte store
+    unsigned int seq;           // sequence number of this launch (the host spins on it instead of waiting for an event)
     int *d_ni;                  // device copy of n_i (read by k_hd_correct)
     double *d_tnext;
 };
@@ -254,10 +268,8 @@ k_hd_select(HdState S, HdBlock B, HdCorr C, int correct_first)
     if (tid == 0) {
         *B.d_ni = ni;
         *B.d_tnext = tnext;
-        *B.h_tnext = tnext;
-        __threadfence_system();
-        *B.h_ni = ni;
         *B.ticket = 0u;
+        hd_notify(B.h_note, tnext, ni, B.seq);
     }
 }
 
@@ -329,9 +341,7 @@ k_hd_shared_apply(HdState S, HdBlock B, const unsigned long long *bits)
     if (p == 0) {
         *B.d_ni = S.n;
         *B.d_tnext = tn;
-        *B.h_tnext = tn;
-        __threadfence_system();
-        *B.h_ni = S.n;
+        hd_notify(B.h_note, tn, S.n, B.seq);
     }
 }
 

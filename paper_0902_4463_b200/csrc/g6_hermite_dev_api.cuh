@@ -5,6 +5,7 @@
 #include "../../include/g6_hermite.h"
 #include "g6_hermite_dev.cuh"
 
+#include <atomic>
 #include <chrono>
 
 struct g6hd_system {
@@ -14,9 +15,8 @@ struct g6hd_system {
     HdBlock B{};
     double *a1 = nullptr, *ad1 = nullptr, *pot = nullptr;      // forces of the current block [n][3], [n]
     unsigned long long *dt_min_bits = nullptr;                // smallest step used so far (bits of a positive double)
-    int *h_ni = nullptr;                                       // mapped host memory
-    double *h_tnext = nullptr;
-    cudaEvent_t ev = nullptr;
+    HdNote *h_note = nullptr;                                  // mapped host memory
+    unsigned int seq = 0;
     int last_ni = 0;
     bool shared = false;                                       // one common step for all particles (reading 21)
     unsigned long long *shared_bits = nullptr;                 // the common step of the next shared step (bits of a double)
@@ -38,9 +38,7 @@ void hd_free(g6hd_system *s)
     cudaFree(s->B.act); cudaFree(s->B.cand); cudaFree(s->B.xi); cudaFree(s->B.vi); cudaFree(s->B.bmin); cudaFree(s->B.bcnt); cudaFree(s->B.boff); cudaFree(s->B.ticket);
     cudaFree(s->B.d_ni); cudaFree(s->B.d_tnext);
     cudaFree(s->a1); cudaFree(s->ad1); cudaFree(s->pot); cudaFree(s->dt_min_bits); cudaFree(s->shared_bits);
-    if (s->h_ni) cudaFreeHost(s->h_ni);
-    if (s->h_tnext) cudaFreeHost(s->h_tnext);
-    if (s->ev) cudaEventDestroy(s->ev);
+    if (s->h_note) cudaFreeHost(s->h_note);
     for (auto &e : s->pe) if (e) cudaEventDestroy(e);
     delete s;
 }
@@ -56,6 +54,28 @@ int hd_force(Cluster &c, g6hd_system &s, int ni, double tn)
                            s.ad1 + 3 * (size_t)i0, s.pot + i0, nullptr, nullptr, nullptr, nullptr, nullptr);
         if (rc) return rc;
     }
+    return G6_OK;
+}
+
+// Wait for the notification of launch `seq` (hd_notify): spin on the mapped record -- a few microseconds sooner than an
+// event wait -- and look at the stream now and then so that a failed launch cannot hang the host.
+int hd_wait_note(Cluster &c, g6hd_system &s, unsigned int seq, int &ni, double &tn)
+{
+    volatile HdNote *h = s.h_note;
+    for (unsigned long long spins = 1;; ++spins) {
+        if (h->seq == seq) break;
+        if ((spins & 0x3fff) == 0) {
+            const cudaError_t q = cudaStreamQuery(c.stream);
+            if (q == cudaSuccess) {
+                if (h->seq == seq) break;
+                return fail(c, G6_ERR_CUDA, "block selection finished without its notification (seq %u)", seq);
+            }
+            if (q != cudaErrorNotReady) return fail(c, G6_ERR_CUDA, "block selection failed: %s", cudaGetErrorString(q));
+        }
+    }
+    std::atomic_thread_fence(std::memory_order_acquire);
+    ni = h->ni;
+    tn = h->tnext;
     return G6_OK;
 }
 
@@ -98,11 +118,9 @@ g6hd_system *g6hd_create(int clusterid, int n, const double x[][3], const double
         CK(dalloc(s->B.act, n)); CK(dalloc(s->B.cand, (size_t)nb * HD_PER_BLOCK)); CK(dalloc(s->B.xi, n3)); CK(dalloc(s->B.vi, n3));
         CK(dalloc(s->B.bmin, nb)); CK(dalloc(s->B.bcnt, nb)); CK(dalloc(s->B.boff, nb)); CK(dalloc(s->B.ticket, 1)); CK(dalloc(s->B.d_ni, 1)); CK(dalloc(s->B.d_tnext, 1));
         CK(dalloc(s->a1, n3)); CK(dalloc(s->ad1, n3)); CK(dalloc(s->pot, n)); CK(dalloc(s->dt_min_bits, 1)); CK(dalloc(s->shared_bits, 1));
-        CK(cudaHostAlloc((void **)&s->h_ni, sizeof(int), cudaHostAllocMapped));
-        CK(cudaHostAlloc((void **)&s->h_tnext, sizeof(double), cudaHostAllocMapped));
-        CK(cudaHostGetDevicePointer((void **)&s->B.h_ni, s->h_ni, 0));
-        CK(cudaHostGetDevicePointer((void **)&s->B.h_tnext, s->h_tnext, 0));
-        CK(cudaEventCreateWithFlags(&s->ev, cudaEventDisableTiming));
+        CK(cudaHostAlloc((void **)&s->h_note, sizeof(HdNote), cudaHostAllocMapped));
+        memset(s->h_note, 0, sizeof(HdNote));
+        CK(cudaHostGetDevicePointer((void **)&s->B.h_note, s->h_note, 0));
         s->profile = env_int("G6_HD_PROFILE", 0) != 0;
         if (s->profile) for (auto &e : s->pe) CK(cudaEventCreate(&e));
         CK(cudaMemsetAsync(s->B.ticket, 0, sizeof(unsigned int), c.stream));
@@ -162,12 +180,14 @@ int g6hd_evolve(g6hd_system *sp, double t_end, long long max_block_steps)
         const int g = (s.n + HD_THREADS - 1) / HD_THREADS;
         k_hd_set_u64<<<1, 1, 0, c.stream>>>(s.shared_bits, 0x7ff0000000000000ULL);
         k_hd_min_dt<<<g, HD_THREADS, 0, c.stream>>>(s.S, s.shared_bits);
+        s.B.seq = ++s.seq;
         k_hd_shared_apply<<<g, HD_THREADS, 0, c.stream>>>(s.S, s.B, s.shared_bits);
         CK(cudaGetLastError());
-        CK(cudaEventRecord(s.ev, c.stream));
-        CK(cudaEventSynchronize(s.ev));
-        const double tn = *(volatile double *)s.h_tnext;
-        if (!(tn > s.t)) return fail(c, G6_ERR_CUDA, "shared step returned t = %g", tn);
+        int nall = 0;
+        double tn = 0;
+        int rcw = hd_wait_note(c, s, s.B.seq, nall, tn);
+        if (rcw) return rcw;
+        if (!(tn > s.t) || nall != s.n) return fail(c, G6_ERR_CUDA, "shared step returned n = %d, t = %g", nall, tn);
         int rc = hd_force(c, s, s.n, tn);
         if (rc) return rc;
         s.pending = true;
@@ -182,15 +202,18 @@ int g6hd_evolve(g6hd_system *sp, double t_end, long long max_block_steps)
     }
     while (!s.shared && s.t < t_end && (max_block_steps <= 0 || done < max_block_steps)) {
         if (s.profile) CK(cudaEventRecord(s.pe[0], c.stream));
+        s.B.seq = ++s.seq;
         k_hd_select<<<nb, HD_THREADS, 0, c.stream>>>(s.S, s.B, hd_corr(c, s), s.pending ? 1 : 0);
         CK(cudaGetLastError());
         c.pred_valid = false;                           // phase 0 rewrote j-store records
         s.pending = false;
         if (s.profile) CK(cudaEventRecord(s.pe[1], c.stream));
-        CK(cudaEventRecord(s.ev, c.stream));
-        CK(cudaEventSynchronize(s.ev));                 // the one host wait of the block step
-        const int ni = *(volatile int *)s.h_ni;
-        const double tn = *(volatile double *)s.h_tnext;
+        int ni = 0;
+        double tn = 0;
+        {
+            int rcw = hd_wait_note(c, s, s.B.seq, ni, tn);      // the one host wait of the block step
+            if (rcw) return rcw;
+        }
         if (ni < 1 || ni > s.n || !(tn > s.t)) return fail(c, G6_ERR_CUDA, "block selection returned ni = %d, t = %g", ni, tn);
         if (ni > HD_GATHER_INLINE) {
             k_hd_gather<<<nb, HD_THREADS, 0, c.stream>>>(s.S, s.B);
