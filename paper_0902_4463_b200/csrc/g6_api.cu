@@ -6,6 +6,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -68,6 +69,8 @@ struct Cluster {
     int i_cap = 0;
     char *h_iblk = nullptr, *hd_iblk = nullptr, *d_iblk = nullptr;
     char *h_res = nullptr, *hd_res = nullptr, *d_res = nullptr;
+    unsigned int *h_done = nullptr, *hd_done = nullptr;   // mapped word: the block-step kernel's "results are on the host" flag
+    unsigned int done_seq = 0, pend_done_seq = 0;          // pend_done_seq != 0: lasthalf spins on h_done instead of an event
     bool res_on_host = false;   // last call's results were written straight into h_res
     bool iblk_on_device = false;   // last host call left a copy of the i-block in d_iblk
 
@@ -185,7 +188,8 @@ cudaError_t mapped_alloc(T *&h, T *&hd, size_t bytes)
 
 void free_i(Cluster &c)
 {
-    hfree(c.h_iblk); hfree(c.h_res);
+    hfree(c.h_iblk); hfree(c.h_res); hfree(c.h_done);
+    c.hd_done = nullptr;
     dfree(c.d_iblk); dfree(c.d_res);
     c.hd_iblk = c.hd_res = nullptr;
     c.i_cap = 0;
@@ -199,6 +203,9 @@ int ensure_i(Cluster &c, int ni)
     size_t n = std::max(ni, 4096);
     CK(mapped_alloc(c.h_iblk, c.hd_iblk, iblk_bytes(n)));
     CK(mapped_alloc(c.h_res, c.hd_res, res_bytes(n)));
+    CK(mapped_alloc(c.h_done, c.hd_done, sizeof(unsigned int)));
+    *c.h_done = 0;
+    c.done_seq = c.pend_done_seq = 0;
     CK(cudaMalloc((void **)&c.d_iblk, iblk_bytes(n)));
     CK(cudaMalloc((void **)&c.d_res, res_bytes(n)));
     c.i_cap = (int)n;
@@ -458,6 +465,7 @@ int run_force(Cluster &c, int nj, int ni, const int *d_index, const double *d_xi
               double eps2, double *d_acc, double *d_jerk, double *d_pot, int *d_nn_index, double *d_nn_r2,
               cudaEvent_t ev_pred_done, cudaEvent_t ev_force_done, const HostBlock *hb, const NbReq *nb = nullptr)
 {
+    c.pend_done_seq = 0;
     ForceArgs A{};
     A.pred = c.pred;
     A.jraw = c.js.raw;
@@ -505,6 +513,12 @@ int run_force(Cluster &c, int nj, int ni, const int *d_index, const double *d_xi
         B.P.stride_i = G;
         B.counter = c.d_counter;
         B.acc = d_acc; B.jerk = d_jerk; B.pot = d_pot; B.nn_index = d_nn_index; B.nn_r2 = d_nn_r2;
+        if (hb && c.hd_done) {          // host call, results through mapped memory (n_i <= ZC_MAX_I always holds here)
+            if (++c.done_seq == 0) ++c.done_seq;
+            B.done_flag = c.hd_done;
+            B.done_seq = c.done_seq;
+            c.pend_done_seq = c.done_seq;
+        }
         if (nb) {
             rc = ensure_nb_warp(c, (size_t)G * (BS_THREADS / 32) * ni);
             if (rc) return rc;
@@ -888,7 +902,24 @@ int g6calc_lasthalf2(int clusterid, int nj, int ni, const int index[], const dou
         return fail(c, G6_ERR_ARG, "lasthalf (nj=%d, ni=%d) does not match firsthalf (nj=%d, ni=%d)", nj, ni, c.pend_nj, c.pend_ni);
     if (!acc || !jerk || !pot) return fail(c, G6_ERR_ARG, "NULL result array");
     c.pending = false;
-    CK(cudaEventSynchronize(c.ev[5]));
+    if (c.pend_done_seq) {
+        // the block-step kernel flags its results in mapped memory: spin on the word (sooner than an event wait), with a
+        // look at the stream now and then so that a failed launch cannot hang the caller
+        volatile unsigned int *flag = c.h_done;
+        for (unsigned long long spins = 1; *flag != c.pend_done_seq; ++spins) {
+            if ((spins & 0x3fff) == 0) {
+                const cudaError_t q = cudaStreamQuery(c.stream);
+                if (q == cudaSuccess) {
+                    if (*flag == c.pend_done_seq) break;
+                    return fail(c, G6_ERR_CUDA, "force call finished without flagging its results");
+                }
+                if (q != cudaErrorNotReady) return fail(c, G6_ERR_CUDA, "force call failed: %s", cudaGetErrorString(q));
+            }
+        }
+        std::atomic_thread_fence(std::memory_order_acquire);
+    } else {
+        CK(cudaEventSynchronize(c.ev[5]));
+    }
     const RView r = rview(c.h_res, ni);
     memcpy(acc, r.acc, sizeof(double) * 3 * ni);
     memcpy(jerk, r.jerk, sizeof(double) * 3 * ni);

@@ -66,6 +66,8 @@ struct BsArgs {
     double *acc, *jerk, *pot;   // results (device or mapped host memory)
     int *nn_index;
     double *nn_r2;
+    unsigned int *done_flag;    // not NULL: mapped host word that receives done_seq after the results are written
+    unsigned int done_seq;
     // neighbour lists (reading 20); h2 == nullptr: none.  Every warp of the grid keeps its own
     // list per i-particle (it meets its tiles in increasing address order); the last CTA merges them by address.
     const double *h2;           // [ni] neighbour-sphere radius squared
@@ -511,6 +513,16 @@ __device__ __forceinline__ void block_step_body(const BsArgs &A0, const BsInline
         }
     }
     if (tid == 0) *A.counter = 0u;
+    // results that went straight to mapped host memory: tell the host they are complete (it spins on this word instead of
+    // waiting for an event, a few microseconds sooner); the barrier orders the other warps' result stores before the
+    // system-scope fence of this thread
+    if (A.done_flag) {
+        __syncthreads();
+        if (tid == 0) {
+            __threadfence_system();
+            *reinterpret_cast<volatile unsigned int *>(A.done_flag) = A.done_seq;
+        }
+    }
 }
 
 template <int MAXI, bool NEWTON>
