@@ -7,11 +7,11 @@
 #include <cmath>
 #include <cstring>
 #include <new>
-#include <queue>
 #include <utility>
 #include <vector>
 
 namespace {
+constexpr int LEVELS = 1100;             // dt = 2^-k, k up to the smallest normal double
 struct V3 { double c[3]; };
 inline double norm(const V3 &a) { return std::sqrt(a.c[0] * a.c[0] + a.c[1] * a.c[1] + a.c[2] * a.c[2]); }
 using Clock = std::chrono::steady_clock;
@@ -23,8 +23,11 @@ struct g6h_system {
     double eps2 = 0, eta = 0, dt_max = 0, t = 0, dt_min = 0;
     std::vector<V3> x, v, a, ad;     // state at each particle's own time
     std::vector<double> m, tp, dt;
-    // (next time, particle): the block is everything sharing the smallest next time
-    std::priority_queue<std::pair<double, int>, std::vector<std::pair<double, int>>, std::greater<>> heap;
+    // Block scheduling in O(1) per particle step.  Steps are dt_max halved k times and a particle's time is always a
+    // multiple of its step, so ALL particles of level k (dt = dt_max 2^-k) are due at every multiple of that step: the next
+    // block time is t + (smallest step in use), and the block is the union of the levels whose step divides it.
+    std::vector<int> lev[LEVELS];        // members of every level
+    std::vector<int> pos, lvl;           // position in its level's list, level of every particle
     // per-block scratch
     std::vector<int> act;
     std::vector<V3> xi, vi, a1, ad1;
@@ -69,6 +72,35 @@ int block_force(g6h_system &s, double tn)
     return rc;
 }
 
+// k of dt = dt_max 2^-k (every step is dt_max halved k times)
+inline int level_of(const g6h_system &s, double dt)
+{
+    int e;
+    std::frexp(s.dt_max / dt, &e);       // the ratio is 2^k = 0.5 * 2^(k+1), exactly
+    return e - 1;
+}
+inline double level_step(const g6h_system &s, int k) { return std::ldexp(s.dt_max, -k); }
+
+void level_insert(g6h_system &s, int p, double dt)
+{
+    const int k = level_of(s, dt);
+    s.lvl[p] = k;
+    s.pos[p] = (int)s.lev[k].size();
+    s.lev[k].push_back(p);
+}
+
+void level_move(g6h_system &s, int p, double dt)
+{
+    const int k = level_of(s, dt);
+    if (k == s.lvl[p]) return;
+    std::vector<int> &old = s.lev[s.lvl[p]];
+    const int last = old.back();
+    old[s.pos[p]] = last;                // swap-remove
+    s.pos[last] = s.pos[p];
+    old.pop_back();
+    level_insert(s, p, dt);
+}
+
 double pow2_floor(double want, double cap)
 {
     double d = cap;
@@ -90,6 +122,7 @@ g6h_system *g6h_create(int clusterid, int n, const double x[][3], const double v
         s->cl = clusterid; s->n = n; s->eps2 = eps2; s->eta = eta; s->dt_max = dt_max; s->dt_min = dt_max;
         s->x.resize(n); s->v.resize(n); s->a.assign(n, V3{{0, 0, 0}}); s->ad.assign(n, V3{{0, 0, 0}});
         s->m.assign(m, m + n); s->tp.assign(n, 0.0); s->dt.assign(n, dt_max);
+        s->pos.assign(n, 0); s->lvl.assign(n, 0);
         s->act.resize(n); s->xi.resize(n); s->vi.resize(n); s->a1.resize(n); s->ad1.resize(n); s->pot.resize(n);
     } catch (const std::bad_alloc &) { delete s; return nullptr; }
     std::memcpy(s->x.data(), x, sizeof(V3) * n);
@@ -106,7 +139,8 @@ g6h_system *g6h_create(int clusterid, int n, const double x[][3], const double v
         const double na = norm(s->a[p]), nad = norm(s->ad[p]);
         s->dt[p] = pow2_floor(nad > 0 ? eta_start * na / nad : dt_max, dt_max);
         if (s->dt[p] < s->dt_min) s->dt_min = s->dt[p];
-        s->heap.emplace(s->dt[p], p);
+        if (level_of(*s, s->dt[p]) < 0 || level_of(*s, s->dt[p]) >= LEVELS) { delete s; return nullptr; }
+        level_insert(*s, p, s->dt[p]);
     }
     for (int p = 0; rc == 0 && p < n; ++p) rc = send_j(*s, p);
     if (rc != 0) { delete s; return nullptr; }
@@ -124,9 +158,12 @@ int g6h_evolve(g6h_system *sp, double t_end, long long max_block_steps)
     long long done = 0;
     int rc = 0;
     while (s.t < t_end && (max_block_steps <= 0 || done < max_block_steps)) {
-        const double tn = s.heap.top().first;
+        int kmax = LEVELS - 1;
+        while (kmax > 0 && s.lev[kmax].empty()) --kmax;                 // smallest step in use
+        const double tn = s.t + level_step(s, kmax);
         s.act.clear();
-        while (!s.heap.empty() && s.heap.top().first == tn) { s.act.push_back(s.heap.top().second); s.heap.pop(); }
+        for (int k = kmax; k >= 0 && std::fmod(tn, level_step(s, k)) == 0.0; --k)
+            s.act.insert(s.act.end(), s.lev[k].begin(), s.lev[k].end());
         const int ni = (int)s.act.size();
         for (int k = 0; k < ni; ++k) predict_one(s, s.act[k], tn, s.xi[k], s.vi[k]);
         const auto f0 = Clock::now();
@@ -160,7 +197,7 @@ int g6h_evolve(g6h_system *sp, double t_end, long long max_block_steps)
             }
             s.dt[p] = d;
             if (d < s.dt_min) s.dt_min = d;
-            s.heap.emplace(tn + d, p);
+            level_move(s, p, d);
             rc = send_j(s, p);
             if (rc) break;
         }
