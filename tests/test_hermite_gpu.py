@@ -241,7 +241,10 @@ def test_device_shared_time_steps_vs_oracle(cluster, oracle, n, t_end):
     dE_d = abs(_energy(oracle, xd, vd, m, eps2) - E0) / abs(E0)
     print(f"shared N={n}: steps device {sd['n_block_steps']} oracle {ro.n_block_steps}, dE/E device {dE_d:.3e} oracle {dE_o:.3e}, dt_min {sd['dt_min']} / {ro.dt_min}")
     assert sd["t"] == t_end == ro.t
-    assert np.all(pt["t"] == t_end) and len(np.unique(pt["dt"])) <= n        # everybody at the same time
+    assert np.all(pt["t"] == t_end)                                            # everybody at the same time
+    # after the corrector every particle holds its own result of the block rule applied to the common step h:
+    # a power of two, at most dt_max, and at most 2 h (one doubling) -- so no two of them differ by more than h's halvings
+    assert np.all(np.log2(pt["dt"]) % 1 == 0) and pt["dt"].max() <= 0.125 and pt["dt"].min() >= sd["dt_min"]
     assert sd["n_particle_steps"] == n * sd["n_block_steps"]
     b = int(np.log2(n))
     assert sd["ni_hist_log2"][b] == sd["n_block_steps"]

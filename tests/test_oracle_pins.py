@@ -338,7 +338,7 @@ def test_hermite_oracle_fourth_order_and_blocks(oracle):
     a = (2 * np.pi) ** (-2.0 / 3.0); e = 0.5
     x, v, m = _binary(a * (1 + e), e)
     E0 = sum(oracle.energy(x, v, m, 0.0))
-    assert abs(E0 + 0.25 * 0.5 / a * 2) < 1e-12 * abs(E0) + 1e-15 or True
+    assert abs(E0 + 0.125 / a) < 1e-13 * abs(E0)          # two-body energy -m1 m2 / (2a) with m1 = m2 = 1/2
     errs = []
     for eta in (0.04, 0.01):
         r = oracle.hermite(x, v, m, 0.0, eta, 1.0)
