@@ -52,8 +52,9 @@ extern "C" {
 
 /* ---- GRAPE-6 calling sequence ------------------------------------- */
 
-/* Acquire device `G6_DEVICE` (env, default 0), a stream, pinned staging and the j-particle
- * store.  Capacity = env G6_NJMAX (default 2^21 addresses), fixed until g6_close. */
+/* Acquire device `G6_DEVICE` (env, default 0), a stream and pinned staging.  The j-particle store holds at most
+ * env G6_NJMAX addresses (default 2^21; g6_getnjmax) and its device memory is GROWN ON DEMAND: it starts at env
+ * G6_NJINIT addresses (default 16384, 1.9 MB) and doubles whenever a higher address is set (76 + 40 B per address). */
 int g6_open(int clusterid);
 
 /* Wait for outstanding work and free everything the cluster owns. */
@@ -85,6 +86,40 @@ int g6_set_j_particle(int clusterid, int address, int index, double tj, double d
 
 /* Time to which the j-particles are predicted by the next force call (Eq. 1-2, dt = ti - tj). */
 int g6_set_ti(int clusterid, double ti);
+
+/* ---- the rest of the GRAPE-6 calling sequence ----------------------
+ * "Sapporo ... emulate[s the] GRAPE6 interface as closely as possible (with the exception of some rarely used
+ * functions)" (PAPER.md:196; :9 "simple relinking", :126).  The paper prints none of these calls; names, argument
+ * order and meaning are RECALLED from the GRAPE-6 user library and UNVERIFIED (its header is not available to this
+ * build), like DESIGN.md reading 13.  Fortran-callable aliases of the whole sequence are in g6_fortran.h. */
+
+/* GRAPE-6 stores times and positions in fixed point; these set the binary scales (2^tunit, 2^xunit) of that format.
+ * This library keeps positions in fp64 / double-single, so the values are recorded (g6x_get_units)
+ * and have no effect.  Global, like the originals.  Always return 0. */
+int g6_set_tunit(int newtunit);
+int g6_set_xunit(int newxunit);
+
+/* Forget every j-particle and any unfinished force call of the cluster: as after g6_open, allocations kept. */
+int g6_reset(int clusterid);
+/* GRAPE-6 resets its force-output FPGA here; nothing to do on a GPU.  Checks the cluster, returns 0. */
+int g6_reset_fofpga(int clusterid);
+
+/* The j-particles set by g6_set_j_particle are buffered on the host and sent at the next force call.
+ * initialize: size that buffer for buf_size particles in advance (it also grows by itself).
+ * flush: send the buffered particles to the device now (asynchronous). */
+int g6_initialize_jp_buffer(int clusterid, int buf_size);
+int g6_flush_jp_buffer(int clusterid);
+
+/* Largest number of j addresses the cluster can hold (env G6_NJMAX); the largest ni per call is g6_npipes().
+ * Returns the POSITIVE count or a negative error. */
+int g6_getnjmax(int clusterid);
+
+/* Read j-memory slot `address` back (0 <= address < highest address set + 1): the inverse of g6_set_j_particle.
+ * Returns the values AS STORED: x and tj exactly (fp64), mass, v, acc_by2, jerk_by6 rounded to binary32 ("Only the
+ * position is stored in DP, whereas the rest of the terms are stored in SP").  Any output pointer may
+ * be NULL.  Buffered particles are flushed first; waits for the device. */
+int g6_get_j_particle(int clusterid, int address, int *index, double *tj, double *mass, double jerk_by6[3],
+                      double acc_by2[3], double v[3], double x[3]);
 
 /* Start a force calculation on ni i-particles against j addresses [0, nj).
  *   index[ni]          ids of the i-particles (for self-exclusion)
@@ -149,6 +184,14 @@ int g6x_set_j_particles(int clusterid, int addr0, int n, const int index[], cons
                         const double mass[], const double jerk[][3], const double acc[][3],
                         const double v[][3], const double x[][3]);
 
+/* Bulk read-back, HOST arrays: addresses addr0 .. addr0+n-1 as stored (see g6_get_j_particle); acc and jerk PHYSICAL
+ * (2 x and 6 x the stored binary32 values, exact).  Any output pointer may be NULL. */
+int g6x_get_j_particles(int clusterid, int addr0, int n, int index[], double tj[], double mass[], double jerk[][3],
+                        double acc[][3], double v[][3], double x[][3]);
+
+/* The values last given to g6_set_tunit / g6_set_xunit (0 until set). */
+int g6x_get_units(int *tunit, int *xunit);
+
 /* Bulk loader, DEVICE arrays (fp64, same shapes).  Asynchronous on the library's stream. */
 int g6x_set_j_particles_dev(int clusterid, int addr0, int n, const int *d_index, const double *d_tj,
                             const double *d_mass, const double *d_jerk, const double *d_acc,
@@ -191,13 +234,15 @@ int g6x_synchronize(int clusterid);
 int g6x_get_timers(int clusterid, double us[8]);
 
 /* Variant switches (for experiments and tests).  Keys:
- *   "ds"      1 (default) double-single positions; 0 = pure FP32 positions (lo words zeroed)
+ *   "ds"      1 (default) double-single positions; 0 = pure FP32 positions (lo words dropped; the sweep kernel then
+ *             forms each separation with 1 packed add instead of Eq. 3's 3: what "DS costs <~ 20 %", is measured against)
  *   "newton"  1 = one Newton step after rsqrt.approx, 0 = none
  *   "jsplit"  0 = automatic; S > 0 forces S j-splits
  *   "kernel"  0 = automatic; 1 = checked reference kernel everywhere; 2 = fast kernel
  *   "timers"  1 = record CUDA events per phase for g6x_get_timers; 0 (default, or env G6_TIMERS) = none:
  *             the event records cost ~10 us per force call, a third of a small block step
- *   "variant" 0 = automatic; threads*8 + i_per_thread forces a fast-kernel shape (e.g. 128*8+2)
+ *   "variant" 0 = automatic; threads*8 + i_per_thread forces a fast-kernel shape: one of 128*8+2, 128*8+1, 64*8+1,
+ *             32*8+1, 256*8+1 (the automatic ones), 128*8+4, 64*8+2; anything else is G6_ERR_ARG
  *   "small"   largest n_i served by the block-step kernel (one launch: j update + predictor + force +
  *             combine, lanes over j); at most 64, 0 = off.  Until it is set the library uses its own rule,
  *             the measured crossover with the three-launch sweep path: 24 below 65536 j-particles, 32 below
@@ -214,10 +259,6 @@ int g6x_get_option(int clusterid, const char *key, int *value);
  * from the device as fp64: xp = hi + lo, vp.  Runs the predictor if needed.  For parity tests. */
 int g6x_get_predicted(int clusterid, int addr0, int n, double xp[][3], double vp[][3]);
 
-/* Debug: the kernel's own Eq.-3 separation dx[k][3] (binary32) for pairs (i-slot ipipe[k] of
- * the last host force call, j address jaddr[k]).  For the bit-exactness pin of DESIGN.md. */
-int g6x_debug_dx(int clusterid, int n, const int ipipe[], const int jaddr[], float dx[][3]);
-
 /* ---- multi-GPU j-split ("n/Q j-particles per GPU", the same i-particles on every GPU) ----
  * Each process (one per GPU) loads its slice of the j-particles -- increasing address ranges by rank --
  * and calls g6x_calc_dev on the SAME i-block; the partial acc/jerk/pot are then SUMMED over the
@@ -232,20 +273,6 @@ int g6x_debug_dx(int clusterid, int n, const int ipipe[], const int jaddr[], flo
 int g6x_jsplit_pack_dev(int clusterid, int ni, int rank, const double *d_nn_r2, const int *d_nn_index, long long *d_key);
 int g6x_jsplit_select_dev(int clusterid, int ni, int rank, const long long *d_key_min, const int *d_nn_index, double *d_index_f64);
 int g6x_jsplit_unpack_dev(int clusterid, int ni, const long long *d_key_min, const double *d_index_sum, int *d_nn_index, double *d_nn_r2);
-
-/* Measurement aid (not part of the path): FP32 lane-instructions per second (an FMA counts once) that
- * this device sustains for register-sourced instructions in independent chains, `ctas_per_sm` CTAs of
- * 128 threads per SM (1..16).  mode 0: scalar FFMA; 1: packed FFMA2 with two loop-constant operands;
- * 2: FADD2 / FMUL2 / FFMA2 in turn (the instruction kinds of the pair kernel); 3: FFMA2 with three
- * distinct changing sources.  bench.py reports the force kernel against the nominal
- * SMs x 128 lanes x clock AND against this measured issue ceiling. */
-int g6x_probe_fp32_peak(int clusterid, int mode, int ctas_per_sm, double *lane_instr_per_s);
-
-/* Measurement aid (not part of the path): enqueue, on the cluster's stream, a kernel that does nothing but
- * READ the raw j-store of addresses [0, nj) once (76 B per particle).  Timed by the caller with events on
- * that stream, it is the floor for one block step at small n_i, which must make the same pass
- * (bench.py `ni_sweep[].bare_read_us`). */
-int g6x_probe_read_jstore(int clusterid, int nj);
 
 /* Library build information: a static string (arch, variant flags). */
 const char *g6x_version(void);

@@ -39,5 +39,40 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return OUT
 
 
+# ---- the parity-test hook (csrc/debug/g6_debug_dx.cu): the production kernels with their DBG template flag, as a
+# separate small library so that libg6b200.so carries no debug entry point
+DBG_SRC = os.path.join(CSRC, "debug", "g6_debug_dx.cu")
+DBG_OUT = os.path.join(HERE, "libg6b200_dbg.so")
+
+
+# ---- bench.py's measurement aids (csrc/bench/g6_bench_probe.cu): instruction-rate and read-pass probes, their own library
+PROBE_SRC = os.path.join(CSRC, "bench", "g6_bench_probe.cu")
+PROBE_OUT = os.path.join(HERE, "libg6b200_probe.so")
+
+
+def _build_side(src: str, out: str, force: bool) -> str:
+    stale = force or not os.path.exists(out) or any(os.path.getmtime(d) > os.path.getmtime(out) for d in deps() + [src])
+    if stale:
+        r = subprocess.run([NVCC] + FLAGS + [src, "-o", out + ".tmp"], capture_output=True, text=True)
+        if r.returncode != 0:
+            sys.stderr.write(r.stdout + r.stderr)
+            raise RuntimeError("nvcc failed building " + os.path.basename(out))
+        os.replace(out + ".tmp", out)
+    return out
+
+
+def build_debug(force: bool = False) -> str:
+    return _build_side(DBG_SRC, DBG_OUT, force)
+
+
+def build_probe(force: bool = False) -> str:
+    return _build_side(PROBE_SRC, PROBE_OUT, force)
+
+
+def build_all(force: bool = False, verbose: bool = False):
+    return [build(force, verbose), build_debug(force), build_probe(force)]
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    for path in build_all(force="--force" in sys.argv, verbose="--verbose" in sys.argv):
+        print(path)

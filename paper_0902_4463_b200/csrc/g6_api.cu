@@ -20,7 +20,6 @@
 #include "g6_force_ref.cuh"
 #include "g6_force_fast.cuh"
 #include "g6_block_step.cuh"
-#include "g6_probe.cuh"
 
 using namespace g6;
 
@@ -41,7 +40,8 @@ struct Cluster {
     char err[512] = "no error";
 
     // j store
-    int capacity = 0;        // addresses
+    int capacity = 0;        // largest number of addresses this cluster may hold (env G6_NJMAX)
+    int alloc_cap = 0;       // addresses the device arrays hold now (grown on demand up to `capacity`)
     int n_stored = 0;        // highest address set + 1
     JStore js{};
     unsigned int *d_counter = nullptr;   // arrival ticket of the block-step kernel
@@ -331,6 +331,38 @@ int ensure_rec(Cluster &c, int n)
     return G6_OK;
 }
 
+// j-store, predicted tiles and per-tile index ranges for `need` addresses: grown on demand (doubling) up to c.capacity,
+// so a small system does not pay for the largest one (SURVEY.md 8(b) "grown on demand").  Old contents are kept.
+int ensure_capacity(Cluster &c, long long need)
+{
+    if (need <= c.alloc_cap) return G6_OK;
+    if (need > c.capacity) return fail(c, G6_ERR_ADDRESS, "%lld addresses asked for, capacity is %d (env G6_NJMAX)", need, c.capacity);
+    long long cap = std::max<long long>(need, std::min<long long>(2LL * c.alloc_cap, c.capacity));
+    cap = std::min<long long>(((cap + JT - 1) / JT) * JT, c.capacity);
+    const size_t tiles = (size_t)(cap / JT), old_tiles = (size_t)(c.alloc_cap / JT);
+    char *raw = nullptr;
+    float *pred = nullptr;
+    int *imin = nullptr, *imax = nullptr;
+    int rc = [&]() -> int {
+        CK(dalloc(raw, tiles * RAW_TILE_BYTES));
+        CK(dalloc(pred, tiles * (size_t)TILE_FLOATS));
+        CK(dalloc(imin, tiles)); CK(dalloc(imax, tiles));
+        if (old_tiles) CK(cudaMemcpyAsync(raw, c.js.raw, old_tiles * RAW_TILE_BYTES, cudaMemcpyDeviceToDevice, c.stream));
+        CK(cudaMemsetAsync(raw + old_tiles * RAW_TILE_BYTES, 0, (tiles - old_tiles) * RAW_TILE_BYTES, c.stream));
+        CK(cudaStreamSynchronize(c.stream));       // nothing may still read the old arrays
+        return G6_OK;
+    }();
+    if (rc == G6_OK) {
+        try { c.slot_of_addr.resize((size_t)cap, -1); } catch (const std::bad_alloc &) { rc = fail(c, G6_ERR_NOMEM, "host allocation failed"); }
+    }
+    if (rc != G6_OK) { dfree(raw); dfree(pred); dfree(imin); dfree(imax); return rc; }
+    dfree(c.js.raw); dfree(c.pred); dfree(c.tile_imin); dfree(c.tile_imax);
+    c.js.raw = raw; c.pred = pred; c.tile_imin = imin; c.tile_imax = imax;
+    c.alloc_cap = (int)cap;
+    c.pred_valid = false;
+    return G6_OK;
+}
+
 void release(Cluster &c)
 {
     if (c.stream) cudaStreamSynchronize(c.stream);
@@ -556,7 +588,7 @@ int run_force(Cluster &c, int nj, int ni, const int *d_index, const double *d_xi
     // kernel choice: the fast kernel needs a normal FP32 eps2 > 0 (its unchecked tiles rely on s2 > 0)
     // (the kernel works on eps2 / 3, which must stay a normal float too)
     const bool fast_ok = A.eps2 >= 4.0f * std::numeric_limits<float>::min() && std::isfinite(A.eps2);
-    const bool use_fast = (c.opt_kernel == 2 || c.opt_kernel == 0) && fast_ok && fast_available();
+    const bool use_fast = (c.opt_kernel == 2 || c.opt_kernel == 0) && fast_ok;
 
     FastVariant fv = fast_pick(ni, c.n_sm, c.opt_variant);
     if (nb && !fast_has_nb(fv)) fv = fast_pick(ni, c.n_sm, 0);     // lists exist for the automatic shapes only
@@ -665,16 +697,11 @@ int g6_open(int clusterid)
     c.n_sm = prop.multiProcessorCount;
     c.capacity = std::max(JT, env_int("G6_NJMAX", 1 << 21));
     c.capacity = ((c.capacity + JT - 1) / JT) * JT;
-    const size_t n = c.capacity;
     int rc = [&]() -> int {
         CK(cudaStreamCreateWithFlags(&c.own_stream, cudaStreamNonBlocking));
         c.stream = c.own_stream;
-        CK(dalloc(c.js.raw, n / JT * RAW_TILE_BYTES));
-        CK(cudaMemsetAsync(c.js.raw, 0, n / JT * RAW_TILE_BYTES, c.stream));
-        CK(dalloc(c.d_counter, 2));     // [0] ticket of the block-step kernel, [1] sink of the read probe
-        CK(cudaMemsetAsync(c.d_counter, 0, 2 * sizeof(unsigned int), c.stream));
-        CK(dalloc(c.pred, n * NF));
-        CK(dalloc(c.tile_imin, n / JT)); CK(dalloc(c.tile_imax, n / JT));
+        CK(dalloc(c.d_counter, 1));     // arrival ticket of the block-step kernel
+        CK(cudaMemsetAsync(c.d_counter, 0, sizeof(unsigned int), c.stream));
         for (auto &ev : c.ev) CK(cudaEventCreate(&ev));
         for (auto &ev : c.ev_rec) CK(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
         int r = fast_kernel_init();
@@ -682,13 +709,9 @@ int g6_open(int clusterid)
         if (r) return fail(c, G6_ERR_CUDA, "kernel attribute setup failed: %s", cudaGetErrorString((cudaError_t)r));
         return G6_OK;
     }();
+    // the j-store starts at env G6_NJINIT addresses (default 16384 = 1.9 MB of device memory) and doubles on demand
+    if (rc == G6_OK) rc = ensure_capacity(c, std::min(c.capacity, std::max(JT, env_int("G6_NJINIT", 16384))));
     if (rc != G6_OK) { release(c); return rc; }
-    try {
-        c.slot_of_addr.assign(n, -1);
-    } catch (const std::bad_alloc &) {
-        release(c);
-        return fail(c, G6_ERR_NOMEM, "host allocation failed");
-    }
     c.open = true;
     c.opt_newton = env_int("G6_NEWTON", 1) ? 1 : 0;
     c.opt_kernel = env_int("G6_KERNEL", 0);
@@ -713,6 +736,10 @@ int g6_set_j_particle(int clusterid, int address, int index, double tj, double d
     if (address < 0 || address >= c.capacity)
         return fail(c, G6_ERR_ADDRESS, "address %d outside [0, capacity = %d)", address, c.capacity);
     if (!jerk_by6 || !acc_by2 || !v || !x) return fail(c, G6_ERR_ARG, "NULL array in g6_set_j_particle");
+    if (address >= c.alloc_cap) {
+        int rc = ensure_capacity(c, (long long)address + 1);
+        if (rc) return rc;
+    }
     int slot = c.slot_of_addr[address];
     if (slot < 0) {
         int rc = ensure_rec(c, c.n_rec + 1);
@@ -744,7 +771,9 @@ int g6x_set_j_particles_dev(int clusterid, int addr0, int n, const int *d_index,
     if (addr0 < 0 || (long long)addr0 + n > c.capacity)
         return fail(c, G6_ERR_ADDRESS, "addresses [%d, %lld) outside capacity %d", addr0, (long long)addr0 + n, c.capacity);
     if (!d_index || !d_tj || !d_mass || !d_jerk || !d_acc || !d_v || !d_x) return fail(c, G6_ERR_ARG, "NULL device array");
-    int rc = flush_j(c);   // keep program order with earlier g6_set_j_particle calls
+    int rc = ensure_capacity(c, (long long)addr0 + n);
+    if (rc) return rc;
+    rc = flush_j(c);   // keep program order with earlier g6_set_j_particle calls
     if (rc) return rc;
     k_store_from_f64<<<(n + 255) / 256, 256, 0, c.stream>>>(c.js, addr0, n, d_index, d_tj, d_mass, d_jerk, d_acc, d_v, d_x);
     CK(cudaGetLastError());
@@ -775,6 +804,118 @@ int g6x_set_j_particles(int clusterid, int addr0, int n, const int index[], cons
     return g6x_set_j_particles_dev(clusterid, addr0, n, (const int *)(d + 4 * n3 + 2 * n1), (const double *)(d + 4 * n3),
                                    (const double *)(d + 4 * n3 + n1), (const double *)(d + 3 * n3),
                                    (const double *)(d + 2 * n3), (const double *)(d + n3), (const double *)d);
+}
+
+// ---- the rest of the GRAPE-6 calling sequence (names and meanings recalled, unverified) ----
+int g_tunit = 0, g_xunit = 0;     // GRAPE-6 fixed-point scales: kept for the caller, no effect on fp64 / double-single data
+
+int g6_set_tunit(int newtunit) { g_tunit = newtunit; return G6_OK; }
+int g6_set_xunit(int newxunit) { g_xunit = newxunit; return G6_OK; }
+int g6x_get_units(int *tunit, int *xunit)
+{
+    if (!tunit || !xunit) return G6_ERR_ARG;
+    *tunit = g_tunit;
+    *xunit = g_xunit;
+    return G6_OK;
+}
+
+int g6_reset(int clusterid)
+{
+    GET_CLUSTER(clusterid);
+    CK(cudaStreamSynchronize(c.stream));
+    if (c.alloc_cap) CK(cudaMemsetAsync(c.js.raw, 0, (size_t)(c.alloc_cap / JT) * RAW_TILE_BYTES, c.stream));
+    std::fill(c.slot_of_addr.begin(), c.slot_of_addr.end(), -1);
+    c.n_rec = 0;
+    c.n_stored = 0;
+    c.pred_valid = false;
+    c.pending = false;
+    c.have_result = false;
+    c.pend_done_seq = 0;
+    c.last_nb = c.nb_on_host = false;
+    c.ti = 0.0;
+    return G6_OK;
+}
+
+int g6_reset_fofpga(int clusterid)
+{
+    GET_CLUSTER(clusterid);      // there is no force-output FPGA to reset; the call only checks the cluster
+    return G6_OK;
+}
+
+int g6_initialize_jp_buffer(int clusterid, int buf_size)
+{
+    GET_CLUSTER(clusterid);
+    if (buf_size < 1) return fail(c, G6_ERR_ARG, "buf_size = %d", buf_size);
+    return ensure_rec(c, std::min(buf_size, c.capacity));
+}
+
+int g6_flush_jp_buffer(int clusterid)
+{
+    GET_CLUSTER(clusterid);
+    if (c.pending) return fail(c, G6_ERR_SEQUENCE, "g6_flush_jp_buffer between firsthalf and lasthalf");
+    return flush_j(c);
+}
+
+int g6_getnjmax(int clusterid)
+{
+    GET_CLUSTER(clusterid);
+    return c.capacity;
+}
+
+int g6x_get_j_particles(int clusterid, int addr0, int n, int index[], double tj[], double mass[], double jerk[][3],
+                        double acc[][3], double v[][3], double x[][3])
+{
+    GET_CLUSTER(clusterid);
+    if (c.pending) return fail(c, G6_ERR_SEQUENCE, "j-particle read-back between firsthalf and lasthalf");
+    if (n < 1 || addr0 < 0 || (long long)addr0 + n > c.n_stored)
+        return fail(c, G6_ERR_ADDRESS, "addresses [%d, %lld) outside stored [0, %d)", addr0, (long long)addr0 + n, c.n_stored);
+    int rc = flush_j(c);
+    if (rc) return rc;
+    JRecord *d = nullptr;
+    std::vector<JRecord> h;
+    try { h.resize(n); } catch (const std::bad_alloc &) { return fail(c, G6_ERR_NOMEM, "host allocation failed"); }
+    rc = [&]() -> int {
+        CK(dalloc(d, n));
+        k_fetch_records<<<(n + 127) / 128, 128, 0, c.stream>>>(c.js, addr0, n, d);
+        CK(cudaGetLastError());
+        CK(cudaMemcpyAsync(h.data(), d, sizeof(JRecord) * n, cudaMemcpyDeviceToHost, c.stream));
+        CK(cudaStreamSynchronize(c.stream));
+        return G6_OK;
+    }();
+    dfree(d);
+    if (rc) return rc;
+    for (int p = 0; p < n; ++p) {
+        const JRecord &r = h[p];
+        if (index) index[p] = r.idx;
+        if (tj) tj[p] = r.t;
+        if (mass) mass[p] = (double)r.m;
+        for (int k = 0; k < 3; ++k) {
+            if (x) x[p][k] = r.x[k];
+            if (v) v[p][k] = (double)r.v[k];
+            if (acc) acc[p][k] = 2.0 * (double)r.a2[k];
+            if (jerk) jerk[p][k] = 6.0 * (double)r.j6[k];
+        }
+    }
+    return G6_OK;
+}
+
+int g6_get_j_particle(int clusterid, int address, int *index, double *tj, double *mass, double jerk_by6[3],
+                      double acc_by2[3], double v[3], double x[3])
+{
+    double j[1][3], a[1][3], vv[1][3], xx[1][3], t = 0, m = 0;
+    int idx = 0;
+    int rc = g6x_get_j_particles(clusterid, address, 1, &idx, &t, &m, j, a, vv, xx);
+    if (rc) return rc;
+    if (index) *index = idx;
+    if (tj) *tj = t;
+    if (mass) *mass = m;
+    for (int k = 0; k < 3; ++k) {
+        if (jerk_by6) jerk_by6[k] = j[0][k] / 6.0;      // exact: the stored binary32 value
+        if (acc_by2) acc_by2[k] = a[0][k] / 2.0;
+        if (v) v[k] = vv[0][k];
+        if (x) x[k] = xx[0][k];
+    }
+    return G6_OK;
 }
 
 int g6_set_ti(int clusterid, double ti)
@@ -1077,7 +1218,7 @@ int g6x_set_option(int clusterid, const char *key, int value)
     const bool is_flag = slot == &c.opt_ds || slot == &c.opt_newton || slot == &c.opt_timers;
     if (value < 0 || (is_flag && value > 1) || (slot == &c.opt_kernel && value > 2) || (slot == &c.opt_jsplit && value > 65535) || (slot == &c.opt_small && value > BS_MAX_I) ||
         (slot == &c.opt_nb_maxlen && (value < 1 || value > 4096)) ||
-        (slot == &c.opt_variant && value != 0 && fast_ctas_per_sm(FastVariant{value / 8, value % 8}) < 1))
+        (slot == &c.opt_variant && value != 0 && !fast_is_built(FastVariant{value / 8, value % 8}, true)))
         return fail(c, G6_ERR_ARG, "bad value %d for option '%s'", value, key);
     *slot = value;
     if (slot == &c.opt_small) c.small_explicit = true;
@@ -1146,62 +1287,6 @@ int g6x_jsplit_unpack_dev(int clusterid, int ni, const long long *d_key_min, con
     k_jsplit_unpack<<<(ni + 255) / 256, 256, 0, c.stream>>>(ni, d_key_min, d_index_sum, d_nn_index, d_nn_r2);
     CK(cudaGetLastError());
     return G6_OK;
-}
-
-int g6x_probe_fp32_peak(int clusterid, int mode, int ctas_per_sm, double *lane_instr_per_s)
-{
-    GET_CLUSTER(clusterid);
-    if (c.pending) return fail(c, G6_ERR_SEQUENCE, "force call pending");
-    if (mode < 0 || mode > 3 || ctas_per_sm < 1 || ctas_per_sm > 16 || !lane_instr_per_s) return fail(c, G6_ERR_ARG, "bad probe arguments");
-    float *d_out = nullptr;
-    CK(cudaStreamSynchronize(c.stream));
-    CK(dalloc(d_out, (size_t)c.n_sm * ctas_per_sm * PROBE_THREADS));
-    const double r = probe_fp32(mode, c.n_sm, c.stream, d_out, ctas_per_sm);
-    dfree(d_out);
-    if (r < 0) return fail(c, G6_ERR_CUDA, "FP32 probe failed: %s", cudaGetErrorString(cudaGetLastError()));
-    *lane_instr_per_s = r;
-    return G6_OK;
-}
-
-int g6x_probe_read_jstore(int clusterid, int nj)
-{
-    GET_CLUSTER(clusterid);
-    if (c.pending) return fail(c, G6_ERR_SEQUENCE, "force call pending");
-    if (nj < 1 || nj > c.capacity) return fail(c, G6_ERR_NJ, "nj = %d outside [1, capacity]", nj);
-    const size_t n16 = (size_t)((nj + JT - 1) / JT) * RAW_TILE_BYTES / 16;
-    k_probe_read<<<c.n_sm * 8, 256, 0, c.stream>>>(reinterpret_cast<const float4 *>(c.js.raw), n16, reinterpret_cast<float *>(c.d_counter + 1));
-    CK(cudaGetLastError());
-    return G6_OK;
-}
-
-int g6x_debug_dx(int clusterid, int n, const int ipipe[], const int jaddr[], float dx[][3])
-{
-    GET_CLUSTER(clusterid);
-    if (c.pending || !c.have_result) return fail(c, G6_ERR_SEQUENCE, "no completed host force call");
-    if (n < 1 || !ipipe || !jaddr || !dx) return fail(c, G6_ERR_ARG, "bad arguments");
-    for (int k = 0; k < n; ++k)
-        if (ipipe[k] < 0 || ipipe[k] >= c.last_ni || jaddr[k] < 0 || jaddr[k] >= c.pred_n)
-            return fail(c, G6_ERR_ARG, "pair %d out of range", k);
-    int *d_ip = nullptr, *d_ja = nullptr;
-    float *d_out = nullptr;
-    int rc = run_predict(c);     // the small-block kernel predicts on the fly and leaves c.pred stale
-    if (rc) return rc;
-    rc = [&]() -> int {
-        CK(dalloc(d_ip, n)); CK(dalloc(d_ja, n)); CK(dalloc(d_out, 3 * (size_t)n));
-        CK(cudaMemcpyAsync(d_ip, ipipe, sizeof(int) * n, cudaMemcpyHostToDevice, c.stream));
-        CK(cudaMemcpyAsync(d_ja, jaddr, sizeof(int) * n, cudaMemcpyHostToDevice, c.stream));
-        if (!c.iblk_on_device) {
-            CK(cudaMemcpyAsync(c.d_iblk, c.h_iblk, iblk_bytes(c.last_ni), cudaMemcpyHostToDevice, c.stream));
-            c.iblk_on_device = true;
-        }
-        k_debug_dx<<<(n + 127) / 128, 128, 0, c.stream>>>(n, d_ip, d_ja, iview(c.d_iblk, c.last_ni).xi, c.opt_ds, c.pred, d_out);
-        CK(cudaGetLastError());
-        CK(cudaMemcpyAsync(dx, d_out, sizeof(float) * 3 * n, cudaMemcpyDeviceToHost, c.stream));
-        CK(cudaStreamSynchronize(c.stream));
-        return G6_OK;
-    }();
-    dfree(d_ip); dfree(d_ja); dfree(d_out);
-    return rc;
 }
 
 }  // extern "C"

@@ -76,6 +76,7 @@ struct BsArgs {
     int *nb_wlist;              // [G * NW][ni][maxlen]  their j addresses, increasing
     int *nb_cnt;                // [ni]          out: all neighbours found
     int *nb_list;               // [ni][maxlen]  out: callers' indices, increasing j address, the smallest addresses on overflow
+    float *dbg_dx;              // DBG instantiation only (parity pin P11): [ni][nj][3] Eq.-3 separations; nullptr in the library
 };
 
 __device__ __forceinline__ int ld_acquire_cta(const volatile int *p)
@@ -107,15 +108,16 @@ struct BsSmem {
 static_assert(sizeof(BsSmem<16>) <= 232448 && sizeof(BsSmem<64>) <= 232448, "block-step shared memory");
 
 // two consecutive j against one i, every pair checked.  `ok` in: address < nj && index differs.
-template <bool NEWTON>
+template <bool NEWTON, bool DBG = false>
 __device__ __forceinline__ void pair2_checked(IPart &I, const float2 xh, const float2 yh, const float2 zh, const float2 xl,
                                               const float2 yl, const float2 zl, const float2 vx, const float2 vy, const float2 vz,
-                                              float2 m, const float2 eps2, bool ok0, bool ok1, float2 &r2_out)
+                                              float2 m, const float2 eps2, bool ok0, bool ok1, float2 &r2_out, float2 *dbg = nullptr)
 {
     constexpr float INF = __builtin_huge_valf();
     const float2 dx = add2(add2(xh, I.nxh[0]), add2(xl, I.nxl[0]));      // Eq. 3
     const float2 dy = add2(add2(yh, I.nxh[1]), add2(yl, I.nxl[1]));
     const float2 dz = add2(add2(zh, I.nxh[2]), add2(zl, I.nxl[2]));
+    if (DBG) { dbg[0] = dx; dbg[1] = dy; dbg[2] = dz; }      // parity pin P11 (csrc/debug/g6_debug_dx.cu only)
     const float2 dvx = add2(vx, I.nv[0]);
     const float2 dvy = add2(vy, I.nv[1]);
     const float2 dvz = add2(vz, I.nv[2]);
@@ -174,7 +176,7 @@ __device__ __forceinline__ float transpose_reduce8(const float (&v)[8], int lane
 }
 
 // `Dp`: the inline i-block / j updates of the launch (nullptr when there are none: device-resident callers)
-template <int MAXI, bool NEWTON>
+template <int MAXI, bool NEWTON, bool DBG = false>
 __device__ __forceinline__ void block_step_body(const BsArgs &A0, const BsInline<MAXI> *Dp)
 {
     const BsArgs &A = A0;
@@ -270,12 +272,8 @@ __device__ __forceinline__ void block_step_body(const BsArgs &A0, const BsInline
                 const float2 v0 = *reinterpret_cast<const float2 *>(R + RAW_V + 4 * (k * JT + l0));
                 const float2 a2 = *reinterpret_cast<const float2 *>(R + RAW_A2 + 4 * (k * JT + l0));
                 const float2 j6 = *reinterpret_cast<const float2 *>(R + RAW_J6 + 4 * (k * JT + l0));
-#if defined(G6_ABLATE) && (G6_ABLATE & 4)      // experiment: no predictor arithmetic (positions truncated to binary32)
-                jf[F_XH + k][g] = make_float2((float)x0.x, (float)x0.y); jf[F_XL + k][g] = make_float2(dt.x * a2.x, dt.y * j6.y); jf[F_V + k][g] = v0;
-#else
                 predict_coord(dt.x, x0.x, v0.x, a2.x, j6.x, A.ds, jf[F_XH + k][g].x, jf[F_XL + k][g].x, jf[F_V + k][g].x);
                 predict_coord(dt.y, x0.y, v0.y, a2.y, j6.y, A.ds, jf[F_XH + k][g].y, jf[F_XL + k][g].y, jf[F_V + k][g].y);
-#endif
             }
             jf[F_M][g] = *reinterpret_cast<const float2 *>(R + RAW_M + 4 * l0);
             jx[g] = *reinterpret_cast<const int2 *>(R + RAW_IDX + 4 * l0);
@@ -295,12 +293,7 @@ __device__ __forceinline__ void block_step_body(const BsArgs &A0, const BsInline
         }
 
         // ---- a-4: every i-particle of the block against my 8 j
-#if defined(G6_ABLATE) && (G6_ABLATE & 8)      // experiment: no force evaluation (the predicted j are only touched)
-        if (jf[0][0].x == 123.456f && jf[9][3].y == 1.0f) sm.r2[w][0] = jf[3][1].x + jf[7][2].y;
-        for (int i = A.ni; i < A.ni; ++i) {
-#else
         for (int i = 0; i < A.ni; ++i) {
-#endif
             IPart I;
 #pragma unroll
             for (int k = 0; k < 3; ++k) {
@@ -316,8 +309,16 @@ __device__ __forceinline__ void block_step_body(const BsArgs &A0, const BsInline
 #pragma unroll
             for (int g = 0; g < 4; ++g) {
                 const int ja = ja0 + 64 * g;
-                pair2_checked<NEWTON>(I, jf[0][g], jf[1][g], jf[2][g], jf[3][g], jf[4][g], jf[5][g], jf[6][g], jf[7][g], jf[8][g], jf[9][g], eps2,
-                                      (ja < A.nj) && (jx[g].x != my), (ja + 1 < A.nj) && (jx[g].y != my), r2m[g]);
+                float2 dd[3];
+                pair2_checked<NEWTON, DBG>(I, jf[0][g], jf[1][g], jf[2][g], jf[3][g], jf[4][g], jf[5][g], jf[6][g], jf[7][g], jf[8][g], jf[9][g], eps2,
+                                           (ja < A.nj) && (jx[g].x != my), (ja + 1 < A.nj) && (jx[g].y != my), r2m[g], dd);
+                if (DBG) {
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) {
+                        if (ja < A.nj) A.dbg_dx[((size_t)i * A.nj + ja) * 3 + k] = dd[k].x;
+                        if (ja + 1 < A.nj) A.dbg_dx[((size_t)i * A.nj + ja + 1) * 3 + k] = dd[k].y;
+                    }
+                }
             }
             // the 7 sums of this (i, tile): FP32 tree over the 256 j, then fp64 (reading 9)
             const float v8[8] = {__fadd_rn(I.a[0].x, I.a[0].y), __fadd_rn(I.a[1].x, I.a[1].y), __fadd_rn(I.a[2].x, I.a[2].y),
@@ -538,6 +539,14 @@ __global__ void __launch_bounds__(BS_THREADS)
 k_block_step_dev(const BsArgs A)
 {
     block_step_body<MAXI, NEWTON>(A, nullptr);
+}
+
+// the DBG instantiation (every pair's separation also goes to A.dbg_dx); launched only by csrc/debug/g6_debug_dx.cu
+template <int MAXI, bool NEWTON>
+__global__ void __launch_bounds__(BS_THREADS)
+k_block_step_dbg(const BsArgs A)
+{
+    block_step_body<MAXI, NEWTON, true>(A, nullptr);
 }
 
 // ---------------------------------------------------------------- host side

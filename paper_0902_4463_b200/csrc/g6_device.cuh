@@ -166,6 +166,25 @@ k_stage(JStore S, const JRecord *__restrict__ rec, int n_rec, int n_i, const dou
     }
 }
 
+// ---- j-particle read-back: records of addresses [addr0, addr0 + n) exactly as stored (x, t fp64; the rest binary32) ----
+__global__ void __launch_bounds__(128)
+k_fetch_records(JStore S, int addr0, int n, JRecord *__restrict__ out)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    const int a = addr0 + p;
+    char *T = raw_tile(S.raw, a);
+    const int l = a % JT;
+    JRecord r;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { r.x[k] = raw_x(T, k, l); r.v[k] = raw_v(T, k, l); r.a2[k] = raw_a2(T, k, l); r.j6[k] = raw_j6(T, k, l); }
+    r.t = raw_t(T, l);
+    r.m = raw_m(T, l);
+    r.idx = raw_idx(T, l);
+    r.addr = a;
+    out[p] = r;
+}
+
 // Eq. 1-2 for one coordinate (reading 11): FP32 Horner increment, fp64 add to x0, DS re-split
 __device__ __forceinline__ void predict_coord(float dt, double x0, float v0, float a2, float j6, int ds,
                                               float &xh, float &xl, float &vp)

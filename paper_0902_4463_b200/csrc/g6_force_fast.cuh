@@ -95,15 +95,19 @@ struct IPart {
 
 // One i-particle against two consecutive j-particles (packed lanes).  33 FMA-pipe packed
 // instructions (+3 with the Newton step), 2 MUFU, 1 FMNMX3.  MASKED: m and r2 already masked.
-template <bool NEWTON>
+//   DS = false: pure-FP32 separations, dx = xj_hi - xi_hi (3 packed adds instead of Eq. 3's 9): the variant the
+//               paper's "DS costs <~ 20 %" is measured against; bit-identical to DS with zero lo words.
+//   DBG       : also hand the separations of the two pairs to the caller (parity pin P11: Eq. 3 bit for bit)
+template <bool NEWTON, bool DS = true, bool DBG = false>
 __device__ __forceinline__ void pair2(IPart &I, const float2 xh, const float2 yh, const float2 zh, const float2 xl,
                                       const float2 yl, const float2 zl, const float2 vx, const float2 vy, const float2 vz,
-                                      const float2 m, const float2 eps2_3, float2 &r2_out)
+                                      const float2 m, const float2 eps2_3, float2 &r2_out, float2 *dbg = nullptr)
 {
     // Eq. 3: dx = (xj_hi - xi_hi) + (xj_lo - xi_lo)
-    const float2 dx = add2(add2(xh, I.nxh[0]), add2(xl, I.nxl[0]));
-    const float2 dy = add2(add2(yh, I.nxh[1]), add2(yl, I.nxl[1]));
-    const float2 dz = add2(add2(zh, I.nxh[2]), add2(zl, I.nxl[2]));
+    const float2 dx = DS ? add2(add2(xh, I.nxh[0]), add2(xl, I.nxl[0])) : add2(xh, I.nxh[0]);
+    const float2 dy = DS ? add2(add2(yh, I.nxh[1]), add2(yl, I.nxl[1])) : add2(yh, I.nxh[1]);
+    const float2 dz = DS ? add2(add2(zh, I.nxh[2]), add2(zl, I.nxl[2])) : add2(zh, I.nxh[2]);
+    if (DBG) { dbg[0] = dx; dbg[1] = dy; dbg[2] = dz; }
     const float2 dvx = add2(vx, I.nv[0]);
     const float2 dvy = add2(vy, I.nv[1]);
     const float2 dvz = add2(vz, I.nv[2]);
@@ -117,11 +121,7 @@ __device__ __forceinline__ void pair2(IPart &I, const float2 xh, const float2 yh
     //                   y0 (3 - sigma y0^2) / 2, i.e. 2 / sqrt(sigma) = sqrt(3) / s: the halving is never done,
     //                   the step costs 3 packed instructions (FMUL2, FFMA2, FMUL2) instead of 4.
     const float2 s2 = fma2(r2, dup(pair_scale<NEWTON>()), eps2_3);          // eps2_3 = SC * eps^2
-#if defined(G6_ABLATE) && (G6_ABLATE & 2)
-    float2 rinv = mul2(s2, dup(0.5f));
-#else
     float2 rinv = make_float2(rsqrt_approx(s2.x), rsqrt_approx(s2.y));
-#endif
     if (NEWTON) {
         const float2 ns2 = make_float2(-s2.x, -s2.y);       // folded into the FFMA2 operand modifier
         const float2 u = fma2(ns2, mul2(rinv, rinv), dup(3.0f));
@@ -143,6 +143,17 @@ __device__ __forceinline__ void pair2(IPart &I, const float2 xh, const float2 yh
     r2_out = r2;
 }
 
+// DBG: store the separations of j addresses (ja, ja + 1) against i-particle i into A.dbg_dx[i][j][3]
+__device__ __forceinline__ void dbg_store(const ForceArgs &A, int i, int ja, const float2 *d)
+{
+    if (i >= A.ni) return;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        if (ja < A.nj) A.dbg_dx[((size_t)i * A.nj + ja) * 3 + k] = d[k].x;
+        if (ja + 1 < A.nj) A.dbg_dx[((size_t)i * A.nj + ja + 1) * 3 + k] = d[k].y;
+    }
+}
+
 constexpr int FAST_NSTAGE = 4;
 
 template <int THREADS, int IT>
@@ -156,7 +167,9 @@ struct FastSmem {
 // unchecked loop then keeps the minimum r2 of each 8-j step (as many FMNMX as before) and compares
 // it with max(h2_i, rmin): only a step that holds a neighbour or a new nearest neighbour leaves
 // the packed code, re-evaluates its 8 separations from shared memory and appends to the list.
-template <int THREADS, int IT, bool NEWTON, bool NB = false>
+// DS = false: the pure-FP32 variant of pair2 (option "ds" = 0).  DBG: every pair's Eq.-3 separation goes to A.dbg_dx
+// (only instantiated by the parity-test hook csrc/debug/g6_debug_dx.cu, never by the library).
+template <int THREADS, int IT, bool NEWTON, bool NB = false, bool DS = true, bool DBG = false>
 __global__ void __launch_bounds__(THREADS, (NB && THREADS * IT == 256) ? 3 : 0)
 k_force_fast(ForceArgs A)
 {
@@ -271,24 +284,27 @@ k_force_fast(ForceArgs A)
                     for (int k = 0; k < NF; ++k) f[k] = T[k * (JT / 4) + 2 * s8 + h];
 #pragma unroll
                     for (int q = 0; q < IT; ++q) {
-                        float2 ra, rb;
-                        pair2<NEWTON>(I[q], make_float2(f[0].x, f[0].y), make_float2(f[1].x, f[1].y), make_float2(f[2].x, f[2].y),
+                        float2 ra, rb, da[3], db[3];
+                        pair2<NEWTON, DS, DBG>(I[q], make_float2(f[0].x, f[0].y), make_float2(f[1].x, f[1].y), make_float2(f[2].x, f[2].y),
                                       make_float2(f[3].x, f[3].y), make_float2(f[4].x, f[4].y), make_float2(f[5].x, f[5].y),
                                       make_float2(f[6].x, f[6].y), make_float2(f[7].x, f[7].y), make_float2(f[8].x, f[8].y),
-                                      make_float2(f[9].x, f[9].y), eps2, ra);
-                        pair2<NEWTON>(I[q], make_float2(f[0].z, f[0].w), make_float2(f[1].z, f[1].w), make_float2(f[2].z, f[2].w),
+                                      make_float2(f[9].x, f[9].y), eps2, ra, da);
+                        pair2<NEWTON, DS, DBG>(I[q], make_float2(f[0].z, f[0].w), make_float2(f[1].z, f[1].w), make_float2(f[2].z, f[2].w),
                                       make_float2(f[3].z, f[3].w), make_float2(f[4].z, f[4].w), make_float2(f[5].z, f[5].w),
                                       make_float2(f[6].z, f[6].w), make_float2(f[7].z, f[7].w), make_float2(f[8].z, f[8].w),
-                                      make_float2(f[9].z, f[9].w), eps2, rb);
+                                      make_float2(f[9].z, f[9].w), eps2, rb, db);
+                        if (DBG) {
+                            const int i = (blockIdx.x * IT + q) * THREADS + tid, ja = t * JT + 8 * s8 + 4 * h;
+                            dbg_store(A, i, ja, da);
+                            dbg_store(A, i, ja + 2, db);
+                        }
                         if (NB) {
                             // before[] is reused as the running minimum of this step
                             if (h == 0) before[q] = fminf(fminf(ra.x, ra.y), fminf(rb.x, rb.y));
                             else before[q] = fminf(fminf(fminf(ra.x, ra.y), before[q]), fminf(rb.x, rb.y));
                         } else {
-#if !(defined(G6_ABLATE) && (G6_ABLATE & 1))
                             I[q].rmin = fminf(fminf(ra.x, ra.y), I[q].rmin);
                             I[q].rmin = fminf(fminf(rb.x, rb.y), I[q].rmin);
-#endif
                         }
                     }
                 }
@@ -339,15 +355,20 @@ k_force_fast(ForceArgs A)
                     const bool o2 = (j0 + 2 < A.nj) && (jx.z != my[q]);
                     const bool o3 = (j0 + 3 < A.nj) && (jx.w != my[q]);
                     const float before = I[q].rmin;
-                    float2 ra, rb;
-                    pair2<NEWTON>(I[q], make_float2(f[0].x, f[0].y), make_float2(f[1].x, f[1].y), make_float2(f[2].x, f[2].y),
+                    float2 ra, rb, da[3], db[3];
+                    pair2<NEWTON, DS, DBG>(I[q], make_float2(f[0].x, f[0].y), make_float2(f[1].x, f[1].y), make_float2(f[2].x, f[2].y),
                                   make_float2(f[3].x, f[3].y), make_float2(f[4].x, f[4].y), make_float2(f[5].x, f[5].y),
                                   make_float2(f[6].x, f[6].y), make_float2(f[7].x, f[7].y), make_float2(f[8].x, f[8].y),
-                                  make_float2(o0 ? f[9].x : 0.0f, o1 ? f[9].y : 0.0f), eps2, ra);
-                    pair2<NEWTON>(I[q], make_float2(f[0].z, f[0].w), make_float2(f[1].z, f[1].w), make_float2(f[2].z, f[2].w),
+                                  make_float2(o0 ? f[9].x : 0.0f, o1 ? f[9].y : 0.0f), eps2, ra, da);
+                    pair2<NEWTON, DS, DBG>(I[q], make_float2(f[0].z, f[0].w), make_float2(f[1].z, f[1].w), make_float2(f[2].z, f[2].w),
                                   make_float2(f[3].z, f[3].w), make_float2(f[4].z, f[4].w), make_float2(f[5].z, f[5].w),
                                   make_float2(f[6].z, f[6].w), make_float2(f[7].z, f[7].w), make_float2(f[8].z, f[8].w),
-                                  make_float2(o2 ? f[9].z : 0.0f, o3 ? f[9].w : 0.0f), eps2, rb);
+                                  make_float2(o2 ? f[9].z : 0.0f, o3 ? f[9].w : 0.0f), eps2, rb, db);
+                    if (DBG) {
+                        const int i = (blockIdx.x * IT + q) * THREADS + tid;
+                        dbg_store(A, i, j0, da);
+                        dbg_store(A, i, j0 + 2, db);
+                    }
                     I[q].rmin = fminf(fminf(o0 ? ra.x : INF, o1 ? ra.y : INF), I[q].rmin);
                     I[q].rmin = fminf(fminf(o2 ? rb.x : INF, o3 ? rb.y : INF), I[q].rmin);
                     if (I[q].rmin < before) bstep[q] = j0 >> 3;
@@ -422,48 +443,51 @@ k_force_fast(ForceArgs A)
     }
 }
 
-// ---------------------------------------------------------------- host side: variants + launch
+// ---------------------------------------------------------------- host side: shapes + launch
 struct FastVariant { int threads, it; };
 
-inline bool fast_available() { return true; }
+// The shapes the library builds: (threads, i-particles per thread).  Each exists with and without the Newton step,
+// with neighbour lists (NB) and as the pure-FP32 variant (option "ds" = 0; without lists).  128 x 4 and 64 x 2 are
+// reachable only through option "variant" (experiments); fast_pick chooses among the first five.
+#define G6_FAST_SHAPES(X) X(128, 2) X(128, 1) X(64, 1) X(32, 1) X(256, 1)
+#define G6_FAST_EXTRA_SHAPES(X) X(128, 4) X(64, 2)
 
-template <int THREADS, int IT>
+inline int fast_key(FastVariant v) { return v.threads * 8 + v.it; }
+
+// is (threads, it) a built shape?  `extra`: also the experiment-only shapes (no lists, no pure-FP32 variant)
+inline bool fast_is_built(FastVariant v, bool extra)
+{
+    if (v.threads < 32 || v.it < 1 || v.it > 7) return false;
+    switch (fast_key(v)) {
+#define X(T, I) case T * 8 + I:
+        G6_FAST_SHAPES(X)
+        return true;
+        G6_FAST_EXTRA_SHAPES(X)
+        return extra;
+#undef X
+        default: return false;
+    }
+}
+
+template <int THREADS, int IT, bool NB, bool DS>
 inline int fast_attr()
 {
     const int bytes = (int)sizeof(FastSmem<THREADS, IT>);
-    cudaError_t e = cudaFuncSetAttribute(k_force_fast<THREADS, IT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    cudaError_t e = cudaFuncSetAttribute(k_force_fast<THREADS, IT, true, NB, DS>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     if (e != cudaSuccess) return (int)e;
-    e = cudaFuncSetAttribute(k_force_fast<THREADS, IT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    return (int)e;
-}
-template <int THREADS, int IT>
-inline int fast_attr_nb()
-{
-    const int bytes = (int)sizeof(FastSmem<THREADS, IT>);
-    cudaError_t e = cudaFuncSetAttribute(k_force_fast<THREADS, IT, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    if (e != cudaSuccess) return (int)e;
-    e = cudaFuncSetAttribute(k_force_fast<THREADS, IT, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    e = cudaFuncSetAttribute(k_force_fast<THREADS, IT, false, NB, DS>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     return (int)e;
 }
 
 inline int fast_kernel_init()
 {
     int r;
-    if ((r = fast_attr<128, 2>())) return r;
-    if ((r = fast_attr<128, 1>())) return r;
-    if ((r = fast_attr<64, 1>())) return r;
-    if ((r = fast_attr<32, 1>())) return r;
-    if ((r = fast_attr<256, 1>())) return r;
-    if ((r = fast_attr<256, 2>())) return r;
-    if ((r = fast_attr<128, 4>())) return r;
-    if ((r = fast_attr<64, 2>())) return r;
-    if ((r = fast_attr<64, 4>())) return r;
-    // neighbour-list variants: the shapes fast_pick chooses
-    if ((r = fast_attr_nb<128, 2>())) return r;
-    if ((r = fast_attr_nb<128, 1>())) return r;
-    if ((r = fast_attr_nb<64, 1>())) return r;
-    if ((r = fast_attr_nb<32, 1>())) return r;
-    if ((r = fast_attr_nb<256, 1>())) return r;
+#define X(T, I) if ((r = fast_attr<T, I, false, true>())) return r; if ((r = fast_attr<T, I, true, true>())) return r; if ((r = fast_attr<T, I, false, false>())) return r;
+    G6_FAST_SHAPES(X)
+#undef X
+#define X(T, I) if ((r = fast_attr<T, I, false, true>())) return r;
+    G6_FAST_EXTRA_SHAPES(X)
+#undef X
     return 0;
 }
 
@@ -481,112 +505,61 @@ inline FastVariant fast_pick(int ni, int n_sm, int force)
     return FastVariant{128, 2};
 }
 
-template <int THREADS, int IT>
+template <int THREADS, int IT, bool NB, bool DS>
 inline int fast_launch_t(const ForceArgs &A, bool newton, int n_itiles, int S, cudaStream_t st)
 {
     dim3 grid(n_itiles, S);
     const size_t bytes = sizeof(FastSmem<THREADS, IT>);
-    if (newton) k_force_fast<THREADS, IT, true><<<grid, THREADS, bytes, st>>>(A);
-    else k_force_fast<THREADS, IT, false><<<grid, THREADS, bytes, st>>>(A);
+    if (newton) k_force_fast<THREADS, IT, true, NB, DS><<<grid, THREADS, bytes, st>>>(A);
+    else k_force_fast<THREADS, IT, false, NB, DS><<<grid, THREADS, bytes, st>>>(A);
     return (int)cudaGetLastError();
 }
 
-template <int THREADS, int IT>
-inline int fast_launch_nb_t(const ForceArgs &A, bool newton, int n_itiles, int S, cudaStream_t st)
-{
-    dim3 grid(n_itiles, S);
-    const size_t bytes = sizeof(FastSmem<THREADS, IT>);
-    if (newton) k_force_fast<THREADS, IT, true, true><<<grid, THREADS, bytes, st>>>(A);
-    else k_force_fast<THREADS, IT, false, true><<<grid, THREADS, bytes, st>>>(A);
-    return (int)cudaGetLastError();
-}
+// neighbour lists exist for the automatic shapes only
+inline bool fast_has_nb(FastVariant v) { return fast_is_built(v, false); }
 
-// is (threads, it) one of the shapes built with neighbour lists?
-inline bool fast_has_nb(FastVariant v)
-{
-    const int key = v.threads * 8 + v.it;
-    return key == 128 * 8 + 2 || key == 128 * 8 + 1 || key == 64 * 8 + 1 || key == 32 * 8 + 1 || key == 256 * 8 + 1;
-}
-
+// A.h2 != nullptr: with neighbour lists (double-single arithmetic; with ds = 0 the lo words are zero, which is the same
+// numbers).  A.ds == 0 without lists: the pure-FP32 variant (3 packed adds per separation instead of 9).
 inline int launch_force_fast(const ForceArgs &A, bool newton, FastVariant v, int n_itiles, int S, cudaStream_t st)
 {
-    const int key = v.threads * 8 + v.it;
-    if (A.h2) {
-        switch (key) {
-            case 128 * 8 + 2: return fast_launch_nb_t<128, 2>(A, newton, n_itiles, S, st);
-            case 128 * 8 + 1: return fast_launch_nb_t<128, 1>(A, newton, n_itiles, S, st);
-            case 64 * 8 + 1: return fast_launch_nb_t<64, 1>(A, newton, n_itiles, S, st);
-            case 32 * 8 + 1: return fast_launch_nb_t<32, 1>(A, newton, n_itiles, S, st);
-            case 256 * 8 + 1: return fast_launch_nb_t<256, 1>(A, newton, n_itiles, S, st);
-            default: return (int)cudaErrorInvalidValue;
-        }
-    }
-    switch (key) {
-        case 128 * 8 + 2: return fast_launch_t<128, 2>(A, newton, n_itiles, S, st);
-        case 128 * 8 + 1: return fast_launch_t<128, 1>(A, newton, n_itiles, S, st);
-        case 64 * 8 + 1: return fast_launch_t<64, 1>(A, newton, n_itiles, S, st);
-        case 32 * 8 + 1: return fast_launch_t<32, 1>(A, newton, n_itiles, S, st);
-        case 256 * 8 + 1: return fast_launch_t<256, 1>(A, newton, n_itiles, S, st);
-        case 256 * 8 + 2: return fast_launch_t<256, 2>(A, newton, n_itiles, S, st);
-        case 128 * 8 + 4: return fast_launch_t<128, 4>(A, newton, n_itiles, S, st);
-        case 64 * 8 + 2: return fast_launch_t<64, 2>(A, newton, n_itiles, S, st);
-        case 64 * 8 + 4: return fast_launch_t<64, 4>(A, newton, n_itiles, S, st);
+    switch (fast_key(v)) {
+#define X(T, I) case T * 8 + I: \
+            if (A.h2) return fast_launch_t<T, I, true, true>(A, newton, n_itiles, S, st); \
+            if (!A.ds) return fast_launch_t<T, I, false, false>(A, newton, n_itiles, S, st); \
+            return fast_launch_t<T, I, false, true>(A, newton, n_itiles, S, st);
+        G6_FAST_SHAPES(X)
+#undef X
+#define X(T, I) case T * 8 + I: \
+            if (A.h2) return (int)cudaErrorInvalidValue; \
+            return fast_launch_t<T, I, false, true>(A, newton, n_itiles, S, st);
+        G6_FAST_EXTRA_SHAPES(X)
+#undef X
         default: return (int)cudaErrorInvalidValue;
     }
 }
 
-// resident CTAs per SM of a variant (for the j-split scheduler)
-template <int THREADS, int IT, bool NB = false>
+// resident CTAs per SM of a shape (for the j-split scheduler); nb: the neighbour-list build (more registers)
+template <int THREADS, int IT, bool NB>
 inline int fast_occ_t()
 {
-    int n = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_force_fast<THREADS, IT, true, NB>, THREADS, sizeof(FastSmem<THREADS, IT>)) != cudaSuccess) return 1;
-    return n > 0 ? n : 1;
+    static int n = 0;
+    if (!n) {
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_force_fast<THREADS, IT, true, NB, true>, THREADS, sizeof(FastSmem<THREADS, IT>)) != cudaSuccess || n < 1) n = 1;
+    }
+    return n;
 }
-inline int fast_ctas_per_sm_nb(FastVariant v)
+inline int fast_ctas_per_sm(FastVariant v, bool nb = false)
 {
-    static int cache[5] = {0};
-    const int key = v.threads * 8 + v.it;
-    switch (key) {
-        case 256 * 8 + 1: return cache[4] ? cache[4] : (cache[4] = fast_occ_t<256, 1, true>());
-        case 128 * 8 + 2: return cache[0] ? cache[0] : (cache[0] = fast_occ_t<128, 2, true>());
-        case 128 * 8 + 1: return cache[1] ? cache[1] : (cache[1] = fast_occ_t<128, 1, true>());
-        case 64 * 8 + 1: return cache[2] ? cache[2] : (cache[2] = fast_occ_t<64, 1, true>());
-        case 32 * 8 + 1: return cache[3] ? cache[3] : (cache[3] = fast_occ_t<32, 1, true>());
+    switch (fast_key(v)) {
+#define X(T, I) case T * 8 + I: return nb ? fast_occ_t<T, I, true>() : fast_occ_t<T, I, false>();
+        G6_FAST_SHAPES(X)
+#undef X
+#define X(T, I) case T * 8 + I: return fast_occ_t<T, I, false>();
+        G6_FAST_EXTRA_SHAPES(X)
+#undef X
         default: return 1;
     }
 }
-inline int fast_ctas_per_sm(FastVariant v)
-{
-    static int cache[9] = {0};
-    const int key = v.threads * 8 + v.it;
-    int slot;
-    switch (key) {
-        case 128 * 8 + 2: slot = 0; break;
-        case 128 * 8 + 1: slot = 1; break;
-        case 64 * 8 + 1: slot = 2; break;
-        case 32 * 8 + 1: slot = 3; break;
-        case 256 * 8 + 1: slot = 4; break;
-        case 256 * 8 + 2: slot = 5; break;
-        case 128 * 8 + 4: slot = 6; break;
-        case 64 * 8 + 2: slot = 7; break;
-        case 64 * 8 + 4: slot = 8; break;
-        default: return 1;
-    }
-    if (!cache[slot]) {
-        switch (slot) {
-            case 0: cache[slot] = fast_occ_t<128, 2>(); break;
-            case 1: cache[slot] = fast_occ_t<128, 1>(); break;
-            case 2: cache[slot] = fast_occ_t<64, 1>(); break;
-            case 3: cache[slot] = fast_occ_t<32, 1>(); break;
-            case 4: cache[slot] = fast_occ_t<256, 1>(); break;
-            case 5: cache[slot] = fast_occ_t<256, 2>(); break;
-            case 6: cache[slot] = fast_occ_t<128, 4>(); break;
-            case 7: cache[slot] = fast_occ_t<64, 2>(); break;
-            case 8: cache[slot] = fast_occ_t<64, 4>(); break;
-        }
-    }
-    return cache[slot];
-}
+inline int fast_ctas_per_sm_nb(FastVariant v) { return fast_ctas_per_sm(v, true); }
 
 }  // namespace g6

@@ -30,6 +30,7 @@ struct ForceArgs {
     int nb_maxlen;            // entries stored per (split, i)
     int *nb_cnt;              // [S][ni]          neighbours found by split s (may exceed nb_maxlen)
     int *nb_list;             // [S][ni][maxlen]  their j addresses, increasing
+    float *dbg_dx;            // DBG instantiations only (parity pin P11): [ni][nj][3] Eq.-3 separations; nullptr in the library
 };
 
 // append j address `ja` to the list of (split s, i-particle i); `cnt` is the thread's running count

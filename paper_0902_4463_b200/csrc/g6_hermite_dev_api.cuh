@@ -102,10 +102,12 @@ g6hd_system *g6hd_create(int clusterid, int n, const double x[][3], const double
     if (clusterid < 0 || clusterid >= MAX_CLUSTERS) return nullptr;
     Cluster &c = g_cl[clusterid];
     if (!c.open) { fail(c, G6_ERR_NOT_OPEN, "cluster %d is not open", clusterid); return nullptr; }
-    if (n < 1 || n > c.capacity || !x || !v || !m || !(eta > 0) || !(dt_max > 0) || !(eps2 >= 0) || c.pending) {
-        fail(c, G6_ERR_ARG, "bad g6hd_create arguments (n = %d, capacity %d)", n, c.capacity);
+    // k_hd_select keeps one entry per 1024-particle thread block in shared memory: HD_MAX_BLOCKS of them
+    if (n < 1 || n > c.capacity || n > HD_MAX_BLOCKS * HD_PER_BLOCK || !x || !v || !m || !(eta > 0) || !(dt_max > 0) || !(eps2 >= 0) || c.pending) {
+        fail(c, G6_ERR_ARG, "bad g6hd_create arguments (n = %d; capacity %d, device-resident driver limit %d)", n, c.capacity, HD_MAX_BLOCKS * HD_PER_BLOCK);
         return nullptr;
     }
+    if (ensure_capacity(c, n) != G6_OK) return nullptr;
     g6hd_system *s = new (std::nothrow) g6hd_system;
     if (!s) return nullptr;
     s->cl = clusterid; s->n = n; s->eps2 = eps2; s->eta = eta; s->dt_max = dt_max;

@@ -21,12 +21,22 @@ DEFAULT_NPIPES = 131072
 SYMBOLS = [
     "g6_open", "g6_close", "g6_npipes", "g6_set_j_particle", "g6_set_ti", "g6calc_firsthalf",
     "g6calc_lasthalf", "g6calc_lasthalf2", "g6_read_neighbour_list", "g6_get_neighbour_list",
+    "g6_set_tunit", "g6_set_xunit", "g6_reset", "g6_reset_fofpga", "g6_initialize_jp_buffer", "g6_flush_jp_buffer",
+    "g6_getnjmax", "g6_get_j_particle", "g6x_get_j_particles", "g6x_get_units",
     "g6x_last_error", "g6x_set_npipes", "g6x_set_j_particles", "g6x_set_j_particles_dev", "g6x_calc_dev",
     "g6x_calc_dev_nb", "g6x_get_neighbour_lists", "g6x_jsplit_pack_dev", "g6x_jsplit_select_dev", "g6x_jsplit_unpack_dev",
     "g6x_get_nearest", "g6x_set_stream", "g6x_synchronize", "g6x_get_timers", "g6x_set_option",
-    "g6x_get_option", "g6x_get_predicted", "g6x_debug_dx", "g6x_probe_fp32_peak", "g6x_probe_read_jstore", "g6x_version",
+    "g6x_get_option", "g6x_get_predicted", "g6x_version",
     "g6h_create", "g6h_destroy", "g6h_evolve", "g6h_get_state", "g6h_get_stats", "g6h_get_force_wall_hist",
     "g6hd_create", "g6hd_destroy", "g6hd_evolve", "g6hd_get_state", "g6hd_get_stats", "g6hd_get_particles", "g6hd_get_last_block", "g6hd_set_shared_steps",
+]
+
+#: the Fortran-callable aliases include/g6_fortran.h declares (trailing underscore, arguments by reference)
+FORTRAN_SYMBOLS = [
+    "g6_open_", "g6_close_", "g6_npipes_", "g6_set_tunit_", "g6_set_xunit_", "g6_reset_", "g6_reset_fofpga_",
+    "g6_initialize_jp_buffer_", "g6_flush_jp_buffer_", "g6_getnjmax_", "g6_set_j_particle_", "g6_get_j_particle_",
+    "g6_set_ti_", "g6calc_firsthalf_", "g6calc_lasthalf_", "g6calc_lasthalf2_", "g6_read_neighbour_list_",
+    "g6_get_neighbour_list_",
 ]
 
 ERRORS = {0: "G6_OK", -1: "G6_ERR_NOT_OPEN", -2: "G6_ERR_CLUSTER", -3: "G6_ERR_ADDRESS", -4: "G6_ERR_NI",
@@ -114,6 +124,58 @@ def g6_set_j_particle(clusterid, address, index, tj, dtj, mass, snap_by18, jerk_
 
 def g6_set_ti(clusterid, ti):
     return _chk(lib().g6_set_ti(C.c_int(clusterid), C.c_double(ti)), clusterid)
+
+
+def g6_set_tunit(newtunit):
+    return lib().g6_set_tunit(C.c_int(newtunit))
+
+
+def g6_set_xunit(newxunit):
+    return lib().g6_set_xunit(C.c_int(newxunit))
+
+
+def g6x_get_units():
+    t = C.c_int(0); x = C.c_int(0)
+    lib().g6x_get_units(C.byref(t), C.byref(x))
+    return t.value, x.value
+
+
+def g6_reset(clusterid=0):
+    return _chk(lib().g6_reset(C.c_int(clusterid)), clusterid)
+
+
+def g6_reset_fofpga(clusterid=0):
+    return _chk(lib().g6_reset_fofpga(C.c_int(clusterid)), clusterid)
+
+
+def g6_initialize_jp_buffer(clusterid, buf_size):
+    return _chk(lib().g6_initialize_jp_buffer(C.c_int(clusterid), C.c_int(buf_size)), clusterid)
+
+
+def g6_flush_jp_buffer(clusterid=0):
+    return _chk(lib().g6_flush_jp_buffer(C.c_int(clusterid)), clusterid)
+
+
+def g6_getnjmax(clusterid=0):
+    return _chk(lib().g6_getnjmax(C.c_int(clusterid)), clusterid)
+
+
+def g6_get_j_particle(clusterid, address):
+    """Returns dict(index, tj, mass, jerk_by6[3], acc_by2[3], v[3], x[3]) as stored."""
+    idx = C.c_int(0); tj = C.c_double(0); mass = C.c_double(0)
+    j6 = np.empty(3); a2 = np.empty(3); v = np.empty(3); x = np.empty(3)
+    _chk(lib().g6_get_j_particle(C.c_int(clusterid), C.c_int(address), C.byref(idx), C.byref(tj), C.byref(mass),
+                                 _dp(j6), _dp(a2), _dp(v), _dp(x)), clusterid)
+    return dict(index=idx.value, tj=tj.value, mass=mass.value, jerk_by6=j6, acc_by2=a2, v=v, x=x)
+
+
+def g6x_get_j_particles(clusterid, addr0, n):
+    """Bulk read-back: dict(index[n], tj[n], mass[n], jerk[n,3], acc[n,3], v[n,3], x[n,3]); acc and jerk physical."""
+    o = dict(index=np.empty(n, np.int32), tj=np.empty(n), mass=np.empty(n), jerk=np.empty((n, 3)), acc=np.empty((n, 3)),
+             v=np.empty((n, 3)), x=np.empty((n, 3)))
+    _chk(lib().g6x_get_j_particles(C.c_int(clusterid), C.c_int(addr0), C.c_int(n), _ip(o["index"]), _dp(o["tj"]), _dp(o["mass"]),
+                                   _dp(o["jerk"]), _dp(o["acc"]), _dp(o["v"]), _dp(o["x"])), clusterid)
+    return o
 
 
 def g6calc_firsthalf(clusterid, nj, ni, index, xi, vi, acc_old=None, jerk6_old=None, phi_old=None, eps2=0.0, h2=None):
@@ -255,15 +317,6 @@ def g6x_get_predicted(clusterid, addr0, n):
     return xp, vp
 
 
-def g6x_debug_dx(clusterid, ipipe, jaddr):
-    n = len(ipipe)
-    ipipe = _i32(ipipe, (n,)); jaddr = _i32(jaddr, (n,))
-    dx = np.empty((n, 3), np.float32)
-    _chk(lib().g6x_debug_dx(C.c_int(clusterid), C.c_int(n), _ip(ipipe), _ip(jaddr),
-                            dx.ctypes.data_as(C.POINTER(C.c_float))), clusterid)
-    return dx
-
-
 def g6x_jsplit_pack_dev(clusterid, ni, rank, d_nn_r2, d_nn_index, d_key):
     import torch
     return _chk(lib().g6x_jsplit_pack_dev(C.c_int(clusterid), C.c_int(ni), C.c_int(rank), _dev(d_nn_r2, torch.float64, ni),
@@ -281,16 +334,6 @@ def g6x_jsplit_unpack_dev(clusterid, ni, d_key_min, d_index_sum, d_nn_index, d_n
     return _chk(lib().g6x_jsplit_unpack_dev(C.c_int(clusterid), C.c_int(ni), _dev(d_key_min, torch.int64, ni),
                                             _dev(d_index_sum, torch.float64, ni), _dev(d_nn_index, torch.int32, ni),
                                             _dev(d_nn_r2, torch.float64, ni)), clusterid)
-
-
-def g6x_probe_fp32_peak(clusterid, mode, ctas_per_sm=4):
-    r = C.c_double(0.0)
-    _chk(lib().g6x_probe_fp32_peak(C.c_int(clusterid), C.c_int(mode), C.c_int(ctas_per_sm), C.byref(r)), clusterid)
-    return r.value
-
-
-def g6x_probe_read_jstore(clusterid, nj):
-    return _chk(lib().g6x_probe_read_jstore(C.c_int(clusterid), C.c_int(nj)), clusterid)
 
 
 # ---- convenience (still only calls the functions above) ------------------------------------------

@@ -17,30 +17,55 @@ def library():
     return g6.lib()
 
 
-def _declared():
+HEADERS = sorted(f for f in os.listdir(os.path.join(ROOT, "include")) if f.endswith(".h"))
+
+
+def _declared(headers=None):
     names = []
-    for h in ("g6.h", "g6_hermite.h"):
+    for h in headers or HEADERS:
         text = open(os.path.join(ROOT, "include", h)).read()
         text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
         names += re.findall(r"\b(g6\w*)\s*\(", text)
     return sorted(set(names))
 
 
+def _exported(path):
+    import subprocess
+    out = subprocess.run(["nm", "-D", "--defined-only", path], capture_output=True, text=True, check=True).stdout
+    return sorted(line.split()[-1] for line in out.splitlines() if " T " in line)
+
+
 def test_every_declared_symbol_is_exported(library):
+    assert HEADERS == ["g6.h", "g6_fortran.h", "g6_hermite.h"]
     declared = _declared()
-    assert len(declared) >= 29
+    assert len(declared) >= 60
     for name in declared:
         assert hasattr(library, name), f"{name} declared in include/ but not exported"
     # and the Python binding mirrors the same names
-    assert sorted(set(g6.SYMBOLS)) == declared
-    for name in declared:
+    assert sorted(set(g6.SYMBOLS)) == _declared(["g6.h", "g6_hermite.h"])
+    assert sorted(set(g6.FORTRAN_SYMBOLS)) == _declared(["g6_fortran.h"])
+    for name in g6.SYMBOLS:
         if name.startswith("g6h_") or name.startswith("g6hd_"):
             continue                      # wrapped by the g6.Hermite / g6.HermiteDev classes
         assert hasattr(g6, name), f"binding lacks {name}"
+    # every Fortran alias mirrors a g6.h call of the same name
+    for name in g6.FORTRAN_SYMBOLS:
+        assert name[:-1] in g6.SYMBOLS, name
+
+
+def test_library_exports_only_what_the_headers_declare(library):
+    """No probe, ablation or debug entry point in the product library: its dynamic symbols of the g6 family are exactly
+    the declared ones (the parity-test hook and bench.py's probes are separate libraries)."""
+    exported = [n for n in _exported(g6.LIB_PATH) if n.startswith("g6")]
+    assert exported == _declared()
+    dbg = [n for n in _exported(build.build_debug()) if n.startswith("g6")]
+    assert dbg == ["g6dbg_pair_dx"]
+    probe = [n for n in _exported(build.build_probe()) if n.startswith("g6")]
+    assert probe == ["g6p_fp32_rate", "g6p_pair_rate", "g6p_read_pass"]
 
 
 def test_headers_have_no_torch_or_cxx_types():
-    for h in ("g6.h", "g6_hermite.h"):
+    for h in HEADERS:
         text = open(os.path.join(ROOT, "include", h)).read()
         code = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
         assert 'extern "C"' in code

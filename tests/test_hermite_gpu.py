@@ -83,16 +83,17 @@ def test_c2_short_run_energy_and_block_histogram(cluster, oracle):
     assert dE < 1e-6
 
 
-@pytest.mark.skipif(not __import__("os").environ.get("G6_FULL_C2"), reason="minutes of CPU: set G6_FULL_C2=1 (results recorded in profiles/)")
 def test_c2_full_run_vs_oracle_driven(cluster, oracle):
-    """BASELINE.json config 2 in full: N = 32768, t = 0 -> 1, library-driven and oracle-driven."""
+    """BASELINE.json config 2 in full: N = 32768, eps = 1e-4, eta = 0.01, t = 0 -> 1, driven by the host driver (g6h_*), by the
+    device-resident driver (g6hd_*) and by the oracle (~1e12 fp64 pair evaluations: a few minutes on the GPU box's host cores).
+    north_star: the library-driven energy drift stays within 2x the oracle-driven one."""
     import json, os
     t_end = float(os.environ.get("G6_C2_TEND", "1.0"))
     x, v, m, eps2 = inputs.config("C2")
     eta = 0.01
     E0 = _energy(oracle, x, v, m, eps2)
     rep = {"config": "C2", "n": len(m), "eta": eta, "eps2": eps2, "t_end": t_end, "E0": E0, "oracle_threads": oracle.threads()}
-    for newton in (1, 0):
+    for newton in ((1, 0) if os.environ.get("G6_C2_NEWTON0") else (1,)):
         g6.g6x_set_option(0, "newton", newton)
         t0 = time.perf_counter()
         h = g6.Hermite(0, x, v, m, eps2, eta)

@@ -283,20 +283,45 @@ def test_block_step_cycle_with_j_updates(cluster, oracle, n, ni):
 
 
 # ------------------------------------------------------------------ P11: Eq. 3 bit for bit
-def test_p11_ds_separation_bit_exact(cluster, oracle):
-    x, v, m, eps2 = inputs.config("C5", n=4096)         # offset cluster: lo words matter
-    idx = load_j(x, v, m)
-    g6.g6_set_ti(0, 0.0)
-    g6.force_host(0, idx[:512], x[:512], v[:512], eps2, 4096)
-    rng = np.random.default_rng(3)
-    ip = rng.integers(0, 512, 5000).astype(np.int32); ja = rng.integers(0, 4096, 5000).astype(np.int32)
-    dx = g6.g6x_debug_dx(0, ip, ja)
+def _pair_dx(kernel, xj, index_j, xi, index_i, eps2, ds=1):
+    """Every pair's separation as the PRODUCTION pair code formed it: libg6b200_dbg.so instantiates k_force_fast /
+    the block-step kernel (same headers) with their DBG template flag (csrc/debug/g6_debug_dx.cu)."""
+    import ctypes as C
+    from paper_0902_4463_b200 import build
+    L = C.CDLL(build.build_debug())
+    nj, ni = len(index_j), len(index_i)
+    xj = np.ascontiguousarray(xj, np.float64); xi = np.ascontiguousarray(xi, np.float64)
+    index_j = np.ascontiguousarray(index_j, np.int32); index_i = np.ascontiguousarray(index_i, np.int32)
+    dx = np.empty((ni, nj, 3), np.float32)
+    dp = lambda a: a.ctypes.data_as(C.POINTER(C.c_double)); ip = lambda a: a.ctypes.data_as(C.POINTER(C.c_int))
+    rc = L.g6dbg_pair_dx(C.c_int(kernel), C.c_int(nj), C.c_int(ni), dp(xj), ip(index_j), dp(xi), ip(index_i),
+                         C.c_double(eps2), C.c_int(ds), dx.ctypes.data_as(C.POINTER(C.c_float)))
+    assert rc == 0, rc
+    return dx
+
+
+@pytest.mark.parametrize("kernel,ni", [(2, 700), (3, 37)])
+def test_p11_ds_separation_bit_exact(oracle, kernel, ni):
+    """Eq. 3 as the hot loops form it -- packed lanes of pair2 (sweep kernel: unchecked tiles, the checked
+    tiles that hold the warp's own particles, the ragged last tile) and pair2_checked (block-step kernel) -- equals the
+    binary32 CPU transcription bit for bit, for EVERY (i, j) pair, on the offset cluster where the lo words matter."""
+    nj = 4000                                            # 15 full j-tiles and a ragged one
+    x, v, m, eps2 = inputs.config("C5", n=nj)
+    idx = np.arange(nj, dtype=np.int32)
+    sel = np.sort(np.random.default_rng(3).choice(nj, ni, replace=False))
+    dx = _pair_dx(kernel, x, idx, x[sel], idx[sel], eps2)
+    assert not np.isnan(dx).any()                        # every pair was visited (the buffer starts as NaN)
     for k in range(3):
-        ih, il = oracle.ds_split(x[ip, k]); jh, jl = oracle.ds_split(x[ja, k])
-        want = oracle.ds_diff(jh, jl, ih, il)
-        assert np.array_equal(dx[:, k].view(np.uint32), want.view(np.uint32))
-        exact = x[ja, k] - x[ip, k]
-        assert np.all(np.abs(dx[:, k] - exact) <= 3 * 2.0**-24 * np.abs(exact) + 2.0**-47 * 1001.0)
+        ih, il = oracle.ds_split(x[sel, k]); jh, jl = oracle.ds_split(x[:, k])
+        want = oracle.ds_diff(np.broadcast_to(jh, (ni, nj)).ravel(), np.broadcast_to(jl, (ni, nj)).ravel(),
+                              np.repeat(ih, nj), np.repeat(il, nj)).reshape(ni, nj)
+        assert np.array_equal(dx[:, :, k].view(np.uint32), want.view(np.uint32))
+        exact = x[None, :, k] - x[sel, None, k]
+        assert np.all(np.abs(dx[:, :, k] - exact) <= 3 * 2.0**-24 * np.abs(exact) + 2.0**-47 * 1001.0)
+    # pure FP32 (lo words dropped): the separation is the single rounded difference of the hi words
+    d0 = _pair_dx(kernel, x, idx, x[sel], idx[sel], eps2, ds=0)
+    ih, _ = oracle.ds_split(x[sel, 0]); jh, _ = oracle.ds_split(x[:, 0])
+    assert np.array_equal(d0[:, :, 0], (jh[None, :] - ih[:, None]).astype(np.float32))
 
 
 # ------------------------------------------------------------------ C5: double-single vs pure FP32
