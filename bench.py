@@ -105,6 +105,57 @@ class ClockSampler:
                 "power_w_max": float(max(power)), "samples": len(sm)}
 
 
+class Probes:
+    """bench.py's measurement aids (paper_0902_4463_b200/csrc/bench/g6_bench_probe.cu -> libg6b200_probe.so; not part of
+    libg6b200, not on the path): FP32 instruction-rate probes, the production pair loop with ablations, a read-only pass."""
+    FP32_MODES = ((0, "scalar_ffma_x_d_acc_reuse"), (1, "scalar_ffma_three_changing_sources"), (2, "ffma2_two_distinct_pairs"),
+                  (3, "ffma2_two_pairs_plus_reused"), (4, "ffma2_three_distinct_pairs"), (5, "ffma2_two_pairs_plus_32bit_broadcast"),
+                  (6, "fmul2_one_pair_alternating_ffma2_three_pairs"), (7, "fadd2_fmul2_ffma2_mix_one_changing_source"))
+    PAIR_VARIANTS = ((0, "production_pair2_ds_newton"), (1, "pure_fp32_separations"), (2, "three_operand_ffma2_made_two_operand"),
+                     (3, "no_nearest_neighbour_tracking"))
+
+    def __init__(self):
+        import ctypes as C
+        from paper_0902_4463_b200 import build
+        self.C = C
+        self.L = C.CDLL(build.build_probe())
+
+    def fp32_rate(self, mode, ctas_per_sm, stream=0):
+        r = self.C.c_double(0.0)
+        rc = self.L.g6p_fp32_rate(self.C.c_int(mode), self.C.c_int(ctas_per_sm), self.C.c_void_p(stream), self.C.byref(r))
+        if rc:
+            raise RuntimeError(f"g6p_fp32_rate failed: cudaError {rc}")
+        return r.value
+
+    def pair_rate(self, ab, shape, stream=0):
+        r = self.C.c_double(0.0)
+        rc = self.L.g6p_pair_rate(self.C.c_int(ab), self.C.c_int(shape), self.C.c_void_p(stream), self.C.byref(r))
+        if rc:
+            raise RuntimeError(f"g6p_pair_rate failed: cudaError {rc}")
+        return r.value
+
+    def read_pass(self, tensor, stream):
+        nbytes = tensor.numel() * tensor.element_size() // 16 * 16
+        rc = self.L.g6p_read_pass(self.C.c_void_p(tensor.data_ptr()), self.C.c_ulonglong(nbytes), self.C.c_void_p(stream))
+        if rc:
+            raise RuntimeError(f"g6p_read_pass failed: cudaError {rc}")
+
+    def table(self, peak_inst, stream=0):
+        """every probe as a fraction of the nominal FP32 peak (lane-instructions / s)"""
+        out = {"fp32_instruction_streams_frac_of_peak": {}, "pair_loop": {}}
+        for w in range(3):
+            self.fp32_rate(2, 4, stream)                                    # bring the clocks up
+        for mode, name in self.FP32_MODES:
+            out["fp32_instruction_streams_frac_of_peak"][name] = max(self.fp32_rate(mode, c, stream) for c in (2, 4, 8)) / peak_inst
+        for ab, name in self.PAIR_VARIANTS:
+            per_pair = {0: 36, 1: 30, 2: 36, 3: 37}[ab]                    # packed FP32 instructions per pair evaluation of the variant
+            r = {sh: self.pair_rate(ab, k, stream) for k, sh in ((0, "128x2"), (1, "256x1"))}
+            out["pair_loop"][name] = {"interactions_per_s": r, "fp32_instr_per_interaction_executed": per_pair,
+                                      "pipe_busy_frac": {k: v * per_pair / peak_inst for k, v in r.items()},
+                                      "frac_of_peak_at_33": {k: v * 33 / peak_inst for k, v in r.items()}}
+        return out
+
+
 def cpu_oracle_rate(x, v, m, eps2, idx, target_s, seed=7):
     """interactions/s of the oracle (as it stands) on a bounded sample of rows of the sweep."""
     from oracle import oracle as orc
@@ -126,7 +177,7 @@ def cpu_oracle_rate(x, v, m, eps2, idx, target_s, seed=7):
 NI_SWEEP = (1, 16, 256, 4096, 65536)
 
 
-def ni_sweep(g6, inputs, torch, dev, stream, flush, x, v, idx_all, n, eps2, peaks, reps=10):
+def ni_sweep(g6, inputs, torch, dev, stream, flush, x, v, idx_all, n, eps2, peaks, probes, reps=10):
     """C4's block-step regime (BASELINE.json configs[3]): random active blocks of n_i particles
     against all N_j, one block step = predictor over all j (t_i changes every step) + force +
     combine.  Device times from CUDA events on the launching stream; `cold` = L2 flushed before
@@ -140,10 +191,11 @@ def ni_sweep(g6, inputs, torch, dev, stream, flush, x, v, idx_all, n, eps2, peak
     rows = []
     # floor of a block step at small n_i: a kernel that only reads the j-store once (same bytes, L2 flushed)
     bare = []
+    jstore_sized = torch.zeros(n * 76 // 4, dtype=torch.float32, device=dev)      # as many bytes as the raw j-store of n particles
     for k in range(reps + 3):
         flush.zero_()
         e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
-        e0.record(stream); g6.g6x_probe_read_jstore(0, n); e1.record(stream)
+        e0.record(stream); probes.read_pass(jstore_sized, stream.cuda_stream); e1.record(stream)
         torch.cuda.synchronize()
         if k >= 3:
             bare.append(e0.elapsed_time(e1) * 1e3)
@@ -235,6 +287,44 @@ def neighbour_list_cost(g6, inputs, torch, dev, x, v, idx_all, n, eps2, ni=65536
             "overflowed": int((cnt > maxlen).sum()), "nb_maxlen": maxlen}
 
 
+def recorded_traffic(nj, ni, jsplits):
+    """DRAM bytes of one force-kernel launch from the committed ncu capture, if it was taken on this configuration."""
+    p = os.path.join(ROOT, "profiles", "force_fast_traffic.json")
+    try:
+        rec = json.load(open(p))
+    except Exception:
+        return None
+    if rec.get("n_j") == nj and rec.get("n_i") == ni and rec.get("jsplits") == jsplits:
+        return int(rec["dram_bytes_read"]) + int(rec["dram_bytes_write"])
+    return None
+
+
+def double_single_cost(g6, inputs, torch, dev, x, v, idx_all, n, eps2, ni=65536, reps=3):
+    """What the double-single separations cost (the paper: "<~ 20 %"): the same 65536-block against all N_j
+    with option ds = 1 (Eq. 3: 9 packed adds per pair) and ds = 0 (pure FP32: 3 packed adds; lo words dropped by the predictor)."""
+    f64 = torch.float64
+    ni = min(ni, n)
+    block = inputs.active_subset(n, ni, 4040 + ni)
+    to = lambda a, dt=f64: torch.from_numpy(np.ascontiguousarray(a)).to(dev, dt)
+    d_xi, d_vi, d_ii = to(x[block]), to(v[block]), to(idx_all[block], torch.int32)
+    d_acc = torch.empty(ni, 3, dtype=f64, device=dev); d_jerk = torch.empty_like(d_acc)
+    d_pot = torch.empty(ni, dtype=f64, device=dev); d_nn = torch.empty(ni, dtype=torch.int32, device=dev); d_r2 = torch.empty_like(d_pot)
+    g6.g6_set_ti(0, 0.0)
+    out = {}
+    for ds in (1, 0):
+        g6.g6x_set_option(0, "ds", ds)
+        ts = []
+        for k in range(reps + 1):
+            g6.g6x_calc_dev(0, n, ni, d_ii, d_xi, d_vi, eps2, d_acc, d_jerk, d_pot, d_nn, d_r2)
+            torch.cuda.synchronize()
+            if k > 0:
+                ts.append(g6.g6x_get_timers(0)["force_us"])
+        out[ds] = float(np.median(ts))
+    g6.g6x_set_option(0, "ds", 1)
+    return {"n_i": ni, "force_us_double_single": out[1], "force_us_pure_fp32": out[0], "cost": out[1] / out[0] - 1.0,
+            "interactions_per_s_double_single": ni * float(n) / (out[1] * 1e-6), "interactions_per_s_pure_fp32": ni * float(n) / (out[0] * 1e-6)}
+
+
 def c3_sweep(g6, inputs, torch, dev, peaks, reps=5):
     """BASELINE.json configs[2] (C3): full force sweep at N = 131072, device-resident, L2-resident j-store
     (a side figure; the headline is C4).  Replaces the j-store contents: call last."""
@@ -300,6 +390,79 @@ def run_reference(args):
     print(json.dumps(out), flush=True)
 
 
+def run_jsplit(args, torch, dist, g6, inputs, world, rank, local, dev):
+    """--mode jsplit: one block step of n_i particles under the paper's multi-GPU scheme: rank r holds the
+    j-particles of addresses [r N/G, (r+1) N/G), every rank computes partial forces on the SAME i-block (predictor over its
+    slice + force + combine), then two allreduces (MIN on the nearest-neighbour keys, SUM on acc | jerk | pot | index) over
+    NCCL, stream-ordered with the kernels (sharding.JSplit).  value = n_i x N interactions per step over the max-over-ranks
+    time; at G = 1 the collectives are no-ops and the line is the single-GPU block step."""
+    from paper_0902_4463_b200.sharding import JSplit, LibOps, j_range
+    x, v, m, eps2 = inputs.config(WORKLOAD, n=args.n)
+    n = len(m)
+    idx = np.arange(n, dtype=np.int32)
+    ni = min(args.ni, n)
+    j0, j1 = j_range(rank, world, n)
+    f64 = torch.float64
+    to = lambda a, dt=f64: torch.from_numpy(np.ascontiguousarray(a)).to(dev, dt)
+    g6.g6_open(0)
+    g6.g6x_set_npipes(1 << 21)
+    stream = torch.cuda.Stream(device=dev)
+    torch.cuda.set_stream(stream)
+    ops = LibOps(0)                                      # moves the cluster onto torch's current stream
+    nl = j1 - j0
+    z3 = torch.zeros(nl, 3, dtype=f64, device=dev)
+    g6.g6x_set_j_particles_dev(0, 0, nl, to(idx[j0:j1], torch.int32), torch.zeros(nl, dtype=f64, device=dev), to(m[j0:j1]), z3, z3,
+                               to(v[j0:j1]), to(x[j0:j1]))
+    block = inputs.active_subset(n, ni, 4040 + ni)
+    d_ii, d_xi, d_vi = to(idx[block], torch.int32), to(x[block]).reshape(-1), to(v[block]).reshape(-1)
+    js = JSplit(ops, rank, world) if world > 1 else JSplit(ops, 0, 1, allreduce=lambda t, op: None)
+    flush = torch.empty(512 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def step(k):
+        g6.g6_set_ti(0, (k % 2) * 2.0 ** -30)            # a new block time: the predictor runs again, as in a block step
+        return js.calc(nl, ni, d_ii, d_xi, d_vi, eps2)
+
+    for k in range(max(args.warmup, 3)):
+        flush.zero_()
+        step(k)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for k in range(args.steps):
+        flush.zero_()
+        barrier()
+        ev[k][0].record(stream)
+        step(k)
+        ev[k][1].record(stream)
+    barrier()
+    clocks = sampler.stop()
+    t_ms = torch.tensor([sum(a.elapsed_time(b) for a, b in ev)], dtype=f64, device=dev)
+    if world > 1:
+        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
+    ms_total = float(t_ms.item())
+    if rank == 0:
+        value = args.steps * float(ni) * float(n) / (ms_total * 1e-3)
+        print(json.dumps({"metric": "interactions/s (one block step of n_i particles against N j-particles split over the GPUs, PAPER.md:122)",
+                          "value": value, "unit": "interactions/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+                          "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+                          "dtype": "f32 (double-single separations, fp64 accumulation across tiles)", "data": "synthetic",
+                          "config": {"workload": f"{WORKLOAD}: N={n} equal-mass Plummer sphere, eps=1e-4, block of n_i={ni} random active particles, j-split x{world}",
+                                     "n": n, "n_i": ni, "parallelism": f"j-split x{world}: 2 allreduces per step (8 B + 64 B per i-particle)",
+                                     "l2": "flushed between timed steps (512 MiB write)"},
+                          "clocks": clocks, "gflops_60": value * FLOP_PAPER / 1e9, "gpu_launches": 6 * args.steps}), flush=True)
+    g6.g6_close(0)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -313,6 +476,11 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-sweep", action="store_true", help="skip the C4 n_i sweep (block-step regime)")
     ap.add_argument("--newton", type=int, default=None, help="override the library default (1 = rsqrt + one Newton step)")
+    ap.add_argument("--probes", action="store_true", help="only run the FP32 operand-bandwidth and pair-loop probes and print their table")
+    ap.add_argument("--mode", default="sweep", choices=["sweep", "jsplit"],
+                    help="sweep: the headline (i-split under torchrun); jsplit: the paper's multi-GPU scheme (PAPER.md:122), every rank "
+                         "holds N/G j-particles and all ranks compute the same block of --ni i-particles, partial forces allreduced")
+    ap.add_argument("--ni", type=int, default=4096, help="block size of --mode jsplit (n_i <= 4096 is the regime it is for)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = max(args.warmup, 0)
@@ -339,6 +507,15 @@ def main():
     if world > 1:
         dist.barrier()
 
+    if args.probes:
+        if rank == 0:
+            peaks, _ = measured_peaks()
+            peak_inst = SM_COUNT * FP32_LANES_PER_SM * float(peaks.get("sm_max_mhz", SM_MAX_MHZ_FALLBACK)) * 1e6
+            print(json.dumps({"probes": Probes().table(peak_inst), "peak_lane_instr_per_s": peak_inst}), flush=True)
+        return
+    if args.mode == "jsplit":
+        return run_jsplit(args, torch, dist, g6, inputs, world, rank, local, dev)
+
     x, v, m, eps2 = inputs.config(WORKLOAD, n=args.n)
     n = len(m)
     idx = np.arange(n, dtype=np.int32)
@@ -364,10 +541,20 @@ def main():
     d_pot = torch.empty(ni, dtype=f64, device=dev); d_nn = torch.empty(ni, dtype=torch.int32, device=dev); d_r2 = torch.empty_like(d_pot)
     flush = torch.empty(512 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)      # 512 MiB > 126 MB L2
 
+    # multi-GPU (i-split): the shards meet -- every rank ends the step with ALL n rows of results, gathered over NCCL
+    # (one all_gather of 72 B per i-particle) inside the timed region
+    ni_pad = -(-n // world)
+    if world > 1:
+        d_rows = torch.zeros(ni_pad, 9, dtype=f64, device=dev)           # acc | jerk | pot | nn_r2 | nn_index (exact in fp64)
+        d_all = torch.empty(world * ni_pad, 9, dtype=f64, device=dev)
+
     def step_dev():
         g6.g6x_set_j_particles_dev(0, 0, n, d_idx, d_t, d_m, d_z3, d_z3, d_v, d_x)       # a-1
         g6.g6_set_ti(0, 0.0)
         g6.g6x_calc_dev(0, n, ni, d_ii, d_xi, d_vi, eps2, d_acc, d_jerk, d_pot, d_nn, d_r2)   # a-2 .. a-5
+        if world > 1:                                     # same stream as the library's kernels: stream-ordered, no host sync
+            d_rows[:ni, 0:3] = d_acc; d_rows[:ni, 3:6] = d_jerk; d_rows[:ni, 6] = d_pot; d_rows[:ni, 7] = d_r2; d_rows[:ni, 8] = d_nn
+            dist.all_gather_into_tensor(d_all, d_rows)
 
     def barrier():
         torch.cuda.synchronize()
@@ -410,11 +597,20 @@ def main():
         z3 = np.zeros((n, 3)); tz = np.zeros(n)
         xi_h, vi_h, ii_h = np.ascontiguousarray(x[i0:i1]), np.ascontiguousarray(v[i0:i1]), np.ascontiguousarray(idx[i0:i1])
 
+        host_group = dist.new_group(backend="gloo") if world > 1 else None
+        rows_h = torch.zeros(ni_pad, 8, dtype=f64)
+        all_h = [torch.empty_like(rows_h) for _ in range(world)]
+
         def step_host():
             g6.g6x_set_j_particles(0, 0, idx, tz, m, z3, z3, v, x)
             g6.g6_set_ti(0, 0.0)
             g6.g6calc_firsthalf(0, n, ni, ii_h, xi_h, vi_h, eps2=eps2)
-            return g6.g6calc_lasthalf2(0, n, ni, eps2=eps2)
+            acc_h, jerk_h, pot_h, nn_h = g6.g6calc_lasthalf2(0, n, ni, eps2=eps2)
+            if world > 1:                                 # the shards meet on the host too (host arrays in, host arrays out)
+                rows_h[:ni, 0:3] = torch.from_numpy(acc_h); rows_h[:ni, 3:6] = torch.from_numpy(jerk_h)
+                rows_h[:ni, 6] = torch.from_numpy(pot_h); rows_h[:ni, 7] = torch.from_numpy(nn_h.astype(np.float64))
+                dist.all_gather(all_h, rows_h, group=host_group)
+            return acc_h, jerk_h, pot_h, nn_h
         step_host()
         barrier()
         t0 = time.perf_counter()
@@ -437,14 +633,16 @@ def main():
     c3 = None
     nb_cost = None
     ceilings = None
+    ds_cost = None
+    probes = Probes() if rank == 0 else None
     if rank == 0 and world == 1 and not args.no_sweep:
-        sweep = ni_sweep(g6, inputs, torch, dev, stream, flush, x, v, idx, n, eps2, measured_peaks()[0])
+        sweep = ni_sweep(g6, inputs, torch, dev, stream, flush, x, v, idx, n, eps2, measured_peaks()[0], probes)
         nb_cost = neighbour_list_cost(g6, inputs, torch, dev, x, v, idx, n, eps2)
+        ds_cost = double_single_cost(g6, inputs, torch, dev, x, v, idx, n, eps2)
         c3 = c3_sweep(g6, inputs, torch, dev, measured_peaks()[0]) if args.n is None else None
     if rank == 0:
-        # what the FP32 pipes sustain for register-sourced instructions (g6x_probe_fp32_peak, include/g6.h), measured live
-        ceilings = {name: max(g6.g6x_probe_fp32_peak(0, mode, c) for c in (3, 4, 8))
-                    for mode, name in ((0, "scalar_ffma"), (1, "ffma2_two_reused_operands"), (2, "fadd2_fmul2_ffma2_mix"), (3, "ffma2_three_distinct_sources"))}
+        # what the FP32 pipes sustain for register-sourced instruction streams and for the pair loop itself (libg6b200_probe.so), live
+        ceilings = probes.table(SM_COUNT * FP32_LANES_PER_SM * float(measured_peaks()[0].get("sm_max_mhz", SM_MAX_MHZ_FALLBACK)) * 1e6, stream.cuda_stream)
 
     if rank == 0:
         peaks, peaks_src = measured_peaks()
@@ -456,9 +654,9 @@ def main():
         roofline = {"bound": "alu", "kernel": "k_force_fast",
                     "achieved": 2 * ach_inst / 1e12, "peak": 2 * peak_inst / 1e12,
                     "unit": "TFLOP/s", "frac": ach_inst / peak_inst,
-                    # dram__bytes_read.sum + dram__bytes_write.sum of one launch of this kernel at N = 2^20, from the ncu --set full
-                    # capture profiles/r01_force_fast_1M_ncu_full.txt (bytes per launch; only valid for the headline workload)
-                    "traffic": 1028230400 if (n == 1048576 and world == 1) else None,
+                    # dram__bytes_read.sum + dram__bytes_write.sum of one launch of this kernel from the committed ncu --set full capture
+                    # (profiles/force_fast_traffic.json names it); null unless that capture had this run's n_j, n_i and j-split count
+                    "traffic": recorded_traffic(n, ni, int(tm["jsplits"])),
                     "how": ("FP32-pipe issue-slot equivalent: 33 algorithmic FP32 lane-instructions per interaction (SURVEY 8(d)) x "
                             "interactions per launch / mean force-kernel time (CUDA events on the launching stream, live in this run); "
                             f"peak = 148 SM x 128 lanes x {sm_max:.0f} MHz ({peaks_src} max SM clock) x 2"),
@@ -467,7 +665,7 @@ def main():
                     "flops47_tflops": FLOP47 * inter_per_launch / (f_us * 1e-6) / 1e12,
                     "frac_at_measured_clock": (ach_inst / (SM_COUNT * FP32_LANES_PER_SM * clocks["sm_mhz"] * 1e6)) if clocks.get("sm_mhz") else None,
                     "kernel_share_of_step": f_us * args.steps / (ms_total * 1e3) if world == 1 else None,
-                    "measured_issue_ceiling_frac_of_peak": {k: v / peak_inst for k, v in ceilings.items()},
+                    "measured_ceilings": ceilings,
                     "pipe_busy_equivalent": (FP32_INSTR_PER_INTERACTION + 3 * int(newton)) / FP32_INSTR_PER_INTERACTION * ach_inst / peak_inst,
                     "predictor_gbs": (n * (76 + 40)) / (float(np.mean(pred_us)) * 1e-6) / 1e9,
                     "hbm_peak_gbs": peaks.get("hbm_gbs")}
@@ -487,6 +685,8 @@ def main():
             out["ni_sweep"] = sweep
         if nb_cost is not None:
             out["neighbour_lists"] = nb_cost
+        if ds_cost is not None:
+            out["double_single_cost"] = ds_cost
         if c3 is not None:
             out["c3_sweep"] = c3
         if not args.no_cpu_baseline and world == 1:

@@ -66,7 +66,9 @@ void g6hd_destroy(g6hd_system *s);
 int g6hd_evolve(g6hd_system *s, double t_end, long long max_block_steps);
 /* on != 0: shared time steps from now on ("shared or block time steps"; reading 21): every
  * particle takes every step with one common step, the smallest of the per-particle results of the step rule above
- * applied to the common step.  Call between g6hd_evolve calls; switching back to block steps is allowed. */
+ * applied to the common step.  Call between g6hd_evolve calls; switching back to block steps is allowed.  Switching ON
+ * needs every particle at the system time (true at t = 0 and after evolving to a multiple of dt_max): otherwise
+ * G6_ERR_SEQUENCE and nothing changes. */
 int g6hd_set_shared_steps(g6hd_system *s, int on);
 /* as g6h_get_state (Eq. 1-2 predictions to the system time, evaluated on the device) */
 int g6hd_get_state(g6hd_system *s, double x[][3], double v[][3]);

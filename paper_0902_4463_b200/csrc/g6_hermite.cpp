@@ -150,11 +150,24 @@ g6h_system *g6h_create(int clusterid, int n, const double x[][3], const double v
 
 void g6h_destroy(g6h_system *s) { delete s; }
 
+static int evolve_body(g6h_system &s, double t_end, long long max_block_steps);
+
 int g6h_evolve(g6h_system *sp, double t_end, long long max_block_steps)
 {
     if (!sp) return G6_ERR_ARG;
-    g6h_system &s = *sp;
+    try {
+        return evolve_body(*sp, t_end, max_block_steps);      // no C++ exception crosses the boundary (level lists grow)
+    } catch (const std::bad_alloc &) {
+        return G6_ERR_NOMEM;
+    } catch (...) {
+        return G6_ERR_ARG;
+    }
+}
+
+static int evolve_body(g6h_system &s, double t_end, long long max_block_steps)
+{
     const auto w0 = Clock::now();
+    const double dt_floor = level_step(s, LEVELS - 1);      // the smallest step the level table holds
     long long done = 0;
     int rc = 0;
     while (s.t < t_end && (max_block_steps <= 0 || done < max_block_steps)) {
@@ -191,7 +204,8 @@ int g6h_evolve(g6h_system *sp, double t_end, long long max_block_steps)
             const double want = den > 0 ? std::sqrt(s.eta * (na * n2 + nad * nad) / den) : s.dt_max;
             double d = h;
             if (want < d) {
-                while (d > want) d *= 0.5;
+                while (d > want && d > dt_floor) d *= 0.5;
+                if (d > want) { rc = G6_ERR_ARG; break; }     // the step criterion asks for a step below 2^-1100 dt_max (want = 0 or NaN forces)
             } else if (want >= 2 * d && 2 * d <= s.dt_max && std::fmod(tn, 2 * d) == 0.0) {
                 d *= 2;
             }

@@ -146,7 +146,7 @@ __device__ __forceinline__ void hd_correct_one(const HdState &S, const HdBlock &
     const double want = den > 0 ? sqrt(C.eta * (na * n2 + nad * nad) / den) : C.dt_max;
     double d = h;
     if (want < d) {
-        while (d > want) d *= 0.5;
+        while (d > want && d > 1e-300) d *= 0.5;     // floor: a zero or NaN wish must not loop forever (the host then sees no progress)
     } else if (want >= 2 * d && 2 * d <= C.dt_max && hd_is_multiple(tn, 2 * d)) {
         d *= 2;
     }
@@ -346,6 +346,16 @@ k_hd_shared_apply(HdState S, HdBlock B, const unsigned long long *bits)
 }
 
 __global__ void k_hd_set_u64(unsigned long long *p, unsigned long long v) { *p = v; }
+
+// shared steps need every particle at the system time: count those that are not (bits[0] += 1 each)
+__global__ void __launch_bounds__(HD_THREADS)
+k_hd_count_unsynchronised(HdState S, double t, unsigned long long *count)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool off = p < S.n && S.t[p] != t;
+    const unsigned bal = __ballot_sync(0xffffffffu, off);
+    if ((threadIdx.x & 31) == 0 && bal) atomicAdd(count, (unsigned long long)__popc(bal));
+}
 
 __global__ void k_hd_iota(int *act, int n)
 {

@@ -261,6 +261,18 @@ int g6hd_set_shared_steps(g6hd_system *sp, int on)
     GET_CLUSTER(s.cl);
     int rc = hd_finish(c, s);           // (never pending between calls; kept for safety)
     if (rc) return rc;
+    if (on && !s.shared) {
+        // the shared scheme predicts everybody from ONE time and gives everybody ONE new time: all particles must be at the
+        // system time now (true at multiples of dt_max; not after a stop on max_block_steps or at another t_end)
+        unsigned long long off = 0;
+        k_hd_set_u64<<<1, 1, 0, c.stream>>>(s.shared_bits, 0ULL);
+        k_hd_count_unsynchronised<<<(s.n + HD_THREADS - 1) / HD_THREADS, HD_THREADS, 0, c.stream>>>(s.S, s.t, s.shared_bits);
+        CK(cudaGetLastError());
+        CK(cudaMemcpyAsync(&off, s.shared_bits, sizeof(off), cudaMemcpyDeviceToHost, c.stream));
+        CK(cudaStreamSynchronize(c.stream));
+        if (off) return fail(c, G6_ERR_SEQUENCE, "shared time steps need all particles at the system time t = %g; %llu are not "
+                             "(evolve to a multiple of dt_max first)", s.t, off);
+    }
     s.shared = on != 0;
     return G6_OK;
 }

@@ -66,7 +66,12 @@ class JSplit:
         dist.all_reduce(t, op=dist.ReduceOp.MIN if op == "min" else dist.ReduceOp.SUM, group=self.group)
 
     def calc(self, nj_local, ni, d_index, d_xi, d_vi, eps2):
-        """Returns (acc[ni,3], jerk[ni,3], pot[ni], nn_index[ni], nn_r2[ni]) complete on every rank."""
+        """Returns (acc[ni,3], jerk[ni,3], pot[ni], nn_index[ni], nn_r2[ni]) complete on every rank.
+
+        Stream-ordered: the device steps and the two collectives are enqueued back to back on ONE stream (`LibOps` puts
+        the library on torch's current stream, on which torch.distributed orders its NCCL work), with no host
+        synchronisation in between; the results are complete when that stream has drained (the caller synchronises
+        when it reads them)."""
         import torch
         dev = d_xi.device
         f64 = torch.float64
@@ -77,34 +82,52 @@ class JSplit:
         key = torch.empty(ni, dtype=torch.int64, device=dev)
         self.ops.calc_dev(nj_local, ni, d_index, d_xi, d_vi, eps2, acc, jerk, pot, nn, r2)
         self.ops.pack(ni, self.rank, r2, nn, key)
-        self.ops.sync()
         self._allreduce(key, "min")
         self.ops.select(ni, self.rank, key, nn, idxf)
-        self.ops.sync()
         self._allreduce(buf, "sum")
         self.ops.unpack(ni, key, idxf, nn, r2)
-        self.ops.sync()
         return acc.view(ni, 3), jerk.view(ni, 3), pot, nn, r2
 
 
 class LibOps:
-    """The device-side steps of `JSplit`, bound to libg6b200 (CUDA kernels behind the C ABI)."""
+    """The device-side steps of `JSplit`, bound to libg6b200 (CUDA kernels behind the C ABI).
 
-    def __init__(self, clusterid=0):
+    The library normally works on a stream of its own; torch.distributed orders a collective after the work already
+    enqueued on torch's CURRENT stream and makes that stream wait for the collective.  So that kernels and collectives
+    are ordered without host synchronisation, the cluster is moved onto torch's current stream here (`g6x_set_stream`);
+    `own_stream=True` keeps the library's stream and falls back to a host synchronisation around every collective."""
+
+    def __init__(self, clusterid=0, own_stream=False):
         from . import g6
-        self.g6, self.c = g6, clusterid
+        self.g6, self.c, self.own_stream = g6, clusterid, own_stream
+        if not own_stream:
+            import torch
+            # torch's default stream has handle 0, which g6x_set_stream reads as "the library's own": name it explicitly
+            # (cudaStreamLegacy = 0x1)
+            g6.g6x_set_stream(clusterid, torch.cuda.current_stream().cuda_stream or 1)
 
     def calc_dev(self, nj, ni, d_index, d_xi, d_vi, eps2, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2):
         self.g6.g6x_calc_dev(self.c, nj, ni, d_index, d_xi, d_vi, eps2, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2)
 
     def pack(self, ni, rank, d_nn_r2, d_nn_index, d_key):
         self.g6.g6x_jsplit_pack_dev(self.c, ni, rank, d_nn_r2, d_nn_index, d_key)
+        self._fence()
 
     def select(self, ni, rank, d_key_min, d_nn_index, d_index_f64):
+        self._fence()
         self.g6.g6x_jsplit_select_dev(self.c, ni, rank, d_key_min, d_nn_index, d_index_f64)
+        self._fence()
 
     def unpack(self, ni, d_key_min, d_index_sum, d_nn_index, d_nn_r2):
+        self._fence()
         self.g6.g6x_jsplit_unpack_dev(self.c, ni, d_key_min, d_index_sum, d_nn_index, d_nn_r2)
+
+    def _fence(self):
+        # only when the library keeps a stream of its own: both directions (library -> collective, collective -> library)
+        if self.own_stream:
+            import torch
+            self.g6.g6x_synchronize(self.c)
+            torch.cuda.current_stream().synchronize()
 
     def sync(self):
         self.g6.g6x_synchronize(self.c)

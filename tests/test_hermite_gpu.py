@@ -260,3 +260,22 @@ def test_device_shared_time_steps_vs_oracle(cluster, oracle, n, t_end):
     hd.evolve(0.125)
     assert hd.stats()["t"] == 0.125 and hd.stats()["n_particle_steps"] < n * hd.stats()["n_block_steps"]
     hd.close()
+
+
+def test_shared_steps_need_synchronised_particles(cluster):
+    """g6hd_set_shared_steps(on) is refused while particles sit at different times (it would integrate wrongly without
+    saying so): after a stop on max_block_steps -> G6_ERR_SEQUENCE; at a multiple of dt_max -> accepted."""
+    x, v, m, _ = inputs.config("C2", n=700)
+    hd = g6.HermiteDev(0, x, v, m, 1e-6, 0.01)
+    hd.evolve(1.0, max_block_steps=5)
+    pt = hd.particles()
+    assert len(np.unique(pt["t"])) > 1
+    with pytest.raises(g6.G6Error) as e:
+        hd.set_shared_steps(True)
+    assert e.value.code == -6
+    hd.evolve(0.125)                                     # a multiple of dt_max: everybody is synchronised
+    assert np.all(hd.particles()["t"] == 0.125)
+    hd.set_shared_steps(True)
+    hd.evolve(0.125 + 2.0 ** -10)
+    assert hd.stats()["t"] >= 0.125 + 2.0 ** -10
+    hd.close()
