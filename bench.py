@@ -148,7 +148,7 @@ class Probes:
         for mode, name in self.FP32_MODES:
             out["fp32_instruction_streams_frac_of_peak"][name] = max(self.fp32_rate(mode, c, stream) for c in (2, 4, 8)) / peak_inst
         for ab, name in self.PAIR_VARIANTS:
-            per_pair = {0: 36, 1: 30, 2: 36, 3: 37}[ab]                    # packed FP32 instructions per pair evaluation of the variant
+            per_pair = {0: 36, 1: 30, 2: 37, 3: 36.5}[ab]                  # packed FP32 instructions per pair evaluation of the variant (counted in its SASS)
             r = {sh: self.pair_rate(ab, k, stream) for k, sh in ((0, "128x2"), (1, "256x1"))}
             out["pair_loop"][name] = {"interactions_per_s": r, "fp32_instr_per_interaction_executed": per_pair,
                                       "pipe_busy_frac": {k: v * per_pair / peak_inst for k, v in r.items()},

@@ -87,7 +87,7 @@ __device__ __forceinline__ void probe_pair2(IPart &I, const float2 xh, const flo
     const float2 u = fma2(make_float2(-s2.x, -s2.y), mul2(rinv, rinv), dup(3.0f));
     rinv = mul2(rinv, u);
     const float2 rinv2 = mul2(rinv, rinv), mrinv = mul2(m, rinv), mrinv3 = mul2(mrinv, rinv2);
-    const float2 rv = add2(fma2(dz, dz, fma2(dy, dy, mul2(dx, dvx))), mul2(dvy, dvz));      // same count, fewer distinct operands
+    const float2 rv = add2(fma2(dz, dz, fma2(dy, dy, mul2(dx, dvx))), mul2(dvy, dvz));      // one instruction more (37 per pair evaluation), two-operand reads
     const float2 w = mul2(rv, rinv2);
     const float2 alpha = make_float2(-w.x, -w.y);
     I.p = add2(I.p, mrinv);
