@@ -4,6 +4,7 @@
 #pragma once
 #include "../../include/g6_hermite.h"
 #include "g6_hermite_dev.cuh"
+#include "g6_hermite_loop.cuh"
 
 #include <atomic>
 #include <chrono>
@@ -27,7 +28,22 @@ struct g6hd_system {
     bool profile = false;
     cudaEvent_t pe[4] = {};
     double phase_us[3][64] = {};
+    // the block-step loop on the device (g6_hermite_loop.cuh): env G6_HD_LOOP = 0 switches it off (one host wait per block step
+    // instead), env G6_HD_LOOP_MAXI = largest block stepped inside the loop (default HD_LOOP_MAXI_DEFAULT, at most HL_MAX_I)
+    bool loop = false;
+    int loop_max_i = 0, loop_G = 0, loop_K = 0;
+    double *tile_min = nullptr;
+    int *tile_cnt = nullptr;
+    unsigned int *bar = nullptr;
+    HlStatus *h_status = nullptr, *hd_status = nullptr;        // mapped host memory and its device view
+    long long loop_launches = 0, loop_steps = 0;
+    double loop_us[64] = {}, big_us[64] = {}, relaunch_us = 0;    // env G6_HD_LOOP_PROFILE: where the time of a run goes, by block size
+    long long big_n[64] = {};
+    double phase_us_loop[8] = {};
+    bool loop_profile = false;
 };
+
+constexpr int HD_LOOP_MAXI_DEFAULT = 1024;
 
 namespace {
 
@@ -38,6 +54,8 @@ void hd_free(g6hd_system *s)
     cudaFree(s->B.act); cudaFree(s->B.cand); cudaFree(s->B.xi); cudaFree(s->B.vi); cudaFree(s->B.bmin); cudaFree(s->B.bcnt); cudaFree(s->B.boff); cudaFree(s->B.ticket);
     cudaFree(s->B.d_ni); cudaFree(s->B.d_tnext);
     cudaFree(s->a1); cudaFree(s->ad1); cudaFree(s->pot); cudaFree(s->dt_min_bits); cudaFree(s->shared_bits);
+    cudaFree(s->tile_min); cudaFree(s->tile_cnt); cudaFree(s->bar);
+    if (s->h_status) cudaFreeHost(s->h_status);
     if (s->h_note) cudaFreeHost(s->h_note);
     for (auto &e : s->pe) if (e) cudaEventDestroy(e);
     delete s;
@@ -92,6 +110,34 @@ int hd_finish(Cluster &c, g6hd_system &s)
     return G6_OK;
 }
 
+// One launch of the device-side step loop: block steps until t_end, `max_steps` (> 0) or a block larger than loop_max_i.
+// Returns with the stream drained and *st filled in.
+int hd_loop_run(Cluster &c, g6hd_system &s, double t_end, long long max_steps, HlStatus *st)
+{
+    int rc = hd_finish(c, s);                       // the corrector of a block the host stepped
+    if (rc) return rc;
+    const int ntiles = (s.n + JT - 1) / JT;
+    rc = ensure_partials(c, (size_t)s.loop_G * s.loop_max_i);
+    if (rc) return rc;
+    HlArgs A{};
+    A.S = s.S; A.B = s.B; A.C = hd_corr(c, s);
+    A.a1 = s.a1; A.ad1 = s.ad1; A.pot = s.pot;
+    A.ntiles = ntiles; A.K = s.loop_K; A.nj = s.n;
+    A.t_sys = s.t; A.t_end = t_end; A.max_steps = max_steps; A.max_i = s.loop_max_i;
+    A.eps2 = (float)s.eps2; A.ds = c.opt_ds;
+    A.P = c.part; A.P.stride_s = 1; A.P.stride_i = s.loop_G;
+    A.tile_min = s.tile_min; A.tile_cnt = s.tile_cnt; A.bar = s.bar; A.status = s.hd_status;
+    void *args[] = {(void *)&A};
+    const void *fn = c.opt_newton ? (const void *)k_hd_loop<true> : (const void *)k_hd_loop<false>;
+    CK(cudaLaunchCooperativeKernel(fn, dim3(s.loop_G), dim3(HL_THREADS), args, sizeof(HlSmem), c.stream));
+    CK(cudaStreamSynchronize(c.stream));
+    *st = *s.h_status;
+    c.pred_valid = false;                           // the loop rewrote j-store records
+    ++s.loop_launches;
+    s.loop_steps += st->steps;
+    return G6_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -123,6 +169,25 @@ g6hd_system *g6hd_create(int clusterid, int n, const double x[][3], const double
         CK(cudaHostAlloc((void **)&s->h_note, sizeof(HdNote), cudaHostAllocMapped));
         memset(s->h_note, 0, sizeof(HdNote));
         CK(cudaHostGetDevicePointer((void **)&s->B.h_note, s->h_note, 0));
+        // the device-side step loop: CTA c owns the j-tiles c, c + G, ... (at most HL_KMAX of them, resident in shared memory)
+        {
+            const int ntiles = (n + JT - 1) / JT;
+            const int K = (ntiles + std::min(c.n_sm, HL_MAX_G) - 1) / std::min(c.n_sm, HL_MAX_G);
+            s->loop_K = K;
+            s->loop_G = (ntiles + K - 1) / K;
+            s->loop_max_i = std::max(1, std::min(env_int("G6_HD_LOOP_MAXI", HD_LOOP_MAXI_DEFAULT), HL_MAX_I));
+            s->loop = env_int("G6_HD_LOOP", 1) != 0 && K <= HL_KMAX;
+            if (s->loop) {
+                CK(cudaFuncSetAttribute(k_hd_loop<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(HlSmem)));
+                CK(cudaFuncSetAttribute(k_hd_loop<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(HlSmem)));
+                CK(dalloc(s->tile_min, ntiles)); CK(dalloc(s->tile_cnt, ntiles)); CK(dalloc(s->bar, 2));
+                CK(cudaMemsetAsync(s->bar, 0, 2 * sizeof(unsigned int), c.stream));
+                CK(cudaHostAlloc((void **)&s->h_status, sizeof(HlStatus), cudaHostAllocMapped));
+                memset(s->h_status, 0, sizeof(HlStatus));
+                CK(cudaHostGetDevicePointer((void **)&s->hd_status, s->h_status, 0));
+            }
+        }
+        s->loop_profile = env_int("G6_HD_LOOP_PROFILE", 0) != 0;
         s->profile = env_int("G6_HD_PROFILE", 0) != 0;
         if (s->profile) for (auto &e : s->pe) CK(cudaEventCreate(&e));
         CK(cudaMemsetAsync(s->B.ticket, 0, sizeof(unsigned int), c.stream));
@@ -201,6 +266,51 @@ int g6hd_evolve(g6hd_system *sp, double t_end, long long max_block_steps)
         int b = 0;
         while ((1LL << (b + 1)) <= s.n) ++b;
         s.hist[b] += 1;
+    }
+    const auto count_block = [&](int ni) {
+        ++s.nblock; ++done;
+        s.npart += ni;
+        s.inter += (double)ni * (double)s.n;
+        int b = 0;
+        while ((1LL << (b + 1)) <= ni) ++b;
+        s.hist[b] += 1;
+    };
+    // block steps, the loop on the device: one launch steps until t_end, the step budget, or a block too large for it;
+    // such a block comes back selected and predicted, the library's sweep path computes its forces, and the loop resumes
+    while (!s.shared && s.loop && !s.profile && s.t < t_end && (max_block_steps <= 0 || done < max_block_steps)) {
+        HlStatus st;
+        int rc = hd_loop_run(c, s, t_end, max_block_steps > 0 ? max_block_steps - done : 0, &st);
+        if (rc) return rc;
+        if (st.steps > 0) {
+            s.t = st.t;
+            s.last_ni = st.ni_last;
+            s.nblock += st.steps; done += st.steps;
+            s.npart += st.npart;
+            s.inter += (double)st.npart * (double)s.n;
+            for (int b = 0; b < 64; ++b) { s.hist[b] += st.hist[b]; s.loop_us[b] += 1e-3 * (double)st.ns[b]; }
+            for (int k = 0; k < 8; ++k) s.phase_us_loop[k] += (k < 7 ? 1e-3 : 1.0) * (double)st.phase_ns[k];
+        }
+        if (st.reason != HL_BIG) {
+            if (st.reason == HL_END || st.reason == HL_STEPS) continue;        // the loop condition ends it
+            return fail(c, G6_ERR_CUDA, "device step loop returned reason %d", st.reason);
+        }
+        const int ni = st.ni_next;
+        const double tn = st.tnext;
+        if (ni < 1 || ni > s.n || !(tn > s.t)) return fail(c, G6_ERR_CUDA, "device step loop handed over ni = %d, t = %g", ni, tn);
+        const auto b0 = std::chrono::steady_clock::now();
+        rc = hd_force(c, s, ni, tn);
+        if (rc) return rc;
+        s.pending = true;                               // its corrector runs before the loop resumes (hd_finish)
+        s.t = tn;
+        s.last_ni = ni;
+        count_block(ni);
+        if (s.loop_profile) {
+            CK(cudaStreamSynchronize(c.stream));
+            int b = 0;
+            while ((1LL << (b + 1)) <= ni) ++b;
+            s.big_us[b] += 1e6 * std::chrono::duration<double>(std::chrono::steady_clock::now() - b0).count();
+            s.big_n[b] += 1;
+        }
     }
     while (!s.shared && s.t < t_end && (max_block_steps <= 0 || done < max_block_steps)) {
         if (s.profile) CK(cudaEventRecord(s.pe[0], c.stream));
@@ -341,6 +451,18 @@ int g6hd_get_stats(g6hd_system *sp, double stats[8], long long ni_hist_log2[64])
             if (s.hist[b])
                 fprintf(stderr, "g6hd profile: n_i in [2^%d, 2^%d): %lld block steps, select %.1f us, force (from the host wait to its last kernel) %.1f us, correct %.1f us per step\n",
                         b, b + 1, s.hist[b], s.phase_us[0][b] / s.hist[b], s.phase_us[1][b] / s.hist[b], s.phase_us[2][b] / s.hist[b]);
+    if (s.loop_profile) {
+        fprintf(stderr, "g6hd loop profile: %lld launches of the step loop, %lld block steps inside it\n", s.loop_launches, s.loop_steps);
+        if (s.phase_us_loop[7] > 0)
+            fprintf(stderr, "  phases of steps with n_i < 32 (us per step, CTA 0): local min %.2f | barrier1 %.2f | table+select+predict-i %.2f | barrier2 %.2f | force %.2f | barrier3 %.2f | combine+correct %.2f\n",
+                    s.phase_us_loop[0] / s.phase_us_loop[7], s.phase_us_loop[1] / s.phase_us_loop[7], s.phase_us_loop[2] / s.phase_us_loop[7], s.phase_us_loop[3] / s.phase_us_loop[7],
+                    s.phase_us_loop[4] / s.phase_us_loop[7], s.phase_us_loop[5] / s.phase_us_loop[7], s.phase_us_loop[6] / s.phase_us_loop[7]);
+        for (int b = 0; b < 64; ++b)
+            if (s.hist[b])
+                fprintf(stderr, "  n_i in [2^%d, 2^%d): %lld block steps; in the loop %.1f us per step (device clock, %lld steps); handed to the host %lld steps, %.1f us each (wall, force only)\n",
+                        b, b + 1, s.hist[b], (s.hist[b] - s.big_n[b]) ? s.loop_us[b] / (double)(s.hist[b] - s.big_n[b]) : 0.0, s.hist[b] - s.big_n[b],
+                        s.big_n[b], s.big_n[b] ? s.big_us[b] / (double)s.big_n[b] : 0.0);
+    }
     if (ni_hist_log2) memcpy(ni_hist_log2, s.hist, sizeof(s.hist));
     return G6_OK;
 }
