@@ -121,35 +121,57 @@ struct HdCorr {
     unsigned long long *dt_min_bits;
 };
 
-__device__ __forceinline__ void hd_correct_one(const HdState &S, const HdBlock &B, const HdCorr &C, int k, double tn)
+// the arithmetic of one corrector step, by value: step h, old (a0, ad0), new (a1, ad1) forces, predicted (xi, vi) at the new
+// time tn -> corrected x1, v1 and the new step (return value)
+__device__ __forceinline__ double hd_correct_core(double h, const double *a0, const double *ad0, const double *a1, const double *ad1,
+                                                  const double *xi, const double *vi, double tn, double eta, double dt_max,
+                                                  double *x1, double *v1)
 {
-    const int p = B.act[k];
-    const double h = S.dt[p], h2 = h * h, h3 = h2 * h, h4 = h3 * h, h5 = h4 * h;
-    double a2n[3], a3[3], an[3], adn[3];
+    // fp64 division costs ~60 dependent instructions on the device and the corrector sits on the critical path of every small
+    // block step: ONE reciprocal of h (exact when h is a power of two, as the steps are for a power-of-two dt_max) and
+    // reciprocal constants replace the ten divisions per component; results agree with the host driver's to rounding
+    const double h2 = h * h, h3 = h2 * h, h4 = h3 * h, h5 = h4 * h;
+    const double ih = 1.0 / h, ih2 = ih * ih, ih3 = ih2 * ih;
+    constexpr double R6 = 1.0 / 6, R24 = 1.0 / 24, R120 = 1.0 / 120;
+    double a2n[3], a3[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        const double a0 = S.a[3 * (size_t)p + c], ad0 = S.ad[3 * (size_t)p + c];
-        an[c] = C.a1[3 * (size_t)k + c];
-        adn[c] = C.ad1[3 * (size_t)k + c];
-        const double da = a0 - an[c];
-        const double a2 = (-6 * da - h * (4 * ad0 + 2 * adn[c])) / h2;
-        a3[c] = (12 * da + 6 * h * (ad0 + adn[c])) / h3;
-        S.x[3 * (size_t)p + c] = B.xi[3 * (size_t)k + c] + h4 * a2 / 24 + h5 * a3[c] / 120;
-        S.v[3 * (size_t)p + c] = B.vi[3 * (size_t)k + c] + h3 * a2 / 6 + h4 * a3[c] / 24;
+        const double da = a0[c] - a1[c];
+        const double a2 = (-6 * da - h * (4 * ad0[c] + 2 * ad1[c])) * ih2;
+        a3[c] = (12 * da + 6 * h * (ad0[c] + ad1[c])) * ih3;
+        x1[c] = xi[c] + h4 * a2 * R24 + h5 * a3[c] * R120;
+        v1[c] = vi[c] + h3 * a2 * R6 + h4 * a3[c] * R24;
         a2n[c] = a2 + h * a3[c];
-        S.a[3 * (size_t)p + c] = an[c];
-        S.ad[3 * (size_t)p + c] = adn[c];
     }
-    S.t[p] = tn;
-    const double na = hd_norm3(an), nad = hd_norm3(adn), n2 = hd_norm3(a2n), n3 = hd_norm3(a3);
+    const double na = hd_norm3(a1), nad = hd_norm3(ad1), n2 = hd_norm3(a2n), n3 = hd_norm3(a3);
     const double den = nad * n3 + n2 * n2;
-    const double want = den > 0 ? sqrt(C.eta * (na * n2 + nad * nad) / den) : C.dt_max;
+    const double want = den > 0 ? sqrt(eta * (na * n2 + nad * nad) / den) : dt_max;
     double d = h;
     if (want < d) {
         while (d > want && d > 1e-300) d *= 0.5;     // floor: a zero or NaN wish must not loop forever (the host then sees no progress)
-    } else if (want >= 2 * d && 2 * d <= C.dt_max && hd_is_multiple(tn, 2 * d)) {
+    } else if (want >= 2 * d && 2 * d <= dt_max && hd_is_multiple(tn, 2 * d)) {
         d *= 2;
     }
+    return d;
+}
+
+__device__ __forceinline__ void hd_correct_one(const HdState &S, const HdBlock &B, const HdCorr &C, int k, double tn)
+{
+    const int p = B.act[k];
+    double a0[3], ad0[3], a1[3], ad1[3], xi[3], vi[3], x1[3], v1[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        a0[c] = S.a[3 * (size_t)p + c]; ad0[c] = S.ad[3 * (size_t)p + c];
+        a1[c] = C.a1[3 * (size_t)k + c]; ad1[c] = C.ad1[3 * (size_t)k + c];
+        xi[c] = B.xi[3 * (size_t)k + c]; vi[c] = B.vi[3 * (size_t)k + c];
+    }
+    const double d = hd_correct_core(S.dt[p], a0, ad0, a1, ad1, xi, vi, tn, C.eta, C.dt_max, x1, v1);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        S.x[3 * (size_t)p + c] = x1[c]; S.v[3 * (size_t)p + c] = v1[c];
+        S.a[3 * (size_t)p + c] = a1[c]; S.ad[3 * (size_t)p + c] = ad1[c];
+    }
+    S.t[p] = tn;
     S.dt[p] = d;
     atomicMin(C.dt_min_bits, (unsigned long long)__double_as_longlong(d));
     hd_store_j(C.raw, S, p);

@@ -32,14 +32,15 @@ struct g6hd_system {
     // instead), env G6_HD_LOOP_MAXI = largest block stepped inside the loop (default HD_LOOP_MAXI_DEFAULT, at most HL_MAX_I)
     bool loop = false;
     int loop_max_i = 0, loop_G = 0, loop_K = 0;
-    double *tile_min = nullptr;
-    int *tile_cnt = nullptr;
-    unsigned int *bar = nullptr;
+    unsigned long long *rec = nullptr, *chunk = nullptr;       // the loop kernel's exchange words (tile records, partial forces)
+    unsigned int *flag = nullptr;
+    unsigned int loop_gen = 0;                                 // step numbers handed out so far
     HlStatus *h_status = nullptr, *hd_status = nullptr;        // mapped host memory and its device view
     long long loop_launches = 0, loop_steps = 0;
     double loop_us[64] = {}, big_us[64] = {}, relaunch_us = 0;    // env G6_HD_LOOP_PROFILE: where the time of a run goes, by block size
     long long big_n[64] = {};
-    double phase_us_loop[8] = {};
+    long long inline_steps = 0;
+
     bool loop_profile = false;
 };
 
@@ -54,7 +55,7 @@ void hd_free(g6hd_system *s)
     cudaFree(s->B.act); cudaFree(s->B.cand); cudaFree(s->B.xi); cudaFree(s->B.vi); cudaFree(s->B.bmin); cudaFree(s->B.bcnt); cudaFree(s->B.boff); cudaFree(s->B.ticket);
     cudaFree(s->B.d_ni); cudaFree(s->B.d_tnext);
     cudaFree(s->a1); cudaFree(s->ad1); cudaFree(s->pot); cudaFree(s->dt_min_bits); cudaFree(s->shared_bits);
-    cudaFree(s->tile_min); cudaFree(s->tile_cnt); cudaFree(s->bar);
+    cudaFree(s->rec); cudaFree(s->chunk); cudaFree(s->flag);
     if (s->h_status) cudaFreeHost(s->h_status);
     if (s->h_note) cudaFreeHost(s->h_note);
     for (auto &e : s->pe) if (e) cudaEventDestroy(e);
@@ -117,21 +118,21 @@ int hd_loop_run(Cluster &c, g6hd_system &s, double t_end, long long max_steps, H
     int rc = hd_finish(c, s);                       // the corrector of a block the host stepped
     if (rc) return rc;
     const int ntiles = (s.n + JT - 1) / JT;
-    rc = ensure_partials(c, (size_t)s.loop_G * s.loop_max_i);
-    if (rc) return rc;
     HlArgs A{};
     A.S = s.S; A.B = s.B; A.C = hd_corr(c, s);
     A.a1 = s.a1; A.ad1 = s.ad1; A.pot = s.pot;
-    A.ntiles = ntiles; A.K = s.loop_K; A.nj = s.n;
+    A.ntiles = ntiles; A.nj = s.n;
     A.t_sys = s.t; A.t_end = t_end; A.max_steps = max_steps; A.max_i = s.loop_max_i;
     A.eps2 = (float)s.eps2; A.ds = c.opt_ds;
-    A.P = c.part; A.P.stride_s = 1; A.P.stride_i = s.loop_G;
-    A.tile_min = s.tile_min; A.tile_cnt = s.tile_cnt; A.bar = s.bar; A.status = s.hd_status;
+    A.gen0 = s.loop_gen;
+    A.rec = s.rec; A.chunk = s.chunk; A.flag = s.flag; A.status = s.hd_status;
+
     void *args[] = {(void *)&A};
     const void *fn = c.opt_newton ? (const void *)k_hd_loop<true> : (const void *)k_hd_loop<false>;
     CK(cudaLaunchCooperativeKernel(fn, dim3(s.loop_G), dim3(HL_THREADS), args, sizeof(HlSmem), c.stream));
     CK(cudaStreamSynchronize(c.stream));
     *st = *s.h_status;
+    s.loop_gen += (unsigned int)st->steps + 2u;     // step numbers are never reused (a handed-over block consumed one too)
     c.pred_valid = false;                           // the loop rewrote j-store records
     ++s.loop_launches;
     s.loop_steps += st->steps;
@@ -180,8 +181,11 @@ g6hd_system *g6hd_create(int clusterid, int n, const double x[][3], const double
             if (s->loop) {
                 CK(cudaFuncSetAttribute(k_hd_loop<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(HlSmem)));
                 CK(cudaFuncSetAttribute(k_hd_loop<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(HlSmem)));
-                CK(dalloc(s->tile_min, ntiles)); CK(dalloc(s->tile_cnt, ntiles)); CK(dalloc(s->bar, 2));
-                CK(cudaMemsetAsync(s->bar, 0, 2 * sizeof(unsigned int), c.stream));
+                const size_t nrec = 2 * (size_t)s->loop_G * ntiles * HL_REC_WORDS, nchunk = (size_t)s->loop_max_i * HL_CHUNK_WORDS * s->loop_G;
+                CK(dalloc(s->rec, nrec)); CK(dalloc(s->chunk, nchunk)); CK(dalloc(s->flag, s->loop_G));
+                CK(cudaMemsetAsync(s->rec, 0, nrec * sizeof(unsigned long long), c.stream));           // step number 0 = never written
+                CK(cudaMemsetAsync(s->chunk, 0, nchunk * sizeof(unsigned long long), c.stream));
+                CK(cudaMemsetAsync(s->flag, 0, s->loop_G * sizeof(unsigned int), c.stream));
                 CK(cudaHostAlloc((void **)&s->h_status, sizeof(HlStatus), cudaHostAllocMapped));
                 memset(s->h_status, 0, sizeof(HlStatus));
                 CK(cudaHostGetDevicePointer((void **)&s->hd_status, s->h_status, 0));
@@ -288,7 +292,7 @@ int g6hd_evolve(g6hd_system *sp, double t_end, long long max_block_steps)
             s.npart += st.npart;
             s.inter += (double)st.npart * (double)s.n;
             for (int b = 0; b < 64; ++b) { s.hist[b] += st.hist[b]; s.loop_us[b] += 1e-3 * (double)st.ns[b]; }
-            for (int k = 0; k < 8; ++k) s.phase_us_loop[k] += (k < 7 ? 1e-3 : 1.0) * (double)st.phase_ns[k];
+            s.inline_steps += st.inline_steps;
         }
         if (st.reason != HL_BIG) {
             if (st.reason == HL_END || st.reason == HL_STEPS) continue;        // the loop condition ends it
@@ -453,10 +457,7 @@ int g6hd_get_stats(g6hd_system *sp, double stats[8], long long ni_hist_log2[64])
                         b, b + 1, s.hist[b], s.phase_us[0][b] / s.hist[b], s.phase_us[1][b] / s.hist[b], s.phase_us[2][b] / s.hist[b]);
     if (s.loop_profile) {
         fprintf(stderr, "g6hd loop profile: %lld launches of the step loop, %lld block steps inside it\n", s.loop_launches, s.loop_steps);
-        if (s.phase_us_loop[7] > 0)
-            fprintf(stderr, "  phases of steps with n_i < 32 (us per step, CTA 0): local min %.2f | barrier1 %.2f | table+select+predict-i %.2f | barrier2 %.2f | force %.2f | barrier3 %.2f | combine+correct %.2f\n",
-                    s.phase_us_loop[0] / s.phase_us_loop[7], s.phase_us_loop[1] / s.phase_us_loop[7], s.phase_us_loop[2] / s.phase_us_loop[7], s.phase_us_loop[3] / s.phase_us_loop[7],
-                    s.phase_us_loop[4] / s.phase_us_loop[7], s.phase_us_loop[5] / s.phase_us_loop[7], s.phase_us_loop[6] / s.phase_us_loop[7]);
+        fprintf(stderr, "  %lld of them predicted their i-block in every CTA (one exchange less)\n", s.inline_steps);
         for (int b = 0; b < 64; ++b)
             if (s.hist[b])
                 fprintf(stderr, "  n_i in [2^%d, 2^%d): %lld block steps; in the loop %.1f us per step (device clock, %lld steps); handed to the host %lld steps, %.1f us each (wall, force only)\n",

@@ -9,19 +9,26 @@
 //  * CTA c (one per SM, all co-resident) OWNS the raw j-tiles c, c + G, ... (at most HL_KMAX) and keeps them IN SHARED MEMORY
 //    for the whole run, together with t + dt of their particles: per block step no j-particle is read from HBM or L2 at all;
 //    the owner patches the staged record of a particle it has just corrected and writes it through to the j-store.
-//  * a block step has three grid-wide barriers (one atomic arrival + a generation word, ~1.5 us each):
-//      A  every CTA publishes (min, count at the min) of t + dt per owned tile          -> barrier 1
-//         everybody derives t_next = global min, n_i and each tile's offset in the active list (increasing address);
-//         owners predict their active particles in fp64 (Eq. 1-2) into the shared i-block     -> barrier 2
-//      B  every CTA: i-block -> double-single in shared memory, Eq. 1-2 of its resident j-particles (same routine as
-//         k_predict), then all pairs with the packed, checked pair code of the block-step kernel (pair2_checked; Eq. 3).
-//         Lanes of a warp = (i-particle, j-sub-range): "several threads share an i and split the j";
-//         the lanes of one i are summed by a fixed shuffle tree ONCE per step, the warps and the CTAs in fixed order in fp64
-//         (reading 9): bit-reproducible.  One partial per (i, CTA)                                  -> barrier 3
-//      C  the owner of each active particle sums its G partials (a warp per particle, the order of k_combine_wide), runs
-//         the corrector, the Aarseth step and the power-of-two rule (hd_correct_one), and updates its resident tile.
-//  * a block with n_i > max_i is selected and predicted (phase A) and handed to the host, which runs the library's sweep path
-//    on it (hd_force) and re-enters the loop.
+//  * the CTAs meet through SELF-VALIDATING 8-byte words {32 bits of payload, 32-bit step number} written and polled with
+//    single 64-bit accesses (single-copy atomic): the data is its own flag, so an exchange costs one store and one L2 round
+//    trip, with no separate barrier and no fence (the protocol NCCL calls LL).  A block step has two such exchanges:
+//      A  per owned tile: (min of t + dt, count at the min, slots of the first HL_INLINE particles at the min)  -> records
+//         every CTA polls all records: t_next = global min, n_i, the active list in increasing address.  If no tile holds more
+//         than HL_INLINE active particles EVERY CTA reads the Hermite state of all n_i particles and predicts them itself in
+//         fp64 (Eq. 1-2): no second exchange.  Otherwise the owners predict into the global i-block and the CTAs
+//         meet at a flag barrier.
+//      B  i-block -> double-single in shared memory, Eq. 1-2 of the resident j-particles (same routine as k_predict), then all
+//         pairs with the packed, checked pair code of the block-step kernel (pair2_checked; Eq. 3).  Lanes of a warp
+//         = (i-particle, j-sub-range): "several threads share an i and split the j"; the lanes of one i are
+//         summed by a fixed shuffle tree once per step, then the warps and the CTAs in fixed order in fp64 (reading 9):
+//         bit-reproducible.  One partial per (i, CTA)                                                          -> chunks
+//      C  the owner of each active particle polls its G partials (a warp per particle, summed in the order of k_combine_wide),
+//         runs the corrector, the Aarseth step and the power-of-two rule (hd_correct_core), updates its resident tile.
+//    Records are double-buffered by step parity (an owner without active particles may run one step ahead of a slow poller);
+//    partials need no second buffer (a CTA writes those of step s + 1 only after every CTA has published its records of s + 1,
+//    i.e. has finished step s).
+//  * a block with n_i > max_i is selected and predicted by its owners and handed to the host, which runs the library's sweep
+//    path on it (hd_force) and re-enters the loop.
 // The nearest neighbour is not tracked (the Hermite driver does not use it).
 #pragma once
 #include "g6_block_step.cuh"
@@ -29,12 +36,17 @@
 
 namespace g6 {
 
-constexpr int HL_THREADS = 256;
+constexpr int HL_THREADS = 512;
 constexpr int HL_NW = HL_THREADS / 32;
 constexpr int HL_KMAX = 4;                    // resident raw tiles per CTA
-constexpr int HL_MAX_I = 1024;                // largest block the loop can step itself
-constexpr int HL_MAX_G = 160;                 // CTAs (one per SM)
+constexpr int HL_MAX_I = 768;                 // largest block the loop can step itself
+constexpr int HL_MAX_G = 148;                 // CTAs (one per SM)
 constexpr int HL_MAX_TILES = HL_MAX_G * HL_KMAX;
+constexpr int HL_INLINE = 8;                  // active particles per tile that travel inside the tile's record
+constexpr int HL_REC_WORDS = 5;               // tmin lo, tmin hi, count, slots 0-3, slots 4-7
+constexpr int HL_CHUNK_WORDS = 14;            // 7 fp64 sums = 14 halves
+constexpr int HL_CQ = 3;                      // particles whose partials an owner gathers at a time (staged in the idle wsum)
+constexpr int HL_CPOLL = 4;                   // words a thread polls per round
 
 enum { HL_END = 0, HL_BIG = 1, HL_STEPS = 2 };
 
@@ -49,7 +61,7 @@ struct HlStatus {
     int pad;
     long long hist[64];    // block steps by log2(n_i)
     long long ns[64];      // device time (globaltimer, ns) spent in the block steps of each bin, as seen by CTA 0
-    long long phase_ns[8]; // PROFILING: time between the phase boundaries of steps with n_i < 32 (CTA 0)
+    long long inline_steps;  // steps whose i-block every CTA predicted itself (no second exchange)
 };
 
 struct HlArgs {
@@ -57,16 +69,16 @@ struct HlArgs {
     HdBlock B;
     HdCorr C;
     double *a1, *ad1, *pot;        // forces of the current block (= C.a1, C.ad1), writable
-    int ntiles, K, nj;
+    int ntiles, nj;
     double t_sys, t_end;
     long long max_steps;
     int max_i;
     float eps2;
     int ds;
-    Partials P;                    // [k][G]: stride_s = 1, stride_i = G
-    double *tile_min;              // [ntiles] per-tile minimum of t + dt
-    int *tile_cnt;                 // [ntiles] particles of the tile at that minimum
-    unsigned int *bar;             // [2] arrival count, generation
+    unsigned int gen0;             // step numbers of this launch are gen0 + 1, gen0 + 2, ... (never 0, never reused)
+    unsigned long long *rec;       // [2][G][ntiles][HL_REC_WORDS]   tile records: double-buffered by step parity, one copy per consumer CTA
+    unsigned long long *chunk;     // [max_i][HL_CHUNK_WORDS][G]  partial forces
+    unsigned int *flag;            // [G] flag barrier of the non-inline path
     HlStatus *status;              // device-visible (mapped host memory)
 };
 
@@ -75,55 +87,85 @@ struct HlSmem {
     alignas(16) float pred[HL_KMAX][TILE_FLOATS];       // their Eq. 1-2 predictions at the block time
     double tnext[HL_KMAX][JT];                          // t + dt of the own particles (+inf past the end)
     float ipart[HL_MAX_I][9];                           // i-block: hi[3], lo[3], v[3]
-    int iidx[HL_MAX_I];
-    double wsum[HL_NW][32][8];                          // per-warp sums of one i-chunk
-    double s_tm[HL_MAX_TILES];
+    int iidx[HL_MAX_I];                                 // ... and the particles' addresses (= indices)
+    double wsum[HL_NW][32][7];                          // per-warp sums of one i-chunk
+    double s_tm[HL_MAX_TILES];                          // the tile records of this step
     int s_tc[HL_MAX_TILES];
     int s_off[HL_MAX_TILES];
+    unsigned int s_sl[HL_MAX_TILES][2];
     int own_k[HL_KMAX * JT], own_l[HL_KMAX * JT];       // my active particles: position in the active list, slot kk * JT + l
-    double red[HL_NW][HL_KMAX];
-    int redc[HL_NW][HL_KMAX];
+    double own_st[HL_KMAX * HL_INLINE][20];             // inline path: xi[3] vi[3] a0[3] ad0[3] h, of my active particles
+    double red[HL_NW][2];
+    unsigned int bal[HL_KMAX][JT / 32];
+    unsigned int recw[HL_KMAX][HL_REC_WORDS];
+    int nown_prev;
+    double tmin[HL_KMAX];
     double gmin;
-    int ni, nown;
+    int ni, nown, inl;
 };
 static_assert(sizeof(HlSmem) <= 232448, "loop kernel shared memory");
+static_assert(sizeof(double) * HL_NW * 32 * 7 >= sizeof(unsigned int) * HL_CQ * HL_CHUNK_WORDS * HL_MAX_G, "chunk staging fits in wsum");
 
-// grid-wide barrier: sense by generation; every CTA of the (cooperative) launch must call it
-__device__ __forceinline__ void hl_grid_barrier(unsigned int *bar, unsigned int G)
+__device__ __forceinline__ void hl_store_word(unsigned long long *p, unsigned int payload, unsigned int gen)
+{
+    const unsigned long long v = (unsigned long long)payload | ((unsigned long long)gen << 32);
+    asm volatile("st.volatile.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long hl_load_word(const unsigned long long *p)
+{
+    unsigned long long v;
+    asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+// spin until the N words p[0], p[stride], ... all carry step number `gen` (all N loads of a round are in flight together);
+// a protocol error fails the launch instead of hanging the device
+template <int N>
+__device__ __forceinline__ void hl_wait_words(const unsigned long long *p, size_t stride, unsigned int gen, unsigned int (&out)[N])
+{
+    unsigned int spins = 0;
+    for (;;) {
+        unsigned long long v[N];
+#pragma unroll
+        for (int k = 0; k < N; ++k) v[k] = hl_load_word(p + k * stride);
+        bool ok = true;
+#pragma unroll
+        for (int k = 0; k < N; ++k) { ok = ok && (unsigned int)(v[k] >> 32) == gen; out[k] = (unsigned int)v[k]; }
+        if (ok) return;
+        if (++spins > (1u << 26)) __trap();
+    }
+}
+
+// flag barrier (non-inline path only): every CTA publishes the step number, everybody polls all flags
+__device__ __forceinline__ void hl_flag_barrier(unsigned int *flag, unsigned int G, unsigned int gen)
 {
     __syncthreads();
     if (threadIdx.x == 0) {
-        unsigned int gen;
-        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(gen) : "l"(bar + 1) : "memory");
         __threadfence();
-        if (atomicAdd(bar, 1u) == G - 1u) {
-            bar[0] = 0u;
-            __threadfence();
-            asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(bar + 1), "r"(gen + 1u) : "memory");
-        } else {
-            unsigned int now, spins = 0;
-            do {
-                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(now) : "l"(bar + 1) : "memory");
-                if (++spins > (1u << 28)) __trap();          // a protocol error fails the launch instead of hanging the device
-            } while (now == gen);
-        }
+        asm volatile("st.volatile.global.u32 [%0], %1;" ::"l"(flag + blockIdx.x), "r"(gen) : "memory");
+    }
+    for (unsigned int s = threadIdx.x; s < G; s += HL_THREADS) {
+        unsigned int v, spins = 0;
+        do {
+            asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(v) : "l"(flag + s) : "memory");
+            if (++spins > (1u << 26)) __trap();
+        } while (v != gen);
         __threadfence();
     }
     __syncthreads();
 }
 
-// particle p's Hermite state -> slot l of a raw tile in shared memory (what hd_store_j writes to the j-store)
-__device__ __forceinline__ void hl_store_tile(char *T, int l, const HdState &S, int p)
+// particle p's new Hermite state -> slot l of a raw tile (shared memory or the j-store): what hd_store_j writes
+__device__ __forceinline__ void hl_store_tile(char *T, int l, int p, const double *x, const double *v, const double *a, const double *ad, double t, float m)
 {
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-        raw_x(T, k, l) = S.x[3 * (size_t)p + k];
-        raw_v(T, k, l) = (float)S.v[3 * (size_t)p + k];
-        raw_a2(T, k, l) = (float)(S.a[3 * (size_t)p + k] / 2);
-        raw_j6(T, k, l) = (float)(S.ad[3 * (size_t)p + k] / 6);
+        raw_x(T, k, l) = x[k];
+        raw_v(T, k, l) = (float)v[k];
+        raw_a2(T, k, l) = (float)(a[k] / 2);
+        raw_j6(T, k, l) = (float)(ad[k] / 6);
     }
-    raw_t(T, l) = S.t[p];
-    raw_m(T, l) = (float)S.m[p];
+    raw_t(T, l) = t;
+    raw_m(T, l) = m;
     raw_idx(T, l) = p;
 }
 
@@ -135,6 +177,7 @@ k_hd_loop(const HlArgs A)
     HlSmem &sm = *reinterpret_cast<HlSmem *>(smem_raw);
     const unsigned FULL = 0xffffffffu;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const int slot = tid & (JT - 1), half = tid / JT, ws = slot >> 5;       // a particle slot and which half of the CTA works on it
     const int G = gridDim.x, cta = blockIdx.x;
     const double INF = __longlong_as_double(0x7ff0000000000000LL);
     const int Kc = cta < A.ntiles ? (A.ntiles - cta + G - 1) / G : 0;       // my tiles: cta, cta + G, ...
@@ -144,19 +187,19 @@ k_hd_loop(const HlArgs A)
         const int4 *src = reinterpret_cast<const int4 *>(A.C.raw + (size_t)(cta + kk * G) * RAW_TILE_BYTES);
         int4 *dst = reinterpret_cast<int4 *>(sm.raw[kk]);
         for (int q = tid; q < RAW_TILE_BYTES / 16; q += HL_THREADS) dst[q] = __ldcg(src + q);
-        const int p = (cta + kk * G) * JT + tid;
-        sm.tnext[kk][tid] = p < A.S.n ? A.S.t[p] + A.S.dt[p] : INF;
+        if (half == 0) {
+            const int p = (cta + kk * G) * JT + slot;
+            sm.tnext[kk][slot] = p < A.S.n ? __ldcg(A.S.t + p) + __ldcg(A.S.dt + p) : INF;
+        }
     }
     __syncthreads();
 
+    if (tid == 0) sm.nown_prev = 0;
     double t_sys = A.t_sys;
-    long long steps = 0, npart = 0;
+    long long steps = 0, npart = 0, n_inline = 0;
     long long hist = 0, hist_ns = 0;       // thread b < 64 of CTA 0 counts bin b
     unsigned long long t_step = 0;
     if (cta == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_step));
-    long long ph[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    unsigned long long stamp[8];
-#define HL_STAMP(k) do { if (cta == 0 && tid == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(stamp[k])); } while (0)
     int reason = HL_END, ni_next = 0, ni_last = 0;
     double t_big = 0.0;
     const float2 eps2 = dup(A.eps2);
@@ -164,52 +207,73 @@ k_hd_loop(const HlArgs A)
     for (;;) {
         if (!(t_sys < A.t_end)) { reason = HL_END; break; }
         if (A.max_steps > 0 && steps >= A.max_steps) { reason = HL_STEPS; break; }
+        const unsigned int gen = A.gen0 + 1u + (unsigned int)steps;
+        // this step's records: [consumer CTA][tile][word] -- every consumer polls its OWN copy (a word polled by all CTAs at once
+        // is a hot spot in its L2 slice: the publisher's store then queues behind hundreds of loads, measured 3-5 us)
+        unsigned long long *rec = A.rec + (size_t)(gen & 1u) * G * A.ntiles * HL_REC_WORDS;
 
-        HL_STAMP(0);
-        // ================= phase A: (min, count) of t + dt per own tile
-        {
-            double v[HL_KMAX];
+        // ================= phase A: per own tile (min, count, first slots at the min) of t + dt -> its record
+        // the two halves of the CTA take the tiles of their parity; a warp holds 32 consecutive slots of one tile
+        for (int kk = half; kk < Kc; kk += 2) {
+            double m = sm.tnext[kk][slot];
 #pragma unroll
-            for (int kk = 0; kk < HL_KMAX; ++kk) {
-                v[kk] = kk < Kc ? sm.tnext[kk][tid] : INF;
-                double m = v[kk];
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) m = fmin(m, __shfl_xor_sync(FULL, m, o));
-                if (lane == 0) sm.red[w][kk] = m;
-            }
-            __syncthreads();
-#pragma unroll
-            for (int kk = 0; kk < HL_KMAX; ++kk) {
-                double m = sm.red[0][kk];
-#pragma unroll
-                for (int q = 1; q < HL_NW; ++q) m = fmin(m, sm.red[q][kk]);
-                const unsigned bal = __ballot_sync(FULL, kk < Kc && v[kk] == m);
-                if (lane == 0) sm.redc[w][kk] = __popc(bal);
-                v[kk] = m;
-            }
-            __syncthreads();
-            if (tid < Kc) {
-                int c = 0;
-                double m = sm.red[0][tid];
-#pragma unroll
-                for (int q = 0; q < HL_NW; ++q) { c += sm.redc[q][tid]; m = fmin(m, sm.red[q][tid]); }
-                __stcg(A.tile_min + cta + tid * G, m);
-                __stcg(A.tile_cnt + cta + tid * G, c);
-            }
+            for (int o = 16; o > 0; o >>= 1) m = fmin(m, __shfl_xor_sync(FULL, m, o));
+            if (lane == 0) sm.red[w][kk >> 1] = m;
         }
-        HL_STAMP(1);
-        hl_grid_barrier(A.bar, G);
-        HL_STAMP(2);
+        __syncthreads();
+        for (int kk = half; kk < Kc; kk += 2) {
+            double m = sm.red[half * (JT / 32)][kk >> 1];
+#pragma unroll
+            for (int q = 1; q < JT / 32; ++q) m = fmin(m, sm.red[half * (JT / 32) + q][kk >> 1]);
+            const unsigned b = __ballot_sync(FULL, sm.tnext[kk][slot] == m);
+            if (lane == 0) sm.bal[kk][ws] = b;
+            if (slot == 0) sm.tmin[kk] = m;
+        }
+        __syncthreads();
+        if (tid < Kc) {
+            // thread kk: count and the first HL_INLINE slots at the minimum of tile kk, from the eight warp ballots
+            const int kk = tid;
+            int c = 0;
+            unsigned int sl[2] = {0u, 0u};
+            for (int q = 0; q < JT / 32; ++q) {
+                unsigned b = sm.bal[kk][q];
+                while (b) {
+                    const int l = __ffs(b) - 1;
+                    b &= b - 1;
+                    if (c < HL_INLINE) sl[c >> 2] |= (unsigned)(32 * q + l) << (8 * (c & 3));
+                    ++c;
+                }
+            }
+            const unsigned long long tb = (unsigned long long)__double_as_longlong(sm.tmin[kk]);
+            sm.recw[kk][0] = (unsigned int)tb;
+            sm.recw[kk][1] = (unsigned int)(tb >> 32);
+            sm.recw[kk][2] = (unsigned int)c;
+            sm.recw[kk][3] = sl[0];
+            sm.recw[kk][4] = sl[1];
+        }
+        // Release: the Hermite state of my particles that phase C of the last step wrote must be visible to whoever reads the
+        // records (only a CTA that corrected particles has anything to release)
+        if (tid == 0 && sm.nown_prev > 0) __threadfence();
+        __syncthreads();
+        for (int e = tid; e < G * Kc * HL_REC_WORDS; e += HL_THREADS) {
+            const int c = e / (Kc * HL_REC_WORDS), r = e % (Kc * HL_REC_WORDS), kk = r / HL_REC_WORDS, wd = r % HL_REC_WORDS;
+            hl_store_word(rec + ((size_t)c * A.ntiles + (cta + kk * G)) * HL_REC_WORDS + wd, sm.recw[kk][wd], gen);
+        }
 
-        // everybody: t_next, n_i, offsets of the tiles in the active list (tile order = increasing address)
+        // everybody polls every record: t_next, n_i, offsets of the tiles in the active list (tile order = increasing address)
         {
             double m = INF;
             for (int T = tid; T < A.ntiles; T += HL_THREADS) {
-                const double tm = __ldcg(A.tile_min + T);
+                unsigned int wd[HL_REC_WORDS];
+                hl_wait_words<HL_REC_WORDS>(rec + ((size_t)cta * A.ntiles + T) * HL_REC_WORDS, 1, gen, wd);
+                const double tm = __longlong_as_double((long long)(((unsigned long long)wd[1] << 32) | wd[0]));
                 sm.s_tm[T] = tm;
-                sm.s_tc[T] = __ldcg(A.tile_cnt + T);
+                sm.s_tc[T] = (int)wd[2];
+                sm.s_sl[T][0] = wd[3];
+                sm.s_sl[T][1] = wd[4];
                 m = fmin(m, tm);
             }
+            __threadfence();                               // acquire: what the records' writers published before them
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) m = fmin(m, __shfl_xor_sync(FULL, m, o));
             if (lane == 0) sm.red[w][0] = m;
@@ -218,11 +282,12 @@ k_hd_loop(const HlArgs A)
 #pragma unroll
             for (int q = 1; q < HL_NW; ++q) m = fmin(m, sm.red[q][0]);
             if (w == 0) {
-                int run = 0;
+                int run = 0, over = 0;
                 for (int T0 = 0; T0 < A.ntiles; T0 += 32) {
                     const int T = T0 + lane;
                     const bool hit = T < A.ntiles && sm.s_tm[T] == m;
                     const int c = hit ? sm.s_tc[T] : 0;
+                    over |= c > HL_INLINE;
                     int inc = c;
 #pragma unroll
                     for (int o = 1; o < 32; o <<= 1) {
@@ -232,147 +297,239 @@ k_hd_loop(const HlArgs A)
                     if (T < A.ntiles) sm.s_off[T] = hit ? run + inc - c : -1;
                     run += __shfl_sync(FULL, inc, 31);
                 }
-                if (lane == 0) { sm.ni = run; sm.gmin = m; }
+                over = __any_sync(FULL, over);
+                if (lane == 0) { sm.ni = run; sm.gmin = m; sm.inl = !over && run <= A.max_i; }
             }
             __syncthreads();
         }
         const double tn = sm.gmin;
         const int ni = sm.ni;
-        const bool big = ni > A.max_i;
+        const bool big = ni > A.max_i, inl = sm.inl != 0;
 
-        // owners: active particles of my tiles, in address order, predicted in fp64 into the shared i-block
-        {
+        if (inl) {
+            // ---- every CTA builds the active list and predicts all n_i particles itself (fp64 Eq. 1-2), straight into its i-block
+            for (int T = tid; T < A.ntiles; T += HL_THREADS) {
+                const int base = sm.s_off[T];
+                if (base < 0) continue;
+                const int c = sm.s_tc[T];
+                for (int r = 0; r < c; ++r) sm.iidx[base + r] = T * JT + (int)((sm.s_sl[T][r >> 2] >> (8 * (r & 3))) & 0xffu);
+            }
+            __syncthreads();
+            int nown = 0;
+            for (int k = tid; k < ni; k += HL_THREADS) {
+                const int p = sm.iidx[k];
+                const double tp = __ldcg(A.S.t + p);
+                const double h = tn - tp, h2 = h * h / 2, h3 = h * h * h / 6;
+                const int T = p / JT;
+                const bool mine = (T % G) == cta;
+                double xi[3], vi[3];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const double x = __ldcg(A.S.x + 3 * (size_t)p + c), v = __ldcg(A.S.v + 3 * (size_t)p + c);
+                    const double a = __ldcg(A.S.a + 3 * (size_t)p + c), ad = __ldcg(A.S.ad + 3 * (size_t)p + c);
+                    xi[c] = x + v * h + a * h2 + ad * h3;              // same expressions as hd_predict
+                    vi[c] = v + a * h + ad * h2;
+                    float hi, lo;
+                    ds_split(xi[c], hi, lo);
+                    sm.ipart[k][c] = hi;
+                    sm.ipart[k][3 + c] = A.ds ? lo : 0.0f;
+                    sm.ipart[k][6 + c] = (float)vi[c];
+                    if (mine) {
+                        double *st = sm.own_st[(T / G) * HL_INLINE + (k - sm.s_off[T])];
+                        st[c] = xi[c]; st[3 + c] = vi[c]; st[6 + c] = a; st[9 + c] = ad;
+                    }
+                    if (cta == 0) { A.B.xi[3 * (size_t)k + c] = xi[c]; A.B.vi[3 * (size_t)k + c] = vi[c]; }     // read-back only
+                }
+                if (mine) sm.own_st[(T / G) * HL_INLINE + (k - sm.s_off[T])][12] = h;
+                if (cta == 0) A.B.act[k] = p;
+            }
+            // my active particles: (position in the list, slot), tile by tile
+            if (tid == 0) {
+                for (int kk = 0; kk < Kc; ++kk) {
+                    const int T = cta + kk * G, base = sm.s_off[T];
+                    if (base < 0) continue;
+                    for (int r = 0; r < sm.s_tc[T]; ++r) {
+                        sm.own_k[nown] = base + r;
+                        sm.own_l[nown] = kk * JT + (int)((sm.s_sl[T][r >> 2] >> (8 * (r & 3))) & 0xffu);
+                        ++nown;
+                    }
+                }
+                sm.nown = nown;
+            }
+        } else {
+            // ---- owners: active particles of my tiles, in address order, predicted in fp64 into the global i-block
             int nown = 0;
             for (int kk = 0; kk < Kc; ++kk) {
                 const int T = cta + kk * G;
                 const int base = sm.s_off[T];
                 if (base < 0) continue;                                     // uniform over the CTA
-                const bool on = sm.tnext[kk][tid] == tn;
-                const unsigned bal = __ballot_sync(FULL, on);
-                if (lane == 0) sm.redc[w][0] = __popc(bal);
-                __syncthreads();
-                int before = 0, total = 0;
-#pragma unroll
-                for (int q = 0; q < HL_NW; ++q) { const int cw = sm.redc[q][0]; before += q < w ? cw : 0; total += cw; }
-                if (on) {
-                    const int r = before + __popc(bal & ((1u << lane) - 1u));
-                    const int k = base + r, p = T * JT + tid;
-                    A.B.act[k] = p;
-                    hd_predict(A.S, p, tn, A.B.xi + 3 * (size_t)k, A.B.vi + 3 * (size_t)k);
-                    if (!big) { sm.own_k[nown + r] = k; sm.own_l[nown + r] = kk * JT + tid; }
+                if (half == 0) {
+                    const bool on = sm.tnext[kk][slot] == tn;
+                    int before = 0;
+                    for (int q = 0; q < ws; ++q) before += __popc(sm.bal[kk][q]);
+                    if (on) {
+                        const int r = before + __popc(sm.bal[kk][ws] & ((1u << lane) - 1u));
+                        const int k = base + r, p = T * JT + slot;
+                        A.B.act[k] = p;
+                        hd_predict(A.S, p, tn, A.B.xi + 3 * (size_t)k, A.B.vi + 3 * (size_t)k);
+                        if (!big) { sm.own_k[nown + r] = k; sm.own_l[nown + r] = kk * JT + slot; }
+                    }
                 }
-                nown += total;
-                __syncthreads();
+                nown += sm.s_tc[T];
             }
             if (tid == 0) sm.nown = nown;
+            if (big) { reason = HL_BIG; ni_next = ni; t_big = tn; break; }   // the kernel's end publishes the i-block
+            hl_flag_barrier(A.flag, G, gen);
+            for (int q = tid; q < ni * 3; q += HL_THREADS) {
+                const int i = q / 3, c = q % 3;
+                float hi, lo;
+                ds_split(__ldcg(A.B.xi + q), hi, lo);
+                sm.ipart[i][c] = hi;
+                sm.ipart[i][3 + c] = A.ds ? lo : 0.0f;
+                sm.ipart[i][6 + c] = (float)__ldcg(A.B.vi + q);
+            }
+            for (int i = tid; i < ni; i += HL_THREADS) sm.iidx[i] = __ldcg(A.B.act + i);
         }
-        HL_STAMP(3);
-        hl_grid_barrier(A.bar, G);
-        HL_STAMP(4);
-        if (big) { reason = HL_BIG; ni_next = ni; t_big = tn; break; }
 
-        // ================= phase B: i-block -> double-single, my j-particles -> Eq. 1-2 at tn, all pairs
-        for (int q = tid; q < ni * 3; q += HL_THREADS) {
-            const int i = q / 3, c = q % 3;
-            float hi, lo;
-            ds_split(__ldcg(A.B.xi + q), hi, lo);
-            sm.ipart[i][c] = hi;
-            sm.ipart[i][3 + c] = A.ds ? lo : 0.0f;
-            sm.ipart[i][6 + c] = (float)__ldcg(A.B.vi + q);
-        }
-        for (int i = tid; i < ni; i += HL_THREADS) sm.iidx[i] = __ldcg(A.B.act + i);
-        for (int kk = 0; kk < Kc; ++kk) {
+        // ================= phase B: my j-particles -> Eq. 1-2 at tn, then all pairs
+        for (int q = tid; q < Kc * JT; q += HL_THREADS) {
+            const int kk = q / JT, l = q % JT;
             char *R = sm.raw[kk];
             float *Pj = sm.pred[kk];
-            const float dt = (float)(tn - raw_t(R, tid));
+            const float dt = (float)(tn - raw_t(R, l));
 #pragma unroll
             for (int k = 0; k < 3; ++k)
-                predict_coord(dt, raw_x(R, k, tid), raw_v(R, k, tid), raw_a2(R, k, tid), raw_j6(R, k, tid), A.ds,
-                              Pj[(F_XH + k) * JT + tid], Pj[(F_XL + k) * JT + tid], Pj[(F_V + k) * JT + tid]);
-            Pj[F_M * JT + tid] = raw_m(R, tid);
+                predict_coord(dt, raw_x(R, k, l), raw_v(R, k, l), raw_a2(R, k, l), raw_j6(R, k, l), A.ds,
+                              Pj[(F_XH + k) * JT + l], Pj[(F_XL + k) * JT + l], Pj[(F_V + k) * JT + l]);
+            Pj[F_M * JT + l] = raw_m(R, l);
         }
         __syncthreads();
 
-        for (int c0 = 0; c0 < ni; c0 += 32) {
-            const int nic = min(32, ni - c0);
-            int lg = 1;                                   // lanes per warp = 2^lg i-particles x 2^(5-lg) j-sub-ranges of 2^lg j each
-            while ((1 << lg) < nic) ++lg;
-            const int pw = 1 << lg;
-            const int ii = lane & (pw - 1), jsub = lane >> lg;
-            const bool act = ii < nic;
-            IPart I;
-            int my = -1;
+        // The pairs.  i-particles in chunks of 32, C = 1, 2, .. 16 chunks at a time; a chunk is worked on by HL_NW / C warps, each
+        // taking a j-slice of JT C / HL_NW particles of every tile (small blocks: one chunk, 16 slices of 16 j; 512 particles:
+        // 16 chunks at once, every warp sweeps whole tiles and no two warps share an i-particle).  Inside a warp the lanes are
+        // 2^lg i-particles x 2^(5 - lg) j-sub-ranges (lg >= 2: every lane has whole packed pairs).  FP32 sums run over one
+        // tile slice (<= 256 j) and are folded into fp64 (reading 9); the lanes of one i-particle are then added by a
+        // fixed shuffle tree, the slices in slice order, the CTAs in CTA order (phase C): bit-reproducible.
+        {
+            const int nch = (ni + 31) / 32;
+            int C = 1;
+            while (C < HL_NW && C < nch) C <<= 1;
+            const int nsl = HL_NW / C, cw = w / nsl, sw = w % nsl, jper = JT / nsl;
+            for (int r0 = 0; r0 < nch; r0 += C) {
+                const int c0 = (r0 + cw) * 32;
+                const int nic = max(0, min(32, ni - c0));
+                int lg = 2;
+                while ((1 << lg) < nic) ++lg;
+                const int pw = 1 << lg, jn = (jper * pw) >> 5;          // j-particles per lane and tile
+                const int ii = lane & (pw - 1), jsub = lane >> lg;
+                const bool act = ii < nic;
+                double acc7[7] = {0, 0, 0, 0, 0, 0, 0};
+                if (act) {
+                    IPart I;
 #pragma unroll
-            for (int k = 0; k < 3; ++k) {
-                I.nxh[k] = dup(act ? -sm.ipart[c0 + ii][k] : 0.0f);
-                I.nxl[k] = dup(act ? -sm.ipart[c0 + ii][3 + k] : 0.0f);
-                I.nv[k] = dup(act ? -sm.ipart[c0 + ii][6 + k] : 0.0f);
-                I.a[k] = dup(0.0f);
-                I.j[k] = dup(0.0f);
-            }
-            I.p = dup(0.0f);
-            if (act) my = sm.iidx[c0 + ii];
-            if (act) {
-                for (int kk = 0; kk < Kc; ++kk) {
-                    const float *Pj = sm.pred[kk];
-                    const int *JX = reinterpret_cast<const int *>(sm.raw[kk] + RAW_IDX);
-                    const int jl0 = 32 * w + jsub * pw;
-                    const int ja0 = (cta + kk * G) * JT + jl0;
-                    for (int q = 0; q < pw; q += 2) {
-                        const int jl = jl0 + q, ja = ja0 + q;
-                        float2 f[NF];
+                    for (int k = 0; k < 3; ++k) {
+                        I.nxh[k] = dup(-sm.ipart[c0 + ii][k]);
+                        I.nxl[k] = dup(-sm.ipart[c0 + ii][3 + k]);
+                        I.nv[k] = dup(-sm.ipart[c0 + ii][6 + k]);
+                    }
+                    const int my = sm.iidx[c0 + ii];
+                    for (int kk = 0; kk < Kc; ++kk) {
 #pragma unroll
-                        for (int k = 0; k < NF; ++k) f[k] = *reinterpret_cast<const float2 *>(Pj + k * JT + jl);
-                        const int2 jx = *reinterpret_cast<const int2 *>(JX + jl);
-                        float2 r2;
-                        pair2_checked<NEWTON>(I, f[0], f[1], f[2], f[3], f[4], f[5], f[6], f[7], f[8], f[9], eps2,
-                                              (ja < A.nj) && (jx.x != my), (ja + 1 < A.nj) && (jx.y != my), r2);
+                        for (int k = 0; k < 3; ++k) { I.a[k] = dup(0.0f); I.j[k] = dup(0.0f); }
+                        I.p = dup(0.0f);
+                        const float *Pj = sm.pred[kk];
+                        const int *JX = reinterpret_cast<const int *>(sm.raw[kk] + RAW_IDX);
+                        const int jl0 = jper * sw + jsub * jn;
+                        const int ja0 = (cta + kk * G) * JT + jl0;
+#pragma unroll 2
+                        for (int q = 0; q < jn; q += 2) {
+                            const int jl = jl0 + q, ja = ja0 + q;
+                            float2 f[NF];
+#pragma unroll
+                            for (int k = 0; k < NF; ++k) f[k] = *reinterpret_cast<const float2 *>(Pj + k * JT + jl);
+                            const int2 jx = *reinterpret_cast<const int2 *>(JX + jl);
+                            float2 r2;
+                            pair2_checked<NEWTON>(I, f[0], f[1], f[2], f[3], f[4], f[5], f[6], f[7], f[8], f[9], eps2,
+                                                  (ja < A.nj) && (jx.x != my), (ja + 1 < A.nj) && (jx.y != my), r2);
+                        }
+#pragma unroll
+                        for (int k = 0; k < 3; ++k) {
+                            acc7[k] += (double)I.a[k].x + (double)I.a[k].y;
+                            acc7[3 + k] += (double)I.j[k].x + (double)I.j[k].y;
+                        }
+                        acc7[6] -= (double)I.p.x + (double)I.p.y;
                     }
                 }
-            }
-            // the lanes of one i-particle (its j-sub-ranges): fixed shuffle tree, FP32 (chains of <= 256 pairs, reading 9)
-            float v7[7] = {__fadd_rn(I.a[0].x, I.a[0].y), __fadd_rn(I.a[1].x, I.a[1].y), __fadd_rn(I.a[2].x, I.a[2].y),
-                           __fadd_rn(I.j[0].x, I.j[0].y), __fadd_rn(I.j[1].x, I.j[1].y), __fadd_rn(I.j[2].x, I.j[2].y),
-                           __fadd_rn(I.p.x, I.p.y)};
-            for (int o = pw; o < 32; o <<= 1) {
+                for (int o = pw; o < 32; o <<= 1) {
 #pragma unroll
-                for (int k = 0; k < 7; ++k) v7[k] = __fadd_rn(v7[k], __shfl_xor_sync(FULL, v7[k], o));
-            }
-            if (lane < pw) {
-#pragma unroll
-                for (int k = 0; k < 7; ++k) sm.wsum[w][lane][k] = (double)v7[k];
-            }
-            __syncthreads();
-            if (tid < nic) {                              // the warps in warp order, fp64: one partial per (i, CTA)
-                double s7[7];
-#pragma unroll
-                for (int k = 0; k < 7; ++k) s7[k] = sm.wsum[0][tid][k];
-#pragma unroll
-                for (int q = 1; q < HL_NW; ++q) {
-#pragma unroll
-                    for (int k = 0; k < 7; ++k) s7[k] += sm.wsum[q][tid][k];
+                    for (int k = 0; k < 7; ++k) acc7[k] += __shfl_xor_sync(FULL, acc7[k], o);
                 }
-                const size_t o = (size_t)cta * A.P.stride_s + (size_t)(c0 + tid) * A.P.stride_i;
+                if (lane < pw) {
 #pragma unroll
-                for (int k = 0; k < 3; ++k) { __stcg(A.P.acc[k] + o, s7[k]); __stcg(A.P.jrk[k] + o, s7[3 + k]); }
-                __stcg(A.P.pot + o, -s7[6]);
+                    for (int k = 0; k < 7; ++k) sm.wsum[w][lane][k] = acc7[k];
+                }
+                __syncthreads();
+                // the slices of every chunk in slice order: one partial per (i, CTA), published as 14 self-validating words
+                for (int q = tid; q < C * 32 * 7; q += HL_THREADS) {
+                    const int cq = q / (32 * 7), i = (q / 7) % 32, k = q % 7;
+                    const int gi = (r0 + cq) * 32 + i;
+                    if (gi < ni) {
+                        double sv = sm.wsum[cq * nsl][i][k];
+                        for (int u = 1; u < nsl; ++u) sv += sm.wsum[cq * nsl + u][i][k];
+                        const unsigned long long b = (unsigned long long)__double_as_longlong(sv);
+                        unsigned long long *ch = A.chunk + ((size_t)gi * HL_CHUNK_WORDS + 2 * k) * G + cta;
+                        hl_store_word(ch, (unsigned int)b, gen);
+                        hl_store_word(ch + G, (unsigned int)(b >> 32), gen);
+                    }
+                }
+                __syncthreads();
+            }
+        }
+
+        // ================= phase C: owners poll the G partials of their particles (fixed order), correct, update the resident tile
+        // The partials of HL_CQ particles at a time: every thread polls its share of their nq x 14 x G words (all loads of a round in
+        // flight together: one L2 round trip after the last writer), the payloads go to shared memory (the idle wsum), then one
+        // warp per particle adds them in fixed order.
+        const int nown = sm.nown;
+        unsigned int *stage = reinterpret_cast<unsigned int *>(&sm.wsum[0][0][0]);       // [HL_CQ][14][G]
+        for (int q0 = 0; q0 < nown; q0 += HL_CQ) {
+            const int nq = min(HL_CQ, nown - q0);
+            const int nwords = nq * HL_CHUNK_WORDS * G;
+            for (int e0 = 0; e0 < nwords; e0 += HL_THREADS * HL_CPOLL) {
+                unsigned int spins = 0;
+                bool done[HL_CPOLL];
+#pragma unroll
+                for (int r = 0; r < HL_CPOLL; ++r) done[r] = e0 + r * HL_THREADS + tid >= nwords;
+                for (;;) {
+                    unsigned long long v[HL_CPOLL];
+#pragma unroll
+                    for (int r = 0; r < HL_CPOLL; ++r) {
+                        const int e = e0 + r * HL_THREADS + tid;
+                        if (!done[r]) v[r] = hl_load_word(A.chunk + (size_t)sm.own_k[q0 + e / (HL_CHUNK_WORDS * G)] * HL_CHUNK_WORDS * G + e % (HL_CHUNK_WORDS * G));
+                    }
+                    bool all = true;
+#pragma unroll
+                    for (int r = 0; r < HL_CPOLL; ++r) {
+                        if (!done[r]) {
+                            if ((unsigned int)(v[r] >> 32) == gen) { stage[e0 + r * HL_THREADS + tid] = (unsigned int)v[r]; done[r] = true; }
+                            else all = false;
+                        }
+                    }
+                    if (all) break;
+                    if (++spins > (1u << 26)) __trap();
+                }
             }
             __syncthreads();
-        }
-        HL_STAMP(5);
-        hl_grid_barrier(A.bar, G);
-        HL_STAMP(6);
-
-        // ================= phase C: owners combine (fixed order) and correct their particles
-        const int nown = sm.nown;
-        for (int q = w; q < nown; q += HL_NW) {
-            const int k = sm.own_k[q], slot = sm.own_l[q];
+            if (w < nq) {
+            const int q = q0 + w;
+            const int k = sm.own_k[q], sl = sm.own_l[q];
+            const unsigned int *sg = stage + (size_t)w * HL_CHUNK_WORDS * G;
             double v[7] = {0, 0, 0, 0, 0, 0, 0};
             for (int s = lane; s < G; s += 32) {
-                const size_t o = (size_t)s * A.P.stride_s + (size_t)k * A.P.stride_i;
 #pragma unroll
-                for (int c = 0; c < 3; ++c) { v[c] += __ldcg(A.P.acc[c] + o); v[3 + c] += __ldcg(A.P.jrk[c] + o); }
-                v[6] += __ldcg(A.P.pot + o);
+                for (int c = 0; c < 7; ++c)
+                    v[c] += __longlong_as_double((long long)(((unsigned long long)sg[(2 * c + 1) * G + s] << 32) | sg[2 * c * G + s]));
             }
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) {
@@ -380,22 +537,47 @@ k_hd_loop(const HlArgs A)
                 for (int c = 0; c < 7; ++c) v[c] += __shfl_xor_sync(FULL, v[c], o);
             }
             if (lane == 0) {
-#pragma unroll
-                for (int c = 0; c < 3; ++c) { A.a1[3 * (size_t)k + c] = v[c]; A.ad1[3 * (size_t)k + c] = v[3 + c]; }
-                A.pot[k] = v[6];
-                hd_correct_one(A.S, A.B, A.C, k, tn);      // corrector, new step, j-store record (global)
-                const int kk = slot / JT, l = slot % JT;
+                const int kk = sl / JT, l = sl % JT;
                 const int p = (cta + kk * G) * JT + l;
-                hl_store_tile(sm.raw[kk], l, A.S, p);       // ... and my resident copy
-                sm.tnext[kk][l] = tn + A.S.dt[p];
+                double a0[3], ad0[3], xi[3], vi[3], x1[3], v1[3], h;
+                if (inl) {
+                    const double *st = sm.own_st[kk * HL_INLINE + (k - sm.s_off[cta + kk * G])];
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) { xi[c] = st[c]; vi[c] = st[3 + c]; a0[c] = st[6 + c]; ad0[c] = st[9 + c]; }
+                    h = st[12];
+                } else {
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        xi[c] = A.B.xi[3 * (size_t)k + c]; vi[c] = A.B.vi[3 * (size_t)k + c];
+                        a0[c] = A.S.a[3 * (size_t)p + c]; ad0[c] = A.S.ad[3 * (size_t)p + c];
+                    }
+                    h = A.S.dt[p];
+                }
+                const double d = hd_correct_core(h, a0, ad0, v, v + 3, xi, vi, tn, A.C.eta, A.C.dt_max, x1, v1);
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    A.a1[3 * (size_t)k + c] = v[c]; A.ad1[3 * (size_t)k + c] = v[3 + c];
+                    A.S.x[3 * (size_t)p + c] = x1[c]; A.S.v[3 * (size_t)p + c] = v1[c];
+                    A.S.a[3 * (size_t)p + c] = v[c]; A.S.ad[3 * (size_t)p + c] = v[3 + c];
+                }
+                A.pot[k] = v[6];
+                A.S.t[p] = tn;
+                A.S.dt[p] = d;
+                atomicMin(A.C.dt_min_bits, (unsigned long long)__double_as_longlong(d));
+                const float m = raw_m(sm.raw[kk], l);
+                hl_store_tile(sm.raw[kk], l, p, x1, v1, v, v + 3, tn, m);                                   // my resident copy
+                hl_store_tile(A.C.raw + (size_t)(cta + kk * G) * RAW_TILE_BYTES, l, p, x1, v1, v, v + 3, tn, m);   // the j-store
+                sm.tnext[kk][l] = tn + d;
             }
+            }
+            __syncthreads();
         }
-        HL_STAMP(7);
-        if (cta == 0 && tid == 0 && ni < 32) { for (int k = 0; k < 7; ++k) ph[k] += (long long)(stamp[k + 1] - stamp[k]); ph[7] += 1; }
+        if (tid == 0) sm.nown_prev = nown;
         t_sys = tn;
         ++steps;
         npart += ni;
         ni_last = ni;
+        n_inline += inl ? 1 : 0;
         if (cta == 0) {
             unsigned long long now;
             asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
@@ -415,7 +597,7 @@ k_hd_loop(const HlArgs A)
             A.status->reason = reason;
             A.status->ni_next = ni_next;
             A.status->ni_last = ni_last;
-            for (int k = 0; k < 8; ++k) A.status->phase_ns[k] = ph[k];
+            A.status->inline_steps = n_inline;
             if (reason == HL_BIG) { *A.B.d_ni = ni_next; *A.B.d_tnext = t_big; }
             else if (ni_last > 0) { *A.B.d_ni = ni_last; *A.B.d_tnext = t_sys; }
         }
