@@ -41,6 +41,7 @@ struct g6hd_system {
     long long big_n[64] = {};
     long long inline_steps = 0;
 
+
     bool loop_profile = false;
 };
 
@@ -126,6 +127,7 @@ int hd_loop_run(Cluster &c, g6hd_system &s, double t_end, long long max_steps, H
     A.eps2 = (float)s.eps2; A.ds = c.opt_ds;
     A.gen0 = s.loop_gen;
     A.rec = s.rec; A.chunk = s.chunk; A.flag = s.flag; A.status = s.hd_status;
+
 
     void *args[] = {(void *)&A};
     const void *fn = c.opt_newton ? (const void *)k_hd_loop<true> : (const void *)k_hd_loop<false>;

@@ -106,6 +106,10 @@ struct HlSmem {
 static_assert(sizeof(HlSmem) <= 232448, "loop kernel shared memory");
 static_assert(sizeof(double) * HL_NW * 32 * 7 >= sizeof(unsigned int) * HL_CQ * HL_CHUNK_WORDS * HL_MAX_G, "chunk staging fits in wsum");
 
+// acquire-release fence at device scope.  (__threadfence() is the sequentially consistent fence and, on sm_100, also invalidates the
+// whole L1: MEMBAR.SC.GPU + CCTL.IVALL, measured several microseconds per step with the exchange stores in flight.)
+__device__ __forceinline__ void hl_fence() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
+
 __device__ __forceinline__ void hl_store_word(unsigned long long *p, unsigned int payload, unsigned int gen)
 {
     const unsigned long long v = (unsigned long long)payload | ((unsigned long long)gen << 32);
@@ -140,7 +144,7 @@ __device__ __forceinline__ void hl_flag_barrier(unsigned int *flag, unsigned int
 {
     __syncthreads();
     if (threadIdx.x == 0) {
-        __threadfence();
+        hl_fence();
         asm volatile("st.volatile.global.u32 [%0], %1;" ::"l"(flag + blockIdx.x), "r"(gen) : "memory");
     }
     for (unsigned int s = threadIdx.x; s < G; s += HL_THREADS) {
@@ -149,7 +153,7 @@ __device__ __forceinline__ void hl_flag_barrier(unsigned int *flag, unsigned int
             asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(v) : "l"(flag + s) : "memory");
             if (++spins > (1u << 26)) __trap();
         } while (v != gen);
-        __threadfence();
+        hl_fence();
     }
     __syncthreads();
 }
@@ -167,6 +171,28 @@ __device__ __forceinline__ void hl_store_tile(char *T, int l, int p, const doubl
     raw_t(T, l) = t;
     raw_m(T, l) = m;
     raw_idx(T, l) = p;
+}
+
+// the record of one tile from the eight ballots of "slot is at the tile's minimum": count and the first HL_INLINE slots (increasing)
+__device__ __forceinline__ void hl_make_record(const unsigned int *bal, double tmin, unsigned int *recw)
+{
+    int c = 0;
+    unsigned int sl[2] = {0u, 0u};
+    for (int q = 0; q < JT / 32; ++q) {
+        unsigned b = bal[q];
+        while (b) {
+            const int l = __ffs(b) - 1;
+            b &= b - 1;
+            if (c < HL_INLINE) sl[c >> 2] |= (unsigned)(32 * q + l) << (8 * (c & 3));
+            ++c;
+        }
+    }
+    const unsigned long long tb = (unsigned long long)__double_as_longlong(tmin);
+    recw[0] = (unsigned int)tb;
+    recw[1] = (unsigned int)(tb >> 32);
+    recw[2] = (unsigned int)c;
+    recw[3] = sl[0];
+    recw[4] = sl[1];
 }
 
 template <bool NEWTON>
@@ -195,6 +221,7 @@ k_hd_loop(const HlArgs A)
     __syncthreads();
 
     if (tid == 0) sm.nown_prev = 0;
+    bool rescan = true;                    // my tiles' records must be recomputed (start; after I corrected particles)
     double t_sys = A.t_sys;
     long long steps = 0, npart = 0, n_inline = 0;
     long long hist = 0, hist_ns = 0;       // thread b < 64 of CTA 0 counts bin b
@@ -213,110 +240,154 @@ k_hd_loop(const HlArgs A)
         unsigned long long *rec = A.rec + (size_t)(gen & 1u) * G * A.ntiles * HL_REC_WORDS;
 
         // ================= phase A: per own tile (min, count, first slots at the min) of t + dt -> its record
-        // the two halves of the CTA take the tiles of their parity; a warp holds 32 consecutive slots of one tile
-        for (int kk = half; kk < Kc; kk += 2) {
-            double m = sm.tnext[kk][slot];
+        // Only a CTA that corrected particles in the last step (or starts) has anything to recompute; the others republish what
+        // they had under the new step number.  Several resident tiles: the whole CTA rescans (its two halves take the tiles of
+        // their parity, a warp holds 32 consecutive slots); one tile: warp 0 does it alone, with no block-wide barrier.
+        if (rescan && Kc > 1) {
+            for (int kk = half; kk < Kc; kk += 2) {
+                double m = sm.tnext[kk][slot];
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) m = fmin(m, __shfl_xor_sync(FULL, m, o));
-            if (lane == 0) sm.red[w][kk >> 1] = m;
-        }
-        __syncthreads();
-        for (int kk = half; kk < Kc; kk += 2) {
-            double m = sm.red[half * (JT / 32)][kk >> 1];
-#pragma unroll
-            for (int q = 1; q < JT / 32; ++q) m = fmin(m, sm.red[half * (JT / 32) + q][kk >> 1]);
-            const unsigned b = __ballot_sync(FULL, sm.tnext[kk][slot] == m);
-            if (lane == 0) sm.bal[kk][ws] = b;
-            if (slot == 0) sm.tmin[kk] = m;
-        }
-        __syncthreads();
-        if (tid < Kc) {
-            // thread kk: count and the first HL_INLINE slots at the minimum of tile kk, from the eight warp ballots
-            const int kk = tid;
-            int c = 0;
-            unsigned int sl[2] = {0u, 0u};
-            for (int q = 0; q < JT / 32; ++q) {
-                unsigned b = sm.bal[kk][q];
-                while (b) {
-                    const int l = __ffs(b) - 1;
-                    b &= b - 1;
-                    if (c < HL_INLINE) sl[c >> 2] |= (unsigned)(32 * q + l) << (8 * (c & 3));
-                    ++c;
-                }
+                for (int o = 16; o > 0; o >>= 1) m = fmin(m, __shfl_xor_sync(FULL, m, o));
+                if (lane == 0) sm.red[w][kk >> 1] = m;
             }
-            const unsigned long long tb = (unsigned long long)__double_as_longlong(sm.tmin[kk]);
-            sm.recw[kk][0] = (unsigned int)tb;
-            sm.recw[kk][1] = (unsigned int)(tb >> 32);
-            sm.recw[kk][2] = (unsigned int)c;
-            sm.recw[kk][3] = sl[0];
-            sm.recw[kk][4] = sl[1];
+            __syncthreads();
+            for (int kk = half; kk < Kc; kk += 2) {
+                double m = sm.red[half * (JT / 32)][kk >> 1];
+#pragma unroll
+                for (int q = 1; q < JT / 32; ++q) m = fmin(m, sm.red[half * (JT / 32) + q][kk >> 1]);
+                const unsigned b = __ballot_sync(FULL, sm.tnext[kk][slot] == m);
+                if (lane == 0) sm.bal[kk][ws] = b;
+                if (slot == 0) sm.tmin[kk] = m;
+            }
+            __syncthreads();
+            if (tid < Kc) hl_make_record(sm.bal[tid], sm.tmin[tid], sm.recw[tid]);
+            __syncthreads();
         }
-        // Release: the Hermite state of my particles that phase C of the last step wrote must be visible to whoever reads the
-        // records (only a CTA that corrected particles has anything to release)
-        if (tid == 0 && sm.nown_prev > 0) __threadfence();
-        __syncthreads();
-        for (int e = tid; e < G * Kc * HL_REC_WORDS; e += HL_THREADS) {
-            const int c = e / (Kc * HL_REC_WORDS), r = e % (Kc * HL_REC_WORDS), kk = r / HL_REC_WORDS, wd = r % HL_REC_WORDS;
-            hl_store_word(rec + ((size_t)c * A.ntiles + (cta + kk * G)) * HL_REC_WORDS + wd, sm.recw[kk][wd], gen);
-        }
+        if (w == 0) {
+            // everything from here to the barrier below is warp 0's: rescan (one tile), publish, poll, select
+            if (rescan && Kc == 1) {
+                double v[JT / 32], m = INF;                   // lane holds the slots lane, lane + 32, ...
+#pragma unroll
+                for (int r = 0; r < JT / 32; ++r) { v[r] = sm.tnext[0][32 * r + lane]; m = fmin(m, v[r]); }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) m = fmin(m, __shfl_xor_sync(FULL, m, o));
+#pragma unroll
+                for (int r = 0; r < JT / 32; ++r) {
+                    const unsigned b = __ballot_sync(FULL, v[r] == m);
+                    if (lane == 0) sm.bal[0][r] = b;
+                }
+                __syncwarp();
+                if (lane == 0) hl_make_record(sm.bal[0], m, sm.recw[0]);
+            }
+            // Release: the Hermite state of my particles that phase C of the last step wrote (other warps, ordered before this
+            // point by the barriers of phase C) must be visible to whoever reads the records
+            if (lane == 0 && sm.nown_prev > 0) hl_fence();
+            __syncwarp();
+            for (int e = lane; e < G * Kc * HL_REC_WORDS; e += 32) {
+                const int c = e / (Kc * HL_REC_WORDS), r = e % (Kc * HL_REC_WORDS), kk = r / HL_REC_WORDS, wd = r % HL_REC_WORDS;
+                hl_store_word(rec + ((size_t)c * A.ntiles + (cta + kk * G)) * HL_REC_WORDS + wd, sm.recw[kk][wd], gen);
+            }
 
-        // everybody polls every record: t_next, n_i, offsets of the tiles in the active list (tile order = increasing address)
-        {
+            // poll every tile's record (my private copy): lane takes the tiles lane, lane + 32, ..., four at a time
             double m = INF;
-            for (int T = tid; T < A.ntiles; T += HL_THREADS) {
-                unsigned int wd[HL_REC_WORDS];
-                hl_wait_words<HL_REC_WORDS>(rec + ((size_t)cta * A.ntiles + T) * HL_REC_WORDS, 1, gen, wd);
-                const double tm = __longlong_as_double((long long)(((unsigned long long)wd[1] << 32) | wd[0]));
-                sm.s_tm[T] = tm;
-                sm.s_tc[T] = (int)wd[2];
-                sm.s_sl[T][0] = wd[3];
-                sm.s_sl[T][1] = wd[4];
-                m = fmin(m, tm);
+            for (int g0 = 0; g0 < A.ntiles; g0 += 128) {
+                bool done[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) done[u] = g0 + lane + 32 * u >= A.ntiles;
+                unsigned int spins = 0;
+                for (;;) {
+                    unsigned long long v[4][HL_REC_WORDS];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        if (!done[u]) {
+                            const unsigned long long *r = rec + ((size_t)cta * A.ntiles + g0 + lane + 32 * u) * HL_REC_WORDS;
+#pragma unroll
+                            for (int k = 0; k < HL_REC_WORDS; ++k) v[u][k] = hl_load_word(r + k);
+                        }
+                    }
+                    bool all = true;
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        if (!done[u]) {
+                            bool ok = true;
+#pragma unroll
+                            for (int k = 0; k < HL_REC_WORDS; ++k) ok = ok && (unsigned int)(v[u][k] >> 32) == gen;
+                            if (ok) {
+                                const int T = g0 + lane + 32 * u;
+                                const double tm = __longlong_as_double((long long)((v[u][1] << 32) | (v[u][0] & 0xffffffffull)));
+                                sm.s_tm[T] = tm;
+                                sm.s_tc[T] = (int)(unsigned int)v[u][2];
+                                sm.s_sl[T][0] = (unsigned int)v[u][3];
+                                sm.s_sl[T][1] = (unsigned int)v[u][4];
+                                m = fmin(m, tm);
+                                done[u] = true;
+                            } else {
+                                all = false;
+                            }
+                        }
+                    }
+                    if (all) break;
+                    if (++spins > (1u << 26)) __trap();
+                }
             }
-            __threadfence();                               // acquire: what the records' writers published before them
+            hl_fence();                               // acquire: what the records' writers published before them
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) m = fmin(m, __shfl_xor_sync(FULL, m, o));
-            if (lane == 0) sm.red[w][0] = m;
-            __syncthreads();
-            m = sm.red[0][0];
+            // t_next = m; offsets of the tiles in the active list (tile order = increasing address); n_i
+            int run = 0, over = 0;
+            for (int T0 = 0; T0 < A.ntiles; T0 += 32) {
+                const int T = T0 + lane;
+                const bool hit = T < A.ntiles && sm.s_tm[T] == m;
+                const int c = hit ? sm.s_tc[T] : 0;
+                over |= c > HL_INLINE;
+                int inc = c;
 #pragma unroll
-            for (int q = 1; q < HL_NW; ++q) m = fmin(m, sm.red[q][0]);
-            if (w == 0) {
-                int run = 0, over = 0;
-                for (int T0 = 0; T0 < A.ntiles; T0 += 32) {
-                    const int T = T0 + lane;
-                    const bool hit = T < A.ntiles && sm.s_tm[T] == m;
-                    const int c = hit ? sm.s_tc[T] : 0;
-                    over |= c > HL_INLINE;
-                    int inc = c;
-#pragma unroll
-                    for (int o = 1; o < 32; o <<= 1) {
-                        const int u = __shfl_up_sync(FULL, inc, o);
-                        if (lane >= o) inc += u;
-                    }
-                    if (T < A.ntiles) sm.s_off[T] = hit ? run + inc - c : -1;
-                    run += __shfl_sync(FULL, inc, 31);
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int u = __shfl_up_sync(FULL, inc, o);
+                    if (lane >= o) inc += u;
                 }
-                over = __any_sync(FULL, over);
-                if (lane == 0) { sm.ni = run; sm.gmin = m; sm.inl = !over && run <= A.max_i; }
+                if (T < A.ntiles) sm.s_off[T] = hit ? run + inc - c : -1;
+                run += __shfl_sync(FULL, inc, 31);
             }
-            __syncthreads();
+            over = __any_sync(FULL, over);
+            const bool inl_w = !over && run <= A.max_i;
+            if (inl_w) {
+                // the active list, from the slots inside the records
+                for (int T = lane; T < A.ntiles; T += 32) {
+                    const int base = sm.s_off[T];
+                    if (base < 0) continue;
+                    const int c = sm.s_tc[T];
+                    for (int r = 0; r < c; ++r) sm.iidx[base + r] = T * JT + (int)((sm.s_sl[T][r >> 2] >> (8 * (r & 3))) & 0xffu);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) {
+                sm.ni = run; sm.gmin = m; sm.inl = inl_w;
+                if (inl_w) {
+                    // my active particles: (position in the list, slot), tile by tile
+                    int nown = 0;
+                    for (int kk = 0; kk < Kc; ++kk) {
+                        const int T = cta + kk * G, base = sm.s_off[T];
+                        if (base < 0) continue;
+                        for (int r = 0; r < sm.s_tc[T]; ++r) {
+                            sm.own_k[nown] = base + r;
+                            sm.own_l[nown] = kk * JT + (int)((sm.s_sl[T][r >> 2] >> (8 * (r & 3))) & 0xffu);
+                            ++nown;
+                        }
+                    }
+                    sm.nown = nown;
+                }
+            }
         }
+        __syncthreads();
         const double tn = sm.gmin;
         const int ni = sm.ni;
         const bool big = ni > A.max_i, inl = sm.inl != 0;
 
         if (inl) {
-            // ---- every CTA builds the active list and predicts all n_i particles itself (fp64 Eq. 1-2), straight into its i-block
-            for (int T = tid; T < A.ntiles; T += HL_THREADS) {
-                const int base = sm.s_off[T];
-                if (base < 0) continue;
-                const int c = sm.s_tc[T];
-                for (int r = 0; r < c; ++r) sm.iidx[base + r] = T * JT + (int)((sm.s_sl[T][r >> 2] >> (8 * (r & 3))) & 0xffu);
-            }
-            __syncthreads();
-            int nown = 0;
-            for (int k = tid; k < ni; k += HL_THREADS) {
+            // ---- every CTA predicts all n_i particles itself (fp64 Eq. 1-2), straight into its i-block: the lower half of the
+            // CTA; the upper half predicts the resident j-particles meanwhile (below)
+            for (int k = tid; k < ni && tid < HL_THREADS / 2; k += HL_THREADS / 2) {
                 const int p = sm.iidx[k];
                 const double tp = __ldcg(A.S.t + p);
                 const double h = tn - tp, h2 = h * h / 2, h3 = h * h * h / 6;
@@ -342,19 +413,6 @@ k_hd_loop(const HlArgs A)
                 }
                 if (mine) sm.own_st[(T / G) * HL_INLINE + (k - sm.s_off[T])][12] = h;
                 if (cta == 0) A.B.act[k] = p;
-            }
-            // my active particles: (position in the list, slot), tile by tile
-            if (tid == 0) {
-                for (int kk = 0; kk < Kc; ++kk) {
-                    const int T = cta + kk * G, base = sm.s_off[T];
-                    if (base < 0) continue;
-                    for (int r = 0; r < sm.s_tc[T]; ++r) {
-                        sm.own_k[nown] = base + r;
-                        sm.own_l[nown] = kk * JT + (int)((sm.s_sl[T][r >> 2] >> (8 * (r & 3))) & 0xffu);
-                        ++nown;
-                    }
-                }
-                sm.nown = nown;
             }
         } else {
             // ---- owners: active particles of my tiles, in address order, predicted in fp64 into the global i-block
@@ -392,7 +450,7 @@ k_hd_loop(const HlArgs A)
         }
 
         // ================= phase B: my j-particles -> Eq. 1-2 at tn, then all pairs
-        for (int q = tid; q < Kc * JT; q += HL_THREADS) {
+        for (int q = inl ? tid - HL_THREADS / 2 : tid; q >= 0 && q < Kc * JT; q += inl ? HL_THREADS / 2 : HL_THREADS) {
             const int kk = q / JT, l = q % JT;
             char *R = sm.raw[kk];
             float *Pj = sm.pred[kk];
@@ -573,6 +631,7 @@ k_hd_loop(const HlArgs A)
             __syncthreads();
         }
         if (tid == 0) sm.nown_prev = nown;
+        rescan = nown > 0;
         t_sys = tn;
         ++steps;
         npart += ni;
@@ -584,7 +643,8 @@ k_hd_loop(const HlArgs A)
             if (tid < 30 && ni >= (1 << tid) && ni < (2 << tid)) { ++hist; hist_ns += (long long)(now - t_step); }
             t_step = now;
         }
-        __syncthreads();
+        // no barrier here: after the force phase's last barrier only phase C (which ends with one) touches shared memory, and the
+        // next step begins with warp 0 alone up to the barrier that follows its selection
     }
 
     if (cta == 0) {
