@@ -110,7 +110,7 @@ struct Cluster {
     int last_kernel = 0;       // force kernel of the last call: 1 checked reference, 2 fast sweep kernel, 3 block-step kernel
 
     // options
-    int opt_ds = 1, opt_newton = 1, opt_jsplit = 0, opt_kernel = 0, opt_timers = 0, opt_variant = 0, opt_small = 32, opt_nb_maxlen = 256;
+    int opt_ds = 1, opt_newton = 1, opt_jsplit = 0, opt_kernel = 0, opt_timers = 0, opt_variant = 0, opt_small = 32, opt_nb_maxlen = 256, opt_bs_design = 0;
     bool small_explicit = false;   // option "small" was set by the caller (else the N_j-dependent rule of small_limit)
 };
 
@@ -480,7 +480,7 @@ int small_limit(const Cluster &c, int nj)
 {
     if (c.small_explicit) return c.opt_small;
     const int ntiles = (nj + JT - 1) / JT;
-    return ntiles >= 1024 ? 48 : (ntiles >= 256 ? 32 : 24);
+    return ntiles >= 1024 ? 64 : (ntiles >= 256 ? 40 : 28);
 }
 
 bool use_block_step(const Cluster &c, int ni, int nj, bool nb = false)
@@ -563,6 +563,11 @@ int run_force(Cluster &c, int nj, int ni, const int *d_index, const double *d_xi
         }
         if (ev_pred_done) CK(cudaEventRecord(ev_pred_done, c.stream));     // predictor fused: no separate phase
         const JRecord *upd = inline_upd ? c.h_rec[c.rec_cur] : nullptr;
+        // without neighbour lists: the second design (lanes = i-particle x j-sub-range in the pair phase); option "bs_design" = 1 pins the first
+        if (!nb && c.opt_bs_design != 1)
+            rc = big ? bs2_launch_t<BS_MAX_I>(B, c.opt_newton != 0, G, hb ? hb->xi : nullptr, hb ? hb->vi : nullptr, hb ? hb->index : nullptr, upd, c.stream)
+                     : bs2_launch_t<16>(B, c.opt_newton != 0, G, hb ? hb->xi : nullptr, hb ? hb->vi : nullptr, hb ? hb->index : nullptr, upd, c.stream);
+        else
         rc = big ? bs_launch_t<BS_MAX_I>(B, c.opt_newton != 0, G, hb ? hb->xi : nullptr, hb ? hb->vi : nullptr, hb ? hb->index : nullptr, upd, c.stream)
                  : bs_launch_t<16>(B, c.opt_newton != 0, G, hb ? hb->xi : nullptr, hb ? hb->vi : nullptr, hb ? hb->index : nullptr, upd, c.stream);
         if (rc) return fail(c, G6_ERR_CUDA, "block-step kernel launch failed: %s", cudaGetErrorString((cudaError_t)rc));
@@ -1207,6 +1212,7 @@ static int *option_slot(Cluster &c, const char *key)
     if (!strcmp(key, "variant")) return &c.opt_variant;
     if (!strcmp(key, "small")) return &c.opt_small;
     if (!strcmp(key, "nb_maxlen")) return &c.opt_nb_maxlen;
+    if (!strcmp(key, "bs_design")) return &c.opt_bs_design;
     return nullptr;
 }
 
@@ -1216,7 +1222,7 @@ int g6x_set_option(int clusterid, const char *key, int value)
     int *slot = option_slot(c, key);
     if (!slot) return fail(c, G6_ERR_ARG, "unknown option '%s'", key ? key : "(null)");
     const bool is_flag = slot == &c.opt_ds || slot == &c.opt_newton || slot == &c.opt_timers;
-    if (value < 0 || (is_flag && value > 1) || (slot == &c.opt_kernel && value > 2) || (slot == &c.opt_jsplit && value > 65535) || (slot == &c.opt_small && value > BS_MAX_I) ||
+    if (value < 0 || (is_flag && value > 1) || (slot == &c.opt_kernel && value > 2) || (slot == &c.opt_jsplit && value > 65535) || (slot == &c.opt_small && value > BS_MAX_I) || (slot == &c.opt_bs_design && value > 2) ||
         (slot == &c.opt_nb_maxlen && (value < 1 || value > 4096)) ||
         (slot == &c.opt_variant && value != 0 && !fast_is_built(FastVariant{value / 8, value % 8}, true)))
         return fail(c, G6_ERR_ARG, "bad value %d for option '%s'", value, key);

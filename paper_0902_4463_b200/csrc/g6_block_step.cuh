@@ -549,6 +549,373 @@ k_block_step_dbg(const BsArgs A)
     block_step_body<MAXI, NEWTON, true>(A, nullptr);
 }
 
+// ================================================================================================
+// k_block_step2 -- the block-step kernel without neighbour lists (the common case), second design.
+//
+// Same launch, same a-1 .. a-5 in one kernel, same ring of raw j-tiles fed by one TMA bulk copy per tile, same last-CTA
+// combine; what changes is the pair phase.  The first design kept lanes over j for the forces too and therefore had to
+// reduce the seven sums of every (i-particle, tile) over the warp (9 shuffles + two warp-wide integer reductions for the
+// nearest neighbour): a third of the instructions of a small block step.  Here a warp predicts its tile (lanes over j,
+// as before), writes the predicted particles to its OWN 11 KB buffer in shared memory and hands the raw slot back to the
+// ring at once; the pairs are then evaluated with LANES = (i-particle, j-sub-range) -- "several threads share an i and
+// split the j" -- so that every lane keeps the sums and the nearest neighbour of ITS i-particle in
+// registers across all the tiles the warp works on (FP32 over one tile slice, folded into fp64 per tile: DESIGN.md reading
+// 9), and the lanes of one i are reduced by a fixed shuffle tree ONCE, at the end of the kernel.  Blocks above 32 particles
+// take their i-particles in chunks of 32 (the predicted tile is re-read from shared memory, not re-predicted).
+// 8 warps; 6 ring slots for blocks up to 16 particles, 5 up to 64 (their fp64 sums take the room).  Measured at N_j = 2^20: 12 warps
+// with the 4 slots that then fit are 4 % faster at n_i = 16 but 14 % slower at n_i = 1, where the stream from HBM is everything
+__host__ __device__ constexpr int bs2_threads(int maxi) { return maxi <= 64 ? 256 : 256; }
+__host__ __device__ constexpr int bs2_nslots(int maxi) { return maxi <= 16 ? 6 : 5; }
+constexpr int BS2_PRED_BYTES = TILE_BYTES + JT * 4;      // predicted tile + the 256 indices
+
+template <int MAXI>
+struct Bs2Smem {
+    alignas(128) char raw[bs2_nslots(MAXI)][RAW_TILE_BYTES];  // ring of raw tiles: tile `it` of the CTA lives in slot it % NS
+    alignas(16) char pred[bs2_threads(MAXI) / 32][BS2_PRED_BYTES];            // per warp: its current tile, predicted (field-major floats) + indices
+    double acc[bs2_threads(MAXI) / 32][MAXI][8];                              // per-warp fp64 sums of every i (filled once, at the end)
+    float r2[bs2_threads(MAXI) / 32][MAXI];
+    int addr[bs2_threads(MAXI) / 32][MAXI];
+    float ipart[MAXI][9];
+    int iidx[MAXI];
+    int uaddr[MAXI];
+    alignas(8) uint64_t full[bs2_nslots(MAXI)];
+    volatile int armed[bs2_nslots(MAXI)];
+    int is_last;
+};
+static_assert(sizeof(Bs2Smem<16>) <= 232448 && sizeof(Bs2Smem<64>) <= 232448, "block-step (2) shared memory");
+
+template <int MAXI, bool NEWTON>
+__device__ __forceinline__ void block_step2_body(const BsArgs &A, const BsInline<MAXI> *Dp)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    Bs2Smem<MAXI> &sm = *reinterpret_cast<Bs2Smem<MAXI> *>(smem_raw);
+    constexpr float INF = __builtin_huge_valf();
+    constexpr int BS2_THREADS = bs2_threads(MAXI), NW = BS2_THREADS / 32, NS = bs2_nslots(MAXI), NCH = (MAXI + 31) / 32;
+    const unsigned FULL = 0xffffffffu;
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const int G = gridDim.x, cta = blockIdx.x;
+    const int nt = cta < A.ntiles ? (A.ntiles - cta + G - 1) / G : 0;
+
+    if (tid == 0) {
+#pragma unroll
+        for (int k = 0; k < NS; ++k) { mbar_init(&sm.full[k], 1); sm.armed[k] = k; }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+#pragma unroll
+        for (int k = 0; k < NS; ++k)
+            if (k < nt) {
+                mbar_expect_tx(&sm.full[k], RAW_TILE_BYTES);
+                tma_load_1d(sm.raw[k], A.raw + (size_t)(cta + k * G) * RAW_TILE_BYTES, RAW_TILE_BYTES, &sm.full[k]);
+            }
+    }
+    // i-block -> shared memory (double-single split here: the host hands fp64)
+    for (int k = tid; k < A.ni * 3; k += BS2_THREADS) {
+        const int i = k / 3, c = k % 3;
+        const double x = A.inline_i ? Dp->xi[i][c] : A.xi[k];
+        const double v = A.inline_i ? Dp->vi[i][c] : A.vi[k];
+        float hi, lo;
+        ds_split(x, hi, lo);
+        sm.ipart[i][c] = hi;
+        sm.ipart[i][3 + c] = A.ds ? lo : 0.0f;
+        sm.ipart[i][6 + c] = (float)v;
+    }
+    for (int i = tid; i < MAXI; i += BS2_THREADS) {
+        if (i < A.ni) sm.iidx[i] = A.inline_i ? Dp->index[i] : A.i_index[i];
+        sm.uaddr[i] = i < A.n_upd ? Dp->upd[i].addr : -1;
+    }
+    __syncthreads();
+
+    // my place in every chunk of 32 i-particles: lanes = 2^lg i-particles x 2^(5 - lg) j-sub-ranges of 8 x 2^lg j
+    int lg[NCH], ii[NCH], my[NCH];
+    bool act[NCH];
+    double acc7[NCH][7];
+    float best[NCH];
+    int baddr[NCH];
+#pragma unroll
+    for (int ch = 0; ch < NCH; ++ch) {
+        const int nic = max(0, min(32, A.ni - 32 * ch));
+        lg[ch] = 0;
+        while ((1 << lg[ch]) < nic) ++lg[ch];
+        ii[ch] = lane & ((1 << lg[ch]) - 1);
+        act[ch] = ii[ch] < nic;
+        my[ch] = act[ch] ? sm.iidx[32 * ch + ii[ch]] : -1;
+        best[ch] = INF;
+        baddr[ch] = 0x7fffffff;
+#pragma unroll
+        for (int k = 0; k < 7; ++k) acc7[ch][k] = 0.0;
+    }
+    const float2 eps2 = dup(A.eps2);
+    // the unchecked pair code needs s2 > 0 for every pair: a normal positive binary32 eps2 (as for the sweep kernel)
+    const bool fast_ok = A.eps2 >= 4.0f * 1.17549435e-38f && A.eps2 < INF;
+    const float2 eps2s = dup(pair_scale<NEWTON>() * A.eps2);
+    const double kP = NEWTON ? 0.5 * sqrt((double)FOUR_THIRDS) : sqrt((double)THIRD), kA = kP * kP * kP;
+    float *Pj = reinterpret_cast<float *>(sm.pred[w]);
+    int *JX = reinterpret_cast<int *>(sm.pred[w] + TILE_BYTES);
+
+    for (int it = w; it < nt; it += NW) {
+        const int tile = cta + it * G;
+        const int slot = it % NS;
+        char *R = sm.raw[slot];
+        // the copy of THIS tile must have been issued before its phase is waited for (a parity wait cannot tell phase
+        // p + 1 from the completed phase p - 1); with fewer slots than warps that holds from the first round on
+        if (it >= NS) {
+            uint32_t spins = 0;
+            while (ld_acquire_cta(&sm.armed[slot]) != it) { if (++spins > (1u << 26)) __trap(); }
+        }
+        mbar_wait(&sm.full[slot], (uint32_t)(it / NS) & 1u);
+
+        // ---- a-1: particles corrected in the last step that live in this tile: patch the staged copy, write through
+        if (A.n_upd > 0) {
+            for (int u = lane; u < A.n_upd; u += 32)
+                if (sm.uaddr[u] / JT == tile) {
+                    const JRecord r = Dp->upd[u];
+                    store_record(R, r.addr % JT, r);
+                    store_record(A.raw + (size_t)tile * RAW_TILE_BYTES, r.addr % JT, r);
+                }
+            __syncwarp();
+        }
+        // ---- a-2: predict my 8 j (lane l owns the pairs {2l, 2l + 1} + 64 g: conflict-free vector loads) into my warp's buffer
+        const bool ragged = tile * JT + JT > A.nj;
+        int id_lo = INT32_MAX, id_hi = INT32_MIN;
+#pragma unroll
+        for (int g = 0; g < 4; ++g) {
+            const int l0 = 2 * lane + 64 * g;
+            const double2 tj = *reinterpret_cast<const double2 *>(R + RAW_T + 8 * l0);
+            const float2 dt = make_float2((float)(A.ti - tj.x), (float)(A.ti - tj.y));
+            float2 f[NF];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const double2 x0 = *reinterpret_cast<const double2 *>(R + RAW_X + 8 * (k * JT + l0));
+                const float2 v0 = *reinterpret_cast<const float2 *>(R + RAW_V + 4 * (k * JT + l0));
+                const float2 a2 = *reinterpret_cast<const float2 *>(R + RAW_A2 + 4 * (k * JT + l0));
+                const float2 j6 = *reinterpret_cast<const float2 *>(R + RAW_J6 + 4 * (k * JT + l0));
+                predict_coord(dt.x, x0.x, v0.x, a2.x, j6.x, A.ds, f[F_XH + k].x, f[F_XL + k].x, f[F_V + k].x);
+                predict_coord(dt.y, x0.y, v0.y, a2.y, j6.y, A.ds, f[F_XH + k].y, f[F_XL + k].y, f[F_V + k].y);
+            }
+            f[F_M] = *reinterpret_cast<const float2 *>(R + RAW_M + 4 * l0);
+            if (ragged) {                                     // addresses >= nj: finite and massless
+                const bool in0 = tile * JT + l0 < A.nj, in1 = tile * JT + l0 + 1 < A.nj;
+#pragma unroll
+                for (int k = 0; k < NF; ++k) f[k] = make_float2(in0 ? f[k].x : 0.0f, in1 ? f[k].y : 0.0f);
+            }
+#pragma unroll
+            for (int k = 0; k < NF; ++k) *reinterpret_cast<float2 *>(Pj + k * JT + l0) = f[k];
+            const int2 jx = *reinterpret_cast<const int2 *>(R + RAW_IDX + 4 * l0);
+            *reinterpret_cast<int2 *>(JX + l0) = jx;
+            id_lo = min(id_lo, min(jx.x, jx.y));
+            id_hi = max(id_hi, max(jx.x, jx.y));
+        }
+        // Self-exclusion hoisted to tile level, as in the sweep kernel: if no i-particle of this warp's lanes has its index
+        // inside the tile's index range (and the tile is not the ragged last one) the tile runs the unchecked pair code
+        id_lo = __reduce_min_sync(FULL, id_lo);
+        id_hi = __reduce_max_sync(FULL, id_hi);
+        bool hit = false;
+#pragma unroll
+        for (int ch = 0; ch < NCH; ++ch) hit |= act[ch] && my[ch] >= id_lo && my[ch] <= id_hi;
+        const bool checked = !fast_ok || ragged || __any_sync(FULL, hit);
+        // the slot is consumed: refill it with the tile NS ahead while the forces are computed
+        __syncwarp();
+        if (lane == 0 && it + NS < nt) {
+            if (A.n_upd > 0) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // a-1 wrote the slot through the generic proxy
+            mbar_expect_tx(&sm.full[slot], RAW_TILE_BYTES);
+            tma_load_1d(R, A.raw + (size_t)(tile + NS * G) * RAW_TILE_BYTES, RAW_TILE_BYTES, &sm.full[slot]);
+            st_release_cta(&sm.armed[slot], it + NS);
+        }
+
+        // ---- a-4: the pairs of this tile; my i-particle of every chunk against my j-sub-range
+#pragma unroll
+        for (int ch = 0; ch < NCH; ++ch) {
+            if (!act[ch]) continue;
+            IPart I;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                I.nxh[k] = dup(-sm.ipart[32 * ch + ii[ch]][k]);
+                I.nxl[k] = dup(-sm.ipart[32 * ch + ii[ch]][3 + k]);
+                I.nv[k] = dup(-sm.ipart[32 * ch + ii[ch]][6 + k]);
+                I.a[k] = dup(0.0f);
+                I.j[k] = dup(0.0f);
+            }
+            I.p = dup(0.0f);
+            const int jn = 8 << lg[ch];
+            const int jl0 = (lane >> lg[ch]) * jn;
+            if (checked) {
+#pragma unroll 2
+                for (int q = 0; q < jn; q += 2) {
+                    const int jl = jl0 + q, ja = tile * JT + jl;
+                    float2 f[NF];
+#pragma unroll
+                    for (int k = 0; k < NF; ++k) f[k] = *reinterpret_cast<const float2 *>(Pj + k * JT + jl);
+                    const int2 jx = *reinterpret_cast<const int2 *>(JX + jl);
+                    float2 r2;
+                    pair2_checked<NEWTON>(I, f[0], f[1], f[2], f[3], f[4], f[5], f[6], f[7], f[8], f[9], eps2,
+                                          (ja < A.nj) && (jx.x != my[ch]), (ja + 1 < A.nj) && (jx.y != my[ch]), r2);
+                    // nearest neighbour: strict <, my j ascend => ties keep the smallest address (reading 7)
+                    if (r2.x < best[ch]) { best[ch] = r2.x; baddr[ch] = ja; }
+                    if (r2.y < best[ch]) { best[ch] = r2.y; baddr[ch] = ja + 1; }
+                }
+                // FP32 over one tile slice (<= 128 pairs per chain), then fp64 (reading 9)
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    acc7[ch][k] += (double)I.a[k].x + (double)I.a[k].y;
+                    acc7[ch][3 + k] += (double)I.j[k].x + (double)I.j[k].y;
+                }
+                acc7[ch][6] += (double)I.p.x + (double)I.p.y;
+            } else {
+                // the sweep kernel's pair code (g6_force_fast.cuh pair2: no per-pair test, Newton step in three instructions on the
+                // scaled sigma); its sums come out scaled by (y s) and (y s)^3, undone here in fp64 with the binary32 scale
+#pragma unroll 2
+                for (int q = 0; q < jn; q += 4) {
+                    const int jl = jl0 + q, ja = tile * JT + jl;
+                    float4 f[NF];
+#pragma unroll
+                    for (int k = 0; k < NF; ++k) f[k] = *reinterpret_cast<const float4 *>(Pj + k * JT + jl);
+                    float2 ra, rb;
+                    pair2<NEWTON>(I, make_float2(f[0].x, f[0].y), make_float2(f[1].x, f[1].y), make_float2(f[2].x, f[2].y),
+                                  make_float2(f[3].x, f[3].y), make_float2(f[4].x, f[4].y), make_float2(f[5].x, f[5].y),
+                                  make_float2(f[6].x, f[6].y), make_float2(f[7].x, f[7].y), make_float2(f[8].x, f[8].y),
+                                  make_float2(f[9].x, f[9].y), eps2s, ra);
+                    pair2<NEWTON>(I, make_float2(f[0].z, f[0].w), make_float2(f[1].z, f[1].w), make_float2(f[2].z, f[2].w),
+                                  make_float2(f[3].z, f[3].w), make_float2(f[4].z, f[4].w), make_float2(f[5].z, f[5].w),
+                                  make_float2(f[6].z, f[6].w), make_float2(f[7].z, f[7].w), make_float2(f[8].z, f[8].w),
+                                  make_float2(f[9].z, f[9].w), eps2s, rb);
+                    if (ra.x < best[ch]) { best[ch] = ra.x; baddr[ch] = ja; }
+                    if (ra.y < best[ch]) { best[ch] = ra.y; baddr[ch] = ja + 1; }
+                    if (rb.x < best[ch]) { best[ch] = rb.x; baddr[ch] = ja + 2; }
+                    if (rb.y < best[ch]) { best[ch] = rb.y; baddr[ch] = ja + 3; }
+                }
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    acc7[ch][k] += kA * ((double)I.a[k].x + (double)I.a[k].y);
+                    acc7[ch][3 + k] += kA * ((double)I.j[k].x + (double)I.j[k].y);
+                }
+                acc7[ch][6] += kP * ((double)I.p.x + (double)I.p.y);
+            }
+        }
+        __syncwarp();                                         // the buffer is overwritten by my next tile
+    }
+
+    // ---- the lanes of one i-particle (its j-sub-ranges): fixed shuffle tree, once; then one entry per (warp, i)
+#pragma unroll
+    for (int ch = 0; ch < NCH; ++ch) {
+        for (int o = 1 << lg[ch]; o < 32; o <<= 1) {
+#pragma unroll
+            for (int k = 0; k < 7; ++k) acc7[ch][k] += __shfl_xor_sync(FULL, acc7[ch][k], o);
+            const float r2 = __shfl_xor_sync(FULL, best[ch], o);
+            const int ad = __shfl_xor_sync(FULL, baddr[ch], o);
+            if (r2 < best[ch] || (r2 == best[ch] && ad < baddr[ch])) { best[ch] = r2; baddr[ch] = ad; }
+        }
+        if (act[ch] && lane < (1 << lg[ch])) {
+            const int i = 32 * ch + lane;
+#pragma unroll
+            for (int k = 0; k < 7; ++k) sm.acc[w][i][k] = acc7[ch][k];
+            sm.r2[w][i] = best[ch];
+            sm.addr[w][i] = baddr[ch];
+        }
+    }
+    __syncthreads();
+
+    // ---- a-5, first half: one partial per (i, CTA): the warps' sums in warp order
+    for (int i = tid; i < A.ni; i += BS2_THREADS) {
+        const size_t o = (size_t)cta * A.P.stride_s + (size_t)i * A.P.stride_i;
+        double v[7];
+#pragma unroll
+        for (int k = 0; k < 7; ++k) v[k] = sm.acc[0][i][k];
+        float bst = sm.r2[0][i];
+        int bad = sm.addr[0][i];
+#pragma unroll
+        for (int q = 1; q < NW; ++q) {
+#pragma unroll
+            for (int k = 0; k < 7; ++k) v[k] += sm.acc[q][i][k];
+            const float r2 = sm.r2[q][i];
+            const int ad = sm.addr[q][i];
+            if (r2 < bst || (r2 == bst && ad < bad)) { bst = r2; bad = ad; }
+        }
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { A.P.acc[k][o] = v[k]; A.P.jrk[k][o] = v[3 + k]; }
+        A.P.pot[o] = -v[6];
+        const bool has = bad != 0x7fffffff;
+        A.P.nn_r2[o] = has ? bst : INF;
+        A.P.nn_addr[o] = has ? bad : -1;
+    }
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) {
+        const unsigned ticket = atomicAdd(A.counter, 1u);
+        sm.is_last = (ticket == (unsigned)G - 1u);
+    }
+    __syncthreads();
+    if (!sm.is_last) return;
+    __threadfence();
+
+    // ---- a-5, second half (last CTA only): sum the G partials of every i in CTA order, one warp per i-particle
+    for (int i = w; i < A.ni; i += NW) {
+        double v[7] = {0, 0, 0, 0, 0, 0, 0};
+        float bst = INF;
+        int bad = 0x7fffffff;
+        for (int s0 = 0; s0 < G; s0 += 160) {
+            double t[5][7];
+            float r2[5];
+            int ad[5];
+#pragma unroll
+            for (int q = 0; q < 5; ++q) {
+                const int sq = s0 + lane + 32 * q;
+                const bool in = sq < G;
+                const size_t o = (size_t)(in ? sq : 0) * A.P.stride_s + (size_t)i * A.P.stride_i;
+#pragma unroll
+                for (int k = 0; k < 3; ++k) { t[q][k] = in ? __ldcg(A.P.acc[k] + o) : 0.0; t[q][3 + k] = in ? __ldcg(A.P.jrk[k] + o) : 0.0; }
+                t[q][6] = in ? __ldcg(A.P.pot + o) : 0.0;
+                r2[q] = in ? __ldcg(A.P.nn_r2 + o) : INF;
+                ad[q] = in ? __ldcg(A.P.nn_addr + o) : -1;
+            }
+#pragma unroll
+            for (int q = 0; q < 5; ++q) {
+                if (s0 + lane + 32 * q < G) {
+#pragma unroll
+                    for (int k = 0; k < 7; ++k) v[k] += t[q][k];
+                    if (ad[q] >= 0 && (r2[q] < bst || (r2[q] == bst && ad[q] < bad))) { bst = r2[q]; bad = ad[q]; }
+                }
+            }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+            for (int k = 0; k < 7; ++k) v[k] += __shfl_xor_sync(FULL, v[k], o);
+            const float r2 = __shfl_xor_sync(FULL, bst, o);
+            const int ad = __shfl_xor_sync(FULL, bad, o);
+            if (r2 < bst || (r2 == bst && ad < bad)) { bst = r2; bad = ad; }
+        }
+        if (lane == 0) {
+#pragma unroll
+            for (int k = 0; k < 3; ++k) { A.acc[3 * (size_t)i + k] = v[k]; A.jerk[3 * (size_t)i + k] = v[3 + k]; }
+            A.pot[i] = v[6];
+            const bool has = bad != 0x7fffffff;
+            if (A.nn_index) A.nn_index[i] = has ? j_index(A.raw, bad) : -1;
+            if (A.nn_r2) A.nn_r2[i] = has ? (double)bst : (double)INF;
+        }
+    }
+    if (tid == 0) *A.counter = 0u;
+    if (A.done_flag) {
+        __syncthreads();
+        if (tid == 0) {
+            __threadfence_system();
+            *reinterpret_cast<volatile unsigned int *>(A.done_flag) = A.done_seq;
+        }
+    }
+}
+
+template <int MAXI, bool NEWTON>
+__global__ void __launch_bounds__(bs2_threads(MAXI))
+k_block_step2(const BsArgs A, const __grid_constant__ BsInline<MAXI> D)
+{
+    block_step2_body<MAXI, NEWTON>(A, &D);
+}
+
+template <int MAXI, bool NEWTON>
+__global__ void __launch_bounds__(bs2_threads(MAXI))
+k_block_step2_dev(const BsArgs A)
+{
+    block_step2_body<MAXI, NEWTON>(A, nullptr);
+}
+
 // ---------------------------------------------------------------- host side
 template <int MAXI>
 inline int bs_attr()
@@ -563,11 +930,49 @@ inline int bs_attr()
     return (int)cudaFuncSetAttribute(k_block_step_dev<MAXI, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
 }
 
+template <int MAXI>
+inline int bs2_attr()
+{
+    const int bytes = (int)sizeof(Bs2Smem<MAXI>);
+    cudaError_t e = cudaFuncSetAttribute(k_block_step2<MAXI, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e != cudaSuccess) return (int)e;
+    e = cudaFuncSetAttribute(k_block_step2<MAXI, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e != cudaSuccess) return (int)e;
+    e = cudaFuncSetAttribute(k_block_step2_dev<MAXI, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e != cudaSuccess) return (int)e;
+    return (int)cudaFuncSetAttribute(k_block_step2_dev<MAXI, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+}
+
 inline int bs_kernel_init()
 {
     int r;
     if ((r = bs_attr<16>())) return r;
-    return bs_attr<BS_MAX_I>();
+    if ((r = bs_attr<BS_MAX_I>())) return r;
+    if ((r = bs2_attr<16>())) return r;
+    return bs2_attr<BS_MAX_I>();
+}
+
+// the second design (no neighbour lists); same arguments as bs_launch_t
+template <int MAXI>
+inline int bs2_launch_t(const BsArgs &A, bool newton, int grid, const double *xi, const double *vi, const int *index,
+                        const JRecord *upd, cudaStream_t st)
+{
+    static thread_local BsInline<MAXI> D;
+    if (A.inline_i) {
+        memcpy(D.xi, xi, sizeof(double) * 3 * A.ni);
+        memcpy(D.vi, vi, sizeof(double) * 3 * A.ni);
+        memcpy(D.index, index, sizeof(int) * A.ni);
+    }
+    if (A.n_upd > 0) memcpy(D.upd, upd, sizeof(JRecord) * A.n_upd);
+    const size_t bytes = sizeof(Bs2Smem<MAXI>);
+    if (!A.inline_i && A.n_upd == 0) {
+        if (newton) k_block_step2_dev<MAXI, true><<<grid, bs2_threads(MAXI), bytes, st>>>(A);
+        else k_block_step2_dev<MAXI, false><<<grid, bs2_threads(MAXI), bytes, st>>>(A);
+        return (int)cudaGetLastError();
+    }
+    if (newton) k_block_step2<MAXI, true><<<grid, bs2_threads(MAXI), bytes, st>>>(A, D);
+    else k_block_step2<MAXI, false><<<grid, bs2_threads(MAXI), bytes, st>>>(A, D);
+    return (int)cudaGetLastError();
 }
 
 template <int MAXI>
