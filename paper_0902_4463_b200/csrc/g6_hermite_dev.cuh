@@ -155,6 +155,47 @@ __device__ __forceinline__ double hd_correct_core(double h, const double *a0, co
     return d;
 }
 
+// The same corrector step by the first four lanes of a warp (the step loop's owners: the corrector sits on the critical path of
+// every small block step and a single thread's fp64 latency chain was 2-3 us of it).  Lanes 0-2 take one component each -- the
+// expressions of hd_correct_core, so the same numbers -- the components meet through shuffles, lanes 0-3 take one of the four
+// norms (a square root each), lane 0 the Aarseth formula and the power-of-two rule.  Call with the whole warp converged.
+//   in : h, tn, eta, dt_max (uniform); lane c < 3: a0c, ad0c, a1c, ad1c, xic, vic of component c
+//   out: lane c < 3: x1c, v1c; return value (all lanes): the new step
+__device__ __forceinline__ double hd_correct_warp(int lane, double h, double a0c, double ad0c, double a1c, double ad1c, double xic, double vic,
+                                                  double tn, double eta, double dt_max, double &x1c, double &v1c)
+{
+    const unsigned FULL = 0xffffffffu;
+    const double h2 = h * h, h3 = h2 * h, h4 = h3 * h, h5 = h4 * h;
+    const double ih = 1.0 / h, ih2 = ih * ih, ih3 = ih2 * ih;
+    constexpr double R6 = 1.0 / 6, R24 = 1.0 / 24, R120 = 1.0 / 120;
+    const double da = a0c - a1c;
+    const double a2 = (-6 * da - h * (4 * ad0c + 2 * ad1c)) * ih2;
+    const double a3c = (12 * da + 6 * h * (ad0c + ad1c)) * ih3;
+    x1c = xic + h4 * a2 * R24 + h5 * a3c * R120;
+    v1c = vic + h3 * a2 * R6 + h4 * a3c * R24;
+    const double a2nc = a2 + h * a3c;
+    // lane L < 4 gets vector L of (a1, ad1, a2n, a3)
+    double vec[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const double q0 = __shfl_sync(FULL, a1c, c), q1 = __shfl_sync(FULL, ad1c, c), q2 = __shfl_sync(FULL, a2nc, c), q3 = __shfl_sync(FULL, a3c, c);
+        vec[c] = lane == 0 ? q0 : lane == 1 ? q1 : lane == 2 ? q2 : q3;
+    }
+    const double nrm = hd_norm3(vec);
+    const double na = __shfl_sync(FULL, nrm, 0), nad = __shfl_sync(FULL, nrm, 1), n2 = __shfl_sync(FULL, nrm, 2), n3 = __shfl_sync(FULL, nrm, 3);
+    double d = h;
+    if (lane == 0) {
+        const double den = nad * n3 + n2 * n2;
+        const double want = den > 0 ? sqrt(eta * (na * n2 + nad * nad) / den) : dt_max;
+        if (want < d) {
+            while (d > want && d > 1e-300) d *= 0.5;
+        } else if (want >= 2 * d && 2 * d <= dt_max && hd_is_multiple(tn, 2 * d)) {
+            d *= 2;
+        }
+    }
+    return __shfl_sync(FULL, d, 0);
+}
+
 __device__ __forceinline__ void hd_correct_one(const HdState &S, const HdBlock &B, const HdCorr &C, int k, double tn)
 {
     const int p = B.act[k];

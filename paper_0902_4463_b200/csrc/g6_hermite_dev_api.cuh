@@ -42,7 +42,8 @@ struct g6hd_system {
     long long inline_steps = 0;
 
 
-    bool loop_profile = false;
+    bool loop_profile = false, loop_marks = false;
+    unsigned long long *prof = nullptr;     // [32] the marked build's summed intervals (device)
 };
 
 constexpr int HD_LOOP_MAXI_DEFAULT = 1024;
@@ -56,7 +57,7 @@ void hd_free(g6hd_system *s)
     cudaFree(s->B.act); cudaFree(s->B.cand); cudaFree(s->B.xi); cudaFree(s->B.vi); cudaFree(s->B.bmin); cudaFree(s->B.bcnt); cudaFree(s->B.boff); cudaFree(s->B.ticket);
     cudaFree(s->B.d_ni); cudaFree(s->B.d_tnext);
     cudaFree(s->a1); cudaFree(s->ad1); cudaFree(s->pot); cudaFree(s->dt_min_bits); cudaFree(s->shared_bits);
-    cudaFree(s->rec); cudaFree(s->chunk); cudaFree(s->flag);
+    cudaFree(s->rec); cudaFree(s->chunk); cudaFree(s->flag); cudaFree(s->prof);
     if (s->h_status) cudaFreeHost(s->h_status);
     if (s->h_note) cudaFreeHost(s->h_note);
     for (auto &e : s->pe) if (e) cudaEventDestroy(e);
@@ -126,11 +127,12 @@ int hd_loop_run(Cluster &c, g6hd_system &s, double t_end, long long max_steps, H
     A.t_sys = s.t; A.t_end = t_end; A.max_steps = max_steps; A.max_i = s.loop_max_i;
     A.eps2 = (float)s.eps2; A.ds = c.opt_ds;
     A.gen0 = s.loop_gen;
-    A.rec = s.rec; A.chunk = s.chunk; A.flag = s.flag; A.status = s.hd_status;
+    A.rec = s.rec; A.chunk = s.chunk; A.flag = s.flag; A.status = s.hd_status; A.prof = s.prof;
 
 
     void *args[] = {(void *)&A};
-    const void *fn = c.opt_newton ? (const void *)k_hd_loop<true> : (const void *)k_hd_loop<false>;
+    const void *fn = s.loop_marks ? (c.opt_newton ? (const void *)k_hd_loop<true, true> : (const void *)k_hd_loop<false, true>)
+                                    : (c.opt_newton ? (const void *)k_hd_loop<true> : (const void *)k_hd_loop<false>);
     CK(cudaLaunchCooperativeKernel(fn, dim3(s.loop_G), dim3(HL_THREADS), args, sizeof(HlSmem), c.stream));
     CK(cudaStreamSynchronize(c.stream));
     *st = *s.h_status;
@@ -183,8 +185,11 @@ g6hd_system *g6hd_create(int clusterid, int n, const double x[][3], const double
             if (s->loop) {
                 CK(cudaFuncSetAttribute(k_hd_loop<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(HlSmem)));
                 CK(cudaFuncSetAttribute(k_hd_loop<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(HlSmem)));
+                CK(cudaFuncSetAttribute(k_hd_loop<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(HlSmem)));
+                CK(cudaFuncSetAttribute(k_hd_loop<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(HlSmem)));
                 const size_t nrec = 2 * (size_t)s->loop_G * ntiles * HL_REC_WORDS, nchunk = (size_t)s->loop_max_i * HL_CHUNK_WORDS * s->loop_G;
-                CK(dalloc(s->rec, nrec)); CK(dalloc(s->chunk, nchunk)); CK(dalloc(s->flag, s->loop_G));
+                CK(dalloc(s->rec, nrec)); CK(dalloc(s->chunk, nchunk)); CK(dalloc(s->flag, s->loop_G)); CK(dalloc(s->prof, 32));
+                CK(cudaMemset(s->prof, 0, 32 * sizeof(unsigned long long)));
                 CK(cudaMemsetAsync(s->rec, 0, nrec * sizeof(unsigned long long), c.stream));           // step number 0 = never written
                 CK(cudaMemsetAsync(s->chunk, 0, nchunk * sizeof(unsigned long long), c.stream));
                 CK(cudaMemsetAsync(s->flag, 0, s->loop_G * sizeof(unsigned int), c.stream));
@@ -193,7 +198,8 @@ g6hd_system *g6hd_create(int clusterid, int n, const double x[][3], const double
                 CK(cudaHostGetDevicePointer((void **)&s->hd_status, s->h_status, 0));
             }
         }
-        s->loop_profile = env_int("G6_HD_LOOP_PROFILE", 0) != 0;
+        s->loop_profile = env_int("G6_HD_LOOP_PROFILE", 0) != 0;      // 1: the build with phase marks; 2: the production loop, per-bin times only
+        s->loop_marks = env_int("G6_HD_LOOP_PROFILE", 0) == 1;
         s->profile = env_int("G6_HD_PROFILE", 0) != 0;
         if (s->profile) for (auto &e : s->pe) CK(cudaEventCreate(&e));
         CK(cudaMemsetAsync(s->B.ticket, 0, sizeof(unsigned int), c.stream));
@@ -460,6 +466,23 @@ int g6hd_get_stats(g6hd_system *sp, double stats[8], long long ni_hist_log2[64])
     if (s.loop_profile) {
         fprintf(stderr, "g6hd loop profile: %lld launches of the step loop, %lld block steps inside it\n", s.loop_launches, s.loop_steps);
         fprintf(stderr, "  %lld of them predicted their i-block in every CTA (one exchange less)\n", s.inline_steps);
+        if (s.loop_marks && s.prof) {
+            unsigned long long pr[32];
+            CK(cudaMemcpy(pr, s.prof, sizeof(pr), cudaMemcpyDeviceToHost));
+            if (pr[15]) {
+                const double n = (double)pr[15];
+                fprintf(stderr, "  steps with n_i < 8 as CTA 0 walks them, SM cycles per step: publish %.0f | poll: own lane %.0f, all lanes %.0f | select %.0f | barrier %.0f | predict i, j %.0f | "
+                        "pairs + shuffle tree %.0f | barrier %.0f | slice sums + partials out %.0f | gather + correct (if owner) %.0f\n",
+                        pr[0] / n, pr[1] / n, pr[2] / n, pr[3] / n, pr[4] / n, pr[5] / n, pr[6] / n, pr[7] / n, pr[8] / n, pr[9] / n);
+                fprintf(stderr, "    select in parts: counts per lane %.0f | scan over the lanes %.0f | offsets and active list %.0f | own list %.0f\n", pr[11] / n, pr[12] / n, pr[13] / n, pr[14] / n);
+            }
+            if (pr[31]) {
+                const double n = (double)pr[31];
+                fprintf(stderr, "  the CTAs that own an active particle of such a step (<= %d of them): gather poll %.0f | barrier %.0f | sum of the %d partials %.0f | corrector %.0f | stores %.0f | "
+                        "barrier %.0f | to the rescan's end %.0f | release fence %.0f | publish %.0f\n", HL_CQ, pr[16] / n, pr[17] / n, s.loop_G, pr[18] / n, pr[19] / n, pr[20] / n,
+                        pr[21] / n, pr[22] / n, pr[23] / n, pr[24] / n);
+            }
+        }
         for (int b = 0; b < 64; ++b)
             if (s.hist[b])
                 fprintf(stderr, "  n_i in [2^%d, 2^%d): %lld block steps; in the loop %.1f us per step (device clock, %lld steps); handed to the host %lld steps, %.1f us each (wall, force only)\n",

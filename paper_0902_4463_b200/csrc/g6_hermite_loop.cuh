@@ -43,10 +43,11 @@ constexpr int HL_MAX_I = 768;                 // largest block the loop can step
 constexpr int HL_MAX_G = 148;                 // CTAs (one per SM)
 constexpr int HL_MAX_TILES = HL_MAX_G * HL_KMAX;
 constexpr int HL_INLINE = 8;                  // active particles per tile that travel inside the tile's record
-constexpr int HL_REC_WORDS = 5;               // tmin lo, tmin hi, count, slots 0-3, slots 4-7
+constexpr int HL_REC_WORDS = 6;               // tmin lo, tmin hi, count, slots 0-3, slots 4-7, (pad): three 16-byte stores / loads
 constexpr int HL_CHUNK_WORDS = 14;            // 7 fp64 sums = 14 halves
+static_assert(true, "");
 constexpr int HL_CQ = 3;                      // particles whose partials an owner gathers at a time (staged in the idle wsum)
-constexpr int HL_CPOLL = 4;                   // words a thread polls per round
+constexpr int HL_CPOLL = 6;                   // 16-byte word pairs a thread polls per round: the HL_CQ x 7 x G pairs of one gather are all in flight together
 
 enum { HL_END = 0, HL_BIG = 1, HL_STEPS = 2 };
 
@@ -77,9 +78,10 @@ struct HlArgs {
     int ds;
     unsigned int gen0;             // step numbers of this launch are gen0 + 1, gen0 + 2, ... (never 0, never reused)
     unsigned long long *rec;       // [2][G][ntiles][HL_REC_WORDS]   tile records: double-buffered by step parity, one copy per consumer CTA
-    unsigned long long *chunk;     // [max_i][HL_CHUNK_WORDS][G]  partial forces
+    unsigned long long *chunk;     // [max_i][G][HL_CHUNK_WORDS]  partial forces: the 14 words of one (particle, CTA) are contiguous (seven 16-byte stores)
     unsigned int *flag;            // [G] flag barrier of the non-inline path
     HlStatus *status;              // device-visible (mapped host memory)
+    unsigned long long *prof;      // [32] PROF build only: summed clock64() intervals between the marks (see HL_MK), steps with n_i < 8
 };
 
 struct HlSmem {
@@ -99,6 +101,8 @@ struct HlSmem {
     unsigned int bal[HL_KMAX][JT / 32];
     unsigned int recw[HL_KMAX][HL_REC_WORDS];
     int nown_prev;
+    long long mk[32];                                   // PROF build: clock64() marks of thread 0
+    int mk_open;
     double tmin[HL_KMAX];
     double gmin;
     int ni, nown, inl;
@@ -113,13 +117,24 @@ __device__ __forceinline__ void hl_fence() { asm volatile("fence.acq_rel.gpu;" :
 __device__ __forceinline__ void hl_store_word(unsigned long long *p, unsigned int payload, unsigned int gen)
 {
     const unsigned long long v = (unsigned long long)payload | ((unsigned long long)gen << 32);
-    asm volatile("st.volatile.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 __device__ __forceinline__ unsigned long long hl_load_word(const unsigned long long *p)
 {
     unsigned long long v;
-    asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return v;
+}
+// two consecutive words (16-byte aligned) with one instruction; each 8-byte half is single-copy atomic, which is all the
+// self-validating words need
+__device__ __forceinline__ void hl_store_word2(unsigned long long *p, unsigned int pay0, unsigned int pay1, unsigned int gen)
+{
+    const unsigned long long g = (unsigned long long)gen << 32;
+    asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(g | pay0), "l"(g | pay1) : "memory");
+}
+__device__ __forceinline__ void hl_load_word2(const unsigned long long *p, unsigned long long &a, unsigned long long &b)
+{
+    asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "l"(p) : "memory");
 }
 // spin until the N words p[0], p[stride], ... all carry step number `gen` (all N loads of a round are in flight together);
 // a protocol error fails the launch instead of hanging the device
@@ -193,9 +208,12 @@ __device__ __forceinline__ void hl_make_record(const unsigned int *bal, double t
     recw[2] = (unsigned int)c;
     recw[3] = sl[0];
     recw[4] = sl[1];
+    recw[5] = 0u;
 }
 
-template <bool NEWTON>
+// PROF: thread 0 of every CTA also takes clock64() marks along the step (HlStatus::ph, ::own); a build of its own (env
+// G6_HD_LOOP_PROFILE) because the marks cost registers the production loop does not have to spare
+template <bool NEWTON, bool PROF = false>
 __global__ void __launch_bounds__(HL_THREADS, 1)
 k_hd_loop(const HlArgs A)
 {
@@ -229,12 +247,21 @@ k_hd_loop(const HlArgs A)
     if (cta == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_step));
     int reason = HL_END, ni_next = 0, ni_last = 0;
     double t_big = 0.0;
+    // PROF: thread 0 of every CTA marks the clock along the step: 0-10 the step as every CTA walks it (summed for CTA 0), 16-25 the
+    // chain of a CTA that owns an active particle (gather .. publish of the next step), summed over all owners
+#define HL_MK(q) do { if (PROF && tid == 0) sm.mk[q] = clock64(); } while (0)
+    if (PROF && tid == 0) sm.mk_open = 0;
     const float2 eps2 = dup(A.eps2);
+    // the unchecked pair code needs s2 > 0 for every pair: a normal positive binary32 eps2 (as for the sweep kernel)
+    const bool fast_ok = A.eps2 >= 4.0f * 1.17549435e-38f && A.eps2 < __builtin_huge_valf();
+    const float2 eps2s = dup(pair_scale<NEWTON>() * A.eps2);
+    const double kP = NEWTON ? 0.5 * sqrt((double)FOUR_THIRDS) : sqrt((double)THIRD), kA = kP * kP * kP;
 
     for (;;) {
         if (!(t_sys < A.t_end)) { reason = HL_END; break; }
         if (A.max_steps > 0 && steps >= A.max_steps) { reason = HL_STEPS; break; }
         const unsigned int gen = A.gen0 + 1u + (unsigned int)steps;
+        HL_MK(0);
         // this step's records: [consumer CTA][tile][word] -- every consumer polls its OWN copy (a word polled by all CTAs at once
         // is a hot spot in its L2 slice: the publisher's store then queues behind hundreds of loads, measured 3-5 us)
         unsigned long long *rec = A.rec + (size_t)(gen & 1u) * G * A.ntiles * HL_REC_WORDS;
@@ -266,28 +293,48 @@ k_hd_loop(const HlArgs A)
         if (w == 0) {
             // everything from here to the barrier below is warp 0's: rescan (one tile), publish, poll, select
             if (rescan && Kc == 1) {
-                double v[JT / 32], m = INF;                   // lane holds the slots lane, lane + 32, ...
+                // t + dt >= 0 (or +inf): the doubles order like their bit patterns, and the minimum of 64-bit patterns over the
+                // warp is two 32-bit warp reductions (high words, then the low words of the lanes at the high minimum)
+                unsigned long long v[JT / 32], m = ~0ull;     // lane holds the slots lane, lane + 32, ...
 #pragma unroll
-                for (int r = 0; r < JT / 32; ++r) { v[r] = sm.tnext[0][32 * r + lane]; m = fmin(m, v[r]); }
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) m = fmin(m, __shfl_xor_sync(FULL, m, o));
+                for (int r = 0; r < JT / 32; ++r) { v[r] = (unsigned long long)__double_as_longlong(sm.tnext[0][32 * r + lane]); m = v[r] < m ? v[r] : m; }
+                const unsigned int mh = __reduce_min_sync(FULL, (unsigned int)(m >> 32));
+                const unsigned int ml = __reduce_min_sync(FULL, (unsigned int)(m >> 32) == mh ? (unsigned int)m : 0xffffffffu);
+                m = ((unsigned long long)mh << 32) | ml;
+                unsigned int bal[JT / 32];
 #pragma unroll
                 for (int r = 0; r < JT / 32; ++r) {
-                    const unsigned b = __ballot_sync(FULL, v[r] == m);
-                    if (lane == 0) sm.bal[0][r] = b;
+                    bal[r] = __ballot_sync(FULL, v[r] == m);
+                    if (lane == 0) sm.bal[0][r] = bal[r];      // (the non-inline path of phase A reads them)
                 }
+                // every lane has the ballots: the record in registers, no round trip through shared memory
+                if (lane == 0) hl_make_record(bal, __longlong_as_double((long long)m), sm.recw[0]);
                 __syncwarp();
-                if (lane == 0) hl_make_record(sm.bal[0], m, sm.recw[0]);
             }
             // Release: the Hermite state of my particles that phase C of the last step wrote (other warps, ordered before this
             // point by the barriers of phase C) must be visible to whoever reads the records
+            HL_MK(23);
             if (lane == 0 && sm.nown_prev > 0) hl_fence();
             __syncwarp();
-            for (int e = lane; e < G * Kc * HL_REC_WORDS; e += 32) {
-                const int c = e / (Kc * HL_REC_WORDS), r = e % (Kc * HL_REC_WORDS), kk = r / HL_REC_WORDS, wd = r % HL_REC_WORDS;
-                hl_store_word(rec + ((size_t)c * A.ntiles + (cta + kk * G)) * HL_REC_WORDS + wd, sm.recw[kk][wd], gen);
+            HL_MK(24);
+            for (int kk = 0; kk < Kc; ++kk) {
+                unsigned int rw[HL_REC_WORDS];
+#pragma unroll
+                for (int wd = 0; wd < HL_REC_WORDS; ++wd) rw[wd] = sm.recw[kk][wd];
+                for (int c = lane; c < G; c += 32) {                 // consumer c's private copy
+                    unsigned long long *r = rec + ((size_t)c * A.ntiles + (cta + kk * G)) * HL_REC_WORDS;
+#pragma unroll
+                    for (int wd = 0; wd < HL_REC_WORDS; wd += 2) hl_store_word2(r + wd, rw[wd], rw[wd + 1], gen);
+                }
             }
 
+            HL_MK(1);
+            HL_MK(25);
+            if (PROF && tid == 0 && sm.mk_open) {
+                for (int q = 16; q < 25; ++q) atomicAdd(A.prof + q, (unsigned long long)(sm.mk[q + 1] - sm.mk[q]));
+                atomicAdd(A.prof + 31, 1ull);
+                sm.mk_open = 0;
+            }
             // poll every tile's record (my private copy): lane takes the tiles lane, lane + 32, ..., four at a time
             double m = INF;
             for (int g0 = 0; g0 < A.ntiles; g0 += 128) {
@@ -302,7 +349,7 @@ k_hd_loop(const HlArgs A)
                         if (!done[u]) {
                             const unsigned long long *r = rec + ((size_t)cta * A.ntiles + g0 + lane + 32 * u) * HL_REC_WORDS;
 #pragma unroll
-                            for (int k = 0; k < HL_REC_WORDS; ++k) v[u][k] = hl_load_word(r + k);
+                            for (int k = 0; k < HL_REC_WORDS; k += 2) hl_load_word2(r + k, v[u][k], v[u][k + 1]);
                         }
                     }
                     bool all = true;
@@ -330,37 +377,77 @@ k_hd_loop(const HlArgs A)
                     if (++spins > (1u << 26)) __trap();
                 }
             }
-            hl_fence();                               // acquire: what the records' writers published before them
+            HL_MK(2);
+            // No acquire fence here.  Everything read after this point that another CTA wrote (the Hermite state of the active
+            // particles, the i-block) is read with ld.global.cg / ld.volatile, i.e. from L2, by instructions ISSUED after the poll
+            // loop has seen the records (the loop's exit depends on the loaded words); the writers made that data visible before
+            // their records (fence.acq_rel.gpu in front of the record stores).  A fence here has to wait for this warp's own
+            // G x 5 record stores to be acknowledged and cost 3-4 us per block step (measured with the phase marks below).
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) m = fmin(m, __shfl_xor_sync(FULL, m, o));
-            // t_next = m; offsets of the tiles in the active list (tile order = increasing address); n_i
-            int run = 0, over = 0;
-            for (int T0 = 0; T0 < A.ntiles; T0 += 32) {
-                const int T = T0 + lane;
-                const bool hit = T < A.ntiles && sm.s_tm[T] == m;
-                const int c = hit ? sm.s_tc[T] : 0;
-                over |= c > HL_INLINE;
-                int inc = c;
+            HL_MK(3);
+            // t_next = m; offsets of the tiles in the active list (tile order = increasing address); n_i.  Lane l takes the
+            // tiles [l R, l R + R): its own running count, one scan over the lanes, and it writes the offsets and (inline path)
+            // the addresses of its tiles' active particles
+            __syncwarp();                                     // the polling lanes' s_tm / s_tc / s_sl
+            const int R = (A.ntiles + 31) >> 5;
+            const unsigned long long mb = (unsigned long long)__double_as_longlong(m);        // bit patterns compare like the times
+            const unsigned long long *tmb = reinterpret_cast<const unsigned long long *>(sm.s_tm);
+            int mine = 0, over = 0;
+            for (int r0 = 0; r0 < R; r0 += 4) {               // four tiles' loads in flight together
+                unsigned long long tb[4];
+                int tc[4];
 #pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const int u = __shfl_up_sync(FULL, inc, o);
-                    if (lane >= o) inc += u;
+                for (int u = 0; u < 4; ++u) {
+                    const int T = min(lane * R + r0 + u, A.ntiles - 1);
+                    tb[u] = tmb[T];
+                    tc[u] = sm.s_tc[T];
                 }
-                if (T < A.ntiles) sm.s_off[T] = hit ? run + inc - c : -1;
-                run += __shfl_sync(FULL, inc, 31);
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int c = (r0 + u < R && lane * R + r0 + u < A.ntiles && tb[u] == mb) ? tc[u] : 0;
+                    over |= c > HL_INLINE;
+                    mine += c;
+                }
             }
+            HL_MK(11);
+            int inc = mine;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int u = __shfl_up_sync(FULL, inc, o);
+                if (lane >= o) inc += u;
+            }
+            const int run = __shfl_sync(FULL, inc, 31);
             over = __any_sync(FULL, over);
             const bool inl_w = !over && run <= A.max_i;
-            if (inl_w) {
-                // the active list, from the slots inside the records
-                for (int T = lane; T < A.ntiles; T += 32) {
-                    const int base = sm.s_off[T];
-                    if (base < 0) continue;
-                    const int c = sm.s_tc[T];
-                    for (int r = 0; r < c; ++r) sm.iidx[base + r] = T * JT + (int)((sm.s_sl[T][r >> 2] >> (8 * (r & 3))) & 0xffu);
+            HL_MK(12);
+            {
+                int base = inc - mine;
+                for (int r0 = 0; r0 < R; r0 += 4) {
+                    unsigned long long tb[4];
+                    int tc[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int T = min(lane * R + r0 + u, A.ntiles - 1);
+                        tb[u] = tmb[T];
+                        tc[u] = sm.s_tc[T];
+                    }
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int T = lane * R + r0 + u;
+                        if (r0 + u < R && T < A.ntiles) {
+                            const bool hit = tb[u] == mb;
+                            const int c = hit ? tc[u] : 0;
+                            sm.s_off[T] = hit ? base : -1;
+                            if (inl_w)
+                                for (int q = 0; q < c; ++q) sm.iidx[base + q] = T * JT + (int)((sm.s_sl[T][q >> 2] >> (8 * (q & 3))) & 0xffu);
+                            base += c;
+                        }
+                    }
                 }
             }
             __syncwarp();
+            HL_MK(13);
             if (lane == 0) {
                 sm.ni = run; sm.gmin = m; sm.inl = inl_w;
                 if (inl_w) {
@@ -379,7 +466,9 @@ k_hd_loop(const HlArgs A)
                 }
             }
         }
+        HL_MK(4);
         __syncthreads();
+        HL_MK(5);
         const double tn = sm.gmin;
         const int ni = sm.ni;
         const bool big = ni > A.max_i, inl = sm.inl != 0;
@@ -463,6 +552,7 @@ k_hd_loop(const HlArgs A)
         }
         __syncthreads();
 
+        HL_MK(6);
         // The pairs.  i-particles in chunks of 32, C = 1, 2, .. 16 chunks at a time; a chunk is worked on by HL_NW / C warps, each
         // taking a j-slice of JT C / HL_NW particles of every tile (small blocks: one chunk, 16 slices of 16 j; 512 particles:
         // 16 chunks at once, every warp sweeps whole tiles and no two warps share an i-particle).  Inside a warp the lanes are
@@ -483,23 +573,31 @@ k_hd_loop(const HlArgs A)
                 const int ii = lane & (pw - 1), jsub = lane >> lg;
                 const bool act = ii < nic;
                 double acc7[7] = {0, 0, 0, 0, 0, 0, 0};
+                IPart I;
+                int my = -1;
                 if (act) {
-                    IPart I;
 #pragma unroll
                     for (int k = 0; k < 3; ++k) {
                         I.nxh[k] = dup(-sm.ipart[c0 + ii][k]);
                         I.nxl[k] = dup(-sm.ipart[c0 + ii][3 + k]);
                         I.nv[k] = dup(-sm.ipart[c0 + ii][6 + k]);
                     }
-                    const int my = sm.iidx[c0 + ii];
-                    for (int kk = 0; kk < Kc; ++kk) {
+                    my = sm.iidx[c0 + ii];
+                }
+                for (int kk = 0; kk < Kc; ++kk) {
+                    // Self-exclusion hoisted to tile level, as in the sweep kernel: a warp takes the checked pair code only on
+                    // the tile that holds one of its i-particles (addresses are indices here) or on the ragged last tile
+                    const int T = cta + kk * G;
+                    const bool checked = !fast_ok || T * JT + JT > A.nj || __any_sync(FULL, act && my / JT == T);
+                    if (!act) continue;
 #pragma unroll
-                        for (int k = 0; k < 3; ++k) { I.a[k] = dup(0.0f); I.j[k] = dup(0.0f); }
-                        I.p = dup(0.0f);
-                        const float *Pj = sm.pred[kk];
-                        const int *JX = reinterpret_cast<const int *>(sm.raw[kk] + RAW_IDX);
-                        const int jl0 = jper * sw + jsub * jn;
-                        const int ja0 = (cta + kk * G) * JT + jl0;
+                    for (int k = 0; k < 3; ++k) { I.a[k] = dup(0.0f); I.j[k] = dup(0.0f); }
+                    I.p = dup(0.0f);
+                    const float *Pj = sm.pred[kk];
+                    const int *JX = reinterpret_cast<const int *>(sm.raw[kk] + RAW_IDX);
+                    const int jl0 = jper * sw + jsub * jn;
+                    const int ja0 = T * JT + jl0;
+                    if (checked) {
 #pragma unroll 2
                         for (int q = 0; q < jn; q += 2) {
                             const int jl = jl0 + q, ja = ja0 + q;
@@ -517,17 +615,37 @@ k_hd_loop(const HlArgs A)
                             acc7[3 + k] += (double)I.j[k].x + (double)I.j[k].y;
                         }
                         acc7[6] -= (double)I.p.x + (double)I.p.y;
+                    } else {
+                        // the sweep kernel's pair code (no per-pair test, Newton step in three instructions on the scaled sigma);
+                        // its sums come out scaled by (y s) and (y s)^3, undone here in fp64 with the binary32 scale
+#pragma unroll 2
+                        for (int q = 0; q < jn; q += 2) {
+                            const int jl = jl0 + q;
+                            float2 f[NF];
+#pragma unroll
+                            for (int k = 0; k < NF; ++k) f[k] = *reinterpret_cast<const float2 *>(Pj + k * JT + jl);
+                            float2 r2;
+                            pair2<NEWTON>(I, f[0], f[1], f[2], f[3], f[4], f[5], f[6], f[7], f[8], f[9], eps2s, r2);
+                        }
+#pragma unroll
+                        for (int k = 0; k < 3; ++k) {
+                            acc7[k] += kA * ((double)I.a[k].x + (double)I.a[k].y);
+                            acc7[3 + k] += kA * ((double)I.j[k].x + (double)I.j[k].y);
+                        }
+                        acc7[6] -= kP * ((double)I.p.x + (double)I.p.y);
                     }
                 }
                 for (int o = pw; o < 32; o <<= 1) {
 #pragma unroll
                     for (int k = 0; k < 7; ++k) acc7[k] += __shfl_xor_sync(FULL, acc7[k], o);
                 }
+                HL_MK(7);
                 if (lane < pw) {
 #pragma unroll
                     for (int k = 0; k < 7; ++k) sm.wsum[w][lane][k] = acc7[k];
                 }
                 __syncthreads();
+                HL_MK(8);
                 // the slices of every chunk in slice order: one partial per (i, CTA), published as 14 self-validating words
                 for (int q = tid; q < C * 32 * 7; q += HL_THREADS) {
                     const int cq = q / (32 * 7), i = (q / 7) % 32, k = q % 7;
@@ -536,9 +654,7 @@ k_hd_loop(const HlArgs A)
                         double sv = sm.wsum[cq * nsl][i][k];
                         for (int u = 1; u < nsl; ++u) sv += sm.wsum[cq * nsl + u][i][k];
                         const unsigned long long b = (unsigned long long)__double_as_longlong(sv);
-                        unsigned long long *ch = A.chunk + ((size_t)gi * HL_CHUNK_WORDS + 2 * k) * G + cta;
-                        hl_store_word(ch, (unsigned int)b, gen);
-                        hl_store_word(ch + G, (unsigned int)(b >> 32), gen);
+                        hl_store_word2(A.chunk + ((size_t)gi * G + cta) * HL_CHUNK_WORDS + 2 * k, (unsigned int)b, (unsigned int)(b >> 32), gen);
                     }
                 }
                 __syncthreads();
@@ -549,86 +665,118 @@ k_hd_loop(const HlArgs A)
         // The partials of HL_CQ particles at a time: every thread polls its share of their nq x 14 x G words (all loads of a round in
         // flight together: one L2 round trip after the last writer), the payloads go to shared memory (the idle wsum), then one
         // warp per particle adds them in fixed order.
+        HL_MK(9);
         const int nown = sm.nown;
+        HL_MK(16);
         unsigned int *stage = reinterpret_cast<unsigned int *>(&sm.wsum[0][0][0]);       // [HL_CQ][14][G]
         for (int q0 = 0; q0 < nown; q0 += HL_CQ) {
             const int nq = min(HL_CQ, nown - q0);
-            const int nwords = nq * HL_CHUNK_WORDS * G;
-            for (int e0 = 0; e0 < nwords; e0 += HL_THREADS * HL_CPOLL) {
+            const int perq = (HL_CHUNK_WORDS / 2) * G, npairs = nq * perq;          // 16-byte pairs: (CTA, component) of each particle
+            for (int e0 = 0; e0 < npairs; e0 += HL_THREADS * HL_CPOLL) {
                 unsigned int spins = 0;
                 bool done[HL_CPOLL];
 #pragma unroll
-                for (int r = 0; r < HL_CPOLL; ++r) done[r] = e0 + r * HL_THREADS + tid >= nwords;
+                for (int r = 0; r < HL_CPOLL; ++r) done[r] = e0 + r * HL_THREADS + tid >= npairs;
                 for (;;) {
-                    unsigned long long v[HL_CPOLL];
+                    unsigned long long v[HL_CPOLL][2];
 #pragma unroll
                     for (int r = 0; r < HL_CPOLL; ++r) {
                         const int e = e0 + r * HL_THREADS + tid;
-                        if (!done[r]) v[r] = hl_load_word(A.chunk + (size_t)sm.own_k[q0 + e / (HL_CHUNK_WORDS * G)] * HL_CHUNK_WORDS * G + e % (HL_CHUNK_WORDS * G));
+                        const int qq = (e >= perq) + (e >= 2 * perq);           // which of the <= HL_CQ particles (no division on this path)
+                        if (!done[r]) hl_load_word2(A.chunk + ((size_t)sm.own_k[q0 + qq] * perq + (e - qq * perq)) * 2, v[r][0], v[r][1]);
                     }
                     bool all = true;
 #pragma unroll
                     for (int r = 0; r < HL_CPOLL; ++r) {
                         if (!done[r]) {
-                            if ((unsigned int)(v[r] >> 32) == gen) { stage[e0 + r * HL_THREADS + tid] = (unsigned int)v[r]; done[r] = true; }
-                            else all = false;
+                            if ((unsigned int)(v[r][0] >> 32) == gen && (unsigned int)(v[r][1] >> 32) == gen) {
+                                *reinterpret_cast<uint2 *>(stage + 2 * (e0 + r * HL_THREADS + tid)) = make_uint2((unsigned int)v[r][0], (unsigned int)v[r][1]);
+                                done[r] = true;
+                            } else all = false;
                         }
                     }
                     if (all) break;
                     if (++spins > (1u << 26)) __trap();
                 }
             }
+            if (q0 == 0) HL_MK(17);
             __syncthreads();
+            if (q0 == 0) HL_MK(18);
             if (w < nq) {
             const int q = q0 + w;
             const int k = sm.own_k[q], sl = sm.own_l[q];
-            const unsigned int *sg = stage + (size_t)w * HL_CHUNK_WORDS * G;
+            const uint2 *sg = reinterpret_cast<const uint2 *>(stage) + (size_t)w * (HL_CHUNK_WORDS / 2) * G;      // [CTA][component]
             double v[7] = {0, 0, 0, 0, 0, 0, 0};
             for (int s = lane; s < G; s += 32) {
 #pragma unroll
-                for (int c = 0; c < 7; ++c)
-                    v[c] += __longlong_as_double((long long)(((unsigned long long)sg[(2 * c + 1) * G + s] << 32) | sg[2 * c * G + s]));
+                for (int c = 0; c < 7; ++c) {
+                    const uint2 u = sg[s * 7 + c];
+                    v[c] += __longlong_as_double((long long)(((unsigned long long)u.y << 32) | u.x));
+                }
             }
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) {
 #pragma unroll
                 for (int c = 0; c < 7; ++c) v[c] += __shfl_xor_sync(FULL, v[c], o);
             }
-            if (lane == 0) {
+            if (q0 == 0) HL_MK(19);
+            {
+                // the corrector, the Aarseth step and the power-of-two rule: lanes 0-2 one component each (hd_correct_warp), and
+                // each of them stores its own component of the new state, of the resident tile and of the j-store record
                 const int kk = sl / JT, l = sl % JT;
                 const int p = (cta + kk * G) * JT + l;
-                double a0[3], ad0[3], xi[3], vi[3], x1[3], v1[3], h;
+                const int c = lane < 3 ? lane : 0;
+                double a0c, ad0c, xic, vic, h;
                 if (inl) {
                     const double *st = sm.own_st[kk * HL_INLINE + (k - sm.s_off[cta + kk * G])];
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) { xi[c] = st[c]; vi[c] = st[3 + c]; a0[c] = st[6 + c]; ad0[c] = st[9 + c]; }
+                    xic = st[c]; vic = st[3 + c]; a0c = st[6 + c]; ad0c = st[9 + c];
                     h = st[12];
                 } else {
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) {
-                        xi[c] = A.B.xi[3 * (size_t)k + c]; vi[c] = A.B.vi[3 * (size_t)k + c];
-                        a0[c] = A.S.a[3 * (size_t)p + c]; ad0[c] = A.S.ad[3 * (size_t)p + c];
-                    }
+                    xic = A.B.xi[3 * (size_t)k + c]; vic = A.B.vi[3 * (size_t)k + c];
+                    a0c = A.S.a[3 * (size_t)p + c]; ad0c = A.S.ad[3 * (size_t)p + c];
                     h = A.S.dt[p];
                 }
-                const double d = hd_correct_core(h, a0, ad0, v, v + 3, xi, vi, tn, A.C.eta, A.C.dt_max, x1, v1);
-#pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    A.a1[3 * (size_t)k + c] = v[c]; A.ad1[3 * (size_t)k + c] = v[3 + c];
-                    A.S.x[3 * (size_t)p + c] = x1[c]; A.S.v[3 * (size_t)p + c] = v1[c];
-                    A.S.a[3 * (size_t)p + c] = v[c]; A.S.ad[3 * (size_t)p + c] = v[3 + c];
+                const double a1c = c == 0 ? v[0] : c == 1 ? v[1] : v[2], ad1c = c == 0 ? v[3] : c == 1 ? v[4] : v[5];
+                double x1c, v1c;
+                const double d = hd_correct_warp(lane, h, a0c, ad0c, a1c, ad1c, xic, vic, tn, A.C.eta, A.C.dt_max, x1c, v1c);
+                if (q0 == 0) HL_MK(20);
+                char *Ts = sm.raw[kk], *Tg = A.C.raw + (size_t)(cta + kk * G) * RAW_TILE_BYTES;      // my resident copy, the j-store
+                if (lane < 3) {
+                    A.a1[3 * (size_t)k + c] = a1c; A.ad1[3 * (size_t)k + c] = ad1c;
+                    A.S.x[3 * (size_t)p + c] = x1c; A.S.v[3 * (size_t)p + c] = v1c;
+                    A.S.a[3 * (size_t)p + c] = a1c; A.S.ad[3 * (size_t)p + c] = ad1c;
+                    raw_x(Ts, c, l) = x1c; raw_v(Ts, c, l) = (float)v1c; raw_a2(Ts, c, l) = (float)(a1c / 2); raw_j6(Ts, c, l) = (float)(ad1c / 6);
+                    raw_x(Tg, c, l) = x1c; raw_v(Tg, c, l) = (float)v1c; raw_a2(Tg, c, l) = (float)(a1c / 2); raw_j6(Tg, c, l) = (float)(ad1c / 6);
                 }
-                A.pot[k] = v[6];
-                A.S.t[p] = tn;
-                A.S.dt[p] = d;
-                atomicMin(A.C.dt_min_bits, (unsigned long long)__double_as_longlong(d));
-                const float m = raw_m(sm.raw[kk], l);
-                hl_store_tile(sm.raw[kk], l, p, x1, v1, v, v + 3, tn, m);                                   // my resident copy
-                hl_store_tile(A.C.raw + (size_t)(cta + kk * G) * RAW_TILE_BYTES, l, p, x1, v1, v, v + 3, tn, m);   // the j-store
-                sm.tnext[kk][l] = tn + d;
+                if (lane == 3) {
+                    A.pot[k] = v[6];
+                    A.S.t[p] = tn;
+                    A.S.dt[p] = d;
+                    atomicMin(A.C.dt_min_bits, (unsigned long long)__double_as_longlong(d));
+                }
+                if (lane == 4) {
+                    const float m = raw_m(Ts, l);
+                    raw_t(Ts, l) = tn; raw_idx(Ts, l) = p;              // (mass and index do not change; hl_store_tile wrote them too)
+                    raw_t(Tg, l) = tn; raw_m(Tg, l) = m; raw_idx(Tg, l) = p;
+                    sm.tnext[kk][l] = tn + d;
+                }
+                if (q0 == 0) HL_MK(21);
             }
             }
             __syncthreads();
+        }
+        HL_MK(10);
+        HL_MK(22);
+        if (PROF && tid == 0) {
+            sm.mk_open = nown > 0 && nown <= HL_CQ && ni < 8;
+            if (cta == 0 && ni < 8) {
+                for (int q = 0; q < 10; ++q) atomicAdd(A.prof + q, (unsigned long long)(sm.mk[q + 1] - sm.mk[q]));
+                atomicAdd(A.prof + 11, (unsigned long long)(sm.mk[11] - sm.mk[3]));
+                atomicAdd(A.prof + 12, (unsigned long long)(sm.mk[12] - sm.mk[11]));
+                atomicAdd(A.prof + 13, (unsigned long long)(sm.mk[13] - sm.mk[12]));
+                atomicAdd(A.prof + 14, (unsigned long long)(sm.mk[4] - sm.mk[13]));
+                atomicAdd(A.prof + 15, 1ull);
+            }
         }
         if (tid == 0) sm.nown_prev = nown;
         rescan = nown > 0;

@@ -132,14 +132,18 @@ def test_c2_full_run_vs_oracle_driven(cluster, oracle):
 
 
 # ------------------------------------------------------------------ device-resident integrator (NEXT-3, g6hd_*)
-def test_device_corrector_and_selection_against_oracle(cluster, oracle):
-    """One block step at a time: the block the device selects is the set of particles with the smallest
+@pytest.mark.parametrize("loop", [1, 0])
+def test_device_corrector_and_selection_against_oracle(cluster, oracle, monkeypatch, loop):
+    """(loop = 1: the persistent step-loop kernel k_hd_loop, one step per launch here; loop = 0: k_hd_select / the library's
+    force path / k_hd_correct with one host wait per step -- env G6_HD_LOOP, read by g6hd_create.)
+    One block step at a time: the block the device selects is the set of particles with the smallest
     t + dt, in address order; its i-particles are Eq. 1-2 predictions (oracle.predict); the corrector kernel's
     new x, v equal oracle.hermite_correct and the new step follows oracle.aarseth_dt and the power-of-two
     rule, given the forces the device used."""
     n = 3000
     x, v, m, _ = inputs.config("C2", n=n)
     eps2, eta, dt_max = 1e-4 ** 2, 0.01, 0.125
+    monkeypatch.setenv("G6_HD_LOOP", str(loop))
     h = g6.HermiteDev(0, x, v, m, eps2, eta)
     before = h.particles()
     assert np.all(before["t"] == 0) and np.all(before["dt"] <= dt_max) and np.all(np.log2(before["dt"]) % 1 == 0)
