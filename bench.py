@@ -289,7 +289,7 @@ def neighbour_list_cost(g6, inputs, torch, dev, x, v, idx_all, n, eps2, ni=65536
 
 def recorded_traffic(nj, ni, jsplits):
     """DRAM bytes of one force-kernel launch from the committed ncu capture, if it was taken on this configuration."""
-    p = os.path.join(ROOT, "profiles", "force_fast_traffic.json")
+    p = os.path.join(ROOT, "profiles", "r02_force_fast_traffic.json")
     try:
         rec = json.load(open(p))
     except Exception:
@@ -352,6 +352,29 @@ def c3_sweep(g6, inputs, torch, dev, peaks, reps=5):
     return {"workload": f"C3: N={n} equal-mass Plummer, eps=1e-4, full sweep", "ms_per_step": ms, "interactions_per_s": float(n) * n / (ms * 1e-3),
             "gflops_60": FLOP_PAPER * float(n) * n / (ms * 1e-3) / 1e9, "force_kernel_ms": f_us / 1e3,
             "fp32_frac_force_kernel": FP32_INSTR_PER_INTERACTION * float(n) * n / (f_us * 1e-6) / peak_inst}
+
+
+def c2_hermite(g6, inputs, t_end=1.0):
+    """BASELINE.json configs[1] (C2): N = 32768 equal-mass Plummer, eps = 1e-4, 4th-order Hermite with block time steps (eta = 0.01,
+    power-of-two steps) to t = 1, with the device-resident driver (g6hd_*: the block-step loop as one persistent kernel, blocks above
+    1024 particles through the sweep path).  A side figure: wall time of g6hd_evolve and the block-size histogram; the energy drift is
+    the parity suite's business (tests/test_hermite_gpu.py::test_c2_full_run_vs_oracle_driven).  Replaces the j-store contents: call last."""
+    x, v, m, eps2 = inputs.config("C2")
+    t0 = time.perf_counter()
+    h = g6.HermiteDev(0, x, v, m, eps2, 0.01)
+    t_init = time.perf_counter() - t0
+    try:
+        t0 = time.perf_counter()
+        h.evolve(t_end)
+        wall = time.perf_counter() - t0
+        st = h.stats()
+    finally:
+        h.close()
+    return {"workload": f"C2: N={len(m)} equal-mass Plummer, eps=1e-4, Hermite block time steps eta=0.01, t=0..{t_end:g}", "driver": "device-resident (g6hd_*)",
+            "wall_s": wall, "init_s": t_init, "block_steps": st["n_block_steps"], "particle_steps": st["n_particle_steps"],
+            "us_per_block_step": 1e6 * wall / max(1, st["n_block_steps"]), "interactions": st["interactions"],
+            "interactions_per_s": st["interactions"] / wall, "gflops_60": FLOP_PAPER * st["interactions"] / wall / 1e9,
+            "dt_min": st["dt_min"], "ni_hist_log2": [int(c) for c in st["ni_hist_log2"][:17]]}
 
 
 def run_reference(args):
@@ -631,6 +654,7 @@ def main():
 
     sweep = None
     c3 = None
+    c2 = None
     nb_cost = None
     ceilings = None
     ds_cost = None
@@ -640,6 +664,7 @@ def main():
         nb_cost = neighbour_list_cost(g6, inputs, torch, dev, x, v, idx, n, eps2)
         ds_cost = double_single_cost(g6, inputs, torch, dev, x, v, idx, n, eps2)
         c3 = c3_sweep(g6, inputs, torch, dev, measured_peaks()[0]) if args.n is None else None
+        c2 = c2_hermite(g6, inputs) if args.n is None else None
     if rank == 0:
         # what the FP32 pipes sustain for register-sourced instruction streams and for the pair loop itself (libg6b200_probe.so), live
         ceilings = probes.table(SM_COUNT * FP32_LANES_PER_SM * float(measured_peaks()[0].get("sm_max_mhz", SM_MAX_MHZ_FALLBACK)) * 1e6, stream.cuda_stream)
@@ -655,7 +680,7 @@ def main():
                     "achieved": 2 * ach_inst / 1e12, "peak": 2 * peak_inst / 1e12,
                     "unit": "TFLOP/s", "frac": ach_inst / peak_inst,
                     # dram__bytes_read.sum + dram__bytes_write.sum of one launch of this kernel from the committed ncu --set full capture
-                    # (profiles/force_fast_traffic.json names it); null unless that capture had this run's n_j, n_i and j-split count
+                    # (profiles/r02_force_fast_traffic.json names it); null unless that capture had this run's n_j, n_i and j-split count
                     "traffic": recorded_traffic(n, ni, int(tm["jsplits"])),
                     "how": ("FP32-pipe issue-slot equivalent: 33 algorithmic FP32 lane-instructions per interaction (SURVEY 8(d)) x "
                             "interactions per launch / mean force-kernel time (CUDA events on the launching stream, live in this run); "
@@ -689,6 +714,8 @@ def main():
             out["double_single_cost"] = ds_cost
         if c3 is not None:
             out["c3_sweep"] = c3
+        if c2 is not None:
+            out["c2_hermite"] = c2
         if not args.no_cpu_baseline and world == 1:
             rate, rows, dt, cores = cpu_oracle_rate(x, v, m, eps2, idx, args.cpu_seconds)
             out["cpu_baseline"] = {"value": rate, "unit": "interactions/s", "cores": cores, "kind": "oracle",

@@ -561,8 +561,17 @@ k_hd_loop(const HlArgs A)
         // fixed shuffle tree, the slices in slice order, the CTAs in CTA order (phase C): bit-reproducible.
         {
             const int nch = (ni + 31) / 32;
+            // C chunks at a time, each by HL_NW / C warps: a pass costs about C + 1/2 (in sixteenths of a tile per warp, plus its
+            // barriers and partial sums), so take the C that minimises passes x (C + 1/2); ties go to the larger C (fewer barriers).
+            // 24 chunks: three passes of 8 instead of 16 + 8; 6 chunks: three passes of 2 instead of one pass that idles a quarter
             int C = 1;
-            while (C < HL_NW && C < nch) C <<= 1;
+            {
+                int best = 1 << 30;
+                for (int c = 1; c <= HL_NW; c <<= 1) {
+                    const int cost = ((nch + c - 1) / c) * (2 * c + 1);
+                    if (cost <= best) { best = cost; C = c; }
+                }
+            }
             const int nsl = HL_NW / C, cw = w / nsl, sw = w % nsl, jper = JT / nsl;
             for (int r0 = 0; r0 < nch; r0 += C) {
                 const int c0 = (r0 + cw) * 32;

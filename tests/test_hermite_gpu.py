@@ -2,6 +2,8 @@
 integrator (oracle/hermite_oracle.c) on the same seeded inputs."""
 import time
 
+import os
+
 import numpy as np
 import pytest
 
@@ -227,6 +229,34 @@ def test_device_driver_edge_sizes_match_host_driver(cluster, oracle, n):
     assert np.abs(xd - xh).max() < 1e-7 and np.abs(vd - vh).max() < 1e-6
     if n == 1:          # a lone particle feels nothing: straight line
         assert np.allclose(xd, x + v * t_end, rtol=0, atol=1e-15)
+
+
+@pytest.mark.parametrize("n", [40000, 80000])
+def test_step_loop_with_several_resident_tiles_per_cta(cluster, oracle, n):
+    """More than 148 j-tiles: every CTA of the step loop keeps two (N = 40000) or three (N = 80000) raw tiles resident -- the
+    whole-CTA rescan, the per-tile records and the tile loops of the pair phase.  Against the same run without the loop
+    (G6_HD_LOOP = 0: k_hd_select / sweep path / k_hd_correct)."""
+    x, v, m, _ = inputs.config("C2", n=n)
+    eps2, eta, t_end = 1e-3 ** 2, 0.01, 2.0 ** -9
+    runs = {}
+    for loop in (1, 0):
+        os.environ["G6_HD_LOOP"] = str(loop)
+        try:
+            h = g6.HermiteDev(0, x, v, m, eps2, eta)
+        finally:
+            del os.environ["G6_HD_LOOP"]
+        h.evolve(t_end)
+        runs[loop] = (h.state(), h.stats(), h.particles(), h.last_block())
+        h.close()
+    (x1, v1), s1, p1, b1 = runs[1]
+    (x0, v0), s0, p0, b0 = runs[0]
+    assert s1["t"] == t_end == s0["t"] and s1["n_block_steps"] > 4
+    # same block schedule (FP32 force differences between the two pair codes may move a borderline step)
+    assert abs(s1["n_particle_steps"] - s0["n_particle_steps"]) <= 0.002 * s0["n_particle_steps"] + 2
+    assert np.abs(x1 - x0).max() < 1e-9 and np.abs(v1 - v0).max() < 1e-7
+    # the no-loop path is what the oracle-driven comparisons above pin; the last blocks of the two runs are the same particles
+    assert np.array_equal(b1["act"], b0["act"])
+    assert np.allclose(b1["acc"], b0["acc"], rtol=2e-5, atol=0) and np.allclose(b1["xi"], b0["xi"], rtol=0, atol=1e-9)
 
 
 @pytest.mark.parametrize("n,t_end", [(512, 0.0625), (3000, 0.015625)])
