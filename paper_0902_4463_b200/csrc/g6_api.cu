@@ -200,7 +200,9 @@ int ensure_i(Cluster &c, int ni)
     if (ni <= c.i_cap) return G6_OK;
     CK(cudaStreamSynchronize(c.stream));
     free_i(c);
-    size_t n = std::max(ni, 4096);
+    // grown geometrically: the block sizes of a Hermite run creep upwards, and every reallocation is a stream synchronisation plus
+    // cudaFree / cudaMalloc / cudaHostAlloc calls (measured: 1 ms to hundreds of ms each on the B200 box)
+    size_t n = std::max<size_t>(std::max(ni, 4096), (size_t)c.i_cap + c.i_cap / 2);
     CK(mapped_alloc(c.h_iblk, c.hd_iblk, iblk_bytes(n)));
     CK(mapped_alloc(c.h_res, c.hd_res, res_bytes(n)));
     CK(mapped_alloc(c.h_done, c.hd_done, sizeof(unsigned int)));
@@ -216,10 +218,12 @@ int ensure_i(Cluster &c, int ni)
 int ensure_partials(Cluster &c, size_t elems)
 {
     if (elems <= c.part_elems) return G6_OK;
+    const size_t prev = c.part_elems;
     CK(cudaStreamSynchronize(c.stream));
     if (c.part_block) cudaFree(c.part_block);
     c.part_block = nullptr;
     c.part_elems = 0;
+    elems = std::max(elems, prev + prev / 2);          // geometric growth (see ensure_i)
     elems = (elems + 63) & ~(size_t)63;
     CK(cudaMalloc(&c.part_block, elems * (7 * sizeof(double) + sizeof(float) + sizeof(int))));
     double *d = (double *)c.part_block;
@@ -261,6 +265,7 @@ int ensure_nb_part(Cluster &c, size_t rows)
     int rc = nb_check_maxlen(c);
     if (rc) return rc;
     if (rows <= c.nb_part_rows) return G6_OK;
+    rows = std::max(rows, c.nb_part_rows + c.nb_part_rows / 2);
     CK(cudaStreamSynchronize(c.stream));
     dfree(c.d_nb_pcnt); dfree(c.d_nb_plist);
     c.nb_part_rows = 0;
@@ -275,6 +280,7 @@ int ensure_nb_warp(Cluster &c, size_t rows)
     int rc = nb_check_maxlen(c);
     if (rc) return rc;
     if (rows <= c.nb_w_rows) return G6_OK;
+    rows = std::max(rows, c.nb_w_rows + c.nb_w_rows / 2);
     CK(cudaStreamSynchronize(c.stream));
     dfree(c.d_nb_wcnt); dfree(c.d_nb_wlist);
     c.nb_w_rows = 0;
@@ -289,12 +295,13 @@ int ensure_nb_host(Cluster &c, int ni)
     int rc = nb_check_maxlen(c);
     if (rc) return rc;
     if (ni <= c.nb_cap) return G6_OK;
+    const int prev_cap = c.nb_cap;
     CK(cudaStreamSynchronize(c.stream));
     dfree(c.d_nb_cnt); dfree(c.d_nb_list); dfree(c.d_h2);
     hfree(c.h_nb_cnt); hfree(c.h_nb_list); hfree(c.h_h2);
     c.nb_cap = 0;
     c.last_nb = c.nb_on_host = false;
-    const size_t n = std::max(ni, 1024), ml = c.opt_nb_maxlen;
+    const size_t n = std::max<size_t>(std::max(ni, 1024), (size_t)prev_cap + prev_cap / 2), ml = c.opt_nb_maxlen;
     CK(dalloc(c.d_nb_cnt, n)); CK(dalloc(c.d_nb_list, n * ml)); CK(dalloc(c.d_h2, n));
     CK(halloc(c.h_nb_cnt, n)); CK(halloc(c.h_nb_list, n * ml)); CK(halloc(c.h_h2, n));
     c.nb_cap = (int)n;
@@ -304,6 +311,7 @@ int ensure_nb_host(Cluster &c, int ni)
 int ensure_bulk(Cluster &c, size_t bytes)
 {
     if (bytes <= c.bulk_bytes) return G6_OK;
+    bytes = std::max(bytes, c.bulk_bytes + c.bulk_bytes / 2);
     CK(cudaStreamSynchronize(c.stream));
     if (c.h_bulk) cudaFreeHost(c.h_bulk);
     if (c.d_bulk) cudaFree(c.d_bulk);
