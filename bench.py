@@ -357,7 +357,7 @@ def c3_sweep(g6, inputs, torch, dev, peaks, reps=5):
 def c2_hermite(g6, inputs, t_end=1.0):
     """BASELINE.json configs[1] (C2): N = 32768 equal-mass Plummer, eps = 1e-4, 4th-order Hermite with block time steps (eta = 0.01,
     power-of-two steps) to t = 1, with the device-resident driver (g6hd_*: the block-step loop as one persistent kernel, blocks above
-    1024 particles through the sweep path).  A side figure: wall time of g6hd_evolve and the block-size histogram; the energy drift is
+    768 particles through the sweep path).  A side figure: wall time of g6hd_evolve and the block-size histogram; the energy drift is
     the parity suite's business (tests/test_hermite_gpu.py::test_c2_full_run_vs_oracle_driven).  Replaces the j-store contents: call last."""
     x, v, m, eps2 = inputs.config("C2")
     t0 = time.perf_counter()

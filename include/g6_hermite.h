@@ -54,8 +54,16 @@ int g6h_get_force_wall_hist(g6h_system *s, double wall_s_log2[64]);
 /* ---- device-resident variant -----------------------------------------------
  * The same integrator with the particle state kept in device memory and the O(n_i) steps -- block
  * selection, prediction of the i-particles, corrector, step choice, j-store update --
- * run as CUDA kernels; the force is the library's own path.  Per block step the host waits once, for
- * (n_i, t_next).  The paper leaves these steps on the CPU because GRAPE host codes did.
+ * run as CUDA kernels; the force is the library's own path.  The paper leaves these steps on the CPU
+ * because GRAPE host codes did.
+ * Block steps of up to 768 particles ("block sizes are typically small on average") run inside ONE persistent
+ * cooperative kernel (g6_hermite_loop.cuh: j-tiles resident in shared memory, the CTAs meet through self-validating exchange
+ * words) which returns to the host only for a larger block -- whose forces the library's sweep path
+ * computes -- at t_end, or when the step budget is used up.  Needs n <= 4 x 256 x (number of SMs) particles; beyond that, or
+ * with env G6_HD_LOOP = 0, every block step is two or three launches and one host wait for (n_i, t_next).
+ * Environment (read by g6hd_create): G6_HD_LOOP (default 1), G6_HD_LOOP_MAXI (largest block stepped inside the loop, default
+ * and at most 768), G6_HD_LOOP_PROFILE (1: the loop built with clock marks, 2: the production loop; both print the time per
+ * block-size bin from g6hd_get_stats to stderr), G6_HD_PROFILE (CUDA-event phase times of the path without the loop).
  * Same formulas as above, fp64 (the device contracts a*b+c into FMAs, so results agree with g6h_* to
  * rounding, not bit for bit).  Same argument and error conventions; n <= the cluster's capacity. */
 typedef struct g6hd_system g6hd_system;

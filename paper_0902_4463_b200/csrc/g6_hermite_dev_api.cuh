@@ -46,7 +46,7 @@ struct g6hd_system {
     unsigned long long *prof = nullptr;     // [32] the marked build's summed intervals (device)
 };
 
-constexpr int HD_LOOP_MAXI_DEFAULT = 1024;
+constexpr int HD_LOOP_MAXI_DEFAULT = HL_MAX_I;
 
 namespace {
 
