@@ -393,15 +393,17 @@ __device__ __forceinline__ void block_step_body(const BsArgs &A0, const BsInline
             const int i = k / NW, q = k % NW;
             A.nb_wcnt[(size_t)i * (G * NW) + cta * NW + q] = sm.nbcnt[q][i];
         }
-    __threadfence();
+    // the ticket: the barrier orders the CTA's partial stores before thread 0, whose release fence is cumulative; the last CTA's
+    // acquire fence sits between the ticket and its reads of the partials (ld.global.cg)
     __syncthreads();
     if (tid == 0) {
+        fence_acq_rel_gpu();
         const unsigned ticket = atomicAdd(A.counter, 1u);
         sm.is_last = (ticket == (unsigned)G - 1u);
+        if (sm.is_last) fence_acq_rel_gpu();
     }
     __syncthreads();
     if (!sm.is_last) return;
-    __threadfence();
 
     // ---- a-5, second half (last CTA only): sum the G partials of every i in CTA order
     for (int i = w; i < A.ni; i += BS_THREADS / 32) {
@@ -836,15 +838,17 @@ __device__ __forceinline__ void block_step2_body(const BsArgs &A, const BsInline
         A.P.nn_r2[o] = has ? bst : INF;
         A.P.nn_addr[o] = has ? bad : -1;
     }
-    __threadfence();
+    // the ticket: the barrier orders the CTA's partial stores before thread 0, whose release fence is cumulative; the last CTA's
+    // acquire fence sits between the ticket and its reads of the partials (ld.global.cg)
     __syncthreads();
     if (tid == 0) {
+        fence_acq_rel_gpu();
         const unsigned ticket = atomicAdd(A.counter, 1u);
         sm.is_last = (ticket == (unsigned)G - 1u);
+        if (sm.is_last) fence_acq_rel_gpu();
     }
     __syncthreads();
     if (!sm.is_last) return;
-    __threadfence();
 
     // ---- a-5, second half (last CTA only): sum the G partials of every i in CTA order, one warp per i-particle
     for (int i = w; i < A.ni; i += NW) {

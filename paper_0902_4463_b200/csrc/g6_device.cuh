@@ -11,6 +11,12 @@
 
 namespace g6 {
 
+// acquire-release fence at device scope.  __threadfence() is the sequentially consistent fence and on sm_100 compiles to MEMBAR.SC.GPU
+// plus a whole-L1 invalidate (CCTL.IVALL), microseconds when stores are in flight; the "last CTA" patterns of this library only need
+// release (partials before the ticket) and acquire (ticket before the partials, which are then read with ld.global.cg).
+__device__ __forceinline__ void fence_acq_rel_gpu() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
+
+
 // ---- j-particle store (raw Hermite state at t_j): tiles of JT particles, field-major in a tile --
 // "Only the position is stored in DP, whereas the rest of the terms are stored in SP".
 // Tile k = RAW_TILE_BYTES bytes at raw + k * RAW_TILE_BYTES:

@@ -70,10 +70,12 @@ __device__ __forceinline__ double hd_block_min(double v, double *sm)
 // Eq. 1-2 in fp64 for particle p at time tn
 __device__ __forceinline__ void hd_predict(const HdState &S, int p, double tn, double *xp, double *vp)
 {
-    const double h = tn - S.t[p], h2 = h * h / 2, h3 = h * h * h / 6;
+    // read from L2 (ld.global.cg): the state may have been written by another thread block of the same launch (the corrector of the
+    // last-block patterns, the owners of the step loop), and nothing on this path invalidates L1
+    const double h = tn - __ldcg(S.t + p), h2 = h * h / 2, h3 = h * h * h / 6;
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-        const double x = S.x[3 * (size_t)p + k], v = S.v[3 * (size_t)p + k], a = S.a[3 * (size_t)p + k], ad = S.ad[3 * (size_t)p + k];
+        const double x = __ldcg(S.x + 3 * (size_t)p + k), v = __ldcg(S.v + 3 * (size_t)p + k), a = __ldcg(S.a + 3 * (size_t)p + k), ad = __ldcg(S.ad + 3 * (size_t)p + k);
         xp[k] = x + v * h + a * h2 + ad * h3;
         vp[k] = v + a * h + ad * h2;
     }
@@ -281,12 +283,14 @@ k_hd_select(HdState S, HdBlock B, HdCorr C, int correct_first)
         B.bmin[b] = bm;
         B.bcnt[b] = off;
     }
-    __threadfence();
     __syncthreads();
-    if (tid == 0) s_last = atomicAdd(B.ticket, 1u) == (unsigned)nb - 1u;
+    if (tid == 0) {
+        fence_acq_rel_gpu();                              // release: this block's minimum, count and candidates (ordered before by the barrier)
+        s_last = atomicAdd(B.ticket, 1u) == (unsigned)nb - 1u;
+        if (s_last) fence_acq_rel_gpu();                  // acquire: the other blocks' (read with ld.global.cg below)
+    }
     __syncthreads();
     if (!s_last) return;
-    __threadfence();
 
     // ---- last thread block
     double g = INF;
