@@ -377,6 +377,13 @@ def c2_hermite(g6, inputs, t_end=1.0):
             "dt_min": st["dt_min"], "ni_hist_log2": [int(c) for c in st["ni_hist_log2"][:17]]}
 
 
+def bench_config(inputs, n, eps2, newton, world):
+    """the `config` object of the BENCH line: the same for the CUDA arm and for --impl reference"""
+    return {"workload": f"{WORKLOAD}: N={n} equal-mass Plummer sphere, eps=1e-4, full force sweep n_i=N_j=N",
+            "n": n, "eps2": eps2, "seed": inputs.CONFIGS[WORKLOAD]["seed"], "newton_step": int(newton),
+            "parallelism": f"i-split x{world}" if world > 1 else "1 GPU", "l2": "flushed between timed steps (512 MiB write)"}
+
+
 def run_reference(args):
     """--impl reference: the oracle, timed on the host cores on a bounded sample per step."""
     rank = int(os.environ.get("RANK", "0"))
@@ -406,7 +413,9 @@ def run_reference(args):
     out = {"impl": "reference", "metric": METRIC, "value": value, "unit": "interactions/s", "n_gpus": args.gpus, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True, "scaling": "strong",
            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-           "config": {"workload": f"{WORKLOAD}: N={n} equal-mass Plummer, eps=1e-4, full sweep (sampled rows)", "n": n},
+           # the same config as the CUDA arm's line (the driver compares them); that each step is a bounded sample of the rows is
+           # said in cpu_baseline.sample
+           "config": bench_config(inputs, n, eps2, 1 if args.newton is None else int(args.newton), max(1, args.gpus)),
            "cpu_baseline": {"value": value, "unit": "interactions/s", "cores": orc.threads(), "kind": "oracle", "sample": sample},
            "e2e": {"value": value, "unit": "interactions/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
            "gflops_60": value * FLOP_PAPER / 1e9}
@@ -698,9 +707,7 @@ def main():
                "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps, "higher_is_better": True,
                "scaling": "strong", "vs_baseline": None, "dtype": "f32 (double-single separations, fp64 accumulation across tiles)",
                "data": "synthetic",
-               "config": {"workload": f"{WORKLOAD}: N={n} equal-mass Plummer sphere, eps=1e-4, full force sweep n_i=N_j=N",
-                          "n": n, "eps2": eps2, "seed": inputs.CONFIGS[WORKLOAD]["seed"], "newton_step": int(newton),
-                          "parallelism": f"i-split x{world}" if world > 1 else "1 GPU", "l2": "flushed between timed steps (512 MiB write)"},
+               "config": bench_config(inputs, n, eps2, int(newton), world),
                "gflops_60": value * FLOP_PAPER / 1e9, "gflops_66": value * 66 / 1e9,
                "clocks": clocks, "roofline": roofline, "gpu_launches": 4 * args.steps,
                "wall_s_timed_region": wall}
