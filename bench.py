@@ -140,6 +140,51 @@ class Probes:
         if rc:
             raise RuntimeError(f"g6p_read_pass failed: cudaError {rc}")
 
+    MIX_KINDS = ((1, "lds"), (2, "mov_imm"), (3, "iadd"), (4, "lop3_two_reads"), (5, "fmnmx"), (6, "fmnmx3"), (7, "vimnmx3"),
+                 (8, "scalar_ffma"), (9, "mufu_rsq"))
+    OPERAND_MODES = ((0, "ffma2_acc_x_shared_vector_pair_reuse"), (1, "ffma2_acc_x_uniform_register_pair"), (2, "ffma2_acc_x_32bit_broadcast"),
+                     (3, "fadd2_acc_shared_vector_pair"), (4, "fadd2_acc_uniform_register_pair"), (5, "ffma2_three_distinct_vector_pairs"))
+
+    def mix_cycles(self, kind, extra, sm_hz, stream=0):
+        r = self.C.c_double(0.0)
+        rc = self.L.g6p_mix_cycles(self.C.c_int(kind), self.C.c_int(extra), self.C.c_double(sm_hz), self.C.c_void_p(stream), self.C.byref(r))
+        if rc:
+            raise RuntimeError(f"g6p_mix_cycles failed: cudaError {rc}")
+        return r.value
+
+    def operand_rate(self, mode, stream=0):
+        r = self.C.c_double(0.0)
+        rc = self.L.g6p_operand_rate(self.C.c_int(mode), self.C.c_void_p(stream), self.C.byref(r))
+        if rc:
+            raise RuntimeError(f"g6p_operand_rate failed: cudaError {rc}")
+        return r.value
+
+    def pair_rate_cbank(self, shape, stream=0):
+        r = self.C.c_double(0.0)
+        rc = self.L.g6p_pair_rate_cbank(self.C.c_int(shape), self.C.c_void_p(stream), self.C.byref(r))
+        if rc:
+            raise RuntimeError(f"g6p_pair_rate_cbank failed: cudaError {rc}")
+        return r.value
+
+    def extended(self, peak_inst, sm_hz, stream=0):
+        """--probes only (profiles/r02_fp32_operand_probes.md): what one non-FMA instruction costs next to a saturated FFMA2 stream,
+        which operand forms cost no vector-register read, and the pair loop with its j-tiles in the constant bank"""
+        out = {}
+        base = self.mix_cycles(0, 0, sm_hz, stream)
+        mix = {"twelve_ffma2_alone_cycles": base}
+        for kind, name in self.MIX_KINDS:
+            row = {}
+            for extra in ((1, 2, 4) if name == "mufu_rsq" else (4, 12)):
+                c = self.mix_cycles(kind, extra, sm_hz, stream)
+                row[f"plus_{extra}"] = {"cycles": c, "cost_each": (c - base) / extra}
+            mix[name] = row
+        out["non_fma_instruction_next_to_12_ffma2"] = mix
+        out["operand_forms_frac_of_peak"] = {name: self.operand_rate(mode, stream) / peak_inst for mode, name in self.OPERAND_MODES}
+        cb = {sh: self.pair_rate_cbank(k, stream) for k, sh in ((0, "128x2"), (1, "128x1"))}
+        out["pair_loop_j_tiles_in_constant_bank"] = {"interactions_per_s": cb, "pipe_busy_frac": {k: v * 36 / peak_inst for k, v in cb.items()},
+                                                     "frac_of_peak_at_33": {k: v * 33 / peak_inst for k, v in cb.items()}}
+        return out
+
     def table(self, peak_inst, stream=0):
         """every probe as a fraction of the nominal FP32 peak (lane-instructions / s)"""
         out = {"fp32_instruction_streams_frac_of_peak": {}, "pair_loop": {}}
@@ -543,7 +588,10 @@ def main():
         if rank == 0:
             peaks, _ = measured_peaks()
             peak_inst = SM_COUNT * FP32_LANES_PER_SM * float(peaks.get("sm_max_mhz", SM_MAX_MHZ_FALLBACK)) * 1e6
-            print(json.dumps({"probes": Probes().table(peak_inst), "peak_lane_instr_per_s": peak_inst}), flush=True)
+            pr = Probes()
+            sm_hz = float(peaks.get("sm_max_mhz", SM_MAX_MHZ_FALLBACK)) * 1e6
+            print(json.dumps({"probes": pr.table(peak_inst), "probes_extended": pr.extended(peak_inst, sm_hz), "peak_lane_instr_per_s": peak_inst,
+                              "sm_hz_assumed": sm_hz}), flush=True)
         return
     if args.mode == "jsplit":
         return run_jsplit(args, torch, dist, g6, inputs, world, rank, local, dev)
