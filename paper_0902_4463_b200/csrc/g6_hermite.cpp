@@ -5,6 +5,8 @@
 
 #include <chrono>
 #include <cmath>
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <utility>
@@ -34,6 +36,7 @@ struct g6h_system {
     std::vector<double> pot;
     long long nblock = 0, npart = 0, hist[64] = {};
     double inter = 0, wall = 0, wall_force = 0, wall_force_hist[64] = {};
+    double wall_predict = 0, wall_correct = 0;       // where the host's own time goes (printed with env G6H_PROFILE)
 };
 
 namespace {
@@ -178,12 +181,15 @@ static int evolve_body(g6h_system &s, double t_end, long long max_block_steps)
         for (int k = kmax; k >= 0 && std::fmod(tn, level_step(s, k)) == 0.0; --k)
             s.act.insert(s.act.end(), s.lev[k].begin(), s.lev[k].end());
         const int ni = (int)s.act.size();
+        const auto p0 = Clock::now();
         for (int k = 0; k < ni; ++k) predict_one(s, s.act[k], tn, s.xi[k], s.vi[k]);
         const auto f0 = Clock::now();
+        s.wall_predict += secs(p0, f0);
         rc = block_force(s, tn);
         const double wf = secs(f0, Clock::now());
         s.wall_force += wf;
         if (rc) break;
+        const auto c0 = Clock::now();
         for (int k = 0; k < ni; ++k) {
             const int p = s.act[k];
             const double h = s.dt[p], h2 = h * h, h3 = h2 * h, h4 = h3 * h, h5 = h4 * h;
@@ -215,6 +221,7 @@ static int evolve_body(g6h_system &s, double t_end, long long max_block_steps)
             rc = send_j(s, p);
             if (rc) break;
         }
+        s.wall_correct += secs(c0, Clock::now());
         if (rc) break;
         s.t = tn;
         ++s.nblock; ++done;
@@ -226,6 +233,12 @@ static int evolve_body(g6h_system &s, double t_end, long long max_block_steps)
         s.wall_force_hist[b] += wf;
     }
     s.wall += secs(w0, Clock::now());
+    // (measured on C2: 3.4 s = force calls 2.3 + i-prediction 0.17 + corrector, level lists and g6_set_j_particle 0.87; computing the
+    // corrector of large blocks on 8 threads and updating lists and j-particles afterwards was slower, 1.18 s: the scattered
+    // particle state, not the arithmetic, is what costs)
+    if (std::getenv("G6H_PROFILE"))
+        std::fprintf(stderr, "g6h profile: wall %.3f s, force calls %.3f, i-prediction %.3f, corrector + level lists + g6_set_j_particle %.3f, block selection and the rest %.3f\n",
+                     s.wall, s.wall_force, s.wall_predict, s.wall_correct, s.wall - s.wall_force - s.wall_predict - s.wall_correct);
     return rc;
 }
 
