@@ -61,7 +61,7 @@ def test_library_exports_only_what_the_headers_declare(library):
     dbg = [n for n in _exported(build.build_debug()) if n.startswith("g6")]
     assert dbg == ["g6dbg_pair_dx"]
     probe = [n for n in _exported(build.build_probe()) if n.startswith("g6")]
-    assert probe == ["g6p_fp32_rate", "g6p_pair_rate", "g6p_read_pass"]
+    assert probe == ["g6p_fp32_rate", "g6p_mix_cycles", "g6p_operand_rate", "g6p_pair_rate", "g6p_pair_rate_cbank", "g6p_read_pass"]
 
 
 def test_headers_have_no_torch_or_cxx_types():
