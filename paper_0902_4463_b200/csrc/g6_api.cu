@@ -201,9 +201,9 @@ void free_i(Cluster &c)
 // split over a few threads (contiguous pieces: the result is the same bytes).
 void big_memcpy(void *dst, const void *src, size_t bytes)
 {
-    constexpr size_t MIN_PER_THREAD = 8u << 20;
+    constexpr size_t MIN_PER_THREAD = 4u << 20;
     const unsigned hw = std::thread::hardware_concurrency();
-    const size_t nt = std::min<size_t>(std::min<size_t>(hw ? hw : 1, 6), bytes / MIN_PER_THREAD);
+    const size_t nt = std::min<size_t>(std::min<size_t>(hw ? hw : 1, 12), bytes / MIN_PER_THREAD);
     if (nt < 2) { memcpy(dst, src, bytes); return; }
     std::vector<std::thread> th;
     const size_t per = ((bytes / nt) + 4095) & ~(size_t)4095;
