@@ -257,6 +257,27 @@ k_hd_loop(const HlArgs A)
     const float2 eps2s = dup(pair_scale<NEWTON>() * A.eps2);
     const double kP = NEWTON ? 0.5 * sqrt((double)FOUR_THIRDS) : sqrt((double)THIRD), kA = kP * kP * kP;
 
+    // (min, count, first slots at the min) of t + dt of my one resident tile -> sm.recw[0], sm.bal[0]; one whole warp
+    const auto rescan_tile0 = [&]() {
+        // t + dt >= 0 (or +inf): the doubles order like their bit patterns, and the minimum of 64-bit patterns over the
+        // warp is two 32-bit warp reductions (high words, then the low words of the lanes at the high minimum)
+        unsigned long long v[JT / 32], m = ~0ull;     // lane holds the slots lane, lane + 32, ...
+#pragma unroll
+        for (int r = 0; r < JT / 32; ++r) { v[r] = (unsigned long long)__double_as_longlong(sm.tnext[0][32 * r + lane]); m = v[r] < m ? v[r] : m; }
+        const unsigned int mh = __reduce_min_sync(FULL, (unsigned int)(m >> 32));
+        const unsigned int ml = __reduce_min_sync(FULL, (unsigned int)(m >> 32) == mh ? (unsigned int)m : 0xffffffffu);
+        m = ((unsigned long long)mh << 32) | ml;
+        unsigned int bal[JT / 32];
+#pragma unroll
+        for (int r = 0; r < JT / 32; ++r) {
+            bal[r] = __ballot_sync(FULL, v[r] == m);
+            if (lane == 0) sm.bal[0][r] = bal[r];      // (the non-inline path of phase A reads them)
+        }
+        // every lane has the ballots: the record in registers, no round trip through shared memory
+        if (lane == 0) hl_make_record(bal, __longlong_as_double((long long)m), sm.recw[0]);
+        __syncwarp();
+    };
+    bool pre_scanned = false;              // an idle warp rescanned my tile at the end of phase C (Kc == 1, I corrected particles)
     for (;;) {
         if (!(t_sys < A.t_end)) { reason = HL_END; break; }
         if (A.max_steps > 0 && steps >= A.max_steps) { reason = HL_STEPS; break; }
@@ -292,30 +313,9 @@ k_hd_loop(const HlArgs A)
         }
         if (w == 0) {
             // everything from here to the barrier below is warp 0's: rescan (one tile), publish, poll, select
-            if (rescan && Kc == 1) {
-                // t + dt >= 0 (or +inf): the doubles order like their bit patterns, and the minimum of 64-bit patterns over the
-                // warp is two 32-bit warp reductions (high words, then the low words of the lanes at the high minimum)
-                unsigned long long v[JT / 32], m = ~0ull;     // lane holds the slots lane, lane + 32, ...
-#pragma unroll
-                for (int r = 0; r < JT / 32; ++r) { v[r] = (unsigned long long)__double_as_longlong(sm.tnext[0][32 * r + lane]); m = v[r] < m ? v[r] : m; }
-                const unsigned int mh = __reduce_min_sync(FULL, (unsigned int)(m >> 32));
-                const unsigned int ml = __reduce_min_sync(FULL, (unsigned int)(m >> 32) == mh ? (unsigned int)m : 0xffffffffu);
-                m = ((unsigned long long)mh << 32) | ml;
-                unsigned int bal[JT / 32];
-#pragma unroll
-                for (int r = 0; r < JT / 32; ++r) {
-                    bal[r] = __ballot_sync(FULL, v[r] == m);
-                    if (lane == 0) sm.bal[0][r] = bal[r];      // (the non-inline path of phase A reads them)
-                }
-                // every lane has the ballots: the record in registers, no round trip through shared memory
-                if (lane == 0) hl_make_record(bal, __longlong_as_double((long long)m), sm.recw[0]);
-                __syncwarp();
-            }
-            // Release: the Hermite state of my particles that phase C of the last step wrote (other warps, ordered before this
-            // point by the barriers of phase C) must be visible to whoever reads the records
+            if (rescan && Kc == 1 && !pre_scanned) rescan_tile0();
+            // (release: the owners' warps fenced after their state stores in phase C of the last step, before its closing barrier)
             HL_MK(23);
-            if (lane == 0 && sm.nown_prev > 0) hl_fence();
-            __syncwarp();
             HL_MK(24);
             for (int kk = 0; kk < Kc; ++kk) {
                 unsigned int rw[HL_REC_WORDS];
@@ -711,6 +711,13 @@ k_hd_loop(const HlArgs A)
             if (q0 == 0) HL_MK(17);
             __syncthreads();
             if (q0 == 0) HL_MK(18);
+            // The owner's chain is the critical path of a small block step (the other CTAs wait for its records), so it is ordered
+            // for overlap: corrector and new step first -> t + dt into shared memory -> (last round, one tile) barrier -> an idle warp
+            // rescans the tile for the next records WHILE the particle's warp stores the new state and runs the release fence.
+            const bool last_round = Kc == 1 && q0 + HL_CQ >= nown;
+            bool have = false;
+            int c_k = 0, c_kk = 0, c_l = 0, c_p = 0, c_c = 0;
+            double x1c = 0, v1c = 0, a1c = 0, ad1c = 0, d_new = 0, pot_new = 0;
             if (w < nq) {
             const int q = q0 + w;
             const int k = sm.own_k[q], sl = sm.own_l[q];
@@ -729,9 +736,7 @@ k_hd_loop(const HlArgs A)
                 for (int c = 0; c < 7; ++c) v[c] += __shfl_xor_sync(FULL, v[c], o);
             }
             if (q0 == 0) HL_MK(19);
-            {
-                // the corrector, the Aarseth step and the power-of-two rule: lanes 0-2 one component each (hd_correct_warp), and
-                // each of them stores its own component of the new state, of the resident tile and of the j-store record
+                // the corrector, the Aarseth step and the power-of-two rule: lanes 0-2 one component each (hd_correct_warp)
                 const int kk = sl / JT, l = sl % JT;
                 const int p = (cta + kk * G) * JT + l;
                 const int c = lane < 3 ? lane : 0;
@@ -745,10 +750,18 @@ k_hd_loop(const HlArgs A)
                     a0c = A.S.a[3 * (size_t)p + c]; ad0c = A.S.ad[3 * (size_t)p + c];
                     h = A.S.dt[p];
                 }
-                const double a1c = c == 0 ? v[0] : c == 1 ? v[1] : v[2], ad1c = c == 0 ? v[3] : c == 1 ? v[4] : v[5];
-                double x1c, v1c;
-                const double d = hd_correct_warp(lane, h, a0c, ad0c, a1c, ad1c, xic, vic, tn, A.C.eta, A.C.dt_max, x1c, v1c);
+                a1c = c == 0 ? v[0] : c == 1 ? v[1] : v[2];
+                ad1c = c == 0 ? v[3] : c == 1 ? v[4] : v[5];
+                d_new = hd_correct_warp(lane, h, a0c, ad0c, a1c, ad1c, xic, vic, tn, A.C.eta, A.C.dt_max, x1c, v1c);
+                if (lane == 4) sm.tnext[kk][l] = tn + d_new;
+                pot_new = v[6];
+                have = true; c_k = k; c_kk = kk; c_l = l; c_p = p; c_c = c;
                 if (q0 == 0) HL_MK(20);
+            }
+            if (last_round) __syncthreads();                     // every corrected particle's t + dt is in place
+            if (have) {
+                // each of lanes 0-2 stores its own component of the new state, of the resident tile and of the j-store record
+                const int k = c_k, kk = c_kk, l = c_l, p = c_p, c = c_c;
                 char *Ts = sm.raw[kk], *Tg = A.C.raw + (size_t)(cta + kk * G) * RAW_TILE_BYTES;      // my resident copy, the j-store
                 if (lane < 3) {
                     A.a1[3 * (size_t)k + c] = a1c; A.ad1[3 * (size_t)k + c] = ad1c;
@@ -758,19 +771,23 @@ k_hd_loop(const HlArgs A)
                     raw_x(Tg, c, l) = x1c; raw_v(Tg, c, l) = (float)v1c; raw_a2(Tg, c, l) = (float)(a1c / 2); raw_j6(Tg, c, l) = (float)(ad1c / 6);
                 }
                 if (lane == 3) {
-                    A.pot[k] = v[6];
+                    A.pot[k] = pot_new;
                     A.S.t[p] = tn;
-                    A.S.dt[p] = d;
-                    atomicMin(A.C.dt_min_bits, (unsigned long long)__double_as_longlong(d));
+                    A.S.dt[p] = d_new;
+                    atomicMin(A.C.dt_min_bits, (unsigned long long)__double_as_longlong(d_new));
                 }
                 if (lane == 4) {
                     const float m = raw_m(Ts, l);
-                    raw_t(Ts, l) = tn; raw_idx(Ts, l) = p;              // (mass and index do not change; hl_store_tile wrote them too)
+                    raw_t(Ts, l) = tn; raw_idx(Ts, l) = p;              // (mass and index do not change)
                     raw_t(Tg, l) = tn; raw_m(Tg, l) = m; raw_idx(Tg, l) = p;
-                    sm.tnext[kk][l] = tn + d;
                 }
+                // release: the new Hermite state must be visible to whoever reads this CTA's next records; the warp's stores are
+                // ordered before lane 0's fence by the warp barrier, the fence before the records by the closing CTA barrier
+                __syncwarp();
+                if (lane == 0) hl_fence();
                 if (q0 == 0) HL_MK(21);
-            }
+            } else if (last_round && w == HL_NW - 1) {
+                rescan_tile0();
             }
             __syncthreads();
         }
@@ -789,6 +806,7 @@ k_hd_loop(const HlArgs A)
         }
         if (tid == 0) sm.nown_prev = nown;
         rescan = nown > 0;
+        pre_scanned = nown > 0 && Kc == 1;      // (the last round of phase C rescanned the tile)
         t_sys = tn;
         ++steps;
         npart += ni;
