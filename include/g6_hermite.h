@@ -12,6 +12,12 @@
  *   step       dt_want = sqrt(eta (|a1||a2'| + |adot1|^2) / (|adot1||a3| + |a2'|^2)),  a2' = a2 + h a3;
  *              power-of-two steps, halved while dt > dt_want, doubled only when dt_want >= 2 dt and the
  *              time is a multiple of 2 dt, dt <= dt_max; first step eta_start |a| / |adot| rounded down.
+ *   dt_max     should be a POWER OF TWO (the configurations of BASELINE.json use 1/8): all steps are dt_max halved k times, so the
+ *              particle times are then exact binary fractions and the particles of one step level share their block times bit for
+ *              bit -- which is what "the same block" means in all three drivers.  Any other positive value is accepted and
+ *              integrates correctly, but sums of steps are then rounded, particles that reached a time by different step sequences
+ *              no longer compare equal, and the blocks fragment (measured with dt_max = 0.1: two to five times as many block steps,
+ *              and a block schedule that depends on the last bit of the forces).
  *
  * All pointers are HOST pointers, [][3] arrays row-major fp64; the caller owns them.
  * Functions return 0 or a negative G6_ERR_* code (g6h_create: NULL on failure; the text is in
