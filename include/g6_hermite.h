@@ -15,9 +15,8 @@
  *   dt_max     should be a POWER OF TWO (the configurations of BASELINE.json use 1/8): all steps are dt_max halved k times, so the
  *              particle times are then exact binary fractions and the particles of one step level share their block times bit for
  *              bit -- which is what "the same block" means in all three drivers.  Any other positive value is accepted and
- *              integrates correctly, but sums of steps are then rounded, particles that reached a time by different step sequences
- *              no longer compare equal, and the blocks fragment (measured with dt_max = 0.1: two to five times as many block steps,
- *              and a block schedule that depends on the last bit of the forces).
+ *              integrates correctly (the drivers agree with each other, tested by random comparison at dt_max = 0.1), but sums of
+ *              steps are then rounded and particles that reached a time by different step sequences may not compare equal.
  *
  * All pointers are HOST pointers, [][3] arrays row-major fp64; the caller owns them.
  * Functions return 0 or a negative G6_ERR_* code (g6h_create: NULL on failure; the text is in

@@ -500,7 +500,7 @@ k_hd_loop(const HlArgs A)
                     }
                     if (cta == 0) { A.B.xi[3 * (size_t)k + c] = xi[c]; A.B.vi[3 * (size_t)k + c] = vi[c]; }     // read-back only
                 }
-                if (mine) sm.own_st[(T / G) * HL_INLINE + (k - sm.s_off[T])][12] = h;
+                if (mine) sm.own_st[(T / G) * HL_INLINE + (k - sm.s_off[T])][12] = A.S.dt[p];      // the stored step (= h when dt_max is a power of two)
                 if (cta == 0) A.B.act[k] = p;
             }
         } else {
