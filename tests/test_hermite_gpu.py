@@ -262,6 +262,31 @@ def test_step_loop_with_several_resident_tiles_per_cta(cluster, oracle, n):
         assert rel.max() <= 2e-5 and np.allclose(b1["xi"], b0["xi"], rtol=0, atol=1e-8)
 
 
+def test_step_loop_with_a_largest_step_that_is_not_a_power_of_two(cluster, oracle):
+    """dt_max = 0.1: the steps are 0.1 / 2^k, sums of steps are rounded, and t_next - t is no longer bit for bit the stored step.
+    The loop and the path without it must still take the same block steps (the loop's corrector once started from t_next - t:
+    3709 block steps against 2186 on this case)."""
+    n = 3426
+    x, v, m, _ = inputs.config("C2", n=n)
+    eps2, eta, dt_max, t_end = 1e-2 ** 2, 0.01, 0.1, 0.05
+    runs = {}
+    for loop in (1, 0):
+        os.environ["G6_HD_LOOP"] = str(loop)
+        try:
+            h = g6.HermiteDev(0, x, v, m, eps2, eta, dt_max=dt_max)
+        finally:
+            del os.environ["G6_HD_LOOP"]
+        h.evolve(t_end)
+        runs[loop] = (h.state(), h.stats())
+        h.close()
+    (x1, v1), s1 = runs[1]
+    (x0, v0), s0 = runs[0]
+    assert s1["t"] == t_end == s0["t"]
+    assert abs(s1["n_block_steps"] - s0["n_block_steps"]) <= 0.01 * s0["n_block_steps"] + 2
+    assert abs(s1["n_particle_steps"] - s0["n_particle_steps"]) <= 0.005 * s0["n_particle_steps"] + 2
+    assert np.abs(x1 - x0).max() < 1e-8 and np.abs(v1 - v0).max() < 1e-5
+
+
 @pytest.mark.parametrize("n,t_end", [(512, 0.0625), (3000, 0.015625)])
 def test_device_shared_time_steps_vs_oracle(cluster, oracle, n, t_end):
     """shared-time-step variant (reading 21) on the device against the oracle's: every particle takes every
