@@ -287,6 +287,37 @@ def test_step_loop_with_a_largest_step_that_is_not_a_power_of_two(cluster, oracl
     assert np.abs(x1 - x0).max() < 1e-8 and np.abs(v1 - v0).max() < 1e-5
 
 
+def test_step_loop_random_walk_against_the_path_without_it(cluster, oracle):
+    """seeded random sizes, softenings, accuracies and largest steps (0.1 included): the two device paths take the same block steps and
+    end in the same state"""
+    rng = np.random.default_rng(20261105)
+    for case in range(10):
+        n = int(rng.choice([rng.integers(2, 600), rng.integers(600, 9000), rng.integers(9000, 70000)]))
+        eps2 = float(rng.choice([1e-2, 1e-3, 1e-4])) ** 2
+        eta = float(rng.choice([0.005, 0.01, 0.02, 0.03]))
+        dt_max = float(rng.choice([0.125, 0.0625, 0.1]))
+        t_end = dt_max * float(rng.choice([0.25, 0.5, 1.0])) if n < 9000 else dt_max / 16
+        x, v, m, _ = inputs.config("C2", n=max(n, 2))
+        x, v, m = x[:n], v[:n], m[:n] / m[:n].sum()
+        res = {}
+        for loop in (1, 0):
+            os.environ["G6_HD_LOOP"] = str(loop)
+            try:
+                h = g6.HermiteDev(0, x, v, m, eps2, eta, dt_max=dt_max)
+            finally:
+                del os.environ["G6_HD_LOOP"]
+            h.evolve(t_end)
+            res[loop] = (h.state(), h.stats())
+            h.close()
+        (x1, v1), s1 = res[1]
+        (x0, v0), s0 = res[0]
+        what = (case, n, eps2, eta, dt_max, t_end, s1["n_block_steps"], s0["n_block_steps"])
+        assert s1["t"] == s0["t"] == t_end, what
+        assert abs(s1["n_particle_steps"] - s0["n_particle_steps"]) <= 0.005 * s0["n_particle_steps"] + 3, what
+        assert abs(s1["n_block_steps"] - s0["n_block_steps"]) <= 0.15 * s0["n_block_steps"] + 3, what
+        assert np.abs(x1 - x0).max() < 1e-7 and np.abs(v1 - v0).max() < 1e-5, what
+
+
 @pytest.mark.parametrize("n,t_end", [(512, 0.0625), (3000, 0.015625)])
 def test_device_shared_time_steps_vs_oracle(cluster, oracle, n, t_end):
     """shared-time-step variant (reading 21) on the device against the oracle's: every particle takes every
