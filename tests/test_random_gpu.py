@@ -94,3 +94,36 @@ def test_random_block_step_cycles_with_j_updates(cluster, oracle, seed):
                 x[a] = xp[a] + 1e-6 * rng.normal(size=3); v[a] = vp[a]; tj[a] = ti
                 a0[a] = 1e-2 * rng.normal(size=3); j0[a] = 1e-1 * rng.normal(size=3)
                 g6.g6_set_j_particle(0, int(a), int(idx[a]), ti, 2.0 ** -8, m[a], None, j0[a] / 6, a0[a] / 2, v[a], x[a])
+
+
+def test_random_neighbour_lists_with_overflow(cluster, oracle):
+    """radii from a few neighbours to a large part of the cluster, list lengths from 4 to 1024: counts, stored entries (the smallest
+    addresses on overflow) and their order against the oracle, through every kernel that builds lists"""
+    rng = np.random.default_rng(9090)
+    overflowed = 0
+    try:
+        for case in range(12):
+            nj = int(rng.choice([rng.integers(2, 500), rng.integers(500, 6000), rng.integers(6000, 40000)]))
+            ni = int(min(nj, rng.choice([1, 3, 16, 32, 33, 64, 65, 200, 256, 300, 1000])))
+            maxlen = int(rng.choice([4, 8, 64, 256, 1024]))
+            g6.g6x_set_option(0, "kernel", int(rng.choice([0, 0, 1, 2]))); g6.g6x_set_option(0, "bs_design", int(rng.choice([0, 1, 2])))
+            g6.g6x_set_option(0, "nb_maxlen", maxlen)
+            g6.g6x_set_npipes(max(ni, 4096))
+            x, v, m, _ = inputs.config("C2", n=max(nj, 2))
+            x, v, m = x[:nj].copy(), v[:nj].copy(), m[:nj] / m[:nj].sum()
+            idx = rng.permutation(nj).astype(np.int32)
+            z = np.zeros((nj, 3))
+            g6.g6_reset(0)
+            g6.g6x_set_j_particles(0, 0, idx, np.zeros(nj), m, z, z, v, x)
+            g6.g6_set_ti(0, 0.0)
+            sel = np.sort(rng.choice(nj, ni, replace=False))
+            h2 = 10.0 ** rng.uniform(-3.5, -0.3, ni)
+            g6.force_host(0, idx[sel], x[sel], v[sel], 1e-6, nj, h2=h2)
+            g6.g6_read_neighbour_list(0)
+            cnt, lst, _ = g6.g6x_get_neighbour_lists(0, ni, maxlen)
+            oc, ol = oracle.neighbours(idx[sel], x[sel], h2, idx, x, maxlen=nj)
+            check_neighbours(cnt, lst, oc, ol, idx, x[sel], x, h2, maxlen)
+            overflowed += int((oc > maxlen).sum())
+    finally:
+        g6.g6x_set_option(0, "nb_maxlen", 256)
+    assert overflowed > 0
