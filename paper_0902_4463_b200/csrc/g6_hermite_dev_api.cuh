@@ -478,9 +478,9 @@ int g6hd_get_stats(g6hd_system *sp, double stats[8], long long ni_hist_log2[64])
             }
             if (pr[31]) {
                 const double n = (double)pr[31];
-                fprintf(stderr, "  the CTAs that own an active particle of such a step (<= %d of them): gather poll %.0f | barrier %.0f | sum of the %d partials %.0f | corrector %.0f | stores %.0f | "
-                        "barrier %.0f | to the rescan's end %.0f | release fence %.0f | publish %.0f\n", HL_CQ, pr[16] / n, pr[17] / n, s.loop_G, pr[18] / n, pr[19] / n, pr[20] / n,
-                        pr[21] / n, pr[22] / n, pr[23] / n, pr[24] / n);
+                fprintf(stderr, "  the CTAs that own an active particle of such a step (<= %d of them): gather poll %.0f | barrier %.0f | sum of the %d partials %.0f | corrector %.0f | "
+                        "barrier + stores + release fence (an idle warp rescans the tile meanwhile) %.0f | closing barrier %.0f | to the top of the next step %.0f | publish %.0f\n",
+                        HL_CQ, pr[16] / n, pr[17] / n, s.loop_G, pr[18] / n, pr[19] / n, pr[20] / n, pr[21] / n, (pr[22] + pr[23]) / n, pr[24] / n);
             }
         }
         for (int b = 0; b < 64; ++b)
