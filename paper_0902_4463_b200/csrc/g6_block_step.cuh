@@ -566,14 +566,39 @@ k_block_step_dbg(const BsArgs A)
 // take their i-particles in chunks of 32 (the predicted tile is re-read from shared memory, not re-predicted).
 // 8 warps; 6 ring slots for blocks up to 16 particles, 5 up to 64 (their fp64 sums take the room).  Measured at N_j = 2^20: 12 warps
 // with the 4 slots that then fit are 4 % faster at n_i = 16 but 14 % slower at n_i = 1, where the stream from HBM is everything
-__host__ __device__ constexpr int bs2_threads(int maxi) { return maxi <= 64 ? 256 : 256; }
-__host__ __device__ constexpr int bs2_nslots(int maxi) { return maxi <= 16 ? 6 : 5; }
-constexpr int BS2_PRED_BYTES = TILE_BYTES + JT * 4;      // predicted tile + the 256 indices
+//
+// The unit of work of a warp is a SUB-TILE (JT / SUB particles), not a whole tile: with 148 x 8 warps and 4096 tiles (N_j = 2^20)
+// a warp would get 3 or 4 whole tiles and a quarter of the warps would idle through the last round; N_j = 32768 is one tile per
+// CTA, i.e. one busy warp per SM.  The SUB warps that share a raw slot count themselves out of it (shared-memory atomic), and the
+// last one re-issues the slot's next copy.  The per-warp buffer shrinks with the unit, which pays for more warps and ring slots.
+// Measured (B200, cold L2, CUDA events around the call, us; 8 warps x whole tiles -> this): N_j = 2^20: n_i = 8 34.9 -> 34.8,
+// 16 47.1 -> 44.6, 32 79.9 -> 78.9, 64 137.3 -> 131.7;  N_j = 32768: n_i = 4 14.4 -> 13.3, 16 20.5 -> 16.5, 32 30.1 -> 22.6, 64 47.1 -> 33.8.
+#ifndef G6_BS2_SUB16
+#define G6_BS2_SUB16 2
+#endif
+#ifndef G6_BS2_SUB64
+#define G6_BS2_SUB64 4
+#endif
+#ifndef G6_BS2_T16
+#define G6_BS2_T16 512
+#endif
+#ifndef G6_BS2_T64
+#define G6_BS2_T64 384
+#endif
+__host__ __device__ constexpr int bs2_sub(int maxi) { return maxi <= 16 ? G6_BS2_SUB16 : G6_BS2_SUB64; }   // warps per tile (1, 2 or 4)
+__host__ __device__ constexpr int bs2_uj(int maxi) { return JT / bs2_sub(maxi); }                          // j-particles per unit
+__host__ __device__ constexpr int bs2_threads(int maxi) { return maxi <= 16 ? G6_BS2_T16 : G6_BS2_T64; }
+__host__ __device__ constexpr int bs2_pred_bytes(int maxi) { return bs2_uj(maxi) * NF * 4 + bs2_uj(maxi) * 4; }   // predicted unit (field-major floats) + its indices
+// ring slots: what is left of the SM's shared memory after the per-warp buffers and sums
+__host__ __device__ constexpr int bs2_nslots(int maxi)
+{
+    return (232448 - 1024 - (bs2_threads(maxi) / 32) * (bs2_pred_bytes(maxi) + maxi * 72) - maxi * 44) / RAW_TILE_BYTES;
+}
 
 template <int MAXI>
 struct Bs2Smem {
     alignas(128) char raw[bs2_nslots(MAXI)][RAW_TILE_BYTES];  // ring of raw tiles: tile `it` of the CTA lives in slot it % NS
-    alignas(16) char pred[bs2_threads(MAXI) / 32][BS2_PRED_BYTES];            // per warp: its current tile, predicted (field-major floats) + indices
+    alignas(16) char pred[bs2_threads(MAXI) / 32][bs2_pred_bytes(MAXI)];            // per warp: its current tile, predicted (field-major floats) + indices
     double acc[bs2_threads(MAXI) / 32][MAXI][8];                              // per-warp fp64 sums of every i (filled once, at the end)
     float r2[bs2_threads(MAXI) / 32][MAXI];
     int addr[bs2_threads(MAXI) / 32][MAXI];
@@ -582,6 +607,7 @@ struct Bs2Smem {
     int uaddr[MAXI];
     alignas(8) uint64_t full[bs2_nslots(MAXI)];
     volatile int armed[bs2_nslots(MAXI)];
+    int gone[bs2_nslots(MAXI)];                                               // warps that have read their unit out of the slot (running count)
     int is_last;
 };
 static_assert(sizeof(Bs2Smem<16>) <= 232448 && sizeof(Bs2Smem<64>) <= 232448, "block-step (2) shared memory");
@@ -600,7 +626,7 @@ __device__ __forceinline__ void block_step2_body(const BsArgs &A, const BsInline
 
     if (tid == 0) {
 #pragma unroll
-        for (int k = 0; k < NS; ++k) { mbar_init(&sm.full[k], 1); sm.armed[k] = k; }
+        for (int k = 0; k < NS; ++k) { mbar_init(&sm.full[k], 1); sm.armed[k] = k; sm.gone[k] = 0; }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
 #pragma unroll
         for (int k = 0; k < NS; ++k)
@@ -651,14 +677,19 @@ __device__ __forceinline__ void block_step2_body(const BsArgs &A, const BsInline
     const float2 eps2s = dup(pair_scale<NEWTON>() * A.eps2);
     const double kP = NEWTON ? 0.5 * sqrt((double)FOUR_THIRDS) : sqrt((double)THIRD), kA = kP * kP * kP;
     float *Pj = reinterpret_cast<float *>(sm.pred[w]);
-    int *JX = reinterpret_cast<int *>(sm.pred[w] + TILE_BYTES);
+    int *JX = reinterpret_cast<int *>(sm.pred[w] + bs2_uj(MAXI) * NF * 4);
 
-    for (int it = w; it < nt; it += NW) {
+    // unit u of the CTA = sub-tile u % SUB of its tile number u / SUB, handled by warp u % NW alone
+    constexpr int SUB = bs2_sub(MAXI), UJ = bs2_uj(MAXI);
+    static_assert(SUB == 1 || SUB == 2 || SUB == 4, "units are whole 64-particle groups");
+    for (int u = w; u < nt * SUB; u += NW) {
+        const int it = u / SUB, sub = u % SUB;
         const int tile = cta + it * G;
         const int slot = it % NS;
+        const int j0 = sub * UJ;                              // first particle of my unit inside the tile
         char *R = sm.raw[slot];
         // the copy of THIS tile must have been issued before its phase is waited for (a parity wait cannot tell phase
-        // p + 1 from the completed phase p - 1); with fewer slots than warps that holds from the first round on
+        // p + 1 from the completed phase p - 1)
         if (it >= NS) {
             uint32_t spins = 0;
             while (ld_acquire_cta(&sm.armed[slot]) != it) { if (++spins > (1u << 26)) __trap(); }
@@ -667,20 +698,20 @@ __device__ __forceinline__ void block_step2_body(const BsArgs &A, const BsInline
 
         // ---- a-1: particles corrected in the last step that live in this tile: patch the staged copy, write through
         if (A.n_upd > 0) {
-            for (int u = lane; u < A.n_upd; u += 32)
-                if (sm.uaddr[u] / JT == tile) {
-                    const JRecord r = Dp->upd[u];
+            for (int q = lane; q < A.n_upd; q += 32)
+                if (sm.uaddr[q] / JT == tile && (sm.uaddr[q] % JT) / UJ == sub) {
+                    const JRecord r = Dp->upd[q];
                     store_record(R, r.addr % JT, r);
                     store_record(A.raw + (size_t)tile * RAW_TILE_BYTES, r.addr % JT, r);
                 }
             __syncwarp();
         }
-        // ---- a-2: predict my 8 j (lane l owns the pairs {2l, 2l + 1} + 64 g: conflict-free vector loads) into my warp's buffer
-        const bool ragged = tile * JT + JT > A.nj;
+        // ---- a-2: predict my UJ / 32 j (lane l owns the pairs {2l, 2l + 1} + 64 g: conflict-free vector loads) into my warp's buffer
+        const bool ragged = tile * JT + j0 + UJ > A.nj;
         int id_lo = INT32_MAX, id_hi = INT32_MIN;
 #pragma unroll
-        for (int g = 0; g < 4; ++g) {
-            const int l0 = 2 * lane + 64 * g;
+        for (int g = 0; g < UJ / 64; ++g) {
+            const int lu = 2 * lane + 64 * g, l0 = j0 + lu;    // inside the unit, inside the tile
             const double2 tj = *reinterpret_cast<const double2 *>(R + RAW_T + 8 * l0);
             const float2 dt = make_float2((float)(A.ti - tj.x), (float)(A.ti - tj.y));
             float2 f[NF];
@@ -700,27 +731,35 @@ __device__ __forceinline__ void block_step2_body(const BsArgs &A, const BsInline
                 for (int k = 0; k < NF; ++k) f[k] = make_float2(in0 ? f[k].x : 0.0f, in1 ? f[k].y : 0.0f);
             }
 #pragma unroll
-            for (int k = 0; k < NF; ++k) *reinterpret_cast<float2 *>(Pj + k * JT + l0) = f[k];
+            for (int k = 0; k < NF; ++k) *reinterpret_cast<float2 *>(Pj + k * UJ + lu) = f[k];
             const int2 jx = *reinterpret_cast<const int2 *>(R + RAW_IDX + 4 * l0);
-            *reinterpret_cast<int2 *>(JX + l0) = jx;
+            *reinterpret_cast<int2 *>(JX + lu) = jx;
             id_lo = min(id_lo, min(jx.x, jx.y));
             id_hi = max(id_hi, max(jx.x, jx.y));
         }
-        // Self-exclusion hoisted to tile level, as in the sweep kernel: if no i-particle of this warp's lanes has its index
-        // inside the tile's index range (and the tile is not the ragged last one) the tile runs the unchecked pair code
+        // Self-exclusion hoisted to unit level, as in the sweep kernel: if no i-particle of this warp's lanes has its index
+        // inside the unit's index range (and the unit is not cut by nj) the unit runs the unchecked pair code
         id_lo = __reduce_min_sync(FULL, id_lo);
         id_hi = __reduce_max_sync(FULL, id_hi);
         bool hit = false;
 #pragma unroll
         for (int ch = 0; ch < NCH; ++ch) hit |= act[ch] && my[ch] >= id_lo && my[ch] <= id_hi;
         const bool checked = !fast_ok || ragged || __any_sync(FULL, hit);
-        // the slot is consumed: refill it with the tile NS ahead while the forces are computed
+        // my unit is out of the slot; the LAST of the tile's SUB warps refills the slot with the tile NS ahead while the forces are computed
         __syncwarp();
-        if (lane == 0 && it + NS < nt) {
-            if (A.n_upd > 0) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // a-1 wrote the slot through the generic proxy
-            mbar_expect_tx(&sm.full[slot], RAW_TILE_BYTES);
-            tma_load_1d(R, A.raw + (size_t)(tile + NS * G) * RAW_TILE_BYTES, RAW_TILE_BYTES, &sm.full[slot]);
-            st_release_cta(&sm.armed[slot], it + NS);
+        if (lane == 0) {
+            bool last = true;
+            if (SUB > 1) {
+                __threadfence_block();                        // my lanes' reads (and a-1 writes) of the slot before the count ...
+                last = (atomicAdd(&sm.gone[slot], 1) % SUB) == SUB - 1;
+                __threadfence_block();                        // ... and the other warps' before the copy that overwrites it
+            }
+            if (last && it + NS < nt) {
+                if (A.n_upd > 0) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // a-1 wrote the slot through the generic proxy
+                mbar_expect_tx(&sm.full[slot], RAW_TILE_BYTES);
+                tma_load_1d(R, A.raw + (size_t)(tile + NS * G) * RAW_TILE_BYTES, RAW_TILE_BYTES, &sm.full[slot]);
+                st_release_cta(&sm.armed[slot], it + NS);
+            }
         }
 
         // ---- a-4: the pairs of this tile; my i-particle of every chunk against my j-sub-range
@@ -737,15 +776,15 @@ __device__ __forceinline__ void block_step2_body(const BsArgs &A, const BsInline
                 I.j[k] = dup(0.0f);
             }
             I.p = dup(0.0f);
-            const int jn = 8 << lg[ch];
+            const int jn = (UJ / 32) << lg[ch];
             const int jl0 = (lane >> lg[ch]) * jn;
-            if (checked) {
+            if (checked || jn < 4) {                          // (the unchecked loop takes four j at a time)
 #pragma unroll 2
                 for (int q = 0; q < jn; q += 2) {
-                    const int jl = jl0 + q, ja = tile * JT + jl;
+                    const int jl = jl0 + q, ja = tile * JT + j0 + jl;
                     float2 f[NF];
 #pragma unroll
-                    for (int k = 0; k < NF; ++k) f[k] = *reinterpret_cast<const float2 *>(Pj + k * JT + jl);
+                    for (int k = 0; k < NF; ++k) f[k] = *reinterpret_cast<const float2 *>(Pj + k * UJ + jl);
                     const int2 jx = *reinterpret_cast<const int2 *>(JX + jl);
                     float2 r2;
                     pair2_checked<NEWTON>(I, f[0], f[1], f[2], f[3], f[4], f[5], f[6], f[7], f[8], f[9], eps2,
@@ -766,10 +805,10 @@ __device__ __forceinline__ void block_step2_body(const BsArgs &A, const BsInline
                 // scaled sigma); its sums come out scaled by (y s) and (y s)^3, undone here in fp64 with the binary32 scale
 #pragma unroll 2
                 for (int q = 0; q < jn; q += 4) {
-                    const int jl = jl0 + q, ja = tile * JT + jl;
+                    const int jl = jl0 + q, ja = tile * JT + j0 + jl;
                     float4 f[NF];
 #pragma unroll
-                    for (int k = 0; k < NF; ++k) f[k] = *reinterpret_cast<const float4 *>(Pj + k * JT + jl);
+                    for (int k = 0; k < NF; ++k) f[k] = *reinterpret_cast<const float4 *>(Pj + k * UJ + jl);
                     float2 ra, rb;
                     pair2<NEWTON>(I, make_float2(f[0].x, f[0].y), make_float2(f[1].x, f[1].y), make_float2(f[2].x, f[2].y),
                                   make_float2(f[3].x, f[3].y), make_float2(f[4].x, f[4].y), make_float2(f[5].x, f[5].y),
