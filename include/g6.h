@@ -204,6 +204,24 @@ int g6x_calc_dev(int clusterid, int nj, int ni, const int *d_index, const double
                  const double *d_vi, double eps2, double *d_acc, double *d_jerk, double *d_pot,
                  int *d_nn_index, double *d_nn_r2);
 
+/* g6x_calc_dev for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): same arguments, same results (the same predictor, force and combine kernels, PAPER.md section
+ * 2.3, :106), but the per-split partial sums go to a FIXED file-scope device array instead of the on-demand buffer
+ * that g6x_calc_dev grows with cudaMalloc.  The call allocates and frees nothing, on host or device.
+ *  - Limit: (j-splits chosen by the scheduler) x ni <= g6x_noalloc_max_rows() = 65536 rows (4 MiB, held by every GPU
+ *    that loads the library until exit); the splits are capped to fit, ni > 65536 is G6_ERR_NI.
+ *  - Always the sweep path (predictor, force kernel, combine), also for small blocks; no neighbour lists.
+ *  - No j-particle update may be pending (G6_ERR_SEQUENCE): call g6_flush_jp_buffer first -- this call stages nothing.
+ *  - The array is shared by all calls on a device and keeps the last call's partials (every row read is written first,
+ *    nothing needs clearing).  Calls that OVERLAP on the GPU (two clusters / streams on one device) race on it.
+ *  - g6x_noalloc_init resolves the array's device address for the cluster's device (cudaGetSymbolAddress, once per
+ *    device); g6x_calc_dev_noalloc does it itself on first use, so call init before a capture begins. */
+int g6x_calc_dev_noalloc(int clusterid, int nj, int ni, const int *d_index, const double *d_xi,
+                         const double *d_vi, double eps2, double *d_acc, double *d_jerk, double *d_pot,
+                         int *d_nn_index, double *d_nn_r2);
+int g6x_noalloc_init(int clusterid);
+int g6x_noalloc_max_rows(void);
+
 /* g6x_calc_dev with neighbour lists: d_h2[ni] fp64 radii squared in; d_nb_count[ni] (all neighbours
  * found, may exceed nb_maxlen) and d_nb_list[ni][nb_maxlen] (callers' indices, increasing j address;
  * entries past min(count, nb_maxlen) are left untouched) out.  The three pointers are given

@@ -1333,3 +1333,6 @@ int g6x_jsplit_unpack_dev(int clusterid, int ni, const long long *d_key_min, con
 
 // device-resident Hermite integrator (g6hd_*, include/g6_hermite.h): needs the internals above
 #include "g6_hermite_dev_api.cuh"
+
+// force call that allocates nothing (g6x_calc_dev_noalloc): partials in a fixed file-scope device array
+#include "g6_noalloc.cuh"

@@ -24,6 +24,7 @@ SYMBOLS = [
     "g6_set_tunit", "g6_set_xunit", "g6_reset", "g6_reset_fofpga", "g6_initialize_jp_buffer", "g6_flush_jp_buffer",
     "g6_getnjmax", "g6_get_j_particle", "g6x_get_j_particles", "g6x_get_units",
     "g6x_last_error", "g6x_set_npipes", "g6x_set_j_particles", "g6x_set_j_particles_dev", "g6x_calc_dev",
+    "g6x_calc_dev_noalloc", "g6x_noalloc_init", "g6x_noalloc_max_rows",
     "g6x_calc_dev_nb", "g6x_get_neighbour_lists", "g6x_jsplit_pack_dev", "g6x_jsplit_select_dev", "g6x_jsplit_unpack_dev",
     "g6x_get_nearest", "g6x_set_stream", "g6x_synchronize", "g6x_get_timers", "g6x_set_option",
     "g6x_get_option", "g6x_get_predicted", "g6x_version",
@@ -268,6 +269,22 @@ def g6x_calc_dev(clusterid, nj, ni, d_index, d_xi, d_vi, eps2, d_acc, d_jerk, d_
     return _chk(lib().g6x_calc_dev(C.c_int(clusterid), C.c_int(nj), C.c_int(ni), _dev(d_index, i, ni), _dev(d_xi, f, 3 * ni),
                                    _dev(d_vi, f, 3 * ni), C.c_double(eps2), _dev(d_acc, f, 3 * ni), _dev(d_jerk, f, 3 * ni),
                                    _dev(d_pot, f, ni), _dev(d_nn_index, i, ni), _dev(d_nn_r2, f, ni)), clusterid)
+
+
+def g6x_calc_dev_noalloc(clusterid, nj, ni, d_index, d_xi, d_vi, eps2, d_acc, d_jerk, d_pot, d_nn_index=None, d_nn_r2=None):
+    import torch
+    f, i = torch.float64, torch.int32
+    return _chk(lib().g6x_calc_dev_noalloc(C.c_int(clusterid), C.c_int(nj), C.c_int(ni), _dev(d_index, i, ni), _dev(d_xi, f, 3 * ni),
+                                           _dev(d_vi, f, 3 * ni), C.c_double(eps2), _dev(d_acc, f, 3 * ni), _dev(d_jerk, f, 3 * ni),
+                                           _dev(d_pot, f, ni), _dev(d_nn_index, i, ni), _dev(d_nn_r2, f, ni)), clusterid)
+
+
+def g6x_noalloc_init(clusterid):
+    return _chk(lib().g6x_noalloc_init(C.c_int(clusterid)), clusterid)
+
+
+def g6x_noalloc_max_rows():
+    return int(lib().g6x_noalloc_max_rows())
 
 
 def g6x_calc_dev_nb(clusterid, nj, ni, d_index, d_xi, d_vi, eps2, d_acc, d_jerk, d_pot, d_nn_index, d_nn_r2, d_h2, d_nb_count, d_nb_list):
