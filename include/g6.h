@@ -262,9 +262,9 @@ int g6x_get_timers(int clusterid, double us[8]);
  *   "variant" 0 = automatic; threads*8 + i_per_thread forces a fast-kernel shape: one of 128*8+2, 128*8+1, 64*8+1,
  *             32*8+1, 256*8+1 (the automatic ones), 128*8+4, 64*8+2; anything else is G6_ERR_ARG
  *   "small"   largest n_i served by the block-step kernel (one launch: j update + predictor + force +
- *             combine, lanes over j); at most 64, 0 = off.  Until it is set the library uses its own rule,
- *             the measured crossover with the three-launch sweep path: 24 below 65536 j-particles, 32 below
- *             262144, 48 above (g6x_get_option reports 32 then)
+ *             combine); at most 64, 0 = off.  Until it is set the library uses 64: the kernel beats the
+ *             three-launch sweep path at every block size it is built for (with neighbour lists: 28 below 65536
+ *             j-particles, 40 below 262144, 64 above; g6x_get_option reports 32 until the option is set)
  *   "nb_maxlen" neighbours stored per i-particle (1 .. 4096, default G6_NB_MAXLEN = 256; compile-time
  *             in the paper); changing it discards the lists of the last call
  *   "last_kernel" (g6x_get_option only) the force kernel the last call took: 1 checked reference kernel,

@@ -507,12 +507,15 @@ int choose_jsplit(int n_itiles, int ntiles, int slots, int ni, long long s_cap =
 
 // force + combine (steps a-4, a-5) on device-resident i-blocks; all asynchronous
 // small active blocks take the fused block-step kernel unless an experiment switch pins another path
-// Largest block the block-step kernel serves.  Its time grows by ~2.0 us per i-particle per 2^20 j, the sweep path's
-// (predictor + sweep kernel + combine: three launches) starts higher and grows slower; measured crossover n_i = 28 at
-// N_j = 32768 and ~56 at N_j = 2^20.  Option "small" set by the caller overrides the rule.
-int small_limit(const Cluster &c, int nj)
+// Largest block the block-step kernel serves: all it is built for (BS_MAX_I = 64).  Since its warps work on sub-tiles
+// (g6_block_step.cuh) it beats the sweep path (predictor + sweep kernel + combine: three launches) at every block size it
+// takes, measured by CUDA events around the device call, cold L2: n_i = 64 at N_j = 32768 33 us against 50, at N_j = 2^20
+// 131 us against 161 (the earlier crossovers were 28 and ~56).  Option "small" set by the caller overrides the rule.
+// With neighbour lists the first design runs (lanes over j, a reduction per (i, tile)): its crossovers stay as measured.
+int small_limit(const Cluster &c, int nj, bool nb = false)
 {
     if (c.small_explicit) return c.opt_small;
+    if (!nb && c.opt_bs_design != 1) return BS_MAX_I;
     const int ntiles = (nj + JT - 1) / JT;
     return ntiles >= 1024 ? 64 : (ntiles >= 256 ? 40 : 28);
 }
@@ -520,7 +523,7 @@ int small_limit(const Cluster &c, int nj)
 bool use_block_step(const Cluster &c, int ni, int nj, bool nb = false)
 {
     // with neighbour lists the kernel's last-CTA merge holds one list per warp in shared memory
-    return (!nb || c.opt_nb_maxlen <= BS_NB_SCRATCH) && ni <= small_limit(c, nj) && c.opt_kernel != 1 && c.opt_kernel != 2 && c.opt_jsplit == 0;
+    return (!nb || c.opt_nb_maxlen <= BS_NB_SCRATCH) && ni <= small_limit(c, nj, nb) && c.opt_kernel != 1 && c.opt_kernel != 2 && c.opt_jsplit == 0;
 }
 
 struct HostBlock { const double *xi, *vi; const int *index; };   // host copy of the i-block (small blocks travel in kernel parameters)
