@@ -567,26 +567,30 @@ k_block_step_dbg(const BsArgs A)
 // 8 warps; 6 ring slots for blocks up to 16 particles, 5 up to 64 (their fp64 sums take the room).  Measured at N_j = 2^20: 12 warps
 // with the 4 slots that then fit are 4 % faster at n_i = 16 but 14 % slower at n_i = 1, where the stream from HBM is everything
 //
-// The unit of work of a warp is a SUB-TILE (JT / SUB particles), not a whole tile: with 148 x 8 warps and 4096 tiles (N_j = 2^20)
-// a warp would get 3 or 4 whole tiles and a quarter of the warps would idle through the last round; N_j = 32768 is one tile per
-// CTA, i.e. one busy warp per SM.  The SUB warps that share a raw slot count themselves out of it (shared-memory atomic), and the
-// last one re-issues the slot's next copy.  The per-warp buffer shrinks with the unit, which pays for more warps and ring slots.
-// Measured (B200, cold L2, CUDA events around the call, us; 8 warps x whole tiles -> this): N_j = 2^20: n_i = 8 34.9 -> 34.8,
-// 16 47.1 -> 44.6, 32 79.9 -> 78.9, 64 137.3 -> 131.7;  N_j = 32768: n_i = 4 14.4 -> 13.3, 16 20.5 -> 16.5, 32 30.1 -> 22.6, 64 47.1 -> 33.8.
-#ifndef G6_BS2_SUB16
-#define G6_BS2_SUB16 2
+// The unit of work of a warp is a run of QUARTER TILES (64 particles each), not a whole tile: with 148 x 8 warps and 4096 tiles
+// (N_j = 2^20) a warp would get 3 or 4 whole tiles and a quarter of the warps would idle through the last round; N_j = 32768 is
+// one tile per CTA, i.e. one busy warp per SM.  The schedule is static (run-to-run bit-reproducible sums, reading 9):
+// in full rounds every warp takes UQ consecutive quarters (warp w of round r: quarters (r NW + w) UQ ...), the quarters left for
+// the last round are dealt out as evenly as whole quarters allow (the first warps take two while more than NW are left).
+// The warps that share a raw slot count their quarters out of it (shared-memory atomic); the one that completes the four
+// re-issues the slot's next copy.  The per-warp buffer shrinks with the unit, which pays for more warps and ring slots.
+// Measured (B200, cold L2, CUDA events around the call, us; 8 warps x whole tiles -> 16 warps x half / quarter tiles):
+// N_j = 2^20: n_i = 16 47.1 -> 44.0, 32 79.9 -> 74.8, 64 137.3 -> 123.9;  N_j = 32768: 16 20.5 -> 16.5, 32 30.1 -> 22.0, 64 47.1 -> 29.7.
+#ifndef G6_BS2_UQ16
+#define G6_BS2_UQ16 2
 #endif
-#ifndef G6_BS2_SUB64
-#define G6_BS2_SUB64 4
+#ifndef G6_BS2_UQ64
+#define G6_BS2_UQ64 1
 #endif
 #ifndef G6_BS2_T16
 #define G6_BS2_T16 512
 #endif
 #ifndef G6_BS2_T64
-#define G6_BS2_T64 384
+#define G6_BS2_T64 512
 #endif
-__host__ __device__ constexpr int bs2_sub(int maxi) { return maxi <= 16 ? G6_BS2_SUB16 : G6_BS2_SUB64; }   // warps per tile (1, 2 or 4)
-__host__ __device__ constexpr int bs2_uj(int maxi) { return JT / bs2_sub(maxi); }                          // j-particles per unit
+constexpr int BS2_QJ = 64;                                                                                  // particles per quarter tile
+__host__ __device__ constexpr int bs2_uq(int maxi) { return maxi <= 16 ? G6_BS2_UQ16 : G6_BS2_UQ64; }      // quarters per unit in a full round (1 or 2)
+__host__ __device__ constexpr int bs2_uj(int maxi) { return BS2_QJ * bs2_uq(maxi); }                       // j-particles per unit, at most
 __host__ __device__ constexpr int bs2_threads(int maxi) { return maxi <= 16 ? G6_BS2_T16 : G6_BS2_T64; }
 __host__ __device__ constexpr int bs2_pred_bytes(int maxi) { return bs2_uj(maxi) * NF * 4 + bs2_uj(maxi) * 4; }   // predicted unit (field-major floats) + its indices
 // ring slots: what is left of the SM's shared memory after the per-warp buffers and sums
@@ -618,7 +622,7 @@ __device__ __forceinline__ void block_step2_body(const BsArgs &A, const BsInline
     extern __shared__ __align__(128) unsigned char smem_raw[];
     Bs2Smem<MAXI> &sm = *reinterpret_cast<Bs2Smem<MAXI> *>(smem_raw);
     constexpr float INF = __builtin_huge_valf();
-    constexpr int BS2_THREADS = bs2_threads(MAXI), NW = BS2_THREADS / 32, NS = bs2_nslots(MAXI), NCH = (MAXI + 31) / 32;
+    constexpr int BS2_THREADS = bs2_threads(MAXI), NW = BS2_THREADS / 32, NS = bs2_nslots(MAXI), NCH = MAXI <= 16 ? 1 : 2;
     const unsigned FULL = 0xffffffffu;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int G = gridDim.x, cta = blockIdx.x;
@@ -653,6 +657,21 @@ __device__ __forceinline__ void block_step2_body(const BsArgs &A, const BsInline
     __syncthreads();
 
     // my place in every chunk of 32 i-particles: lanes = 2^lg i-particles x 2^(5 - lg) j-sub-ranges of 8 x 2^lg j
+    // The i-block as at most two chunks of a power-of-two number of lanes each (<= 32): one chunk of ceil2(n_i) lanes, or -- where
+    // that wastes lanes -- the largest power of two below n_i plus the rest rounded up (n_i = 24: 16 + 8 lanes' worth of work
+    // instead of 32: 72 -> 61 us at N_j = 2^20; 17: 71 -> 53).  Every chunk is one pass over the warp's predicted unit.  The kernel
+    // for blocks up to 16 keeps a single chunk (a second set of sums costs it 2 us at n_i = 1).
+    int cb[NCH], cn[NCH];
+    cb[0] = 0; cn[0] = A.ni;
+    if (NCH > 1) {
+        const auto ceil2 = [](int n) { int c = 1; while (c < n) c *= 2; return c; };
+        int f = 1;
+        while (2 * f <= min(A.ni, 32)) f *= 2;
+        const int rest = A.ni - f;
+        const bool one = A.ni <= 32 && (rest == 0 || f + ceil2(rest) >= ceil2(A.ni));
+        cn[0] = one ? A.ni : f;
+        cb[NCH - 1] = cn[0]; cn[NCH - 1] = A.ni - cn[0];
+    }
     int lg[NCH], ii[NCH], my[NCH];
     bool act[NCH];
     double acc7[NCH][7];
@@ -660,12 +679,12 @@ __device__ __forceinline__ void block_step2_body(const BsArgs &A, const BsInline
     int baddr[NCH];
 #pragma unroll
     for (int ch = 0; ch < NCH; ++ch) {
-        const int nic = max(0, min(32, A.ni - 32 * ch));
+        const int nic = cn[ch];
         lg[ch] = 0;
         while ((1 << lg[ch]) < nic) ++lg[ch];
         ii[ch] = lane & ((1 << lg[ch]) - 1);
         act[ch] = ii[ch] < nic;
-        my[ch] = act[ch] ? sm.iidx[32 * ch + ii[ch]] : -1;
+        my[ch] = act[ch] ? sm.iidx[cb[ch] + ii[ch]] : -1;
         best[ch] = INF;
         baddr[ch] = 0x7fffffff;
 #pragma unroll
@@ -679,14 +698,20 @@ __device__ __forceinline__ void block_step2_body(const BsArgs &A, const BsInline
     float *Pj = reinterpret_cast<float *>(sm.pred[w]);
     int *JX = reinterpret_cast<int *>(sm.pred[w] + bs2_uj(MAXI) * NF * 4);
 
-    // unit u of the CTA = sub-tile u % SUB of its tile number u / SUB, handled by warp u % NW alone
-    constexpr int SUB = bs2_sub(MAXI), UJ = bs2_uj(MAXI);
-    static_assert(SUB == 1 || SUB == 2 || SUB == 4, "units are whole 64-particle groups");
-    for (int u = w; u < nt * SUB; u += NW) {
-        const int it = u / SUB, sub = u % SUB;
+    // the static schedule (see above): NR full rounds of UQ quarters per warp, then the last round
+    constexpr int UQ = bs2_uq(MAXI), UJ = bs2_uj(MAXI);       // UJ: the stride of the warp's buffer
+    static_assert(UQ == 1 || UQ == 2, "a unit never straddles two tiles");
+    const int Q = 4 * nt, NR = Q / (UQ * NW), rem = Q - NR * UQ * NW;   // NR full rounds
+    const int n2 = UQ == 2 ? max(0, rem - NW) : 0;           // warps that take two quarters in the last round
+    for (int r = 0; r <= NR; ++r) {
+        int qs, nq;
+        if (r < NR) { qs = (r * NW + w) * UQ; nq = UQ; }
+        else if (w < n2) { qs = NR * UQ * NW + 2 * w; nq = 2; }
+        else { qs = NR * UQ * NW + n2 + w; nq = 1; if (qs >= Q) break; }
+        const int it = qs >> 2, q0 = qs & 3;
         const int tile = cta + it * G;
         const int slot = it % NS;
-        const int j0 = sub * UJ;                              // first particle of my unit inside the tile
+        const int j0 = q0 * BS2_QJ, uj = nq * BS2_QJ;         // my unit inside the tile: first particle, particles
         char *R = sm.raw[slot];
         // the copy of THIS tile must have been issued before its phase is waited for (a parity wait cannot tell phase
         // p + 1 from the completed phase p - 1)
@@ -699,18 +724,18 @@ __device__ __forceinline__ void block_step2_body(const BsArgs &A, const BsInline
         // ---- a-1: particles corrected in the last step that live in this tile: patch the staged copy, write through
         if (A.n_upd > 0) {
             for (int q = lane; q < A.n_upd; q += 32)
-                if (sm.uaddr[q] / JT == tile && (sm.uaddr[q] % JT) / UJ == sub) {
+                if (sm.uaddr[q] / JT == tile && (unsigned)((sm.uaddr[q] % JT) / BS2_QJ - q0) < (unsigned)nq) {
                     const JRecord r = Dp->upd[q];
                     store_record(R, r.addr % JT, r);
                     store_record(A.raw + (size_t)tile * RAW_TILE_BYTES, r.addr % JT, r);
                 }
             __syncwarp();
         }
-        // ---- a-2: predict my UJ / 32 j (lane l owns the pairs {2l, 2l + 1} + 64 g: conflict-free vector loads) into my warp's buffer
-        const bool ragged = tile * JT + j0 + UJ > A.nj;
+        // ---- a-2: predict my uj / 32 j (lane l owns the pairs {2l, 2l + 1} + 64 g: conflict-free vector loads) into my warp's buffer
+        const bool ragged = tile * JT + j0 + uj > A.nj;
         int id_lo = INT32_MAX, id_hi = INT32_MIN;
 #pragma unroll
-        for (int g = 0; g < UJ / 64; ++g) {
+        for (int g = 0; g < nq; ++g) {
             const int lu = 2 * lane + 64 * g, l0 = j0 + lu;    // inside the unit, inside the tile
             const double2 tj = *reinterpret_cast<const double2 *>(R + RAW_T + 8 * l0);
             const float2 dt = make_float2((float)(A.ti - tj.x), (float)(A.ti - tj.y));
@@ -745,15 +770,12 @@ __device__ __forceinline__ void block_step2_body(const BsArgs &A, const BsInline
 #pragma unroll
         for (int ch = 0; ch < NCH; ++ch) hit |= act[ch] && my[ch] >= id_lo && my[ch] <= id_hi;
         const bool checked = !fast_ok || ragged || __any_sync(FULL, hit);
-        // my unit is out of the slot; the LAST of the tile's SUB warps refills the slot with the tile NS ahead while the forces are computed
+        // my unit is out of the slot; the warp that takes the tile's last quarters refills the slot with the tile NS ahead while the forces are computed
         __syncwarp();
         if (lane == 0) {
-            bool last = true;
-            if (SUB > 1) {
-                __threadfence_block();                        // my lanes' reads (and a-1 writes) of the slot before the count ...
-                last = (atomicAdd(&sm.gone[slot], 1) % SUB) == SUB - 1;
-                __threadfence_block();                        // ... and the other warps' before the copy that overwrites it
-            }
+            __threadfence_block();                            // my lanes' reads (and a-1 writes) of the slot before the count ...
+            const bool last = ((atomicAdd(&sm.gone[slot], nq) + nq) & 3) == 0;
+            __threadfence_block();                            // ... and the other warps' before the copy that overwrites it
             if (last && it + NS < nt) {
                 if (A.n_upd > 0) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // a-1 wrote the slot through the generic proxy
                 mbar_expect_tx(&sm.full[slot], RAW_TILE_BYTES);
@@ -769,14 +791,14 @@ __device__ __forceinline__ void block_step2_body(const BsArgs &A, const BsInline
             IPart I;
 #pragma unroll
             for (int k = 0; k < 3; ++k) {
-                I.nxh[k] = dup(-sm.ipart[32 * ch + ii[ch]][k]);
-                I.nxl[k] = dup(-sm.ipart[32 * ch + ii[ch]][3 + k]);
-                I.nv[k] = dup(-sm.ipart[32 * ch + ii[ch]][6 + k]);
+                I.nxh[k] = dup(-sm.ipart[cb[ch] + ii[ch]][k]);
+                I.nxl[k] = dup(-sm.ipart[cb[ch] + ii[ch]][3 + k]);
+                I.nv[k] = dup(-sm.ipart[cb[ch] + ii[ch]][6 + k]);
                 I.a[k] = dup(0.0f);
                 I.j[k] = dup(0.0f);
             }
             I.p = dup(0.0f);
-            const int jn = (UJ / 32) << lg[ch];
+            const int jn = (uj / 32) << lg[ch];
             const int jl0 = (lane >> lg[ch]) * jn;
             if (checked || jn < 4) {                          // (the unchecked loop takes four j at a time)
 #pragma unroll 2
@@ -845,7 +867,7 @@ __device__ __forceinline__ void block_step2_body(const BsArgs &A, const BsInline
             if (r2 < best[ch] || (r2 == best[ch] && ad < baddr[ch])) { best[ch] = r2; baddr[ch] = ad; }
         }
         if (act[ch] && lane < (1 << lg[ch])) {
-            const int i = 32 * ch + lane;
+            const int i = cb[ch] + lane;
 #pragma unroll
             for (int k = 0; k < 7; ++k) sm.acc[w][i][k] = acc7[ch][k];
             sm.r2[w][i] = best[ch];
