@@ -203,7 +203,12 @@ def test_eps2_zero_and_coincident_particles(cluster, oracle):
 
 
 # ------------------------------------------------------------------ block-step kernel (one launch: update + predictor + force + combine)
-@pytest.mark.parametrize("n,ni,small", [(5000, 1, 16), (5000, 7, 16), (5000, 16, 16), (1000, 64, 64), (300, 33, 64), (40000, 3, 16)])
+@pytest.mark.parametrize("n,ni,small", [(5000, 1, 16), (5000, 7, 16), (5000, 16, 16), (1000, 64, 64), (300, 33, 64), (40000, 3, 16),
+                                        # blocks of 17..31 as two power-of-two chunks, 33..64 as 32 + the rest
+                                        (5000, 17, 64), (5000, 24, 64), (3000, 31, 64), (3000, 40, 64),
+                                        # the static quarter-tile schedule: full rounds and every shape of the last round
+                                        # (7-8 and 13-14 tiles per CTA: warps with two quarters, one, none; an empty last round)
+                                        (300000, 5, 16), (300000, 20, 64), (530000, 16, 16), (530000, 24, 64)])
 def test_small_block_kernel_fused_predictor(cluster, oracle, n, ni, small):
     """n_i <= `small`: one pass over the raw j-store, Eq. 1-2 evaluated on the fly, t_i != t_j, the
     block's own particles present as j; must agree with the oracle and with the two-kernel path."""
