@@ -701,13 +701,24 @@ __device__ __forceinline__ void block_step2_body(const BsArgs &A, const BsInline
     // the static schedule (see above): NR full rounds of UQ quarters per warp, then the last round
     constexpr int UQ = bs2_uq(MAXI), UJ = bs2_uj(MAXI);       // UJ: the stride of the warp's buffer
     static_assert(UQ == 1 || UQ == 2, "a unit never straddles two tiles");
-    const int Q = 4 * nt, NR = Q / (UQ * NW), rem = Q - NR * UQ * NW;   // NR full rounds
+    // Staggered start (UQ == 2, 16 warps, at least 12 tiles): the four warps of one scheduler (w, w + 4, w + 8, w + 12) would
+    // otherwise predict together and evaluate pairs together, so the FP32 pipe idles through every prediction; in a round of its
+    // own, ahead of the others, the warps 4-7 and 12-15 take ONE quarter and run half a unit ahead from then on
+    // (quarters 0-7: warps 0-3 by two; 8-11: warps 4-7; 12-19: warps 8-11 by two; 20-23: warps 12-15).
+#ifndef G6_BS2_STAGGER
+#define G6_BS2_STAGGER 1
+#endif
+    const int Q = 4 * nt;
+    const bool stag = G6_BS2_STAGGER && UQ == 2 && NW == 16 && Q >= 48;
+    const int Q0 = stag ? 24 : 0;                            // quarters of the staggered round
+    const int NR = (Q - Q0) / (UQ * NW), rem = (Q - Q0) - NR * UQ * NW;   // NR full rounds
     const int n2 = UQ == 2 ? max(0, rem - NW) : 0;           // warps that take two quarters in the last round
-    for (int r = 0; r <= NR; ++r) {
+    for (int r = stag ? -1 : 0; r <= NR; ++r) {
         int qs, nq;
-        if (r < NR) { qs = (r * NW + w) * UQ; nq = UQ; }
-        else if (w < n2) { qs = NR * UQ * NW + 2 * w; nq = 2; }
-        else { qs = NR * UQ * NW + n2 + w; nq = 1; if (qs >= Q) break; }
+        if (r < 0) { const int g = w >> 2, k = w & 3; nq = (g & 1) ? 1 : 2; qs = (g >> 1) * 12 + ((g & 1) ? 8 + k : 2 * k); }
+        else if (r < NR) { qs = Q0 + (r * NW + w) * UQ; nq = UQ; }
+        else if (w < n2) { qs = Q0 + NR * UQ * NW + 2 * w; nq = 2; }
+        else { qs = Q0 + NR * UQ * NW + n2 + w; nq = 1; if (qs >= Q) break; }
         const int it = qs >> 2, q0 = qs & 3;
         const int tile = cta + it * G;
         const int slot = it % NS;
