@@ -557,15 +557,16 @@ k_block_step_dbg(const BsArgs A)
 // Same launch, same a-1 .. a-5 in one kernel, same ring of raw j-tiles fed by one TMA bulk copy per tile, same last-CTA
 // combine; what changes is the pair phase.  The first design kept lanes over j for the forces too and therefore had to
 // reduce the seven sums of every (i-particle, tile) over the warp (9 shuffles + two warp-wide integer reductions for the
-// nearest neighbour): a third of the instructions of a small block step.  Here a warp predicts its tile (lanes over j,
-// as before), writes the predicted particles to its OWN 11 KB buffer in shared memory and hands the raw slot back to the
-// ring at once; the pairs are then evaluated with LANES = (i-particle, j-sub-range) -- "several threads share an i and
+// nearest neighbour): a third of the instructions of a small block step.  Here a warp predicts its unit (a half or a quarter
+// tile, see below; lanes over j, as before), writes the predicted particles to its OWN buffer in shared memory and hands its
+// share of the raw slot back to the ring at once; the pairs are then evaluated with LANES = (i-particle, j-sub-range) -- "several threads share an i and
 // split the j" -- so that every lane keeps the sums and the nearest neighbour of ITS i-particle in
 // registers across all the tiles the warp works on (FP32 over one tile slice, folded into fp64 per tile: DESIGN.md reading
-// 9), and the lanes of one i are reduced by a fixed shuffle tree ONCE, at the end of the kernel.  Blocks above 32 particles
-// take their i-particles in chunks of 32 (the predicted tile is re-read from shared memory, not re-predicted).
-// 8 warps; 6 ring slots for blocks up to 16 particles, 5 up to 64 (their fp64 sums take the room).  Measured at N_j = 2^20: 12 warps
-// with the 4 slots that then fit are 4 % faster at n_i = 16 but 14 % slower at n_i = 1, where the stream from HBM is everything
+// 9), and the lanes of one i are reduced by a fixed shuffle tree ONCE, at the end of the kernel.  Blocks above 16 particles
+// take their i-particles in at most two power-of-two chunks (the predicted unit is re-read from shared memory, not re-predicted).
+// 16 warps; 6 ring slots for blocks up to 16 particles, 5 up to 64 (their fp64 sums take the room).  Warps and ring depth as
+// measured at N_j = 2^20 by kernel duration (profiles/r02_block_step_ncu.md): 8 warps with 9 slots and 12 with 7 are no faster
+// at n_i = 1 (the launch is a fixed 9.7 us plus the stream at the HBM rate) and 7 - 18 % slower at n_i = 16.
 //
 // The unit of work of a warp is a run of QUARTER TILES (64 particles each), not a whole tile: with 148 x 8 warps and 4096 tiles
 // (N_j = 2^20) a warp would get 3 or 4 whole tiles and a quarter of the warps would idle through the last round; N_j = 32768 is
