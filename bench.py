@@ -280,7 +280,7 @@ def ni_sweep(g6, inputs, torch, dev, stream, flush, x, v, idx_all, n, eps2, peak
             g6.g6x_set_option(0, "timers", 1)
             res[mode] = dict(step_us=float(np.median(tot)), force_us=float(np.median(frc)), predict_us=float(np.median(prd)),
                              combine_us=float(np.median(cmb)), jsplits=tm["jsplits"], ctas=tm["force_ctas"])
-        fused = ni <= g6.g6x_get_option(0, "small")
+        fused = g6.g6x_get_option(0, "last_kernel") == 3          # the block-step kernel took the call (n_i <= 64)
         bytes_step = n * (76 if fused else 156)
         c = res["cold"]
         rows.append({"n_i": ni, "cold": res["cold"], "warm": res["warm"], "fused_predictor": bool(fused),
